@@ -1,0 +1,387 @@
+/* kf_oracle.c -- fp64 CPU ORACLE for batched Kalman-filter track fitting and building.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the cpu_baseline /
+ * --impl reference legs of bench.py may load it.  It shares no code, header, table or constant generator with
+ * the CUDA path under paper_1711_06571_b200/csrc/ and include/kf.h; neither includes the other.
+ *
+ * What it follows.  The paper (arxiv 1711.06571, /root/reference/PAPER.md) is a prose report with no formulas:
+ *   - three stages, building = project outwards, collect compatible hits, branch, keep the best; final KF fit
+ *     (sec. 2);
+ *   - hybrid coordinates: global Cartesian position + polar momentum (sec. 3);
+ *   - ideal barrel, uniform longitudinal field, Gaussian-smeared hits (sec. 3);
+ *   - small matrices 3x3 .. 6x6 (sec. 2.1); fixed slots per seed, best candidates;
+ *   - the Kalman filter itself is ref. [3] (Fruehwirth 1987).
+ * Everything the paper leaves open is a "reading", listed in DESIGN.md sec. 3 (R1..R18) and cited below as [Rn].
+ * The KF is an iteration, so the oracle follows it step by step, dense 6x6 doubles, plain loops, no packed
+ * storage, no sparsity shortcuts, no blocking/fusion.  The helix-cylinder intersection is found by marching
+ * along the helix until the radius first exceeds R and polishing the bracketed root with safeguarded Newton
+ * (the CUDA path uses a closed form instead).
+ *
+ * Pins (tests/test_oracle_pins.py, all -m "not gpu"): P1 chord closed form from the origin; P2 Jacobian vs central
+ * finite differences of the root-found map; P3 noise-free truth recovery against the simulator's independent
+ * circle-circle transport; P5 B=0 straight-line weighted least squares closed form; P6 Gluckstern curvature
+ * resolution; P7 linear KF vs normal equations; P8 3x3 solve vs LAPACK; P9 rotation / mirror / charge-field
+ * invariances; P10 PSD, C_upd <= C_pred, chi2 >= 0; P11 pulls and chi2/ndf statistics; P12 build vs brute force
+ * without bins; X1-X3 binning / window vs fp64 atan2 and brute force.
+ * PARITY UNPINNED (paper silent, pinned only by self-consistency P11): the Highland form and where Q is added
+ * [R4], seed smearing widths [R6], candidate ranking order [R10], window definition [R11], noise and fake-seed
+ * recipes [R17, R18], guards cos_inc 0.2 / 0.1 [R9].
+ *
+ * State p = (x, y, z, iota = 1/pT, phi, theta), charge q = +-1 separate [R1]; units cm, GeV, Tesla, rad.
+ * Curvature w = dphi/ds_T = -q * k * Bz * iota, k = 0.00299792458 [R3].
+ *
+ * Build: gcc -O2 -std=c11 -fopenmp -ffp-contract=off -fPIC -shared kf_oracle.c -o libkf_oracle.so -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define KFO_KCURV 0.00299792458
+#define KFO_PI 3.14159265358979323846
+
+enum { KFO_UNREACHABLE = 1, KFO_LEFT_Z = 2, KFO_GRAZING = 4, KFO_NUMERIC = 8 };
+
+#define KFO_CMIN 0.1 /* KF-side grazing guard on cos(incidence) [R9] */
+
+/* layer table row: r, zmax, xx0, sig_rphi, sig_z, sig_r */
+#define LR(t, l) ((t)[6 * (l) + 0])
+#define LZMAX(t, l) ((t)[6 * (l) + 1])
+#define LXX0(t, l) ((t)[6 * (l) + 2])
+#define LSRPHI(t, l) ((t)[6 * (l) + 3])
+#define LSZ(t, l) ((t)[6 * (l) + 4])
+#define LSR(t, l) ((t)[6 * (l) + 5])
+
+int kfo_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* phi is wrapped to (-pi, pi] on output only */
+static double wrap_phi(double a) {
+    double w = a - 2.0 * KFO_PI * floor((a + KFO_PI) / (2.0 * KFO_PI));
+    if (w <= -KFO_PI) w += 2.0 * KFO_PI;
+    if (w > KFO_PI) w -= 2.0 * KFO_PI;
+    return w;
+}
+
+/* sin(a)/a */
+static double sinc_(double a) {
+    if (fabs(a) < 1e-2) {
+        double a2 = a * a;
+        return 1.0 - a2 / 6.0 * (1.0 - a2 / 20.0 * (1.0 - a2 / 42.0 * (1.0 - a2 / 72.0)));
+    }
+    return sin(a) / a;
+}
+
+/* Helix at fixed transverse path length s (sec. 8c-2 of SURVEY.md; standard helix in a uniform field along z):
+ *   alpha = w s, X = sin(alpha)/w, Y = (1-cos(alpha))/w   (X -> s, Y -> w s^2/2 as w -> 0)
+ *   x' = x + cos(phi) X - sin(phi) Y,  y' = y + sin(phi) X + cos(phi) Y,  z' = z + s cot(theta),  phi' = phi + alpha */
+static void helix_at(const double p[6], double w, double s, double out[6]) {
+    double a = w * s;
+    double X = s * sinc_(a);
+    double h = sinc_(0.5 * a);
+    double Y = 0.5 * a * s * h * h; /* = 2 sin^2(a/2)/w, regular at w = 0 */
+    double cp = cos(p[4]), sp = sin(p[4]);
+    out[0] = p[0] + cp * X - sp * Y;
+    out[1] = p[1] + sp * X + cp * Y;
+    out[2] = p[2] + s * cos(p[5]) / sin(p[5]);
+    out[3] = p[3];
+    out[4] = p[4] + a;
+    out[5] = p[5];
+}
+
+static double g_of(const double p[6], double w, double s, double R, double* dg) {
+    double o[6];
+    helix_at(p, w, s, o);
+    if (dg) *dg = 2.0 * (o[0] * cos(o[4]) + o[1] * sin(o[4]));
+    return o[0] * o[0] + o[1] * o[1] - R * R;
+}
+
+/* Propagate the state to the cylinder of radius R: smallest positive root of g(s) = x'^2 + y'^2 - R^2 [R2].
+ * J (row-major 6x6) = d p'/d p INCLUDING the path-length term (the state is transported to the surface).
+ * Returns 0 or a flag: KFO_UNREACHABLE (start not inside R, or no crossing within one turn), KFO_GRAZING
+ * (cos(incidence) < KFO_CMIN; outputs are still filled).  s_out = transverse path, cosinc_out = u'/R. */
+int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
+                  double* cosinc_out) {
+    const double w = -(double)q * KFO_KCURV * bz * p[3];
+    const double c_w = -(double)q * KFO_KCURV * bz; /* w = c_w * iota */
+    double r02 = p[0] * p[0] + p[1] * p[1];
+    memcpy(pout, p, 6 * sizeof(double));
+    for (int i = 0; i < 36; ++i) J[i] = (i % 7 == 0) ? 1.0 : 0.0;
+    if (s_out) *s_out = 0.0;
+    if (cosinc_out) *cosinc_out = 0.0;
+    if (!(r02 < R * R) || !isfinite(w) || !isfinite(r02)) return KFO_UNREACHABLE;
+
+    /* march: a circle of radius rho >= R that starts inside the cylinder leaves it within an arc pi R;
+       a tighter circle either crosses within one turn 2 pi rho or never */
+    const int NMARCH = 64;
+    double smax = (fabs(w) * R <= 1.0) ? KFO_PI * R * (1.0 + 1e-9) : 2.0 * KFO_PI / fabs(w);
+    double lo = 0.0, hi = -1.0;
+    for (int k = 1; k <= NMARCH; ++k) {
+        double sk = smax * (double)k / NMARCH;
+        if (g_of(p, w, sk, R, NULL) >= 0.0) { hi = sk; break; }
+        lo = sk;
+    }
+    if (hi < 0.0) return KFO_UNREACHABLE;
+    /* safeguarded Newton inside [lo, hi], g(lo) < 0 <= g(hi) */
+    double s = 0.5 * (lo + hi);
+    for (int it = 0; it < 200; ++it) {
+        double dg, g = g_of(p, w, s, R, &dg);
+        if (g < 0.0) lo = s; else hi = s;
+        double sn = (dg > 0.0) ? s - g / dg : -1.0;
+        if (!(sn > lo && sn < hi)) sn = 0.5 * (lo + hi);
+        double ds = fabs(sn - s);
+        s = sn;
+        if (ds <= 1e-15 * fmax(1.0, fabs(s)) || hi - lo <= 1e-15 * fmax(1.0, fabs(s))) break;
+    }
+    helix_at(p, w, s, pout);
+    const double xn = pout[0], yn = pout[1], phn = pout[4];
+    const double cpn = cos(phn), spn = sin(phn), cp = cos(p[4]), sp = sin(p[4]);
+    const double up = xn * cpn + yn * spn; /* R cos(incidence) */
+    if (s_out) *s_out = s;
+    if (cosinc_out) *cosinc_out = up / R;
+
+    /* fixed-s partial derivatives (sec. 8c-3) */
+    const double a = w * s;
+    double f1, f2; /* f1 = (cos a - sinc a)/a, f2 = (sin a - (1-cos a)/a)/a */
+    if (fabs(a) < 1e-2) {
+        double a2 = a * a;
+        f1 = a * (-1.0 / 3.0 + a2 * (1.0 / 30.0 + a2 * (-1.0 / 840.0 + a2 / 45360.0)));
+        f2 = 0.5 + a2 * (-1.0 / 8.0 + a2 * (1.0 / 144.0 - a2 / 5760.0));
+    } else {
+        f1 = (cos(a) - sin(a) / a) / a;
+        f2 = (sin(a) - (1.0 - cos(a)) / a) / a;
+    }
+    const double dXdi = c_w * s * s * f1; /* dX/d iota at fixed s = (s cos a - X)/iota */
+    const double dYdi = c_w * s * s * f2; /* dY/d iota at fixed s = (s sin a - Y)/iota */
+    const double Fxi = cp * dXdi - sp * dYdi, Fyi = sp * dXdi + cp * dYdi;
+    const double Fxp = -(yn - p[1]), Fyp = xn - p[0];
+    const double cot = cos(p[5]) / sin(p[5]), sin2 = sin(p[5]) * sin(p[5]);
+    /* ds/dp from g(p, s(p)) = 0 */
+    const double sx = -xn / up, sy = -yn / up;
+    const double si = -(xn * Fxi + yn * Fyi) / up, sph = -(xn * Fxp + yn * Fyp) / up;
+    memset(J, 0, 36 * sizeof(double));
+    /* columns: x y z iota phi theta */
+    J[0 * 6 + 0] = 1.0 + cpn * sx; J[0 * 6 + 1] = cpn * sy; J[0 * 6 + 3] = Fxi + cpn * si; J[0 * 6 + 4] = Fxp + cpn * sph;
+    J[1 * 6 + 0] = spn * sx; J[1 * 6 + 1] = 1.0 + spn * sy; J[1 * 6 + 3] = Fyi + spn * si; J[1 * 6 + 4] = Fyp + spn * sph;
+    J[2 * 6 + 0] = cot * sx; J[2 * 6 + 1] = cot * sy; J[2 * 6 + 2] = 1.0; J[2 * 6 + 3] = cot * si; J[2 * 6 + 4] = cot * sph;
+    J[2 * 6 + 5] = -s / sin2;
+    J[3 * 6 + 3] = 1.0;
+    J[4 * 6 + 0] = w * sx; J[4 * 6 + 1] = w * sy; J[4 * 6 + 3] = c_w * s + w * si; J[4 * 6 + 4] = 1.0 + w * sph;
+    J[5 * 6 + 5] = 1.0;
+    if (!(up / R >= KFO_CMIN)) return KFO_GRAZING;
+    return 0;
+}
+
+/* remove the rounding-level asymmetry of the dense loops: C <- (C + C^T)/2 */
+static void symmetrize6(double C[36]) {
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < i; ++j) {
+            double m = 0.5 * (C[i * 6 + j] + C[j * 6 + i]);
+            C[i * 6 + j] = C[j * 6 + i] = m;
+        }
+}
+
+/* C <- J C J^T, dense */
+static void similarity6(const double J[36], const double C[36], double out[36]) {
+    double T[36];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double a = 0.0;
+            for (int k = 0; k < 6; ++k) a += J[i * 6 + k] * C[k * 6 + j];
+            T[i * 6 + j] = a;
+        }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double a = 0.0;
+            for (int k = 0; k < 6; ++k) a += T[i * 6 + k] * J[j * 6 + k];
+            out[i * 6 + j] = a;
+        }
+    symmetrize6(out);
+}
+void kfo_similarity6(const double J[36], const double C[36], double out[36]) { similarity6(J, C, out); }
+
+/* Multiple-scattering noise of a thin layer of thickness xx0 (radiation lengths at normal incidence),
+ * evaluated at the arriving state [R4]: path t = xx0/(sin(theta) cos_inc); Highland, beta = 1, unit charge,
+ * p = 1/(iota sin theta): theta0 = 0.0136 iota sin(theta) sqrt(t) (1 + 0.038 ln t).  Two orthogonal deflections
+ * of variance theta0^2 with |p| conserved give, in (iota, phi, theta):
+ *   Q_thth = th0^2, Q_phph = th0^2/sin^2(theta), Q_ii = iota^2 cot^2(theta) th0^2, Q_ith = -iota cot(theta) th0^2. */
+void kfo_ms_noise(const double p[6], double cosinc, double xx0, double Q[36]) {
+    memset(Q, 0, 36 * sizeof(double));
+    if (!(xx0 > 0.0)) return;
+    double st = sin(p[5]), ct = cos(p[5]);
+    double t = xx0 / (st * cosinc);
+    double th0 = 0.0136 * p[3] * st * sqrt(t) * (1.0 + 0.038 * log(t));
+    double v = th0 * th0, cot = ct / st;
+    Q[5 * 6 + 5] = v;
+    Q[4 * 6 + 4] = v / (st * st);
+    Q[3 * 6 + 3] = p[3] * p[3] * cot * cot * v;
+    Q[3 * 6 + 5] = Q[5 * 6 + 3] = -p[3] * cot * v;
+}
+
+/* 3x3 SPD solve by Cholesky: returns 0 and inv (row-major) or -1 when not positive definite */
+int kfo_inv3_spd(const double S[9], double inv[9]) {
+    double l00, l10, l11, l20, l21, l22;
+    if (!(S[0] > 0.0)) return -1;
+    l00 = sqrt(S[0]); l10 = S[3] / l00; l20 = S[6] / l00;
+    double d1 = S[4] - l10 * l10;
+    if (!(d1 > 0.0)) return -1;
+    l11 = sqrt(d1); l21 = (S[7] - l20 * l10) / l11;
+    double d2 = S[8] - l20 * l20 - l21 * l21;
+    if (!(d2 > 0.0)) return -1;
+    l22 = sqrt(d2);
+    /* invert L (lower) then inv = L^-T L^-1 */
+    double m00 = 1.0 / l00, m11 = 1.0 / l11, m22 = 1.0 / l22;
+    double m10 = -l10 * m00 * m11;
+    double m21 = -l21 * m11 * m22;
+    double m20 = -(l20 * m00 + l21 * m10) * m22;
+    inv[0] = m00 * m00 + m10 * m10 + m20 * m20;
+    inv[1] = inv[3] = m10 * m11 + m20 * m21;
+    inv[2] = inv[6] = m20 * m22;
+    inv[4] = m11 * m11 + m21 * m21;
+    inv[5] = inv[7] = m21 * m22;
+    inv[8] = m22 * m22;
+    return 0;
+}
+
+/* Hit covariance in global Cartesian coordinates from the layer resolutions and the hit's own azimuth [R5]:
+ * c = mx/rm, s = my/rm: Vxx = c^2 sr^2 + s^2 srphi^2, Vyy = s^2 sr^2 + c^2 srphi^2, Vxy = c s (sr^2 - srphi^2), Vzz = sz^2 */
+static void hit_cov(const double m[3], double srphi, double sz, double sr, double V[9]) {
+    double rm = sqrt(m[0] * m[0] + m[1] * m[1]);
+    double c = m[0] / rm, s = m[1] / rm;
+    memset(V, 0, 9 * sizeof(double));
+    V[0] = c * c * sr * sr + s * s * srphi * srphi;
+    V[4] = s * s * sr * sr + c * c * srphi * srphi;
+    V[1] = V[3] = c * s * (sr * sr - srphi * srphi);
+    V[8] = sz * sz;
+}
+
+/* chi2 of hit m against the predicted state (p, C) without updating.  Returns -1 if S is not PD. */
+int kfo_chi2(const double p[6], const double C[36], const double m[3], double srphi, double sz, double sr,
+             double* chi2) {
+    double V[9], S[9], Si[9], r[3];
+    hit_cov(m, srphi, sz, sr, V);
+    for (int i = 0; i < 3; ++i) {
+        r[i] = m[i] - p[i];
+        for (int j = 0; j < 3; ++j) S[i * 3 + j] = C[i * 6 + j] + V[i * 3 + j];
+    }
+    if (kfo_inv3_spd(S, Si)) return -1;
+    double c2 = 0.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c2 += r[i] * Si[i * 3 + j] * r[j];
+    *chi2 = c2;
+    return 0;
+}
+
+/* Kalman update with the 3-D hit m, H = [I3 0] (Fruehwirth 1987, gain-matrix form):
+ *   r = m - p[0:3]; S = C[0:3,0:3] + V; chi2 = r^T S^-1 r; K = C[:,0:3] S^-1; p <- p + K r;
+ *   C <- (I-KH) C (I-KH)^T + K V K^T   (Joseph form: equal to C - K H C in exact arithmetic, symmetric by construction)
+ * Returns 0, or KFO_NUMERIC when S is not PD, the result is not finite or iota <= 0 (outputs then undefined). */
+int kfo_update(const double p[6], const double C[36], const double m[3], double srphi, double sz, double sr,
+               double pout[6], double Cout[36], double* chi2) {
+    double V[9], S[9], Si[9], r[3], K[18], A[36], T[36];
+    hit_cov(m, srphi, sz, sr, V);
+    for (int i = 0; i < 3; ++i) {
+        r[i] = m[i] - p[i];
+        for (int j = 0; j < 3; ++j) S[i * 3 + j] = C[i * 6 + j] + V[i * 3 + j];
+    }
+    if (kfo_inv3_spd(S, Si)) return KFO_NUMERIC;
+    double c2 = 0.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c2 += r[i] * Si[i * 3 + j] * r[j];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double a = 0.0;
+            for (int k = 0; k < 3; ++k) a += C[i * 6 + k] * Si[k * 3 + j];
+            K[i * 3 + j] = a;
+        }
+    for (int i = 0; i < 6; ++i) {
+        double a = p[i];
+        for (int k = 0; k < 3; ++k) a += K[i * 3 + k] * r[k];
+        pout[i] = a;
+    }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) A[i * 6 + j] = (i == j ? 1.0 : 0.0) - (j < 3 ? K[i * 3 + j] : 0.0);
+    similarity6(A, C, T);
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double a = 0.0;
+            for (int k = 0; k < 3; ++k)
+                for (int l = 0; l < 3; ++l) a += K[i * 3 + k] * V[k * 3 + l] * K[j * 3 + l];
+            Cout[i * 6 + j] = T[i * 6 + j] + a;
+        }
+    symmetrize6(Cout);
+    *chi2 = c2;
+    for (int i = 0; i < 6; ++i)
+        if (!isfinite(pout[i])) return KFO_NUMERIC;
+    for (int i = 0; i < 36; ++i)
+        if (!isfinite(Cout[i])) return KFO_NUMERIC;
+    if (!(pout[3] > 0.0) || !isfinite(c2)) return KFO_NUMERIC;
+    return 0;
+}
+
+/* One KF step: propagate to layer l, add Q, (optionally) update with hit m.  Used by fit and build.
+ * Returns flags; on flags != 0 the outputs are not to be used. */
+static int predict(const double* layers, int l, double bz, const double p[6], const double C[36], int q,
+                   double pp[6], double Cp[36]) {
+    double J[36], Q[36], s, ci;
+    int f = kfo_propagate(p, q, bz, LR(layers, l), pp, J, &s, &ci);
+    if (f) return f;
+    similarity6(J, C, Cp);
+    kfo_ms_noise(pp, ci, LXX0(layers, l), Q);
+    for (int i = 0; i < 36; ++i) Cp[i] += Q[i];
+    return 0;
+}
+int kfo_predict(const double* layers, int l, double bz, const double p[6], const double C[36], int q, double pp[6],
+                double Cp[36]) {
+    return predict(layers, l, bz, p, C, q, pp, Cp);
+}
+
+/* kf_fit_ref [R8]: forward (inside-out) filter over the layers in order of increasing radius.
+ * hit_idx[l*ld + t] < 0 -> layer skipped entirely; NULL -> identity.  Hit of track t on layer l is
+ * (hx,hy,hz)[seg_off[ev*L + l] + idx], ev = trk_event ? trk_event[t] : 0.
+ * A propagation failure or a failed update sets the status bit, stops the track and keeps the last good state.
+ * par [6][ld], cov [36][ld] dense in, outputs alike; chi2/nhits/status [n].  chi2_in/nhits_in may be NULL (=0). */
+int kfo_fit(int n_layers, const double* layers, double bz, int64_t n, int64_t ld, const double* par,
+            const double* cov, const int8_t* q, const double* hx, const double* hy, const double* hz,
+            const int64_t* seg_off, const int32_t* hit_idx, const int32_t* trk_event, double* par_out,
+            double* cov_out, double* chi2_out, int32_t* nhits_out, uint32_t* status_out) {
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t t = 0; t < n; ++t) {
+        double p[6], C[36], pp[6], Cp[36], pu[6], Cu[36];
+        for (int i = 0; i < 6; ++i) p[i] = par[i * ld + t];
+        for (int i = 0; i < 36; ++i) C[i] = cov[i * ld + t];
+        double chi2 = 0.0;
+        int nh = 0;
+        uint32_t st = 0;
+        int ev = trk_event ? trk_event[t] : 0;
+        for (int l = 0; l < n_layers; ++l) {
+            int64_t idx = hit_idx ? hit_idx[(int64_t)l * ld + t] : t;
+            if (idx < 0) continue;
+            int f = predict(layers, l, bz, p, C, q[t], pp, Cp);
+            if (f) { st |= (uint32_t)f; break; }
+            int64_t h = seg_off[(int64_t)ev * n_layers + l] + idx;
+            double m[3] = {hx[h], hy[h], hz[h]}, c2;
+            f = kfo_update(pp, Cp, m, LSRPHI(layers, l), LSZ(layers, l), LSR(layers, l), pu, Cu, &c2);
+            if (f) { st |= (uint32_t)f; break; }
+            memcpy(p, pu, sizeof p);
+            memcpy(C, Cu, sizeof C);
+            chi2 += c2;
+            nh += 1;
+        }
+        p[4] = wrap_phi(p[4]);
+        for (int i = 0; i < 6; ++i) par_out[i * ld + t] = p[i];
+        for (int i = 0; i < 36; ++i) cov_out[i * ld + t] = C[i];
+        chi2_out[t] = chi2;
+        nhits_out[t] = nh;
+        status_out[t] = st;
+    }
+    return 0;
+}

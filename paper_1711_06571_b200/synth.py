@@ -1,0 +1,492 @@
+"""Seeded synthetic inputs for the KF tracking hot path (toy Monte Carlo).
+
+Stands in for the paper's standalone toy simulation -- "simplified ideal barrel
+geometry with a uniform longitudinal magnetic field, gaussian-smeared hit
+positions, a particle gun ... flat transverse momentum distribution between 0.5
+and 10 GeV" (sec. 3) -- and for its CMS-simulation events
+(sec. 4.2), which are not available here.  Shapes and
+distributions follow BASELINE.json configs[0..4]; the recipe is restated in
+DESIGN.md "Input recipe".
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds
+none of the Kalman filter: no Jacobian, no covariance transport, no gain, no
+chi2, no binning.  It is a particle *simulator*: truth helices are intersected
+with the barrel cylinders by circle-circle geometry (centre of curvature +
+law of cosines), which is a different derivation from both the oracle's
+march-and-Newton root finder and the kernel's tan-half-angle closed form, so
+the noise-free pin (tests/test_oracle_pins.py::P3) is a real cross-check.
+
+Everything is numpy fp64; hits and seeds are rounded to fp32 ONCE at the end
+and that fp32 data is the common input of oracle and GPU.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+import numpy as np
+
+K_CURV = 0.00299792458  # GeV / (T cm): rho[cm] = pT / (K_CURV * |Bz|)
+MASTER_SEED = 171106571
+
+
+def rng_for(config: int, event: int = 0, stream: int = 0) -> np.random.Generator:
+    return np.random.Generator(np.random.PCG64(np.random.SeedSequence([MASTER_SEED, config, event, stream])))
+
+
+@dataclass
+class Geometry:
+    """Ideal concentric barrel.  One row per layer, increasing radius."""
+    r: np.ndarray
+    zmax: np.ndarray
+    xx0: np.ndarray
+    sig_rphi: np.ndarray
+    sig_z: np.ndarray
+    sig_r: np.ndarray
+    bz: float
+
+    @property
+    def n_layers(self) -> int:
+        return len(self.r)
+
+    def layer_table(self) -> np.ndarray:
+        """[L][6] float64: r, zmax, xx0, sig_rphi, sig_z, sig_r."""
+        return np.stack([self.r, self.zmax, self.xx0, self.sig_rphi, self.sig_z, self.sig_r], axis=1).astype(np.float64)
+
+
+def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0) -> Geometry:
+    """kind 'barrel10' (configs 0,1,3): r = 4,8..40 cm, x/X0 = 0.02.
+    kind 'barrel17' (configs 2,4): 17 layers r = 4..80 uniformly, x/X0 alternating 0.01/0.03."""
+    if kind == "barrel10":
+        r = 4.0 * np.arange(1, 11, dtype=np.float64)
+        xx0 = np.full(10, 0.02)
+    elif kind == "barrel17":
+        r = 4.0 + 4.75 * np.arange(17, dtype=np.float64)
+        xx0 = np.where(np.arange(17) % 2 == 0, 0.01, 0.03)
+    else:
+        raise ValueError(kind)
+    n = len(r)
+    return Geometry(r=r, zmax=np.full(n, 100.0), xx0=xx0 * xx0_scale, sig_rphi=np.full(n, 0.01),
+                    sig_z=np.full(n, 0.1), sig_r=np.full(n, 0.01), bz=bz)
+
+
+def pack_index(i: int, j: int) -> int:
+    """Packed lower-triangular row-major index, k(i,j) = i(i+1)/2 + j for i >= j."""
+    if i < j:
+        i, j = j, i
+    return i * (i + 1) // 2 + j
+
+
+def pack_sym(c: np.ndarray) -> np.ndarray:
+    """[..., 6, 6] -> [..., 21]"""
+    idx = [(i, j) for i in range(6) for j in range(i + 1)]
+    return np.stack([c[..., i, j] for i, j in idx], axis=-1)
+
+
+def unpack_sym(p: np.ndarray) -> np.ndarray:
+    """[..., 21] -> [..., 6, 6]"""
+    out = np.empty(p.shape[:-1] + (6, 6), dtype=p.dtype)
+    for i in range(6):
+        for j in range(i + 1):
+            out[..., i, j] = p[..., pack_index(i, j)]
+            out[..., j, i] = p[..., pack_index(i, j)]
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# particle gun
+# ----------------------------------------------------------------------------------------------
+def particle_gun(rng: np.random.Generator, n: int, kind: str) -> dict:
+    """Truth at the vertex (origin).  kind 'flat' (configs 0,1,3): pT ~ U(0.5,10) GeV, |eta|<1.
+    kind 'wide' (configs 2,4): ln pT ~ U(ln 0.3, ln 100), |eta|<1.5."""
+    phi = rng.uniform(-np.pi, np.pi, n)
+    q = np.where(rng.random(n) < 0.5, -1, 1).astype(np.int8)
+    if kind == "flat":
+        pt = rng.uniform(0.5, 10.0, n)
+        eta = rng.uniform(-1.0, 1.0, n)
+    elif kind == "wide":
+        pt = np.exp(rng.uniform(np.log(0.3), np.log(100.0), n))
+        eta = rng.uniform(-1.5, 1.5, n)
+    else:
+        raise ValueError(kind)
+    theta = 2.0 * np.arctan(np.exp(-eta))
+    z = np.zeros(n)
+    return dict(x=z.copy(), y=z.copy(), z=z.copy(), ipt=1.0 / pt, phi=phi, theta=theta, q=q)
+
+
+# ----------------------------------------------------------------------------------------------
+# truth transport: circle-circle intersection (simulator only)
+# ----------------------------------------------------------------------------------------------
+def cross_cylinder(x, y, z, ipt, phi, theta, q, bz, R):
+    """First outward crossing of the cylinder of radius R by the truth helix.
+
+    Returns (ok, x', y', z', phi', s_T, cos_inc).  Geometry: the transverse projection is a circle of
+    signed curvature w = -q K Bz / pT about the centre c = (x - sin(phi)/w, y + cos(phi)/w); the cylinder
+    is the circle |p| = R about the origin.  The two intersections sit at polar angle gamma +- beta, with
+    gamma the azimuth of c and cos(beta) = (d^2 + R^2 - rho^2) / (2 d R) (law of cosines, d = |c|).
+    The one reached first is the one with the smaller turning angle about c in the sense of rotation.
+    A straight line (w = 0) uses the chord formula instead.
+    """
+    x, y, z, ipt, phi, theta = (np.asarray(a, dtype=np.float64) for a in (x, y, z, ipt, phi, theta))
+    w = -np.asarray(q, dtype=np.float64) * K_CURV * bz * ipt
+    cp, sp = np.cos(phi), np.sin(phi)
+    r02 = x * x + y * y
+    inside = r02 < R * R
+    straight = np.abs(w) * R < 1e-12
+    ws = np.where(straight, 1.0, w)
+    # --- curved branch
+    cx, cy = x - sp / ws, y + cp / ws
+    rho = 1.0 / np.abs(ws)
+    d = np.hypot(cx, cy)
+    cosb = (d * d + R * R - rho * rho) / (2.0 * np.where(d > 0, d, 1.0) * R)
+    reach = (np.abs(cosb) <= 1.0) & (d > 0)
+    beta = np.arccos(np.clip(cosb, -1.0, 1.0))
+    gamma = np.arctan2(cy, cx)
+    psi0 = np.arctan2(y - cy, x - cx)
+    sgn = np.sign(ws)
+    best = np.full(x.shape, np.inf)
+    bx = np.zeros_like(x)
+    by = np.zeros_like(x)
+    for pm in (+1.0, -1.0):
+        px, py = R * np.cos(gamma + pm * beta), R * np.sin(gamma + pm * beta)
+        psi = np.arctan2(py - cy, px - cx)
+        turn = np.mod((psi - psi0) * sgn, 2.0 * np.pi)
+        take = turn < best
+        best = np.where(take, turn, best)
+        bx = np.where(take, px, bx)
+        by = np.where(take, py, by)
+    s_c = best * rho
+    phi_c = phi + sgn * best
+    # --- straight branch: |p + s d|^2 = R^2
+    u = x * cp + y * sp
+    s_l = -u + np.sqrt(np.maximum(u * u + R * R - r02, 0.0))
+    lx, ly = x + s_l * cp, y + s_l * sp
+    xs = np.where(straight, lx, bx)
+    ys = np.where(straight, ly, by)
+    s = np.where(straight, s_l, s_c)
+    phn = np.where(straight, phi, phi_c)
+    ok = inside & (straight | reach)
+    zn = z + s / np.tan(theta)
+    cosinc = (xs * np.cos(phn) + ys * np.sin(phn)) / R
+    return ok, xs, ys, zn, phn, s, cosinc
+
+
+def highland_theta0(ipt, theta, cosinc, xx0):
+    """Highland/PDG width of the projected scattering angle, beta = 1, unit charge, p = 1/(ipt sin theta),
+    path through the layer = xx0 / (sin(theta) * cos_inc)."""
+    t = xx0 / (np.sin(theta) * cosinc)
+    return 0.0136 * ipt * np.sin(theta) * np.sqrt(t) * (1.0 + 0.038 * np.log(t))
+
+
+GEN_MIN_COSINC = 0.2  # a truth crossing shallower than this ends the track (reading A9)
+
+
+def simulate(geom: Geometry, gun: dict, rng: np.random.Generator, ms: bool = True, smear: bool = True) -> dict:
+    """Transport every truth particle outward layer by layer; record the crossing, smear the hit on the
+    cylinder surface (phi by N(0, sig_rphi/R), z by N(0, sig_z)), then apply the thin-scatterer kick.
+
+    A track ends (that layer and all outer ones get no hit) when the layer is unreachable, the crossing has
+    |z| > zmax, or cos(incidence) < GEN_MIN_COSINC.
+    Returns hits [L][n][3] (NaN where absent), valid [L][n], truth [L][n][6] = state just outside the layer.
+    """
+    n = len(gun["phi"])
+    L = geom.n_layers
+    x, y, z = gun["x"].copy(), gun["y"].copy(), gun["z"].copy()
+    ipt, phi, theta, q = gun["ipt"].copy(), gun["phi"].copy(), gun["theta"].copy(), gun["q"]
+    alive = np.ones(n, dtype=bool)
+    hits = np.full((L, n, 3), np.nan)
+    valid = np.zeros((L, n), dtype=bool)
+    truth = np.full((L, n, 6), np.nan)
+    for l in range(L):
+        R = geom.r[l]
+        with np.errstate(invalid="ignore", divide="ignore"):
+            ok, xn, yn, zn, phn, s, ci = cross_cylinder(x, y, z, ipt, phi, theta, q, geom.bz, R)
+        ok = ok & alive & (np.abs(zn) <= geom.zmax[l]) & (ci >= GEN_MIN_COSINC)
+        alive = ok
+        x = np.where(ok, xn, x); y = np.where(ok, yn, y); z = np.where(ok, zn, z); phi = np.where(ok, phn, phi)
+        # hit, smeared on the surface
+        e_phi = rng.standard_normal(n) * (geom.sig_rphi[l] / R if smear else 0.0)
+        e_z = rng.standard_normal(n) * (geom.sig_z[l] if smear else 0.0)
+        az = np.arctan2(y, x) + e_phi
+        hits[l, :, 0] = np.where(ok, R * np.cos(az), np.nan)
+        hits[l, :, 1] = np.where(ok, R * np.sin(az), np.nan)
+        hits[l, :, 2] = np.where(ok, z + e_z, np.nan)
+        valid[l] = ok
+        # multiple scattering: two orthogonal kicks of width theta0, |p| conserved
+        k1 = rng.standard_normal(n)
+        k2 = rng.standard_normal(n)
+        if ms:
+            with np.errstate(invalid="ignore", divide="ignore"):
+                th0 = np.where(ok, highland_theta0(ipt, theta, np.where(ok, ci, 1.0), geom.xx0[l]), 0.0)
+            th_new = theta + k1 * th0
+            phi = phi + k2 * th0 / np.sin(theta)
+            ipt = ipt * np.sin(theta) / np.sin(th_new)
+            theta = th_new
+        truth[l] = np.where(ok[:, None], np.stack([x, y, z, ipt, phi, theta], axis=1), np.nan)
+    return dict(hits=hits, valid=valid, truth=truth)
+
+
+# ----------------------------------------------------------------------------------------------
+# seeds
+# ----------------------------------------------------------------------------------------------
+SEED_SIGMA_POS = 0.05      # cm
+SEED_SIGMA_REL_IPT = 0.05  # "truth smeared 5 %" (BASELINE.json config 0) applies to 1/pT
+SEED_SIGMA_ANG = 0.005     # rad
+
+
+def smear_seed(rng: np.random.Generator, state: np.ndarray) -> tuple[np.ndarray, np.ndarray]:
+    """state [n][6] truth -> (seed [n][6], sigma [n][6]).  Diagonal Gaussian smearing; covariance = diag(sigma^2)."""
+    n = state.shape[0]
+    sig = np.empty((n, 6))
+    sig[:, 0:3] = SEED_SIGMA_POS
+    sig[:, 3] = SEED_SIGMA_REL_IPT * np.abs(state[:, 3])
+    sig[:, 4:6] = SEED_SIGMA_ANG
+    seed = state + rng.standard_normal((n, 6)) * sig
+    return seed, sig
+
+
+def _ld(n: int) -> int:
+    return max(32, (n + 31) // 32 * 32)
+
+
+def _soa_tracks(seed: np.ndarray, sig: np.ndarray, q: np.ndarray) -> dict:
+    """AoS fp64 -> the SoA fp32 store of include/kf.h (par[6][ld], cov[21][ld], q[n])."""
+    n = seed.shape[0]
+    ld = _ld(n)
+    par = np.zeros((6, ld), dtype=np.float32)
+    par[:, :n] = seed.T.astype(np.float32)
+    cov = np.zeros((21, ld), dtype=np.float32)
+    for i in range(6):
+        cov[pack_index(i, i), :n] = (sig[:, i] ** 2).astype(np.float32)
+    # padding lanes: harmless unit state so that kernels may touch them
+    par[3, n:] = 1.0; par[5, n:] = 1.5
+    return dict(n=n, ld=ld, par=par, cov=cov, q=np.ascontiguousarray(q.astype(np.int8)))
+
+
+@dataclass
+class FitInputs:
+    geom: Geometry
+    n: int
+    ld: int
+    par: np.ndarray        # [6][ld] f32 seeds
+    cov: np.ndarray        # [21][ld] f32
+    q: np.ndarray          # [n] i8
+    hit_x: np.ndarray      # [L*ld] f32, segment l at [l*ld, l*ld+n)
+    hit_y: np.ndarray
+    hit_z: np.ndarray
+    seg_off: np.ndarray    # [L+1] i64
+    hit_idx: np.ndarray | None  # [L][ld] i32 (identity or -1), None = identity everywhere
+    truth: np.ndarray      # [L][n][6] f64 (NaN where no hit)
+    valid: np.ndarray      # [L][n] bool
+    gun: dict = field(default_factory=dict)
+
+
+FIT_CONFIGS = {
+    0: dict(n=10_000, geom="barrel10", gun="flat"),
+    1: dict(n=1_000_000, geom="barrel10", gun="flat"),
+    2: dict(n=1_000_000, geom="barrel17", gun="wide"),
+}
+
+
+def fit_inputs(config: int, n: int | None = None, ms: bool = True, smear: bool = True, event: int = 0,
+               force_index: bool = False, bz: float = 3.8) -> FitInputs:
+    """Inputs of kf_fit for BASELINE.json configs 0-2 (n overrides the track count, e.g. for tests)."""
+    cfg = FIT_CONFIGS[config]
+    n = cfg["n"] if n is None else n
+    geom = geometry(cfg["geom"], bz=bz, xx0_scale=1.0 if ms else 0.0)
+    rng = rng_for(config, event)
+    gun = particle_gun(rng, n, cfg["gun"])
+    sim = simulate(geom, gun, rng, ms=ms, smear=smear)
+    vtx = np.stack([gun["x"], gun["y"], gun["z"], gun["ipt"], gun["phi"], gun["theta"]], axis=1)
+    seed, sig = smear_seed(rng, vtx)
+    t = _soa_tracks(seed, sig, gun["q"])
+    L, ld = geom.n_layers, t["ld"]
+    hx = np.zeros((L, ld), dtype=np.float32); hy = np.zeros((L, ld), dtype=np.float32); hz = np.zeros((L, ld), dtype=np.float32)
+    h = np.nan_to_num(sim["hits"], nan=0.0)
+    hx[:, :n] = h[:, :, 0]; hy[:, :n] = h[:, :, 1]; hz[:, :n] = h[:, :, 2]
+    all_valid = bool(sim["valid"].all())
+    hit_idx = None
+    if force_index or not all_valid:
+        hit_idx = np.full((L, ld), -1, dtype=np.int32)
+        ident = np.arange(n, dtype=np.int32)
+        for l in range(L):
+            hit_idx[l, :n] = np.where(sim["valid"][l], ident, -1)
+    seg_off = (np.arange(L + 1, dtype=np.int64) * ld)
+    return FitInputs(geom=geom, n=n, ld=ld, par=t["par"], cov=t["cov"], q=t["q"], hit_x=hx.reshape(-1), hit_y=hy.reshape(-1),
+                     hit_z=hz.reshape(-1), seg_off=seg_off, hit_idx=hit_idx, truth=sim["truth"], valid=sim["valid"], gun=gun)
+
+
+# ----------------------------------------------------------------------------------------------
+# build events (configs 3, 4)
+# ----------------------------------------------------------------------------------------------
+@dataclass
+class BuildInputs:
+    geom: Geometry
+    n_events: int
+    n_phi: int
+    n_z: int
+    K: int
+    chi2_cut: float
+    n_sigma: float
+    first_layer: int
+    hit_x: np.ndarray      # [n_hits] f32, segments (event*L + layer) back to back
+    hit_y: np.ndarray
+    hit_z: np.ndarray
+    seg_off: np.ndarray    # [n_events*L+1] i64
+    hit_truth: np.ndarray  # [n_hits] i32: global truth-track id of the hit, -1 = noise
+    n_seeds: int
+    ld: int
+    par: np.ndarray        # [6][ld] f32 seed states on layer first_layer-1
+    cov: np.ndarray        # [21][ld]
+    q: np.ndarray          # [n_seeds] i8
+    seed_event: np.ndarray    # [n_seeds] i32
+    seed_hit_idx: np.ndarray  # [first_layer][ld] i32 index within segment
+    seed_truth: np.ndarray    # [n_seeds] i32 global truth-track id, -1 = fake seed
+    truth_hit_idx: np.ndarray  # [L][n_tracks_total] i32 index within segment of each truth track's hit, -1 none
+
+
+BUILD_CONFIGS = {
+    3: dict(n_events=16, tracks=2_000, geom="barrel10", gun="flat", noise=5, n_phi=256, n_z=16, fake_frac=0.0),
+    4: dict(n_events=64, tracks=10_000, geom="barrel17", gun="wide", noise=10, n_phi=1024, n_z=32, fake_frac=0.2),
+}
+
+
+def _three_point_seed(p1, p2, p3, bz):
+    """Fake seed from three hits (simulator-side geometry only): circle through the (x,y) points ->
+    curvature and tangent at p3; cot(theta) from dz over arc length between p1 and p3.
+    Returns state[6] at p3 and charge, or None when degenerate."""
+    (x1, y1, z1), (x2, y2, z2), (x3, y3, z3) = p1, p2, p3
+    a = 2.0 * ((x2 - x1) * (y3 - y1) - (y2 - y1) * (x3 - x1))
+    chord = np.hypot(x3 - x1, y3 - y1)
+    if chord <= 0:
+        return None
+    if abs(a) < 1e-12 * chord * chord:
+        w = 0.0
+        phi = np.arctan2(y3 - y1, x3 - x1)
+        arc = chord
+    else:
+        b2, b3 = (x2 * x2 + y2 * y2 - x1 * x1 - y1 * y1), (x3 * x3 + y3 * y3 - x1 * x1 - y1 * y1)
+        cx = (b2 * (y3 - y1) - b3 * (y2 - y1)) / a
+        cy = (b3 * (x2 - x1) - b2 * (x3 - x1)) / a
+        rho = np.hypot(x3 - cx, y3 - cy)
+        sgn = 1.0 if a > 0 else -1.0   # counter-clockwise (w > 0) when p1->p2->p3 turns left
+        w = sgn / rho
+        phi = np.arctan2(sgn * (x3 - cx), -sgn * (y3 - cy))
+        half = min(1.0, chord / (2.0 * rho))
+        arc = 2.0 * rho * np.arcsin(half)
+    cot = (z3 - z1) / arc
+    theta = np.arctan2(1.0, cot)
+    if w == 0.0 or bz == 0.0:
+        return None
+    ipt = abs(w) / (K_CURV * abs(bz))
+    q = 1 if (-w / (K_CURV * bz)) > 0 else -1
+    return np.array([x3, y3, z3, ipt, phi, theta]), q
+
+
+def build_inputs(config: int, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
+                 K: int = 10, chi2_cut: float = 30.0, n_sigma: float = 3.0, noise: float | None = None,
+                 fake_frac: float | None = None, n_phi: int | None = None, n_z: int | None = None,
+                 smear: bool = True, ms: bool = True) -> BuildInputs:
+    """Inputs of kf_bin_hits / kf_build for BASELINE.json configs 3-4 (sizes can be overridden for tests).
+
+    Per event: truth tracks from the particle gun; hits per layer = truth hits + `noise` x (number of truth
+    hits on that layer) uniform in (phi, z) on the cylinder; each segment is shuffled.  One seed per truth
+    track that reaches layer `first_layer-1`: truth state just outside that layer, smeared (smear_seed),
+    diagonal covariance (reading A6b).  Config 4 adds `fake_frac` x tracks fake seeds from random
+    hit triplets on layers 0-2 (reading A18)."""
+    cfg = dict(BUILD_CONFIGS[config])
+    n_events = cfg["n_events"] if n_events is None else n_events
+    tracks = cfg["tracks"] if tracks is None else tracks
+    noise = cfg["noise"] if noise is None else noise
+    fake_frac = cfg["fake_frac"] if fake_frac is None else fake_frac
+    n_phi = cfg["n_phi"] if n_phi is None else n_phi
+    n_z = cfg["n_z"] if n_z is None else n_z
+    geom = geometry(cfg["geom"], xx0_scale=1.0 if ms else 0.0)
+    L = geom.n_layers
+    xs, ys, zs, tr = [], [], [], []
+    seg_off = [0]
+    seeds, sigs, qs, sev, struth, shit = [], [], [], [], [], []
+    truth_hit_idx = np.full((L, n_events * tracks), -1, dtype=np.int32)
+    for ev in range(n_events):
+        rng = rng_for(config, ev)
+        gun = particle_gun(rng, tracks, cfg["gun"])
+        sim = simulate(geom, gun, rng, ms=ms, smear=smear)
+        ev_hits = []
+        for l in range(L):
+            v = sim["valid"][l]
+            ids = np.nonzero(v)[0]
+            n_sig = len(ids)
+            n_noise = int(round(noise * n_sig))
+            az = rng.uniform(-np.pi, np.pi, n_noise)
+            nz = rng.uniform(-geom.zmax[l], geom.zmax[l], n_noise)
+            hx = np.concatenate([sim["hits"][l, ids, 0], geom.r[l] * np.cos(az)])
+            hy = np.concatenate([sim["hits"][l, ids, 1], geom.r[l] * np.sin(az)])
+            hz = np.concatenate([sim["hits"][l, ids, 2], nz])
+            ht = np.concatenate([ids + ev * tracks, np.full(n_noise, -1)]).astype(np.int32)
+            perm = rng.permutation(len(hx))
+            hx, hy, hz, ht = hx[perm], hy[perm], hz[perm], ht[perm]
+            pos = np.empty(len(perm), dtype=np.int64); pos[perm] = np.arange(len(perm))
+            truth_hit_idx[l, ids + ev * tracks] = pos[:n_sig]
+            xs.append(hx.astype(np.float32)); ys.append(hy.astype(np.float32)); zs.append(hz.astype(np.float32)); tr.append(ht)
+            seg_off.append(seg_off[-1] + len(hx))
+            ev_hits.append((hx, hy, hz, ht))
+        # true seeds
+        ok = sim["valid"][first_layer - 1]
+        ids = np.nonzero(ok)[0]
+        sd, sg = smear_seed(rng, sim["truth"][first_layer - 1][ids])
+        seeds.append(sd); sigs.append(sg); qs.append(gun["q"][ids]); sev.append(np.full(len(ids), ev, dtype=np.int32))
+        struth.append((ids + ev * tracks).astype(np.int32))
+        shit.append(truth_hit_idx[:first_layer, ids + ev * tracks])
+        # fake seeds from random hit triplets on layers 0..2
+        n_fake = int(round(fake_frac * tracks))
+        if n_fake:
+            f_sd, f_q, f_hit = [], [], []
+            h0, h1, h2 = ev_hits[0], ev_hits[1], ev_hits[2]
+            az1 = np.arctan2(h1[1], h1[0]); az2 = np.arctan2(h2[1], h2[0])
+            dphi = 3.0 * 2.0 * np.pi / n_phi / 2.0      # "3x3 bin neighbourhood": +-1.5 bins
+            dz = 3.0 * (2.0 * geom.zmax[0] / n_z) / 2.0
+            tries = 0
+            while len(f_sd) < n_fake and tries < 200 * n_fake:
+                tries += 1
+                i0 = int(rng.integers(len(h0[0])))
+                a0 = np.arctan2(h0[1][i0], h0[0][i0]); z0 = h0[2][i0]
+                picks = [i0]
+                fail = False
+                for (hh, azs, l) in ((h1, az1, 1), (h2, az2, 2)):
+                    zexp = z0 * geom.r[l] / geom.r[0]
+                    dd = np.abs(np.mod(azs - a0 + np.pi, 2 * np.pi) - np.pi)
+                    cand = np.nonzero((dd <= dphi) & (np.abs(hh[2] - zexp) <= dz))[0]
+                    if len(cand) == 0:
+                        fail = True; break
+                    picks.append(int(cand[rng.integers(len(cand))]))
+                if fail:
+                    continue
+                t0, t1, t2 = h0[3][picks[0]], h1[3][picks[1]], h2[3][picks[2]]
+                if t0 >= 0 and t0 == t1 == t2:
+                    continue
+                pts = [(hh[0][i], hh[1][i], hh[2][i]) for hh, i in zip((h0, h1, h2), picks)]
+                res = _three_point_seed(*pts, geom.bz)
+                if res is None:
+                    continue
+                st, qq = res
+                if 1.0 / st[3] < 0.3:
+                    continue
+                f_sd.append(st); f_q.append(qq); f_hit.append(picks)
+            if f_sd:
+                f_sd = np.array(f_sd)
+                f_sg = np.empty_like(f_sd)
+                f_sg[:, 0:3] = SEED_SIGMA_POS; f_sg[:, 3] = SEED_SIGMA_REL_IPT * f_sd[:, 3]; f_sg[:, 4:6] = SEED_SIGMA_ANG
+                seeds.append(f_sd); sigs.append(f_sg); qs.append(np.array(f_q, dtype=np.int8))
+                sev.append(np.full(len(f_sd), ev, dtype=np.int32)); struth.append(np.full(len(f_sd), -1, dtype=np.int32))
+                fh = np.array(f_hit, dtype=np.int32).T            # [3][n_fake]
+                if first_layer != 3:
+                    raise ValueError("fake seeds are defined for first_layer == 3")
+                shit.append(fh)
+    seed = np.concatenate(seeds); sig = np.concatenate(sigs); q = np.concatenate(qs)
+    t = _soa_tracks(seed, sig, q)
+    n_seeds, ld = t["n"], t["ld"]
+    seed_hit_idx = np.full((first_layer, ld), -1, dtype=np.int32)
+    seed_hit_idx[:, :n_seeds] = np.concatenate(shit, axis=1)
+    return BuildInputs(geom=geom, n_events=n_events, n_phi=n_phi, n_z=n_z, K=K, chi2_cut=chi2_cut, n_sigma=n_sigma,
+                       first_layer=first_layer, hit_x=np.concatenate(xs), hit_y=np.concatenate(ys), hit_z=np.concatenate(zs),
+                       seg_off=np.array(seg_off, dtype=np.int64), hit_truth=np.concatenate(tr), n_seeds=n_seeds, ld=ld,
+                       par=t["par"], cov=t["cov"], q=t["q"], seed_event=np.concatenate(sev), seed_hit_idx=seed_hit_idx,
+                       seed_truth=np.concatenate(struth), truth_hit_idx=truth_hit_idx)
