@@ -1,0 +1,153 @@
+/* kf.h -- C ABI of libkf_b200: batched Kalman-filter track fitting and combinatorial track building on one
+ * NVIDIA B200 (sm_100a), fp32.
+ *
+ * The operations are the hot path of arxiv 1711.06571:
+ *   - kf_fit:   "a final fit using the KF is performed to provide the best estimate of the track's parameters"
+ *               -- repeated propagate + update over a fixed hit list, no branching (sec. 2);
+ *   - kf_bin_hits / kf_window_lookup: the "data structures used for selecting hit candidates" (sec. 3.1);
+ *   - kf_build: "Track building projects the track candidate outwards to collect additional hits, using the KF to
+ *               estimate which hits represent the most likely continuation ... branching to explore multiple
+ *               candidate tracks per seed", with "a fixed number of slots for each track seed" and
+ *               "rapid identification of the best candidates" (sec. 4.3).
+ * The paper gives no formulas; the arithmetic (state, helix, Jacobian, noise, update, ranking, bins) is fixed by
+ * DESIGN.md sec. 3 "Readings" and restated per entry point below.
+ *
+ * Conventions
+ *   - State p = (x, y, z, 1/pT, phi, theta): global Cartesian position [cm], polar momentum ("hybrid
+ *     coordinate system"); charge q = +-1 separate; field along +z in Tesla; curvature dphi/ds_T = -q k Bz / pT,
+ *     k = 0.00299792458 GeV/(T cm).
+ *   - Covariance: packed lower-triangular row-major, element (i,j), i >= j, at k = i(i+1)/2 + j; 21 floats.
+ *   - Every array argument is a DEVICE pointer unless marked "host".  SoA: component c of track t at [c*ld + t].
+ *   - The library never allocates, frees or retains user memory.  All work is enqueued on `stream`
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream) and the call returns without
+ *     synchronising.  Host-marked arrays are read before the call returns.
+ *   - Return value 0 = OK, negative = kf_status.  No C++ exception crosses the boundary.  kf_last_error() gives
+ *     a thread-local, statically stored description of the last failure on the calling thread.
+ *   - Per-track numerical trouble is data, not an error: it sets bits in `status` and the track keeps its
+ *     last good state.
+ */
+#ifndef KF_B200_H
+#define KF_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KF_MAX_LAYERS 32
+
+typedef enum {
+    KF_OK = 0,
+    KF_ERR_INVALID_ARG = -1,
+    KF_ERR_NULL_PTR = -2,
+    KF_ERR_BAD_GEOM = -3,            /* n_layers outside 1..KF_MAX_LAYERS, radii not increasing, n_phi % 8 != 0 ... */
+    KF_ERR_WORKSPACE_TOO_SMALL = -4,
+    KF_ERR_CUDA = -5,                /* launch / runtime error; text in kf_last_error() */
+    KF_ERR_UNIMPLEMENTED = -6
+} kf_status;
+
+/* per-track status bits */
+#define KF_ST_UNREACHABLE 1u /* layer radius not reached within half a turn, or start radius >= layer radius       */
+#define KF_ST_LEFT_Z 2u      /* kf_build only: predicted |z| beyond zmax + window                                   */
+#define KF_ST_GRAZING 4u     /* cos(incidence) < 0.1 at the crossing                                                */
+#define KF_ST_NUMERIC 8u     /* innovation matrix not positive definite, non-finite result, or 1/pT <= 0            */
+
+/* One barrel layer: cylinder of radius r [cm], half length zmax [cm], thickness xx0 in radiation lengths at
+ * normal incidence, hit resolutions [cm] along r-phi, z and r (sig_r regularises the 3-D update; R5). */
+typedef struct { float r, zmax, xx0, sig_rphi, sig_z, sig_r; } kf_layer;
+
+/* Geometry: n_layers cylinders sorted by increasing r; uniform field bz_tesla along z.  `layers` is a HOST array. */
+typedef struct { int32_t n_layers; float bz_tesla; const kf_layer* layers; } kf_geom;
+
+/* SoA track store.  n tracks, stride ld >= n between components. */
+typedef struct {
+    int64_t n, ld;
+    float* par;       /* [6][ld]  x, y, z, 1/pT, phi, theta                                   */
+    float* cov;       /* [21][ld] packed symmetric                                             */
+    int8_t* q;        /* [n]      charge +-1                                                   */
+    float* chi2;      /* [n]      accumulated chi2 (input value is ignored by kf_fit)          */
+    int32_t* nhits;   /* [n]      number of hits used                                          */
+    uint32_t* status; /* [n]      KF_ST_* bits                                                 */
+} kf_tracks;
+
+/* Hits of all (event, layer) segments back to back, SoA.  Segment (event e, layer l) is
+ * [seg_off[e*n_layers + l], seg_off[e*n_layers + l + 1]).  seg_off is a HOST array of n_events*n_layers + 1
+ * entries; seg_off_dev is a device copy of the same array (required when n_events > 1 or for the build calls,
+ * may be NULL for kf_fit with n_events == 1). */
+typedef struct {
+    int64_t n_hits;
+    const float *x, *y, *z;
+    int32_t n_events;
+    const int64_t* seg_off;
+    const int64_t* seg_off_dev;
+} kf_hits;
+
+/* ---------------------------------------------------------------------------------------------------------
+ * kf_fit -- forward (inside-out) Kalman filter over a fixed hit list (DESIGN.md sec. 2 F1-F9).
+ * For every track t and every layer l in order of increasing radius with hit_idx[l*ld + t] >= 0:
+ *   propagate the state and covariance along the exact helix to the first crossing of the cylinder r_l (Jacobian
+ *   including the path-length term), add the multiple-scattering noise of the layer (Highland), update with the
+ *   3-D hit (residual, 3x3 innovation inverse, chi2, gain, state and covariance update).
+ * hit_idx: [n_layers][seeds->ld] index of the hit within its segment, < 0 = layer skipped; NULL = identity
+ *          (hit of track t on layer l is element t of segment l).
+ * trk_event: [n] event of each track, NULL = event 0.
+ * seeds/out: same n; out->ld may differ; out may alias seeds.  out->q is not written.
+ * A failing layer sets the status bit, ends the track there and leaves the state of the last updated layer.
+ * Output phi is wrapped to (-pi, pi].  Errors: NULL pointers, n < 0, ld < n, bad geometry, CUDA launch failure. */
+int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
+           const kf_tracks* seeds, kf_tracks* out, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Binned hit index (DESIGN.md sec. 2 B0, readings X1-X2).  Filled by kf_bin_hits into
+ * caller-allocated arrays.  Global bin of a hit = ((event*n_layers + layer)*n_z + iz)*n_phi + iphi; iphi from the
+ * azimuth by exact fp32 comparisons against a tangent table (no atan2), iz = clamp(floor((z + zmax)*n_z/(2 zmax))).
+ * Sorted order = ascending (global bin, original index): unique, hence bit-exact testable. */
+typedef struct {
+    int32_t n_phi, n_z;   /* n_phi multiple of 8, 8..4096; n_z 1..1024                                     */
+    float *x, *y, *z;     /* [n_hits] hits in sorted order                                                 */
+    int32_t* perm;        /* [n_hits] sorted position -> original index within its segment                 */
+    int32_t* bin_off;     /* [n_events*n_layers*n_z*n_phi + 1] offsets into the sorted arrays              */
+} kf_binned;
+
+size_t kf_bin_workspace_bytes(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z);
+int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* ws,
+                size_t ws_bytes, void* stream);
+
+/* kf_window_lookup -- test / diagnostic entry: the window hit list of B2-B3 for explicit windows (reading X3).
+ * Query i: event[i], layer[i], azimuth window phi_c +- dphi (phi_c in (-pi, pi], dphi >= 0), z window z_c +- dz.
+ * The list is every hit of the bins touched, rows in ascending iz, bins in ascending (wrapping) iphi, hits in
+ * sorted order.  count[i] = true length even if > cap; sorted_idx[i*cap + j] = global sorted position, j < min(count, cap). */
+int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, int64_t n_query,
+                     const int32_t* event, const int32_t* layer, const float* phi_c, const float* dphi,
+                     const float* z_c, const float* dz, int32_t cap, int32_t* count, int32_t* sorted_idx, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * kf_build -- combinatorial track building (DESIGN.md sec. 2 B1-B6, readings R10-R11).
+ * Per seed, per layer l = first_layer .. n_layers-1: propagate the <= K live candidates, open a window of
+ * n_sigma standard deviations in phi and z, chi2 against every hit of the window, one child per hit with
+ * chi2 < chi2_cut (else one child without hit), keep the best K children by (nhits desc, chi2 asc, parent slot asc,
+ * sorted hit position asc), update the survivors.
+ * Output: slot s*K + k of `cand` (best first), hit_idx[l*ld + slot] = original index within the segment,
+ * -1 = no hit on this layer, -2 = layer not crossed (candidate finished); n_cand[s] = number of valid slots. */
+typedef struct {
+    int32_t K, n_layers;
+    int64_t n_seeds, ld;  /* ld >= n_seeds*K */
+    kf_tracks cand;       /* n = n_seeds*K, cand.ld == ld */
+    int32_t* hit_idx;     /* [n_layers][ld] */
+    int32_t* n_cand;      /* [n_seeds] */
+} kf_cands;
+
+size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K);
+int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
+             const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
+             float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream);
+
+const char* kf_last_error(void);
+int kf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KF_B200_H */

@@ -106,7 +106,7 @@ static double g_of(const double p[6], double w, double s, double R, double* dg) 
 
 /* Propagate the state to the cylinder of radius R: smallest positive root of g(s) = x'^2 + y'^2 - R^2 [R2].
  * J (row-major 6x6) = d p'/d p INCLUDING the path-length term (the state is transported to the surface).
- * Returns 0 or a flag: KFO_UNREACHABLE (start not inside R, or no crossing within one turn), KFO_GRAZING
+ * Returns 0 or a flag: KFO_UNREACHABLE (start not inside R, or no crossing within half a turn), KFO_GRAZING
  * (cos(incidence) < KFO_CMIN; outputs are still filled).  s_out = transverse path, cosinc_out = u'/R. */
 int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
                   double* cosinc_out) {
@@ -119,10 +119,11 @@ int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6],
     if (cosinc_out) *cosinc_out = 0.0;
     if (!(r02 < R * R) || !isfinite(w) || !isfinite(r02)) return KFO_UNREACHABLE;
 
-    /* march: a circle of radius rho >= R that starts inside the cylinder leaves it within an arc pi R;
-       a tighter circle either crosses within one turn 2 pi rho or never */
+    /* march: a circle of radius rho >= R that starts inside the cylinder leaves it within an arc pi R
+       (<= half a turn); a tighter circle must cross within half a turn pi rho, else the layer counts as
+       unreachable [R2] */
     const int NMARCH = 64;
-    double smax = (fabs(w) * R <= 1.0) ? KFO_PI * R * (1.0 + 1e-9) : 2.0 * KFO_PI / fabs(w);
+    double smax = (fabs(w) * R <= 1.0) ? KFO_PI * R * (1.0 + 1e-9) : KFO_PI / fabs(w);
     double lo = 0.0, hi = -1.0;
     for (int k = 1; k <= NMARCH; ++k) {
         double sk = smax * (double)k / NMARCH;

@@ -1,0 +1,192 @@
+"""Thin ctypes binding of libkf_b200.so (include/kf.h).  Argument marshalling only: every step of the path runs
+in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: if the shared library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libkf_b200.so")
+_lib = None
+
+KF_MAX_LAYERS = 32
+ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
+
+EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
+           "kf_build", "kf_last_error", "kf_version"]
+
+
+class KfError(RuntimeError):
+    pass
+
+
+class kf_layer(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("r", "zmax", "xx0", "sig_rphi", "sig_z", "sig_r")]
+
+
+class kf_geom(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("bz_tesla", C.c_float), ("layers", C.POINTER(kf_layer))]
+
+
+class kf_tracks(C.Structure):
+    _fields_ = [("n", C.c_int64), ("ld", C.c_int64), ("par", C.c_void_p), ("cov", C.c_void_p), ("q", C.c_void_p),
+                ("chi2", C.c_void_p), ("nhits", C.c_void_p), ("status", C.c_void_p)]
+
+
+class kf_hits(C.Structure):
+    _fields_ = [("n_hits", C.c_int64), ("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p), ("n_events", C.c_int32),
+                ("seg_off", C.POINTER(C.c_int64)), ("seg_off_dev", C.c_void_p)]
+
+
+class kf_binned(C.Structure):
+    _fields_ = [("n_phi", C.c_int32), ("n_z", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p),
+                ("perm", C.c_void_p), ("bin_off", C.c_void_p)]
+
+
+class kf_cands(C.Structure):
+    _fields_ = [("K", C.c_int32), ("n_layers", C.c_int32), ("n_seeds", C.c_int64), ("ld", C.c_int64), ("cand", kf_tracks),
+                ("hit_idx", C.c_void_p), ("n_cand", C.c_void_p)]
+
+
+def lib() -> C.CDLL:
+    """Loads libkf_b200.so (built in-tree by paper_1711_06571_b200.build_ext).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise KfError(f"{_SO} not built: run `python -m paper_1711_06571_b200.build_ext` (there is no CPU fallback)")
+        l = C.CDLL(_SO)
+        l.kf_last_error.restype = C.c_char_p
+        l.kf_version.restype = C.c_int
+        l.kf_bin_workspace_bytes.restype = C.c_size_t
+        l.kf_build_workspace_bytes.restype = C.c_size_t
+        l.kf_bin_workspace_bytes.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
+        l.kf_build_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+        l.kf_fit.argtypes = [C.c_void_p] * 7
+        l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        _lib = l
+    return _lib
+
+
+def _check(rc: int, who: str):
+    if rc != 0:
+        raise KfError(f"{who} failed with {rc}: {lib().kf_last_error().decode()}")
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise KfError("no CUDA device: the KF path has no CPU fallback")
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device, contiguous tensors only"
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Geom:
+    """Host-side kf_geom built from a [L][6] table (r, zmax, xx0, sig_rphi, sig_z, sig_r) and Bz."""
+
+    def __init__(self, layer_table, bz: float):
+        tab = np.asarray(layer_table, dtype=np.float32)
+        self.n_layers = tab.shape[0]
+        self._arr = (kf_layer * max(1, self.n_layers))()
+        for i in range(self.n_layers):
+            self._arr[i] = kf_layer(*[float(v) for v in tab[i]])
+        self.c = kf_geom(self.n_layers, float(bz), C.cast(self._arr, C.POINTER(kf_layer)))
+        self.table = tab
+        self.bz = float(bz)
+
+
+@dataclass
+class Tracks:
+    """Device SoA track store (kf_tracks)."""
+    n: int
+    ld: int
+    par: torch.Tensor      # [6, ld] f32
+    cov: torch.Tensor      # [21, ld] f32
+    q: torch.Tensor        # [n] i8
+    chi2: torch.Tensor     # [n] f32
+    nhits: torch.Tensor    # [n] i32
+    status: torch.Tensor   # [n] i32 (bit pattern of uint32)
+
+    @staticmethod
+    def empty(n: int, ld: int | None = None, device="cuda") -> "Tracks":
+        ld = max(32, (n + 31) // 32 * 32) if ld is None else ld
+        return Tracks(n, ld, torch.empty((6, ld), dtype=torch.float32, device=device), torch.empty((21, ld), dtype=torch.float32, device=device),
+                      torch.empty(max(n, 1), dtype=torch.int8, device=device)[:n], torch.zeros(max(n, 1), dtype=torch.float32, device=device)[:n],
+                      torch.zeros(max(n, 1), dtype=torch.int32, device=device)[:n], torch.zeros(max(n, 1), dtype=torch.int32, device=device)[:n])
+
+    @staticmethod
+    def from_host(par, cov, q, device="cuda", chi2=None, nhits=None) -> "Tracks":
+        n, ld = len(q), par.shape[1]
+        t = Tracks.empty(n, ld, device)
+        t.par.copy_(torch.from_numpy(np.ascontiguousarray(par, dtype=np.float32)))
+        t.cov.copy_(torch.from_numpy(np.ascontiguousarray(cov, dtype=np.float32)))
+        t.q.copy_(torch.from_numpy(np.ascontiguousarray(q, dtype=np.int8)))
+        if chi2 is not None:
+            t.chi2.copy_(torch.from_numpy(np.ascontiguousarray(chi2, dtype=np.float32)))
+        if nhits is not None:
+            t.nhits.copy_(torch.from_numpy(np.ascontiguousarray(nhits, dtype=np.int32)))
+        return t
+
+    def c(self) -> kf_tracks:
+        return kf_tracks(self.n, self.ld, self.par.data_ptr(), self.cov.data_ptr(), self.q.data_ptr() if self.n else None,
+                         self.chi2.data_ptr() if self.n else None, self.nhits.data_ptr() if self.n else None,
+                         self.status.data_ptr() if self.n else None)
+
+    def to_host(self) -> dict:
+        return dict(par=self.par[:, :self.n].cpu().numpy(), cov=self.cov[:, :self.n].cpu().numpy(), chi2=self.chi2.cpu().numpy(),
+                    nhits=self.nhits.cpu().numpy(), status=self.status.cpu().numpy().view(np.uint32))
+
+
+class Hits:
+    """Device hit store (kf_hits): SoA x, y, z over all (event, layer) segments + host/device segment offsets."""
+
+    def __init__(self, x, y, z, seg_off, n_events: int, device="cuda"):
+        def dev(a):
+            if isinstance(a, torch.Tensor):
+                return a.to(device=device, dtype=torch.float32).contiguous()
+            return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(device)
+        self.x, self.y, self.z = dev(x), dev(y), dev(z)
+        self.n_hits = int(self.x.numel())
+        self.n_events = int(n_events)
+        self.seg_off = np.ascontiguousarray(seg_off, dtype=np.int64)
+        self.seg_off_dev = torch.from_numpy(self.seg_off).to(device)
+        self.c = kf_hits(self.n_hits, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(), self.n_events,
+                         self.seg_off.ctypes.data_as(C.POINTER(C.c_int64)), self.seg_off_dev.data_ptr())
+
+
+def kf_version() -> int:
+    return int(lib().kf_version())
+
+
+def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Tracks | None = None, stream=None) -> Tracks:
+    """include/kf.h kf_fit.  hit_idx: [L, seeds.ld] int32 device tensor or None (identity); trk_event [n] int32 or None."""
+    _require_cuda()
+    if out is None:
+        out = Tracks.empty(seeds.n, seeds.ld, seeds.par.device)
+        out.q = seeds.q
+    if hit_idx is not None:
+        assert tuple(hit_idx.shape) == (geom.n_layers, seeds.ld)
+    sc, oc = seeds.c(), out.c()
+    rc = lib().kf_fit(C.byref(geom.c), C.byref(hits.c), _ptr(hit_idx, torch.int32), _ptr(trk_event, torch.int32),
+                      C.byref(sc), C.byref(oc), _stream(stream))
+    _check(rc, "kf_fit")
+    return out

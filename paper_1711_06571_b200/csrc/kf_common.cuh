@@ -1,0 +1,22 @@
+// kf_common.cuh -- host-side plumbing shared by the entry points: error reporting, geometry checks.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/kf.h"
+#include "kf_math.cuh"
+
+namespace kf {
+
+int fail(int code, const char* fmt, ...);              // records the message for kf_last_error(), returns code
+int check_launch(const char* what);                    // cudaGetLastError() -> KF_OK / KF_ERR_CUDA
+int check_geom(const kf_geom* g, const char* who);
+
+inline LayerC make_layer(const kf_layer& l) {
+    LayerC c;
+    c.r = l.r; c.r2 = l.r * l.r; c.zmax = l.zmax; c.xx0r = l.xx0 * l.r;
+    c.var_rphi = l.sig_rphi * l.sig_rphi; c.var_z = l.sig_z * l.sig_z; c.var_r = l.sig_r * l.sig_r;
+    c.rcmin = l.r * CMIN;
+    return c;
+}
+
+}  // namespace kf

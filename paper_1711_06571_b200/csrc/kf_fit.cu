@@ -1,0 +1,116 @@
+// kf_fit.cu -- fused propagate + update track fit (steps F1-F9).
+//
+// One thread per track; the whole layer loop runs in registers (6 parameters + 21 packed covariance elements),
+// the only HBM traffic being the coalesced SoA load of the seed (F1), one hit (+ optional index) per layer (F6)
+// and the coalesced store of the result (F9).  Per-layer constants arrive as a __grid_constant__ kernel
+// parameter, i.e. through the constant bank: warp-uniform, no global loads.
+#include "kf_common.cuh"
+
+namespace kf {
+
+struct FitArgs {
+    int32_t n_layers, n_events;
+    float kb;                      // k * Bz
+    int64_t n, ld_in, ld_out, ld_idx;
+    const float* par; const float* cov; const int8_t* q;
+    const float *hx, *hy, *hz;
+    const int64_t* seg_off_dev;
+    const int32_t* hit_idx; const int32_t* trk_event;
+    float* par_o; float* cov_o; float* chi2_o; int32_t* nhits_o; uint32_t* status_o;
+    LayerC layer[KF_MAX_LAYERS];
+    int64_t seg0[KF_MAX_LAYERS];   // segment offsets of event 0 (used when trk_event == NULL)
+};
+
+constexpr int FIT_BLOCK = 128;
+
+__global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant__ FitArgs a) {
+    const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
+    if (t >= a.n) return;
+    const float cw = -(float)a.q[t] * a.kb;
+    const int ev = a.trk_event ? a.trk_event[t] : 0;
+    float p[6], C[21];
+    float chi2 = 0.0f;
+    int nh = 0;
+    uint32_t st = 0u;
+    int limit = a.n_layers;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        // F1: coalesced SoA load
+#pragma unroll
+        for (int i = 0; i < 6; ++i) p[i] = a.par[i * a.ld_in + t];
+#pragma unroll
+        for (int i = 0; i < 21; ++i) C[i] = a.cov[i * a.ld_in + t];
+        chi2 = 0.0f;
+        nh = 0;
+        int bad = -1;
+#pragma unroll 1
+        for (int l = 0; l < limit; ++l) {
+            const int64_t idx = a.hit_idx ? (int64_t)a.hit_idx[l * a.ld_idx + t] : t;
+            if (idx < 0) continue;                                   // layer skipped entirely (R8)
+            const int64_t h = (a.trk_event ? a.seg_off_dev[(int64_t)ev * a.n_layers + l] : a.seg0[l]) + idx;
+            const float mx = a.hx[h], my = a.hy[h], mz = a.hz[h];   // F6: issued before the arithmetic
+            const uint32_t flag = predict(p, C, cw, a.layer[l]);     // F2-F5
+            if (flag) { st |= flag; break; }
+            Sym3 Si;
+            float r[3], c2;
+            bool ok = innovation(p, C, mx, my, mz, a.layer[l], Si, r, c2);   // F7
+            if (ok) {
+                gain_update(p, C, Si, r);                                    // F8
+                ok = all_finite(p, C) && p[3] > 0.0f && c2 == c2;
+            }
+            if (!ok) { bad = l; break; }
+            chi2 += c2;
+            nh += 1;
+        }
+        if (bad < 0) break;
+        // numeric failure (rare): the track keeps the state of the last good layer -> redo the layers before it
+        st |= ST_NUMERIC;
+        limit = bad;
+    }
+    // F9: coalesced store
+    p[4] = wrap_phi(p[4]);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) a.par_o[i * a.ld_out + t] = p[i];
+#pragma unroll
+    for (int i = 0; i < 21; ++i) a.cov_o[i * a.ld_out + t] = C[i];
+    a.chi2_o[t] = chi2;
+    a.nhits_o[t] = nh;
+    a.status_o[t] = st;
+}
+
+}  // namespace kf
+
+extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
+                      const kf_tracks* seeds, kf_tracks* out, void* stream) {
+    using namespace kf;
+    if (!geom || !hits || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_fit: NULL struct argument");
+    int rc = check_geom(geom, "kf_fit");
+    if (rc) return rc;
+    if (seeds->n < 0 || seeds->ld < seeds->n || out->n != seeds->n || out->ld < out->n)
+        return fail(KF_ERR_INVALID_ARG, "kf_fit: need 0 <= n <= ld and out->n == seeds->n");
+    if (seeds->n == 0) return KF_OK;
+    if (!seeds->par || !seeds->cov || !seeds->q || !out->par || !out->cov || !out->chi2 || !out->nhits || !out->status)
+        return fail(KF_ERR_NULL_PTR, "kf_fit: NULL track array");
+    if (!hits->x || !hits->y || !hits->z || !hits->seg_off) return fail(KF_ERR_NULL_PTR, "kf_fit: NULL hit array");
+    if (hits->n_events < 1) return fail(KF_ERR_INVALID_ARG, "kf_fit: n_events < 1");
+    if (trk_event && !hits->seg_off_dev) return fail(KF_ERR_NULL_PTR, "kf_fit: trk_event given but hits->seg_off_dev is NULL");
+    FitArgs a;
+    a.n_layers = geom->n_layers; a.n_events = hits->n_events;
+    a.kb = KCURV * geom->bz_tesla;
+    a.n = seeds->n; a.ld_in = seeds->ld; a.ld_out = out->ld; a.ld_idx = seeds->ld;
+    a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q;
+    a.hx = hits->x; a.hy = hits->y; a.hz = hits->z;
+    a.seg_off_dev = hits->seg_off_dev; a.hit_idx = hit_idx; a.trk_event = trk_event;
+    a.par_o = out->par; a.cov_o = out->cov; a.chi2_o = out->chi2; a.nhits_o = out->nhits; a.status_o = out->status;
+    for (int l = 0; l < KF_MAX_LAYERS; ++l) {
+        a.layer[l] = make_layer(l < geom->n_layers ? geom->layers[l] : geom->layers[geom->n_layers - 1]);
+        a.seg0[l] = l < geom->n_layers ? hits->seg_off[l] : 0;
+    }
+    if (!hit_idx) {   // identity indexing: every segment of event 0 must hold n hits
+        for (int l = 0; l < geom->n_layers; ++l)
+            if (!trk_event && hits->seg_off[l + 1] - hits->seg_off[l] < seeds->n)
+                return fail(KF_ERR_INVALID_ARG, "kf_fit: hit_idx == NULL needs >= n hits in every segment");
+    }
+    const int64_t blocks = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
+    kf_fit_kernel<<<(unsigned)blocks, FIT_BLOCK, 0, (cudaStream_t)stream>>>(a);
+    return check_launch("kf_fit");
+}

@@ -1,0 +1,277 @@
+// kf_math.cuh -- register-resident device math of the per-layer Kalman-filter step (fp32, sm_100a).
+//
+// One thread owns one track candidate: 6 parameters + 21 packed covariance elements live in registers for the whole
+// layer loop.  The Jacobian's sparsity (20 non-zeros, 3 of them == 1; cf. "patterns of elements known ... to be zero
+// or one", sec. 2.1) is written out by hand: J C J^T costs 138 FMA instead of 627 dense flops x/2.
+// Formulas: DESIGN.md sec. 3 (R2 closed-form helix/cylinder solve, R3 surface Jacobian, R4 Highland noise,
+// R5 3-D update).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kf {
+
+constexpr float KCURV = 0.00299792458f;  // GeV / (T cm)
+constexpr float CMIN = 0.1f;             // grazing guard on cos(incidence)
+
+enum : uint32_t { ST_UNREACHABLE = 1u, ST_LEFT_Z = 2u, ST_GRAZING = 4u, ST_NUMERIC = 8u };
+
+// per-layer constants, prepared on the host
+struct LayerC {
+    float r, r2, zmax, xx0r;          // radius, radius^2, half length, xx0 * r
+    float var_rphi, var_z, var_r;     // hit variances
+    float rcmin;                      // r * CMIN
+};
+
+// packed lower-triangular index
+__host__ __device__ constexpr int pk(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
+
+// atan(t)/t, |t| <= ~1: odd minimax-free Taylor for small t, library atan otherwise
+__device__ __forceinline__ float atan_over_t(float t) {
+    float t2 = t * t;
+    if (t2 < 0.01f) {   // |t| < 0.1: truncation < t^10/11 = 1e-11
+        return 1.0f + t2 * (-1.0f / 3.0f + t2 * (0.2f + t2 * (-1.0f / 7.0f + t2 * (1.0f / 9.0f))));
+    }
+    return atanf(t) / t;
+}
+
+// f1(a) = (cos a - sin a / a)/a, f2(a) = (sin a - (1 - cos a)/a)/a ; series below |a| = 0.5 (cancellation-free)
+__device__ __forceinline__ void curv_partials(float a, float sa, float ca, float& f1, float& f2) {
+    float a2 = a * a;
+    if (a2 < 0.25f) {
+        f1 = a * (-1.0f / 3.0f + a2 * (1.0f / 30.0f + a2 * (-1.0f / 840.0f + a2 * (1.0f / 45360.0f))));
+        f2 = 0.5f + a2 * (-0.125f + a2 * (1.0f / 144.0f + a2 * (-1.0f / 5760.0f + a2 * (1.0f / 403200.0f))));
+    } else {
+        float ia = 1.0f / a;
+        f1 = (ca - sa * ia) * ia;
+        f2 = (sa - (1.0f - ca) * ia) * ia;
+    }
+}
+
+// Result of the transport to a cylinder (state only).
+struct Transport {
+    float dx, dy;        // x' - x, y' - y
+    float xn, yn, zn;    // position on the cylinder
+    float alpha, s;      // turning angle, transverse path length
+    float sa, ca;        // sin / cos alpha
+    float cpn, spn;      // cos / sin of phi'
+    float up;            // x' cos phi' + y' sin phi' = r cos(incidence)
+    float w;             // curvature
+};
+
+// Closed-form first crossing of the cylinder r (R2): with u, v the position along / across the direction,
+// E = (r^2 - x^2 - y^2)/2, A = 2(1 + v w) - w^2 E, D = u^2 + E A:  tau = tan(alpha/2)/w solves A tau^2 + 2 u tau - E = 0.
+__device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, float cp, float sp, float cot,
+                                              const LayerC& ly, Transport& t) {
+    const float x = p[0], y = p[1];
+    const float w = cw * p[3];
+    const float u = fmaf(x, cp, y * sp);
+    const float v = fmaf(y, cp, -x * sp);
+    const float E = 0.5f * (ly.r2 - fmaf(x, x, y * y));
+    const float A = fmaf(-w * w, E, 2.0f * fmaf(v, w, 1.0f));
+    const float D = fmaf(E, A, u * u);
+    if (!(E > 0.0f) || !(D >= 0.0f)) return ST_UNREACHABLE;
+    const float sq = sqrtf(D);
+    float tau;
+    if (u >= 0.0f) {
+        tau = E / (u + sq);
+    } else {
+        if (!(A > 0.0f)) return ST_UNREACHABLE;   // crossing only after more than half a turn
+        tau = (sq - u) / A;
+    }
+    const float th = w * tau;                     // tan(alpha/2)
+    const float th2 = th * th;
+    const float inv = 1.0f / (1.0f + th2);
+    t.sa = 2.0f * th * inv;
+    t.ca = (1.0f - th2) * inv;
+    const float X = 2.0f * tau * inv;
+    const float Y = X * th;
+    t.dx = fmaf(cp, X, -sp * Y);
+    t.dy = fmaf(sp, X, cp * Y);
+    t.xn = x + t.dx;
+    t.yn = y + t.dy;
+    const float f = atan_over_t(th);
+    t.alpha = 2.0f * th * f;
+    t.s = 2.0f * tau * f;
+    t.zn = fmaf(t.s, cot, p[2]);
+    t.cpn = fmaf(cp, t.ca, -sp * t.sa);
+    t.spn = fmaf(sp, t.ca, cp * t.sa);
+    t.up = fmaf(t.xn, t.cpn, t.yn * t.spn);
+    t.w = w;
+    if (!(t.up >= ly.rcmin)) return (t.up == t.up) ? ST_GRAZING : ST_NUMERIC;
+    return 0u;
+}
+
+// Predict: transport p, C to layer ly, C <- J C J^T + Q.  On a non-zero return p and C are untouched.
+// cw = -q k Bz.  up_out = r cos(incidence) of the crossing.
+__device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], float cw, const LayerC& ly) {
+    float sp, cp, st, ct;
+    sincosf(p[4], &sp, &cp);
+    sincosf(p[5], &st, &ct);
+    const float ist = 1.0f / st;
+    const float cot = ct * ist;
+    Transport t;
+    const uint32_t flag = transport(p, cw, cp, sp, cot, ly, t);
+    if (flag) return flag;
+
+    // ---- Jacobian entries (R3) ----
+    float f1, f2;
+    curv_partials(t.alpha, t.sa, t.ca, f1, f2);
+    const float cs2 = cw * t.s * t.s;
+    const float dXdi = cs2 * f1, dYdi = cs2 * f2;
+    const float Fxi = fmaf(cp, dXdi, -sp * dYdi), Fyi = fmaf(sp, dXdi, cp * dYdi);
+    const float Fxp = -t.dy, Fyp = t.dx;
+    const float iup = 1.0f / t.up;
+    const float sx = -t.xn * iup, sy = -t.yn * iup;
+    const float si = -fmaf(t.xn, Fxi, t.yn * Fyi) * iup;
+    const float sph = -fmaf(t.xn, Fxp, t.yn * Fyp) * iup;
+    const float a0 = fmaf(t.cpn, sx, 1.0f), a1 = t.cpn * sy, a3 = fmaf(t.cpn, si, Fxi), a4 = fmaf(t.cpn, sph, Fxp);
+    const float b0 = t.spn * sx, b1 = fmaf(t.spn, sy, 1.0f), b3 = fmaf(t.spn, si, Fyi), b4 = fmaf(t.spn, sph, Fyp);
+    const float c0 = cot * sx, c1 = cot * sy, c3 = cot * si, c4 = cot * sph, c5 = -t.s * ist * ist;
+    const float d0 = t.w * sx, d1 = t.w * sy, d3 = fmaf(t.w, si, cw * t.s), d4 = fmaf(t.w, sph, 1.0f);
+
+#define CC(i, j) C[pk(i, j)]
+    // ---- T = J C: rows 0, 1, 4 (columns 0,1,3,4,5) and row 2 (all columns) ----
+#define ROW4(c0_, c1_, c3_, c4_, j) fmaf(c0_, CC(0, j), fmaf(c1_, CC(1, j), fmaf(c3_, CC(3, j), c4_ * CC(4, j))))
+    const float T00 = ROW4(a0, a1, a3, a4, 0), T01 = ROW4(a0, a1, a3, a4, 1), T03 = ROW4(a0, a1, a3, a4, 3),
+                T04 = ROW4(a0, a1, a3, a4, 4), T05 = ROW4(a0, a1, a3, a4, 5);
+    const float T10 = ROW4(b0, b1, b3, b4, 0), T11 = ROW4(b0, b1, b3, b4, 1), T13 = ROW4(b0, b1, b3, b4, 3),
+                T14 = ROW4(b0, b1, b3, b4, 4), T15 = ROW4(b0, b1, b3, b4, 5);
+    const float T40 = ROW4(d0, d1, d3, d4, 0), T41 = ROW4(d0, d1, d3, d4, 1), T43 = ROW4(d0, d1, d3, d4, 3),
+                T44 = ROW4(d0, d1, d3, d4, 4), T45 = ROW4(d0, d1, d3, d4, 5);
+#define ROW6(j) (fmaf(c0, CC(0, j), fmaf(c1, CC(1, j), fmaf(c3, CC(3, j), fmaf(c4, CC(4, j), fmaf(c5, CC(5, j), CC(2, j)))))))
+    const float T20 = ROW6(0), T21 = ROW6(1), T22 = ROW6(2), T23 = ROW6(3), T24 = ROW6(4), T25 = ROW6(5);
+#undef ROW4
+#undef ROW6
+    // ---- C' = T J^T, lower triangle; rows 3 and 5 of J are unit rows ----
+#define DOT4(T0, T1, T3, T4, e0, e1, e3, e4) fmaf(T0, e0, fmaf(T1, e1, fmaf(T3, e3, T4 * e4)))
+    const float n00 = DOT4(T00, T01, T03, T04, a0, a1, a3, a4);
+    const float n10 = DOT4(T10, T11, T13, T14, a0, a1, a3, a4);
+    const float n11 = DOT4(T10, T11, T13, T14, b0, b1, b3, b4);
+    const float n20 = DOT4(T20, T21, T23, T24, a0, a1, a3, a4);
+    const float n21 = DOT4(T20, T21, T23, T24, b0, b1, b3, b4);
+    const float n22 = fmaf(T20, c0, fmaf(T21, c1, fmaf(T23, c3, fmaf(T24, c4, fmaf(T25, c5, T22)))));
+    const float n40 = DOT4(T40, T41, T43, T44, a0, a1, a3, a4);
+    const float n41 = DOT4(T40, T41, T43, T44, b0, b1, b3, b4);
+    const float n42 = DOT4(T20, T21, T23, T24, d0, d1, d3, d4);
+    const float n44 = DOT4(T40, T41, T43, T44, d0, d1, d3, d4);
+#undef DOT4
+    // ---- multiple scattering (R4), evaluated at the arriving state ----
+    float q33 = 0.0f, q53 = 0.0f, q44 = 0.0f, q55 = 0.0f;
+    if (ly.xx0r > 0.0f) {
+        const float tms = ly.xx0r * ist * iup;                 // xx0 / (sin(theta) cos(inc))
+        const float lg = fmaf(0.038f, logf(tms), 1.0f);
+        const float h = 0.0136f * p[3] * st * lg;
+        const float v = h * h * tms;                           // theta0^2
+        const float icot = p[3] * cot;
+        q55 = v;
+        q44 = v * ist * ist;
+        q33 = icot * icot * v;
+        q53 = -icot * v;
+    }
+    // commit
+    C[pk(0, 0)] = n00;
+    C[pk(1, 0)] = n10; C[pk(1, 1)] = n11;
+    C[pk(2, 0)] = n20; C[pk(2, 1)] = n21; C[pk(2, 2)] = n22;
+    C[pk(3, 0)] = T03; C[pk(3, 1)] = T13; C[pk(3, 2)] = T23; C[pk(3, 3)] += q33;
+    C[pk(4, 0)] = n40; C[pk(4, 1)] = n41; C[pk(4, 2)] = n42; C[pk(4, 3)] = T43; C[pk(4, 4)] = n44 + q44;
+    C[pk(5, 0)] = T05; C[pk(5, 1)] = T15; C[pk(5, 2)] = T25; C[pk(5, 3)] += q53; C[pk(5, 4)] = T45; C[pk(5, 5)] += q55;
+#undef CC
+    p[0] = t.xn; p[1] = t.yn; p[2] = t.zn; p[4] += t.alpha;
+    return 0u;
+}
+
+// Hit covariance (R5): rotation of diag(var_r, var_rphi) to the hit's azimuth, var_z along z.
+struct HitCov { float xx, xy, yy, zz; };
+__device__ __forceinline__ HitCov hit_cov(float mx, float my, const LayerC& ly) {
+    HitCov V;
+    V.zz = ly.var_z;
+    if (ly.var_r == ly.var_rphi) {
+        V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f;
+    } else {
+        const float ir2 = 1.0f / fmaf(mx, mx, my * my);
+        const float c2 = mx * mx * ir2, s2 = my * my * ir2, cs = mx * my * ir2;
+        V.xx = fmaf(c2, ly.var_r, s2 * ly.var_rphi);
+        V.yy = fmaf(s2, ly.var_r, c2 * ly.var_rphi);
+        V.xy = cs * (ly.var_r - ly.var_rphi);
+    }
+    return V;
+}
+
+// Symmetric 3x3 inverse by cofactors.  Returns false when S is not positive definite (Sylvester).
+struct Sym3 { float m00, m10, m11, m20, m21, m22; };
+__device__ __forceinline__ bool inv_sym3(const Sym3& S, Sym3& I) {
+    const float k00 = fmaf(S.m11, S.m22, -S.m21 * S.m21);
+    const float k10 = fmaf(S.m20, S.m21, -S.m10 * S.m22);
+    const float k20 = fmaf(S.m10, S.m21, -S.m20 * S.m11);
+    const float det = fmaf(S.m00, k00, fmaf(S.m10, k10, S.m20 * k20));
+    const float k22 = fmaf(S.m00, S.m11, -S.m10 * S.m10);
+    if (!(S.m00 > 0.0f) || !(k22 > 0.0f) || !(det > 0.0f)) return false;
+    const float id = 1.0f / det;
+    I.m00 = k00 * id; I.m10 = k10 * id; I.m20 = k20 * id;
+    I.m11 = fmaf(S.m00, S.m22, -S.m20 * S.m20) * id;
+    I.m21 = fmaf(S.m10, S.m20, -S.m00 * S.m21) * id;
+    I.m22 = k22 * id;
+    return true;
+}
+
+// Innovation of hit m against the predicted (p, C): S^-1 and chi2.  r = m - p[0:3].
+__device__ __forceinline__ bool innovation(const float (&p)[6], const float (&C)[21], float mx, float my, float mz,
+                                           const LayerC& ly, Sym3& Si, float (&r)[3], float& chi2) {
+    const HitCov V = hit_cov(mx, my, ly);
+    Sym3 S;
+    S.m00 = C[pk(0, 0)] + V.xx; S.m10 = C[pk(1, 0)] + V.xy; S.m11 = C[pk(1, 1)] + V.yy;
+    S.m20 = C[pk(2, 0)]; S.m21 = C[pk(2, 1)]; S.m22 = C[pk(2, 2)] + V.zz;
+    if (!inv_sym3(S, Si)) return false;
+    r[0] = mx - p[0]; r[1] = my - p[1]; r[2] = mz - p[2];
+    const float t0 = fmaf(Si.m00, r[0], fmaf(Si.m10, r[1], Si.m20 * r[2]));
+    const float t1 = fmaf(Si.m10, r[0], fmaf(Si.m11, r[1], Si.m21 * r[2]));
+    const float t2 = fmaf(Si.m20, r[0], fmaf(Si.m21, r[1], Si.m22 * r[2]));
+    chi2 = fmaf(r[0], t0, fmaf(r[1], t1, r[2] * t2));
+    return true;
+}
+
+// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C -= K C[0:3,:].
+__device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], const Sym3& Si, const float (&r)[3]) {
+    float K[6][3];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        const float ci0 = C[pk(i, 0)], ci1 = C[pk(i, 1)], ci2 = C[pk(i, 2)];
+        K[i][0] = fmaf(ci0, Si.m00, fmaf(ci1, Si.m10, ci2 * Si.m20));
+        K[i][1] = fmaf(ci0, Si.m10, fmaf(ci1, Si.m11, ci2 * Si.m21));
+        K[i][2] = fmaf(ci0, Si.m20, fmaf(ci1, Si.m21, ci2 * Si.m22));
+    }
+#pragma unroll
+    for (int i = 0; i < 6; ++i) p[i] = fmaf(K[i][0], r[0], fmaf(K[i][1], r[1], fmaf(K[i][2], r[2], p[i])));
+    // rows in decreasing order so that C[0:3,:] (rows 0..2 of the old matrix) is still intact when it is read:
+    // element (i,j), j <= i, needs old C[k][j] for k < 3, i.e. packed entries of rows <= max(2, j) <= i.
+    float P[3][6];   // old C[k][j], k < 3, all j
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int j = 0; j < 6; ++j) P[k][j] = C[pk(k, j)];
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+#pragma unroll
+        for (int j = 0; j <= i; ++j)
+            C[pk(i, j)] = fmaf(-K[i][0], P[0][j], fmaf(-K[i][1], P[1][j], fmaf(-K[i][2], P[2][j], C[pk(i, j)])));
+}
+
+__device__ __forceinline__ float wrap_phi(float a) {
+    const float TWO_PI = 6.28318530717958647692f, PI = 3.14159265358979323846f;
+    a -= TWO_PI * floorf((a + PI) * (1.0f / TWO_PI));
+    if (a <= -PI) a += TWO_PI;
+    if (a > PI) a -= TWO_PI;
+    return a;
+}
+
+__device__ __forceinline__ bool all_finite(const float (&p)[6], const float (&C)[21]) {
+    float acc = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) acc = fmaf(0.0f, p[i], acc);
+#pragma unroll
+    for (int i = 0; i < 21; ++i) acc = fmaf(0.0f, C[i], acc);
+    return acc == 0.0f;   // 0 * inf = NaN, 0 * NaN = NaN
+}
+
+}  // namespace kf
