@@ -50,11 +50,12 @@ __global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant
             const float mx = a.hx[h], my = a.hy[h], mz = a.hz[h];   // F6: issued before the arithmetic
             const uint32_t flag = predict(p, C, cw, a.layer[l]);     // F2-F5
             if (flag) { st |= flag; break; }
-            Sym3 Si;
+            Ldl3 Si;
             float r[3], c2;
-            bool ok = innovation(p, C, mx, my, mz, a.layer[l], Si, r, c2);   // F7
+            const HitCov V = hit_cov(mx, my, a.layer[l]);
+            bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);            // F7
             if (ok) {
-                gain_update(p, C, Si, r);                                    // F8
+                gain_update(p, C, Si, V, r);                                 // F8
                 ok = all_finite(p, C) && p[3] > 0.0f && c2 == c2;
             }
             if (!ok) { bad = l; break; }

@@ -198,63 +198,76 @@ __device__ __forceinline__ HitCov hit_cov(float mx, float my, const LayerC& ly) 
     return V;
 }
 
-// Symmetric 3x3 inverse by cofactors.  Returns false when S is not positive definite (Sylvester).
+// Symmetric positive-definite 3x3 system by LDL^T (Cholesky without square roots).  Backward stable for SPD
+// matrices, which a cofactor inverse is not: for low-pT tracks S = C_pos + V has condition number ~1e4 (predicted
+// tangential variance vs hit variance) and the 1/det-scaled rounding errors of cofactors would reach every element.
 struct Sym3 { float m00, m10, m11, m20, m21, m22; };
-__device__ __forceinline__ bool inv_sym3(const Sym3& S, Sym3& I) {
-    const float k00 = fmaf(S.m11, S.m22, -S.m21 * S.m21);
-    const float k10 = fmaf(S.m20, S.m21, -S.m10 * S.m22);
-    const float k20 = fmaf(S.m10, S.m21, -S.m20 * S.m11);
-    const float det = fmaf(S.m00, k00, fmaf(S.m10, k10, S.m20 * k20));
-    const float k22 = fmaf(S.m00, S.m11, -S.m10 * S.m10);
-    if (!(S.m00 > 0.0f) || !(k22 > 0.0f) || !(det > 0.0f)) return false;
-    const float id = 1.0f / det;
-    I.m00 = k00 * id; I.m10 = k10 * id; I.m20 = k20 * id;
-    I.m11 = fmaf(S.m00, S.m22, -S.m20 * S.m20) * id;
-    I.m21 = fmaf(S.m10, S.m20, -S.m00 * S.m21) * id;
-    I.m22 = k22 * id;
+struct Ldl3 { float l10, l20, l21, i0, i1, i2; };
+
+__device__ __forceinline__ bool ldl3(const Sym3& S, Ldl3& F) {
+    if (!(S.m00 > 0.0f)) return false;
+    F.i0 = 1.0f / S.m00;
+    F.l10 = S.m10 * F.i0;
+    F.l20 = S.m20 * F.i0;
+    const float d1 = fmaf(-F.l10, S.m10, S.m11);
+    if (!(d1 > 0.0f)) return false;
+    F.i1 = 1.0f / d1;
+    const float t21 = fmaf(-F.l20, S.m10, S.m21);
+    F.l21 = t21 * F.i1;
+    const float d2 = fmaf(-F.l21, t21, fmaf(-F.l20, S.m20, S.m22));
+    if (!(d2 > 0.0f)) return false;
+    F.i2 = 1.0f / d2;
     return true;
 }
 
-// Innovation of hit m against the predicted (p, C): S^-1 and chi2.  r = m - p[0:3].
+// x = S^-1 b
+__device__ __forceinline__ void ldl3_solve(const Ldl3& F, float b0, float b1, float b2, float& x0, float& x1, float& x2) {
+    const float y1 = fmaf(-F.l10, b0, b1);
+    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, b0, b2));
+    x2 = y2 * F.i2;
+    x1 = fmaf(-F.l21, x2, y1 * F.i1);
+    x0 = fmaf(-F.l20, x2, fmaf(-F.l10, x1, b0 * F.i0));
+}
+
+// Innovation of hit m against the predicted (p, C): factor S = C_pos + V, r = m - p[0:3], chi2 = r^T S^-1 r.
 __device__ __forceinline__ bool innovation(const float (&p)[6], const float (&C)[21], float mx, float my, float mz,
-                                           const LayerC& ly, Sym3& Si, float (&r)[3], float& chi2) {
-    const HitCov V = hit_cov(mx, my, ly);
+                                           const HitCov& V, Ldl3& F, float (&r)[3], float& chi2) {
     Sym3 S;
     S.m00 = C[pk(0, 0)] + V.xx; S.m10 = C[pk(1, 0)] + V.xy; S.m11 = C[pk(1, 1)] + V.yy;
     S.m20 = C[pk(2, 0)]; S.m21 = C[pk(2, 1)]; S.m22 = C[pk(2, 2)] + V.zz;
-    if (!inv_sym3(S, Si)) return false;
+    if (!ldl3(S, F)) return false;
     r[0] = mx - p[0]; r[1] = my - p[1]; r[2] = mz - p[2];
-    const float t0 = fmaf(Si.m00, r[0], fmaf(Si.m10, r[1], Si.m20 * r[2]));
-    const float t1 = fmaf(Si.m10, r[0], fmaf(Si.m11, r[1], Si.m21 * r[2]));
-    const float t2 = fmaf(Si.m20, r[0], fmaf(Si.m21, r[1], Si.m22 * r[2]));
-    chi2 = fmaf(r[0], t0, fmaf(r[1], t1, r[2] * t2));
+    const float y1 = fmaf(-F.l10, r[0], r[1]);
+    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, r[0], r[2]));
+    chi2 = fmaf(r[0] * r[0], F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
     return true;
 }
 
-// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C -= K C[0:3,:].
-__device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], const Sym3& Si, const float (&r)[3]) {
+// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C <- C - K C[0:3,:].
+// The columns that touch the measured block are written in the algebraically identical, cancellation-free form
+//   (C - K H C) H^T = C H^T - K (S - V) = K V          (because K S = C H^T),
+// which matters in fp32: for low-pT tracks at shallow incidence the predicted position variance exceeds the hit
+// variance by 1e3-1e4 and C - K C would lose every significant digit of the updated position block.
+__device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], const Ldl3& F, const HitCov& V,
+                                            const float (&r)[3]) {
     float K[6][3];
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        const float ci0 = C[pk(i, 0)], ci1 = C[pk(i, 1)], ci2 = C[pk(i, 2)];
-        K[i][0] = fmaf(ci0, Si.m00, fmaf(ci1, Si.m10, ci2 * Si.m20));
-        K[i][1] = fmaf(ci0, Si.m10, fmaf(ci1, Si.m11, ci2 * Si.m21));
-        K[i][2] = fmaf(ci0, Si.m20, fmaf(ci1, Si.m21, ci2 * Si.m22));
-    }
+    for (int i = 0; i < 6; ++i) ldl3_solve(F, C[pk(i, 0)], C[pk(i, 1)], C[pk(i, 2)], K[i][0], K[i][1], K[i][2]);
 #pragma unroll
     for (int i = 0; i < 6; ++i) p[i] = fmaf(K[i][0], r[0], fmaf(K[i][1], r[1], fmaf(K[i][2], r[2], p[i])));
-    // rows in decreasing order so that C[0:3,:] (rows 0..2 of the old matrix) is still intact when it is read:
-    // element (i,j), j <= i, needs old C[k][j] for k < 3, i.e. packed entries of rows <= max(2, j) <= i.
-    float P[3][6];   // old C[k][j], k < 3, all j
+    // momentum block (rows/cols 3..5): C_ab -= sum_k K_ak C_kb, with the still-intact old C[b][k]
 #pragma unroll
-    for (int k = 0; k < 3; ++k)
+    for (int a = 3; a < 6; ++a)
 #pragma unroll
-        for (int j = 0; j < 6; ++j) P[k][j] = C[pk(k, j)];
+        for (int b = 3; b <= a; ++b)
+            C[pk(a, b)] = fmaf(-K[a][0], C[pk(b, 0)], fmaf(-K[a][1], C[pk(b, 1)], fmaf(-K[a][2], C[pk(b, 2)], C[pk(a, b)])));
+    // columns 0..2: K V
 #pragma unroll
-    for (int i = 0; i < 6; ++i)
-#pragma unroll
-        for (int j = 0; j <= i; ++j)
-            C[pk(i, j)] = fmaf(-K[i][0], P[0][j], fmaf(-K[i][1], P[1][j], fmaf(-K[i][2], P[2][j], C[pk(i, j)])));
+    for (int i = 0; i < 6; ++i) {
+        C[pk(i, 0)] = fmaf(K[i][0], V.xx, K[i][1] * V.xy);
+        if (i >= 1) C[pk(i, 1)] = fmaf(K[i][0], V.xy, K[i][1] * V.yy);
+        if (i >= 2) C[pk(i, 2)] = K[i][2] * V.zz;
+    }
 }
 
 __device__ __forceinline__ float wrap_phi(float a) {
