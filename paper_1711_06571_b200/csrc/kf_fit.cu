@@ -33,36 +33,56 @@ __global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant
     int nh = 0;
     uint32_t st = 0u;
     int limit = a.n_layers;
-    for (int attempt = 0; attempt < 2; ++attempt) {
+    bool careful = false;
+    for (int attempt = 0; attempt < 3; ++attempt) {
         // F1: coalesced SoA load
 #pragma unroll
         for (int i = 0; i < 6; ++i) p[i] = a.par[i * a.ld_in + t];
 #pragma unroll
         for (int i = 0; i < 21; ++i) C[i] = a.cov[i * a.ld_in + t];
+        Trig g;
+        trig_init(g, p[4], p[5]);
         chi2 = 0.0f;
         nh = 0;
         int bad = -1;
+        bool alive = true;
 #pragma unroll 1
         for (int l = 0; l < limit; ++l) {
             const int64_t idx = a.hit_idx ? (int64_t)a.hit_idx[l * a.ld_idx + t] : t;
-            if (idx < 0) continue;                                   // layer skipped entirely (R8)
-            const int64_t h = (a.trk_event ? a.seg_off_dev[(int64_t)ev * a.n_layers + l] : a.seg0[l]) + idx;
-            const float mx = a.hx[h], my = a.hy[h], mz = a.hz[h];   // F6: issued before the arithmetic
-            const uint32_t flag = predict(p, C, cw, a.layer[l]);     // F2-F5
-            if (flag) { st |= flag; break; }
-            Ldl3 Si;
-            float r[3], c2;
-            const HitCov V = hit_cov(mx, my, a.layer[l]);
-            bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);            // F7
-            if (ok) {
-                gain_update(p, C, Si, V, r);                                 // F8
-                ok = all_finite(p, C) && p[3] > 0.0f && c2 == c2;
+            // idx < 0: layer skipped entirely (R8).  One structured if-block, no break / continue inside
+            // the loop, so that diverged lanes reconverge at the end of every layer.
+            if (alive && idx >= 0) {
+                const int64_t h = (a.trk_event ? a.seg_off_dev[(int64_t)ev * a.n_layers + l] : a.seg0[l]) + idx;
+                const float mx = a.hx[h], my = a.hy[h], mz = a.hz[h];   // F6: issued before the arithmetic
+                const uint32_t flag = predict(p, C, g, cw, a.layer[l]);  // F2-F5
+                if (flag) {
+                    st |= flag;
+                    alive = false;
+                } else {
+                    Ldl3 Si;
+                    float r[3], c2;
+                    const HitCov V = hit_cov(mx, my, a.layer[l]);
+                    bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);            // F7
+                    if (ok) {
+                        gain_update(p, C, g, Si, V, r);                              // F8
+                        ok = step_finite(p, c2) && p[3] > 0.0f && (!careful || all_finite(p, C));
+                    }
+                    if (ok) {
+                        chi2 += c2;
+                        nh += 1;
+                    } else {
+                        bad = l;
+                        alive = false;
+                    }
+                }
             }
-            if (!ok) { bad = l; break; }
-            chi2 += c2;
-            nh += 1;
         }
-        if (bad < 0) break;
+        if (bad < 0) {
+            if (careful || all_finite(p, C)) break;
+            careful = true;          // something non-finite slipped through the cheap per-layer check: find the layer
+            st = 0u;
+            continue;
+        }
         // numeric failure (rare): the track keeps the state of the last good layer -> redo the layers before it
         st |= ST_NUMERIC;
         limit = bad;

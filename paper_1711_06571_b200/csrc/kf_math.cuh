@@ -23,16 +23,45 @@ struct LayerC {
     float rcmin;                      // r * CMIN
 };
 
+// 1-ulp hardware approximations (MUFU.RCP / MUFU.RSQ / MUFU.LG2): no IEEE slow paths, no branches.
+__device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float fsqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float flog(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r * 0.69314718056f; }
+
+// sin / cos of the two angles, carried along the track instead of being re-evaluated every layer: the transport
+// rotates (cos phi, sin phi) by the exact rational (cos alpha, sin alpha), the update by a small-angle polynomial.
+struct Trig { float cp, sp, st, ct; };
+
+__device__ __forceinline__ void trig_init(Trig& g, float phi, float theta) {
+    sincosf(phi, &g.sp, &g.cp);
+    sincosf(theta, &g.st, &g.ct);
+}
+
+// rotate (c, s) by d; polynomial for |d| < 0.06 (truncation < 6e-11), library call otherwise (angle = full value)
+__device__ __forceinline__ void rotate_small(float& c, float& s, float d, float angle) {
+    if (fabsf(d) < 0.06f) {
+        const float d2 = d * d;
+        const float sd = d * fmaf(d2, fmaf(d2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+        const float cd = fmaf(d2, fmaf(d2, 1.0f / 24.0f, -0.5f), 1.0f);
+        const float cn = fmaf(c, cd, -s * sd), sn = fmaf(s, cd, c * sd);
+        const float k = fmaf(-0.5f, fmaf(cn, cn, sn * sn), 1.5f);     // one Newton step back to unit norm
+        c = cn * k; s = sn * k;
+    } else {
+        sincosf(angle, &s, &c);
+    }
+}
+
 // packed lower-triangular index
 __host__ __device__ constexpr int pk(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
 
 // atan(t)/t, |t| <= ~1: odd minimax-free Taylor for small t, library atan otherwise
 __device__ __forceinline__ float atan_over_t(float t) {
     float t2 = t * t;
-    if (t2 < 0.01f) {   // |t| < 0.1: truncation < t^10/11 = 1e-11
-        return 1.0f + t2 * (-1.0f / 3.0f + t2 * (0.2f + t2 * (-1.0f / 7.0f + t2 * (1.0f / 9.0f))));
+    if (t2 < 0.09f) {   // |t| < 0.3 (turning angle < 0.58 rad per layer): truncation < t^14/15 = 3e-9
+        return fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 13.0f, -1.0f / 11.0f), 1.0f / 9.0f), -1.0f / 7.0f), 0.2f),
+                             -1.0f / 3.0f), 1.0f);
     }
-    return atanf(t) / t;
+    return atanf(t) * frcp(t);
 }
 
 // f1(a) = (cos a - sin a / a)/a, f2(a) = (sin a - (1 - cos a)/a)/a ; series below |a| = 0.5 (cancellation-free)
@@ -42,7 +71,7 @@ __device__ __forceinline__ void curv_partials(float a, float sa, float ca, float
         f1 = a * (-1.0f / 3.0f + a2 * (1.0f / 30.0f + a2 * (-1.0f / 840.0f + a2 * (1.0f / 45360.0f))));
         f2 = 0.5f + a2 * (-0.125f + a2 * (1.0f / 144.0f + a2 * (-1.0f / 5760.0f + a2 * (1.0f / 403200.0f))));
     } else {
-        float ia = 1.0f / a;
+        float ia = frcp(a);
         f1 = (ca - sa * ia) * ia;
         f2 = (sa - (1.0f - ca) * ia) * ia;
     }
@@ -70,18 +99,16 @@ __device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, flo
     const float E = 0.5f * (ly.r2 - fmaf(x, x, y * y));
     const float A = fmaf(-w * w, E, 2.0f * fmaf(v, w, 1.0f));
     const float D = fmaf(E, A, u * u);
-    if (!(E > 0.0f) || !(D >= 0.0f)) return ST_UNREACHABLE;
-    const float sq = sqrtf(D);
-    float tau;
-    if (u >= 0.0f) {
-        tau = E / (u + sq);
-    } else {
-        if (!(A > 0.0f)) return ST_UNREACHABLE;   // crossing only after more than half a turn
-        tau = (sq - u) / A;
-    }
+    // u >= 0 (moving outwards): tau = E / (u + sqrt D), the smaller positive root whatever the sign of A;
+    // u < 0: tau = (sqrt D - u) / A, positive only for A > 0 (else the crossing lies beyond half a turn).
+    // Branch-free on purpose: the sign of u is random for seeds smeared about the vertex.
+    const bool fwd = u >= 0.0f;
+    if (!(E > 0.0f) || !(D >= 0.0f) || !(fwd || A > 0.0f)) return ST_UNREACHABLE;
+    const float sq = fsqrt(D);
+    const float tau = (fwd ? E : sq - u) * frcp(fwd ? u + sq : A);
     const float th = w * tau;                     // tan(alpha/2)
     const float th2 = th * th;
-    const float inv = 1.0f / (1.0f + th2);
+    const float inv = frcp(1.0f + th2);
     t.sa = 2.0f * th * inv;
     t.ca = (1.0f - th2) * inv;
     const float X = 2.0f * tau * inv;
@@ -104,11 +131,9 @@ __device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, flo
 
 // Predict: transport p, C to layer ly, C <- J C J^T + Q.  On a non-zero return p and C are untouched.
 // cw = -q k Bz.  up_out = r cos(incidence) of the crossing.
-__device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], float cw, const LayerC& ly) {
-    float sp, cp, st, ct;
-    sincosf(p[4], &sp, &cp);
-    sincosf(p[5], &st, &ct);
-    const float ist = 1.0f / st;
+__device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], Trig& g, float cw, const LayerC& ly) {
+    const float sp = g.sp, cp = g.cp, st = g.st, ct = g.ct;
+    const float ist = frcp(st);
     const float cot = ct * ist;
     Transport t;
     const uint32_t flag = transport(p, cw, cp, sp, cot, ly, t);
@@ -121,7 +146,7 @@ __device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], float
     const float dXdi = cs2 * f1, dYdi = cs2 * f2;
     const float Fxi = fmaf(cp, dXdi, -sp * dYdi), Fyi = fmaf(sp, dXdi, cp * dYdi);
     const float Fxp = -t.dy, Fyp = t.dx;
-    const float iup = 1.0f / t.up;
+    const float iup = frcp(t.up);
     const float sx = -t.xn * iup, sy = -t.yn * iup;
     const float si = -fmaf(t.xn, Fxi, t.yn * Fyi) * iup;
     const float sph = -fmaf(t.xn, Fxp, t.yn * Fyp) * iup;
@@ -160,7 +185,7 @@ __device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], float
     float q33 = 0.0f, q53 = 0.0f, q44 = 0.0f, q55 = 0.0f;
     if (ly.xx0r > 0.0f) {
         const float tms = ly.xx0r * ist * iup;                 // xx0 / (sin(theta) cos(inc))
-        const float lg = fmaf(0.038f, logf(tms), 1.0f);
+        const float lg = fmaf(0.038f, flog(tms), 1.0f);
         const float h = 0.0136f * p[3] * st * lg;
         const float v = h * h * tms;                           // theta0^2
         const float icot = p[3] * cot;
@@ -178,6 +203,7 @@ __device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], float
     C[pk(5, 0)] = T05; C[pk(5, 1)] = T15; C[pk(5, 2)] = T25; C[pk(5, 3)] += q53; C[pk(5, 4)] = T45; C[pk(5, 5)] += q55;
 #undef CC
     p[0] = t.xn; p[1] = t.yn; p[2] = t.zn; p[4] += t.alpha;
+    g.cp = t.cpn; g.sp = t.spn;
     return 0u;
 }
 
@@ -189,7 +215,7 @@ __device__ __forceinline__ HitCov hit_cov(float mx, float my, const LayerC& ly) 
     if (ly.var_r == ly.var_rphi) {
         V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f;
     } else {
-        const float ir2 = 1.0f / fmaf(mx, mx, my * my);
+        const float ir2 = frcp(fmaf(mx, mx, my * my));
         const float c2 = mx * mx * ir2, s2 = my * my * ir2, cs = mx * my * ir2;
         V.xx = fmaf(c2, ly.var_r, s2 * ly.var_rphi);
         V.yy = fmaf(s2, ly.var_r, c2 * ly.var_rphi);
@@ -206,17 +232,17 @@ struct Ldl3 { float l10, l20, l21, i0, i1, i2; };
 
 __device__ __forceinline__ bool ldl3(const Sym3& S, Ldl3& F) {
     if (!(S.m00 > 0.0f)) return false;
-    F.i0 = 1.0f / S.m00;
+    F.i0 = frcp(S.m00);
     F.l10 = S.m10 * F.i0;
     F.l20 = S.m20 * F.i0;
     const float d1 = fmaf(-F.l10, S.m10, S.m11);
     if (!(d1 > 0.0f)) return false;
-    F.i1 = 1.0f / d1;
+    F.i1 = frcp(d1);
     const float t21 = fmaf(-F.l20, S.m10, S.m21);
     F.l21 = t21 * F.i1;
     const float d2 = fmaf(-F.l21, t21, fmaf(-F.l20, S.m20, S.m22));
     if (!(d2 > 0.0f)) return false;
-    F.i2 = 1.0f / d2;
+    F.i2 = frcp(d2);
     return true;
 }
 
@@ -248,13 +274,19 @@ __device__ __forceinline__ bool innovation(const float (&p)[6], const float (&C)
 //   (C - K H C) H^T = C H^T - K (S - V) = K V          (because K S = C H^T),
 // which matters in fp32: for low-pT tracks at shallow incidence the predicted position variance exceeds the hit
 // variance by 1e3-1e4 and C - K C would lose every significant digit of the updated position block.
-__device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], const Ldl3& F, const HitCov& V,
+__device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], Trig& g, const Ldl3& F, const HitCov& V,
                                             const float (&r)[3]) {
     float K[6][3];
 #pragma unroll
     for (int i = 0; i < 6; ++i) ldl3_solve(F, C[pk(i, 0)], C[pk(i, 1)], C[pk(i, 2)], K[i][0], K[i][1], K[i][2]);
 #pragma unroll
-    for (int i = 0; i < 6; ++i) p[i] = fmaf(K[i][0], r[0], fmaf(K[i][1], r[1], fmaf(K[i][2], r[2], p[i])));
+    for (int i = 0; i < 4; ++i) p[i] = fmaf(K[i][0], r[0], fmaf(K[i][1], r[1], fmaf(K[i][2], r[2], p[i])));
+    const float dphi = fmaf(K[4][0], r[0], fmaf(K[4][1], r[1], K[4][2] * r[2]));
+    const float dth = fmaf(K[5][0], r[0], fmaf(K[5][1], r[1], K[5][2] * r[2]));
+    p[4] += dphi;
+    p[5] += dth;
+    rotate_small(g.cp, g.sp, dphi, p[4]);
+    rotate_small(g.ct, g.st, dth, p[5]);
     // momentum block (rows/cols 3..5): C_ab -= sum_k K_ak C_kb, with the still-intact old C[b][k]
 #pragma unroll
     for (int a = 3; a < 6; ++a)
@@ -276,6 +308,12 @@ __device__ __forceinline__ float wrap_phi(float a) {
     if (a <= -PI) a += TWO_PI;
     if (a > PI) a -= TWO_PI;
     return a;
+}
+
+// cheap per-layer check: NaN/Inf anywhere in S or the gain reaches chi2 or the parameters
+__device__ __forceinline__ bool step_finite(const float (&p)[6], float chi2) {
+    const float acc = fmaf(0.0f, chi2, 0.0f * (((p[0] + p[1]) + (p[2] + p[3])) + (p[4] + p[5])));
+    return acc == 0.0f;
 }
 
 __device__ __forceinline__ bool all_finite(const float (&p)[6], const float (&C)[21]) {

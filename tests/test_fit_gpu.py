@@ -35,10 +35,13 @@ def run_ref(fi, idx=None):
                  fi.q[idx], hx, hy, hz, np.arange(L + 1) * m, hi)
 
 
-def check(g, r, min_frac_strict=0.999):
-    assert np.array_equal(g["nhits"], r["nhits"])
-    assert np.array_equal(g["status"], r["status"])
-    rep = compare_tracks(g, r, sel=r["nhits"] > 0)
+def check(g, r, min_frac_strict=0.999, max_decision_mismatch=0.0):
+    """Discrete decisions (which layers were used, status bits) must agree; `max_decision_mismatch` is the fraction of
+    tracks allowed to differ where the inputs sit on a reachability / grazing threshold (reading A16) --
+    zero for the BASELINE configs.  Values are compared on the agreeing tracks."""
+    same = (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
+    assert (~same).sum() <= max_decision_mismatch * len(same), int((~same).sum())
+    rep = compare_tracks(g, r, sel=(r["nhits"] > 0) & same)
     print(rep)
     assert rep["mom_viol"] == 0 and rep["pos_viol"] == 0 and rep["cov_viol"] == 0 and rep["chi2_viol"] == 0, rep
     assert rep["strict_pos_viol"] <= (1 - min_frac_strict) * rep["n"], rep
@@ -75,12 +78,21 @@ def test_fit_explicit_index_equals_identity():
 
 
 def test_fit_stops_and_flags():
-    """Last layer moved out of reach for low pT: status bit 0, state frozen after 9 layers; same decisions as the oracle."""
+    """Last layer moved out to R = 400 cm: unreachable for 2 rho < 400 cm (pT < 2.28 GeV).  Those tracks must carry
+    status bit 0 and the state frozen after 9 layers, with the same decisions as the oracle.  (Tracks that do reach
+    R = 400 are updated with a hit that is not on their helix; only their decision bits are compared.)"""
     fi = synth.fit_inputs(0, n=5000)
     fi.geom.r[9] = 400.0
+    fi.geom.zmax[9] = 4000.0
     g, r = run_gpu(fi), run_ref(fi)
-    assert (r["status"] & o.UNREACHABLE).any() and (r["status"] == 0).any()
-    check(g, r)
+    stopped = (r["status"] & o.UNREACHABLE) != 0
+    assert stopped.sum() > 500 and (r["status"] == 0).sum() > 500
+    same = (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
+    assert (~same).sum() <= 2e-3 * len(same)      # 2 rho within rounding of 400 cm: reading A16
+    sel = stopped & same
+    assert (r["nhits"][sel] == 9).all()
+    rep = compare_tracks(g, r, sel=sel)
+    assert rep["mom_viol"] == 0 and rep["pos_viol"] == 0 and rep["cov_viol"] == 0 and rep["chi2_viol"] == 0, rep
 
 
 def test_fit_in_place():
