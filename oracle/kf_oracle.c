@@ -386,3 +386,296 @@ int kfo_fit(int n_layers, const double* layers, double bz, int64_t n, int64_t ld
     }
     return 0;
 }
+
+/* =====================================================================================================
+ * Hit binning, window lookup, combinatorial building (sec. 2, L54 sec. 3.1, L82-88 sec. 4.3).
+ * The X-series is specified in IEEE fp32 so that CPU and GPU agree bit for bit: every
+ * float expression below is a single rounded operation (this file is compiled with -ffp-contract=off).
+ * ===================================================================================================== */
+
+/* X1 table: T[k] = fl32(tan(2 pi k / N)), k = 0 .. N/8, T[N/8] := 1 */
+void kfo_tan_table(int n_phi, float* tab) {
+    int m = n_phi / 8;
+    for (int k = 0; k < m; ++k) tab[k] = (float)tan(2.0 * KFO_PI * (double)k / (double)n_phi);
+    tab[m] = 1.0f;
+}
+
+/* X1: azimuthal bin of (x, y) from exact fp32 comparisons, no atan2 */
+int kfo_phi_bin(float x, float y, int n_phi, const float* tab) {
+    float ax = fabsf(x), ay = fabsf(y);
+    int swap = ay > ax;
+    float lo = swap ? ax : ay, hi = swap ? ay : ax;
+    float t = (hi > 0.0f) ? lo / hi : 0.0f;
+    int m = n_phi / 8;
+    int j = 0; /* largest k <= m-1 with tab[k] <= t; tab[0] = 0 <= t */
+    for (int k = 1; k < m; ++k)
+        if (tab[k] <= t) j = k;
+    int a = swap ? n_phi / 4 - 1 - j : j;
+    if (x >= 0.0f) return (y >= 0.0f) ? a : n_phi - 1 - a;
+    return (y >= 0.0f) ? n_phi / 2 - 1 - a : n_phi / 2 + a;
+}
+
+/* X2: z bin */
+int kfo_z_bin(float z, float zmax, int n_z) {
+    float inv_dz = (float)n_z / (2.0f * zmax);
+    float f = floorf((z + zmax) * inv_dz);
+    int iz = (f >= (float)n_z) ? n_z - 1 : (f < 0.0f ? 0 : (int)f);
+    return iz;
+}
+
+/* B0: sorted order = ascending (global bin, original index).  seg_off [n_events*L + 1]; outputs sx, sy, sz,
+ * perm [n_hits] (sorted position -> original index within the segment), bin_off [n_events*L*n_z*n_phi + 1]. */
+int kfo_bin_hits(int n_layers, const double* layers, int n_events, const int64_t* seg_off, const float* hx,
+                 const float* hy, const float* hz, int n_phi, int n_z, float* sx, float* sy, float* sz, int32_t* perm,
+                 int32_t* bin_off) {
+    float* tab = (float*)malloc((size_t)(n_phi / 8 + 1) * sizeof(float));
+    kfo_tan_table(n_phi, tab);
+    int64_t nseg = (int64_t)n_events * n_layers;
+    int64_t bins_per_seg = (int64_t)n_phi * n_z;
+    int64_t n_hits = seg_off[nseg];
+    bin_off[0] = 0;
+    int32_t* key = (int32_t*)malloc((size_t)(n_hits > 0 ? n_hits : 1) * sizeof(int32_t));
+    for (int64_t sg = 0; sg < nseg; ++sg) {
+        int l = (int)(sg % n_layers);
+        float zmax = (float)LZMAX(layers, l);
+        int32_t* cnt = (int32_t*)calloc((size_t)bins_per_seg + 1, sizeof(int32_t));
+        for (int64_t h = seg_off[sg]; h < seg_off[sg + 1]; ++h) {
+            int b = kfo_z_bin(hz[h], zmax, n_z) * n_phi + kfo_phi_bin(hx[h], hy[h], n_phi, tab);
+            key[h] = b;
+            cnt[b + 1] += 1;
+        }
+        for (int64_t b = 0; b < bins_per_seg; ++b) cnt[b + 1] += cnt[b];
+        for (int64_t b = 0; b < bins_per_seg; ++b) bin_off[sg * bins_per_seg + b + 1] = (int32_t)(seg_off[sg] + cnt[b + 1]);
+        for (int64_t h = seg_off[sg]; h < seg_off[sg + 1]; ++h) { /* stable: ascending original index within a bin */
+            int64_t pos = seg_off[sg] + cnt[key[h]]++;
+            sx[pos] = hx[h]; sy[pos] = hy[h]; sz[pos] = hz[h];
+            perm[pos] = (int32_t)(h - seg_off[sg]);
+        }
+        free(cnt);
+    }
+    free(key);
+    free(tab);
+    return 0;
+}
+
+/* X3: window (phi_c +- dphi, z_c +- dz) -> first phi bin, number of phi bins (wrapping), z rows [iz_lo, iz_hi] */
+void kfo_window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, int n_phi, int n_z, int* first, int* n_b,
+                     int* iz_lo, int* iz_hi) {
+    float inv_dphi = (float)((double)n_phi / (2.0 * KFO_PI));
+    float f_lo = (phi_c - dphi) * inv_dphi, f_hi = (phi_c + dphi) * inv_dphi;
+    int b_lo = (int)floorf(f_lo), b_hi = (int)floorf(f_hi);
+    int nb = b_hi - b_lo + 1;
+    if (nb > n_phi) nb = n_phi;
+    if (nb < 0) nb = 0;
+    *n_b = nb;
+    *first = ((b_lo % n_phi) + n_phi) % n_phi;
+    *iz_lo = kfo_z_bin(z_c - dz, zmax, n_z);
+    *iz_hi = kfo_z_bin(z_c + dz, zmax, n_z);
+}
+
+/* kf_window_lookup_ref: bin-granular hit list of each query (rows ascending, bins ascending with wrap, hits in
+ * sorted order).  count[i] = full length; sorted_idx[i*cap + j] for j < min(count, cap). */
+int kfo_window_lookup(int n_layers, const double* layers, int n_phi, int n_z, const int32_t* bin_off, int64_t n_query,
+                      const int32_t* event, const int32_t* layer, const float* phi_c, const float* dphi,
+                      const float* z_c, const float* dz, int cap, int32_t* count, int32_t* sorted_idx) {
+    for (int64_t i = 0; i < n_query; ++i) {
+        int first, nb, z0, z1;
+        kfo_window_bins(phi_c[i], dphi[i], z_c[i], dz[i], (float)LZMAX(layers, layer[i]), n_phi, n_z, &first, &nb, &z0, &z1);
+        int64_t seg = (int64_t)event[i] * n_layers + layer[i];
+        int32_t c = 0;
+        for (int iz = z0; iz <= z1; ++iz)
+            for (int k = 0; k < nb; ++k) {
+                int64_t b = (seg * n_z + iz) * n_phi + (first + k) % n_phi;
+                for (int32_t h = bin_off[b]; h < bin_off[b + 1]; ++h) {
+                    if (c < cap) sorted_idx[i * cap + c] = h;
+                    ++c;
+                }
+            }
+        count[i] = c;
+    }
+    return 0;
+}
+
+/* ---- combinatorial building (R10, R11) ---- */
+typedef struct {
+    double p[6], C[36], chi2;
+    int nhits, finished;
+    uint32_t status;
+    int32_t hits[32];
+} kfo_cand;
+
+typedef struct {
+    int parent, kind; /* kind 0 = hit child, 1 = no compatible hit (-1), 2 = finished (-2) */
+    int64_t hitpos;   /* global sorted position; INT64_MAX for kinds 1, 2 */
+    double chi2;
+    int nhits;
+} kfo_child;
+
+static int child_cmp(const void* a_, const void* b_) {
+    const kfo_child *a = (const kfo_child*)a_, *b = (const kfo_child*)b_;
+    if (a->nhits != b->nhits) return a->nhits > b->nhits ? -1 : 1;
+    if (a->chi2 != b->chi2) return a->chi2 < b->chi2 ? -1 : 1;
+    if (a->parent != b->parent) return a->parent < b->parent ? -1 : 1;
+    if (a->hitpos != b->hitpos) return a->hitpos < b->hitpos ? -1 : 1;
+    return 0;
+}
+
+/* kf_build_ref.  Hits are the SORTED arrays of kfo_bin_hits (float), perm / bin_off alike.  Seeds: par [6][ld_seed],
+ * cov dense [36][ld_seed], chi2_in (NULL = 0), seed_hit_idx [first_layer][ld_seed].  use_bins = 0 scans every hit of
+ * the layer's segment (brute force without the spatial index, pin P12).
+ * Outputs, slot = s*K + k: par_o [6][ld_out], cov_o [36][ld_out], chi2_o, nhits_o, status_o [n_seeds*K],
+ * hit_idx_o [n_layers][ld_out], n_cand [n_seeds]; unused slots: nhits 0, chi2 0, status 0, hit_idx -2, par/cov 0.
+ * counters[8]: 0 propagations, 1 hits scanned, 2 pass strict window, 3 pass chi2 cut (hit children), 4 updates,
+ *              5 bin rows touched, 6 seed-layers, 7 children ranked. */
+int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z, const float* sx, const float* sy,
+              const float* sz, const int32_t* perm, const int32_t* bin_off, const int64_t* seg_off, int64_t n_seeds,
+              int64_t ld_seed, const double* par, const double* cov, const int8_t* q, const double* chi2_in,
+              const int32_t* seed_event, const int32_t* seed_hit_idx, int first_layer, int K, double chi2_cut,
+              double n_sigma, int use_bins, int64_t ld_out, double* par_o, double* cov_o, double* chi2_o,
+              int32_t* nhits_o, uint32_t* status_o, int32_t* hit_idx_o, int32_t* n_cand, int64_t* counters) {
+    if (K < 1 || K > 32 || n_layers > 32 || first_layer < 0 || first_layer > n_layers) return -1;
+    int64_t cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : cnt[:8])
+    for (int64_t sd = 0; sd < n_seeds; ++sd) {
+        kfo_cand* cur = (kfo_cand*)calloc((size_t)K, sizeof(kfo_cand));
+        kfo_cand* nxt = (kfo_cand*)calloc((size_t)K, sizeof(kfo_cand));
+        double(*pp)[6] = malloc((size_t)K * sizeof *pp);
+        double(*Cp)[36] = malloc((size_t)K * sizeof *Cp);
+        uint32_t* pflag = (uint32_t*)malloc((size_t)K * sizeof(uint32_t));
+        size_t cap_ch = 256, n_ch = 0;
+        kfo_child* ch = (kfo_child*)malloc(cap_ch * sizeof(kfo_child));
+        int ev = seed_event ? seed_event[sd] : 0;
+        int nc = 1;
+        for (int i = 0; i < 6; ++i) cur[0].p[i] = par[i * ld_seed + sd];
+        for (int i = 0; i < 36; ++i) cur[0].C[i] = cov[i * ld_seed + sd];
+        cur[0].chi2 = chi2_in ? chi2_in[sd] : 0.0;
+        cur[0].nhits = first_layer;
+        for (int l = 0; l < 32; ++l) cur[0].hits[l] = -2;
+        for (int l = 0; l < first_layer; ++l) cur[0].hits[l] = seed_hit_idx ? seed_hit_idx[(int64_t)l * ld_seed + sd] : -1;
+
+        for (int l = first_layer; l < n_layers; ++l) {
+            const double R = LR(layers, l), zmax = LZMAX(layers, l);
+            const double srphi = LSRPHI(layers, l), szz = LSZ(layers, l), sr = LSR(layers, l);
+            const int64_t seg = (int64_t)ev * n_layers + l;
+            n_ch = 0;
+            cnt[6] += 1;
+            for (int c = 0; c < nc; ++c) {
+                kfo_child pass = {c, 2, INT64_MAX, cur[c].chi2, cur[c].nhits};
+                pflag[c] = 0;
+                int f = cur[c].finished ? -1 : predict(layers, l, bz, cur[c].p, cur[c].C, q[sd], pp[c], Cp[c]);
+                if (!cur[c].finished) cnt[0] += 1;
+                double dphi = 0, dzw = 0;
+                if (f == 0) { /* window (R11) */
+                    const double x = pp[c][0], y = pp[c][1], r2 = x * x + y * y;
+                    double varphi = (x * x * Cp[c][1 * 6 + 1] - 2.0 * x * y * Cp[c][0 * 6 + 1] + y * y * Cp[c][0]) / (r2 * r2);
+                    if (varphi < 0.0) varphi = 0.0;
+                    dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R));
+                    dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz);
+                    if (!isfinite(dphi) || !isfinite(dzw)) f = KFO_NUMERIC;
+                    else if (fabs(pp[c][2]) > zmax + dzw) f = KFO_LEFT_Z;
+                }
+                if (f != 0) { /* finished (or just found unpropagatable): state unchanged */
+                    if (f > 0) pflag[c] = (uint32_t)f;
+                    if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
+                    ch[n_ch++] = pass;
+                    continue;
+                }
+                const double x = pp[c][0], y = pp[c][1], zc = pp[c][2], rp = sqrt(x * x + y * y);
+                int first = 0, nb = 1, z0 = 0, z1 = 0;
+                if (use_bins)
+                    kfo_window_bins((float)atan2(y, x), (float)dphi, (float)zc, (float)dzw, (float)zmax, n_phi, n_z, &first, &nb, &z0, &z1);
+                int n_hit_children = 0, s_bad = 0;
+                for (int iz = z0; iz <= z1 && !s_bad; ++iz) {
+                    cnt[5] += use_bins ? 1 : 0;
+                    for (int kb = 0; kb < nb && !s_bad; ++kb) {
+                        int64_t h0, h1;
+                        if (use_bins) {
+                            int64_t b = (seg * n_z + iz) * n_phi + (first + kb) % n_phi;
+                            h0 = bin_off[b]; h1 = bin_off[b + 1];
+                        } else { h0 = seg_off[seg]; h1 = seg_off[seg + 1]; }
+                        for (int64_t h = h0; h < h1; ++h) {
+                            cnt[1] += 1;
+                            const double m[3] = {sx[h], sy[h], sz[h]};
+                            const double rm = sqrt(m[0] * m[0] + m[1] * m[1]);
+                            if (!(fabs(x * m[1] - y * m[0]) <= dphi * rp * rm)) continue;
+                            if (!(x * m[0] + y * m[1] > 0.0)) continue;
+                            if (!(fabs(m[2] - zc) <= dzw)) continue;
+                            cnt[2] += 1;
+                            double c2;
+                            if (kfo_chi2(pp[c], Cp[c], m, srphi, szz, sr, &c2)) { s_bad = 1; break; }
+                            if (!(c2 < chi2_cut)) continue;
+                            cnt[3] += 1;
+                            kfo_child k = {c, 0, h, cur[c].chi2 + c2, cur[c].nhits + 1};
+                            if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
+                            ch[n_ch++] = k;
+                            ++n_hit_children;
+                        }
+                    }
+                }
+                if (s_bad) { /* S not positive definite: drop this parent's hit children, finish it */
+                    n_ch -= (size_t)n_hit_children;
+                    pflag[c] = KFO_NUMERIC;
+                    if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
+                    ch[n_ch++] = pass;
+                } else if (n_hit_children == 0) {
+                    kfo_child miss = {c, 1, INT64_MAX, cur[c].chi2, cur[c].nhits};
+                    if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
+                    ch[n_ch++] = miss;
+                }
+            }
+            cnt[7] += (int64_t)n_ch;
+            qsort(ch, n_ch, sizeof(kfo_child), child_cmp);
+            int nn = n_ch < (size_t)K ? (int)n_ch : K;
+            for (int j = 0; j < nn; ++j) {
+                const kfo_child* k = &ch[j];
+                const kfo_cand* pa = &cur[k->parent];
+                kfo_cand* o = &nxt[j];
+                *o = *pa;
+                if (k->kind == 2) {
+                    o->finished = 1;
+                    o->status |= pflag[k->parent];
+                    o->hits[l] = -2;
+                } else if (k->kind == 1) {
+                    memcpy(o->p, pp[k->parent], sizeof o->p);
+                    memcpy(o->C, Cp[k->parent], sizeof o->C);
+                    o->hits[l] = -1;
+                } else {
+                    const double m[3] = {sx[k->hitpos], sy[k->hitpos], sz[k->hitpos]};
+                    double c2;
+                    cnt[4] += 1;
+                    int f = kfo_update(pp[k->parent], Cp[k->parent], m, srphi, szz, sr, o->p, o->C, &c2);
+                    o->chi2 = k->chi2;
+                    o->nhits = k->nhits;
+                    o->hits[l] = perm[k->hitpos];
+                    if (f) { /* numerically failed update: keep the predicted state, finish the candidate */
+                        memcpy(o->p, pp[k->parent], sizeof o->p);
+                        memcpy(o->C, Cp[k->parent], sizeof o->C);
+                        o->status |= KFO_NUMERIC;
+                        o->finished = 1;
+                    }
+                }
+            }
+            kfo_cand* t = cur; cur = nxt; nxt = t;
+            nc = nn;
+        }
+        n_cand[sd] = nc;
+        for (int k = 0; k < K; ++k) {
+            int64_t slot = sd * K + k;
+            if (k < nc) {
+                const kfo_cand* c = &cur[k];
+                for (int i = 0; i < 6; ++i) par_o[i * ld_out + slot] = (i == 4) ? wrap_phi(c->p[i]) : c->p[i];
+                for (int i = 0; i < 36; ++i) cov_o[i * ld_out + slot] = c->C[i];
+                chi2_o[slot] = c->chi2; nhits_o[slot] = c->nhits; status_o[slot] = c->status;
+                for (int l = 0; l < n_layers; ++l) hit_idx_o[(int64_t)l * ld_out + slot] = c->hits[l];
+            } else {
+                for (int i = 0; i < 6; ++i) par_o[i * ld_out + slot] = 0.0;
+                for (int i = 0; i < 36; ++i) cov_o[i * ld_out + slot] = 0.0;
+                chi2_o[slot] = 0.0; nhits_o[slot] = 0; status_o[slot] = 0;
+                for (int l = 0; l < n_layers; ++l) hit_idx_o[(int64_t)l * ld_out + slot] = -2;
+            }
+        }
+        free(cur); free(nxt); free(pp); free(Cp); free(pflag); free(ch);
+    }
+    if (counters) for (int i = 0; i < 8; ++i) counters[i] = cnt[i];
+    return 0;
+}

@@ -121,3 +121,99 @@ def fit(layers, bz, par, cov21, q, hx, hy, hz, seg_off, hit_idx=None, trk_event=
                   _p(hx), _p(hy), _p(hz), _p(seg_off, C.c_int64), _p(hi, C.c_int32), _p(te, C.c_int32),
                   _p(po), _p(co), _p(c2), _p(nh, C.c_int32), _p(st, C.c_uint32))
     return dict(par=po[:, :n], cov=co[:, :n].T.reshape(n, 6, 6), chi2=c2, nhits=nh, status=st)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# binning / window lookup / building
+# ---------------------------------------------------------------------------------------------------------
+def _f(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _i(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def tan_table(n_phi):
+    tab = np.zeros(n_phi // 8 + 1, dtype=np.float32)
+    lib().kfo_tan_table(C.c_int(n_phi), _p(tab, C.c_float))
+    return tab
+
+
+def phi_bin(x, y, n_phi):
+    l = lib(); l.kfo_phi_bin.restype = C.c_int
+    tab = tan_table(n_phi)
+    x, y = _f(np.atleast_1d(x)), _f(np.atleast_1d(y))
+    return np.array([l.kfo_phi_bin(C.c_float(float(a)), C.c_float(float(b)), C.c_int(n_phi), _p(tab, C.c_float)) for a, b in zip(x, y)], dtype=np.int32)
+
+
+def z_bin(z, zmax, n_z):
+    l = lib(); l.kfo_z_bin.restype = C.c_int
+    return np.array([l.kfo_z_bin(C.c_float(float(a)), C.c_float(float(zmax)), C.c_int(n_z)) for a in _f(np.atleast_1d(z))], dtype=np.int32)
+
+
+def window_bins(phi_c, dphi, z_c, dz, zmax, n_phi, n_z):
+    """X3 -> (first phi bin, n phi bins, iz_lo, iz_hi)"""
+    a, b, c, d = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+    lib().kfo_window_bins(C.c_float(phi_c), C.c_float(dphi), C.c_float(z_c), C.c_float(dz), C.c_float(zmax), C.c_int(n_phi), C.c_int(n_z),
+                          C.byref(a), C.byref(b), C.byref(c), C.byref(d))
+    return a.value, b.value, c.value, d.value
+
+
+def bin_hits(layers, n_events, seg_off, hx, hy, hz, n_phi, n_z):
+    """kf_bin_hits_ref -> dict(x, y, z sorted f32, perm i32, bin_off i32)"""
+    layers = _d(layers); L = layers.shape[0]
+    seg_off = np.ascontiguousarray(seg_off, dtype=np.int64)
+    assert len(seg_off) == n_events * L + 1
+    hx, hy, hz = _f(hx), _f(hy), _f(hz)
+    n = int(seg_off[-1])
+    sx = np.zeros(n, np.float32); sy = np.zeros(n, np.float32); sz = np.zeros(n, np.float32)
+    perm = np.zeros(n, np.int32); bin_off = np.zeros(n_events * L * n_phi * n_z + 1, np.int32)
+    lib().kfo_bin_hits(C.c_int(L), _p(layers), C.c_int(n_events), _p(seg_off, C.c_int64), _p(hx, C.c_float), _p(hy, C.c_float), _p(hz, C.c_float),
+                       C.c_int(n_phi), C.c_int(n_z), _p(sx, C.c_float), _p(sy, C.c_float), _p(sz, C.c_float), _p(perm, C.c_int32), _p(bin_off, C.c_int32))
+    return dict(x=sx, y=sy, z=sz, perm=perm, bin_off=bin_off, n_phi=n_phi, n_z=n_z)
+
+
+def window_lookup(layers, binned, event, layer, phi_c, dphi, z_c, dz, cap):
+    layers = _d(layers)
+    event, layer = _i(event), _i(layer)
+    phi_c, dphi, z_c, dz = _f(phi_c), _f(dphi), _f(z_c), _f(dz)
+    nq = len(event)
+    count = np.zeros(nq, np.int32); idx = np.full((nq, cap), -1, np.int32)
+    lib().kfo_window_lookup(C.c_int(layers.shape[0]), _p(layers), C.c_int(binned["n_phi"]), C.c_int(binned["n_z"]), _p(binned["bin_off"], C.c_int32),
+                            C.c_int64(nq), _p(event, C.c_int32), _p(layer, C.c_int32), _p(phi_c, C.c_float), _p(dphi, C.c_float),
+                            _p(z_c, C.c_float), _p(dz, C.c_float), C.c_int(cap), _p(count, C.c_int32), _p(idx, C.c_int32))
+    return count, idx
+
+
+COUNTERS = ("n_prop", "n_scan", "n_window", "n_children", "n_upd", "n_rows", "n_seed_layers", "n_ranked")
+
+
+def kf_build(layers, bz, binned, seg_off, par, cov21, q, seed_event, seed_hit_idx, first_layer, K, chi2_cut, n_sigma,
+          chi2_in=None, use_bins=True, n=None):
+    """kf_build_ref.  -> dict(par [6][n*K], cov [n*K][6][6], chi2, nhits, status [n*K], hit_idx [L][n*K], n_cand [n], counters)"""
+    layers = _d(layers); L = layers.shape[0]
+    par = _d(par); ld = par.shape[1]
+    n = len(q) if n is None else n
+    cov = _unpack21(_d(cov21))
+    q = np.ascontiguousarray(q, dtype=np.int8)
+    seg_off = np.ascontiguousarray(seg_off, dtype=np.int64)
+    se = None if seed_event is None else _i(seed_event)
+    sh = None if seed_hit_idx is None else _i(seed_hit_idx)
+    if sh is not None:
+        assert sh.shape == (first_layer, ld)
+    ci = None if chi2_in is None else _d(chi2_in)
+    ldo = max(n * K, 1)
+    po = np.zeros((6, ldo)); co = np.zeros((36, ldo)); c2 = np.zeros(ldo); nh = np.zeros(ldo, np.int32); st = np.zeros(ldo, np.uint32)
+    hi = np.zeros((L, ldo), np.int32); nc = np.zeros(max(n, 1), np.int32); cnt = np.zeros(8, np.int64)
+    l = lib(); l.kfo_build.restype = C.c_int
+    rc = l.kfo_build(C.c_int(L), _p(layers), C.c_double(bz), C.c_int(binned["n_phi"]), C.c_int(binned["n_z"]),
+                     _p(binned["x"], C.c_float), _p(binned["y"], C.c_float), _p(binned["z"], C.c_float), _p(binned["perm"], C.c_int32),
+                     _p(binned["bin_off"], C.c_int32), _p(seg_off, C.c_int64), C.c_int64(n), C.c_int64(ld), _p(par), _p(cov), _p(q, C.c_int8),
+                     _p(ci), _p(se, C.c_int32), _p(sh, C.c_int32), C.c_int(first_layer), C.c_int(K), C.c_double(chi2_cut), C.c_double(n_sigma),
+                     C.c_int(1 if use_bins else 0), C.c_int64(ldo), _p(po), _p(co), _p(c2), _p(nh, C.c_int32), _p(st, C.c_uint32),
+                     _p(hi, C.c_int32), _p(nc, C.c_int32), _p(cnt, C.c_int64))
+    assert rc == 0, rc
+    m = n * K
+    return dict(par=po[:, :m], cov=co[:, :m].T.reshape(m, 6, 6), chi2=c2[:m], nhits=nh[:m], status=st[:m], hit_idx=hi[:, :m], n_cand=nc[:n],
+                counters=dict(zip(COUNTERS, (int(v) for v in cnt))))
