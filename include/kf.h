@@ -130,7 +130,8 @@ int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* 
  * chi2 < chi2_cut (else one child without hit), keep the best K children by (nhits desc, chi2 asc, parent slot asc,
  * sorted hit position asc), update the survivors.
  * Output: slot s*K + k of `cand` (best first), hit_idx[l*ld + slot] = original index within the segment,
- * -1 = no hit on this layer, -2 = layer not crossed (candidate finished); n_cand[s] = number of valid slots. */
+ * -1 = no hit on this layer, -2 = layer not crossed (candidate finished); n_cand[s] = number of valid slots.
+ */
 typedef struct {
     int32_t K, n_layers;
     int64_t n_seeds, ld;  /* ld >= n_seeds*K */
@@ -139,7 +140,17 @@ typedef struct {
     int32_t* n_cand;      /* [n_seeds] */
 } kf_cands;
 
+/* Seeds: state on (or near) layer first_layer-1; their chi2 / nhits inputs are ignored: every seed starts with
+ * chi2 = 0 and nhits = first_layer.  seed_event [n] (may be NULL when n_events == 1); seed_hit_idx
+ * [first_layer][seeds->ld] = hits already on the seed (copied to the output lists; NULL = -1).
+ * Slots k >= n_cand[s] get nhits = 0, chi2 = 0, status = 0 and hit_idx = -2; their par / cov are not written.
+ * cand.q is filled with the seed's charge.  A candidate that cannot be propagated to a layer, leaves
+ * |z| <= zmax + window, or fails numerically is finished (status bit set) and carried unchanged.
+ * K in 1..32.  kf_build_workspace_bytes() is 0 in this version (candidates live in shared memory); ws may be NULL.
+ * kf_build_set_lanes(g): tuning hook, lanes of a warp that cooperate on one seed (4, 8, 16, 32; 0 = automatic);
+ * the result does not depend on it. */
 size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K);
+int kf_build_set_lanes(int32_t lanes);
 int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
              float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream);

@@ -20,7 +20,7 @@ KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
 EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
-           "kf_build", "kf_last_error", "kf_version"]
+           "kf_build", "kf_build_set_lanes", "kf_last_error", "kf_version"]
 
 
 class KfError(RuntimeError):
@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
         l.kf_fit.argtypes = [C.c_void_p] * 7
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        l.kf_build_set_lanes.argtypes = [C.c_int32]
         l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = l
     return _lib
@@ -189,4 +190,93 @@ def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Track
     rc = lib().kf_fit(C.byref(geom.c), C.byref(hits.c), _ptr(hit_idx, torch.int32), _ptr(trk_event, torch.int32),
                       C.byref(sc), C.byref(oc), _stream(stream))
     _check(rc, "kf_fit")
+    return out
+
+
+class Binned:
+    """Device arrays of kf_binned, allocated by the caller (here: torch) and filled by kf_bin_hits."""
+
+    def __init__(self, n_hits: int, n_bins: int, n_phi: int, n_z: int, device="cuda"):
+        self.n_phi, self.n_z, self.n_hits = n_phi, n_z, n_hits
+        m = max(n_hits, 1)
+        self.x = torch.empty(m, dtype=torch.float32, device=device)
+        self.y = torch.empty(m, dtype=torch.float32, device=device)
+        self.z = torch.empty(m, dtype=torch.float32, device=device)
+        self.perm = torch.empty(m, dtype=torch.int32, device=device)
+        self.bin_off = torch.empty(n_bins + 1, dtype=torch.int32, device=device)
+        self.c = kf_binned(n_phi, n_z, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(), self.perm.data_ptr(), self.bin_off.data_ptr())
+
+    def to_host(self) -> dict:
+        n = self.n_hits
+        return dict(x=self.x[:n].cpu().numpy(), y=self.y[:n].cpu().numpy(), z=self.z[:n].cpu().numpy(), perm=self.perm[:n].cpu().numpy(),
+                    bin_off=self.bin_off.cpu().numpy(), n_phi=self.n_phi, n_z=self.n_z)
+
+
+def kf_bin_workspace_bytes(geom: Geom, hits: Hits, n_phi: int, n_z: int) -> int:
+    return int(lib().kf_bin_workspace_bytes(C.byref(geom.c), C.byref(hits.c), n_phi, n_z))
+
+
+def kf_bin_hits(geom: Geom, hits: Hits, n_phi: int, n_z: int, out: Binned | None = None, ws: torch.Tensor | None = None, stream=None) -> Binned:
+    """include/kf.h kf_bin_hits.  Allocates the output and the workspace with torch when not given."""
+    _require_cuda()
+    n_bins = hits.n_events * geom.n_layers * n_phi * n_z
+    if out is None:
+        out = Binned(hits.n_hits, n_bins, n_phi, n_z, hits.x.device)
+    need = kf_bin_workspace_bytes(geom, hits, n_phi, n_z)
+    if ws is None:
+        ws = torch.empty(max(need, 1), dtype=torch.uint8, device=hits.x.device)
+    rc = lib().kf_bin_hits(C.byref(geom.c), C.byref(hits.c), n_phi, n_z, C.byref(out.c), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
+    _check(rc, "kf_bin_hits")
+    out._ws = ws    # keep the workspace alive until the stream has consumed it
+    return out
+
+
+def kf_window_lookup(geom: Geom, hits: Hits, binned: Binned, event, layer, phi_c, dphi, z_c, dz, cap: int, stream=None):
+    """include/kf.h kf_window_lookup.  Query arrays are device tensors (int32 / float32).  -> (count [n], sorted_idx [n, cap])"""
+    _require_cuda()
+    n = int(event.numel())
+    count = torch.zeros(max(n, 1), dtype=torch.int32, device=event.device)[:n]
+    idx = torch.full((max(n, 1), max(cap, 1)), -1, dtype=torch.int32, device=event.device)
+    rc = lib().kf_window_lookup(C.byref(geom.c), C.byref(hits.c), C.byref(binned.c), n, _ptr(event, torch.int32), _ptr(layer, torch.int32),
+                                _ptr(phi_c, torch.float32), _ptr(dphi, torch.float32), _ptr(z_c, torch.float32), _ptr(dz, torch.float32),
+                                cap, C.c_void_p(count.data_ptr()), C.c_void_p(idx.data_ptr()), _stream(stream))
+    _check(rc, "kf_window_lookup")
+    return count, idx[:n, :cap]
+
+
+class Cands:
+    """Device arrays of kf_cands: n_seeds*K candidate slots (slot s*K + k, best first)."""
+
+    def __init__(self, n_seeds: int, K: int, n_layers: int, device="cuda"):
+        self.n_seeds, self.K, self.n_layers = n_seeds, K, n_layers
+        n = n_seeds * K
+        self.tracks = Tracks.empty(n, None, device)
+        self.ld = self.tracks.ld
+        self.hit_idx = torch.empty((n_layers, self.ld), dtype=torch.int32, device=device)
+        self.n_cand = torch.zeros(max(n_seeds, 1), dtype=torch.int32, device=device)[:n_seeds]
+        self.c = kf_cands(K, n_layers, n_seeds, self.ld, self.tracks.c(), self.hit_idx.data_ptr(), self.n_cand.data_ptr() if n_seeds else None)
+
+    def to_host(self) -> dict:
+        d = self.tracks.to_host()
+        d["hit_idx"] = self.hit_idx[:, :self.tracks.n].cpu().numpy()
+        d["n_cand"] = self.n_cand.cpu().numpy()
+        return d
+
+
+def kf_build_set_lanes(lanes: int):
+    _check(lib().kf_build_set_lanes(C.c_int32(lanes)), "kf_build_set_lanes")
+
+
+def kf_build(geom: Geom, hits: Hits, binned: Binned, seeds: Tracks, seed_event, seed_hit_idx, first_layer: int, K: int, chi2_cut: float,
+             n_sigma: float, out: Cands | None = None, stream=None) -> Cands:
+    """include/kf.h kf_build.  seed_event [n] int32 device tensor (or None), seed_hit_idx [first_layer, seeds.ld] int32 (or None)."""
+    _require_cuda()
+    if out is None:
+        out = Cands(seeds.n, K, geom.n_layers, seeds.par.device)
+    if seed_hit_idx is not None:
+        assert tuple(seed_hit_idx.shape) == (first_layer, seeds.ld)
+    sc = seeds.c()
+    rc = lib().kf_build(C.byref(geom.c), C.byref(hits.c), C.byref(binned.c), C.byref(sc), _ptr(seed_event, torch.int32), _ptr(seed_hit_idx, torch.int32),
+                        first_layer, K, chi2_cut, n_sigma, C.byref(out.c), None, 0, _stream(stream))
+    _check(rc, "kf_build")
     return out

@@ -1,0 +1,306 @@
+// kf_bin.cu -- binned hit index (B0) and the diagnostic window lookup (B2-B3 list): DESIGN.md readings X1-X3.
+//
+// "data structures used for selecting hit candidates" (sec. 3.1).  Per (event, layer) segment the hits
+// are sorted by (z row, phi bin, original index); bin_off delimits the bins.  Everything here is integer / index
+// work specified in IEEE fp32 single operations (__fdiv_rn, __fmul_rn, __fadd_rn: no contraction), so the result
+// is bit-exact against the CPU oracle.
+//
+// Pipeline (all on the caller's stream, HBM-bound: ~44 B per hit):
+//   1. bin_count:   one thread per hit: key = global bin; atomicAdd into bin_off[key + 1]
+//   2. scan:        in-place inclusive scan of bin_off (three small kernels: block sums, scan of sums, add)
+//   3. bin_scatter: pos = bin_off[key] + atomicAdd(cursor[key]); tmp[pos] = (key, original index)   (order within a
+//                   bin is arbitrary here)
+//   4. bin_place:   one thread per position: rank of its original index inside its bin (bins hold a handful of
+//                   hits) -> final position; writes perm and the gathered x, y, z.  Deterministic and stable.
+#include <cmath>
+#include "kf_common.cuh"
+#include "kf_binmath.cuh"
+
+namespace kf {
+
+constexpr int BIN_BLOCK = 256;
+constexpr int SCAN_ITEMS = 16;                       // per thread
+constexpr int SCAN_TILE = BIN_BLOCK * SCAN_ITEMS;    // per block
+
+struct BinArgs {
+    int32_t n_layers, n_phi, n_z, n_seg;
+    const float *hx, *hy, *hz;
+    const int64_t* seg_off;      // device
+    const float* tan_tab;        // device, n_phi/8 + 1
+    int32_t* key;                // [n_hits]
+    int32_t* bin_off;            // [n_bins + 1]
+    int32_t* cursor;             // [n_bins]
+    int2* tmp;                   // [n_hits] (key, original index within segment)
+    float *sx, *sy, *sz;
+    int32_t* perm;
+    float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
+};
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_constant__ BinArgs a) {
+    extern __shared__ float s_tab[];
+    for (int i = threadIdx.x; i <= a.n_phi / 8; i += BIN_BLOCK) s_tab[i] = a.tan_tab[i];
+    __syncthreads();
+    for (int seg = blockIdx.y; seg < a.n_seg; seg += gridDim.y) {
+        const int l = seg % a.n_layers;
+        const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
+        const int32_t base = seg * a.n_z * a.n_phi;
+        for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
+            const int b = base + z_bin(a.hz[h], a.zmax[l], a.inv_dz[l], a.n_z) * a.n_phi + phi_bin(a.hx[h], a.hy[h], a.n_phi, s_tab);
+            a.key[h] = b;
+            atomicAdd(&a.bin_off[b + 1], 1);
+        }
+    }
+}
+
+// ---- in-place inclusive scan of v[0..n) (int32): block totals, scan of totals by one block, rescan with offsets ----
+__device__ __forceinline__ int block_inclusive_scan(int v, int* s_warp) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += o;
+    }
+    if (lane == 31) s_warp[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        int t = lane < BIN_BLOCK / 32 ? s_warp[lane] : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, t, d);
+            if (lane >= d) t += o;
+        }
+        s_warp[lane] = t;   // inclusive over warps (BIN_BLOCK/32 <= 32)
+    }
+    __syncthreads();
+    if (w > 0) v += s_warp[w - 1];
+    __syncthreads();
+    return v;
+}
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_tile_sums_kernel(const int32_t* v, int64_t n, int32_t* sums) {
+    __shared__ int s_warp[32];
+    const int64_t t0 = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int acc = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) acc += (t0 + i < n) ? v[t0 + i] : 0;
+    const int inc = block_inclusive_scan(acc, s_warp);
+    if (threadIdx.x == BIN_BLOCK - 1) sums[blockIdx.x] = inc;
+}
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_sums_kernel(int32_t* sums, int n_tiles) {   // one block; exclusive, in place
+    __shared__ int s_warp[32];
+    __shared__ int s_carry;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n_tiles; base += BIN_BLOCK) {
+        const int i = base + threadIdx.x;
+        const int x = i < n_tiles ? sums[i] : 0;
+        const int inc = block_inclusive_scan(x, s_warp);
+        const int carry = s_carry;
+        if (i < n_tiles) sums[i] = carry + inc - x;
+        __syncthreads();
+        if (threadIdx.x == BIN_BLOCK - 1) s_carry = carry + inc;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_apply_kernel(int32_t* v, int64_t n, const int32_t* sums) {
+    __shared__ int s_warp[32];
+    const int64_t t0 = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int x[SCAN_ITEMS];
+    int acc = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { x[i] = (t0 + i < n) ? v[t0 + i] : 0; acc += x[i]; }
+    int run = block_inclusive_scan(acc, s_warp) - acc + sums[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { run += x[i]; if (t0 + i < n) v[t0 + i] = run; }
+}
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_bin_scatter_kernel(const __grid_constant__ BinArgs a) {
+    for (int seg = blockIdx.y; seg < a.n_seg; seg += gridDim.y) {
+        const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
+        for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
+            const int b = a.key[h];
+            const int pos = a.bin_off[b] + atomicAdd(&a.cursor[b], 1);
+            a.tmp[pos] = make_int2(b, (int)(h - h0));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_bin_place_kernel(const __grid_constant__ BinArgs a, int64_t n_hits) {
+    const int64_t pos = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
+    if (pos >= n_hits) return;
+    const int2 me = a.tmp[pos];
+    const int o0 = a.bin_off[me.x], o1 = a.bin_off[me.x + 1];
+    int rank = 0;
+    for (int j = o0; j < o1; ++j) rank += a.tmp[j].y < me.y;
+    const int seg = me.x / (a.n_z * a.n_phi);
+    const int64_t src = a.seg_off[seg] + me.y;
+    const int dst = o0 + rank;
+    a.perm[dst] = me.y;
+    a.sx[dst] = a.hx[src];
+    a.sy[dst] = a.hy[src];
+    a.sz[dst] = a.hz[src];
+}
+
+// ---- window lookup (diagnostic entry; the build kernel walks the same ranges) ----
+struct LookupArgs {
+    int32_t n_layers, n_phi, n_z, cap;
+    int64_t n_query;
+    const int32_t *event, *layer;
+    const float *phi_c, *dphi, *z_c, *dz;
+    const int32_t* bin_off;
+    int32_t *count, *sorted_idx;
+    float inv_dphi;
+    float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
+};
+
+__global__ void __launch_bounds__(BIN_BLOCK) kf_window_lookup_kernel(const __grid_constant__ LookupArgs a) {
+    const int64_t i = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
+    if (i >= a.n_query) return;
+    const int l = a.layer[i];
+    const WindowBins w = window_bins(a.phi_c[i], a.dphi[i], a.z_c[i], a.dz[i], a.zmax[l], a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+    const int64_t seg = (int64_t)a.event[i] * a.n_layers + l;
+    int c = 0;
+    for (int iz = w.iz_lo; iz <= w.iz_hi; ++iz) {
+        const int64_t row = (seg * a.n_z + iz) * a.n_phi;
+        for (int k = 0; k < w.n_b; ++k) {
+            int ip = w.first + k;
+            if (ip >= a.n_phi) ip -= a.n_phi;
+            const int h0 = a.bin_off[row + ip], h1 = a.bin_off[row + ip + 1];
+            for (int h = h0; h < h1; ++h) {
+                if (c < a.cap) a.sorted_idx[i * a.cap + c] = h;
+                ++c;
+            }
+        }
+    }
+    a.count[i] = c;
+}
+
+static int check_bins(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, const char* who, int64_t* n_bins) {
+    if (n_phi < 8 || n_phi > 4096 || (n_phi % 8) != 0 || n_z < 1 || n_z > 1024)
+        return fail(KF_ERR_BAD_GEOM, "%s: need n_phi a multiple of 8 in 8..4096 and n_z in 1..1024", who);
+    if (hits->n_events < 1 || hits->n_hits < 0) return fail(KF_ERR_INVALID_ARG, "%s: n_events < 1 or n_hits < 0", who);
+    const int64_t nb = (int64_t)hits->n_events * geom->n_layers * n_phi * n_z;
+    if (nb + 1 >= (int64_t)1 << 31 || hits->n_hits >= (int64_t)1 << 31)
+        return fail(KF_ERR_INVALID_ARG, "%s: bins (%lld) or hits (%lld) exceed the int32 index range", who, (long long)nb, (long long)hits->n_hits);
+    *n_bins = nb;
+    return KF_OK;
+}
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct BinWs { size_t tab, key, cursor, tmp, sums, total; };
+static BinWs bin_ws_layout(int64_t n_hits, int64_t n_bins, int n_phi) {
+    BinWs w;
+    size_t o = 0;
+    w.tab = o; o += align256((size_t)(n_phi / 8 + 1) * sizeof(float));
+    w.key = o; o += align256((size_t)n_hits * sizeof(int32_t));
+    w.cursor = o; o += align256((size_t)n_bins * sizeof(int32_t));
+    w.tmp = o; o += align256((size_t)n_hits * sizeof(int2));
+    w.sums = o; o += align256((size_t)((n_bins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1) * sizeof(int32_t));
+    w.total = o;
+    return w;
+}
+
+}  // namespace kf
+
+extern "C" size_t kf_bin_workspace_bytes(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z) {
+    using namespace kf;
+    if (!geom || !hits) return 0;
+    int64_t nb;
+    if (check_geom(geom, "kf_bin_workspace_bytes") || check_bins(geom, hits, n_phi, n_z, "kf_bin_workspace_bytes", &nb)) return 0;
+    return bin_ws_layout(hits->n_hits, nb, n_phi).total;
+}
+
+extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* ws,
+                           size_t ws_bytes, void* stream) {
+    using namespace kf;
+    if (!geom || !hits || !out) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: NULL struct argument");
+    int rc = check_geom(geom, "kf_bin_hits");
+    if (rc) return rc;
+    int64_t n_bins;
+    rc = check_bins(geom, hits, n_phi, n_z, "kf_bin_hits", &n_bins);
+    if (rc) return rc;
+    if (!hits->seg_off || !hits->seg_off_dev) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: hits->seg_off / seg_off_dev is NULL");
+    if (!out->bin_off) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: out->bin_off is NULL");
+    const int64_t n_hits = hits->n_hits;
+    if (n_hits > 0 && (!hits->x || !hits->y || !hits->z || !out->x || !out->y || !out->z || !out->perm))
+        return fail(KF_ERR_NULL_PTR, "kf_bin_hits: NULL hit array");
+    const int n_seg = hits->n_events * geom->n_layers;
+    if (hits->seg_off[0] != 0 || hits->seg_off[n_seg] != n_hits) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits: seg_off must run from 0 to n_hits");
+    int64_t max_seg = 0;
+    for (int s = 0; s < n_seg; ++s) {
+        const int64_t d = hits->seg_off[s + 1] - hits->seg_off[s];
+        if (d < 0) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits: seg_off not monotonic at segment %d", s);
+        if (d > max_seg) max_seg = d;
+    }
+    const BinWs w = bin_ws_layout(n_hits, n_bins, n_phi);
+    if (!ws || ws_bytes < w.total) return fail(KF_ERR_WORKSPACE_TOO_SMALL, "kf_bin_hits: workspace %zu < %zu bytes", ws_bytes, w.total);
+    cudaStream_t st = (cudaStream_t)stream;
+    char* base = (char*)ws;
+    out->n_phi = n_phi; out->n_z = n_z;
+
+    // X1 table: T[k] = fl32(tan(2 pi k / N)) evaluated in double on the host, T[N/8] = 1
+    float tab[4096 / 8 + 1];
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k = 0; k < n_phi / 8; ++k) tab[k] = (float)std::tan(two_pi * (double)k / (double)n_phi);
+    tab[n_phi / 8] = 1.0f;
+    cudaMemcpyAsync(base + w.tab, tab, (size_t)(n_phi / 8 + 1) * sizeof(float), cudaMemcpyHostToDevice, st);   // pageable source: staged before return
+
+    BinArgs a;
+    a.n_layers = geom->n_layers; a.n_phi = n_phi; a.n_z = n_z; a.n_seg = n_seg;
+    a.hx = hits->x; a.hy = hits->y; a.hz = hits->z; a.seg_off = hits->seg_off_dev;
+    a.tan_tab = (const float*)(base + w.tab);
+    a.key = (int32_t*)(base + w.key); a.bin_off = out->bin_off; a.cursor = (int32_t*)(base + w.cursor); a.tmp = (int2*)(base + w.tmp);
+    a.sx = out->x; a.sy = out->y; a.sz = out->z; a.perm = out->perm;
+    for (int l = 0; l < KF_MAX_LAYERS; ++l) {
+        const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
+        a.zmax[l] = y.zmax;
+        a.inv_dz[l] = (float)n_z / (2.0f * y.zmax);      // one IEEE fp32 division of exact operands (X2)
+    }
+    cudaMemsetAsync(out->bin_off, 0, (size_t)(n_bins + 1) * sizeof(int32_t), st);
+    cudaMemsetAsync(a.cursor, 0, (size_t)n_bins * sizeof(int32_t), st);
+    if (n_hits > 0) {
+        const unsigned gx = (unsigned)std::min<int64_t>((max_seg + BIN_BLOCK - 1) / BIN_BLOCK, 4096);
+        const dim3 grid(gx ? gx : 1, (unsigned)std::min(n_seg, 65535));
+        kf_bin_count_kernel<<<grid, BIN_BLOCK, (size_t)(n_phi / 8 + 1) * sizeof(float), st>>>(a);
+        const int64_t n_scan = n_bins + 1;
+        const int n_tiles = (int)((n_scan + SCAN_TILE - 1) / SCAN_TILE);
+        int32_t* sums = (int32_t*)(base + w.sums);
+        kf_scan_tile_sums_kernel<<<n_tiles, BIN_BLOCK, 0, st>>>(out->bin_off, n_scan, sums);
+        kf_scan_sums_kernel<<<1, BIN_BLOCK, 0, st>>>(sums, n_tiles);
+        kf_scan_apply_kernel<<<n_tiles, BIN_BLOCK, 0, st>>>(out->bin_off, n_scan, sums);
+        kf_bin_scatter_kernel<<<grid, BIN_BLOCK, 0, st>>>(a);
+        kf_bin_place_kernel<<<(unsigned)((n_hits + BIN_BLOCK - 1) / BIN_BLOCK), BIN_BLOCK, 0, st>>>(a, n_hits);
+    }
+    return check_launch("kf_bin_hits");
+}
+
+extern "C" int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, int64_t n_query,
+                                const int32_t* event, const int32_t* layer, const float* phi_c, const float* dphi,
+                                const float* z_c, const float* dz, int32_t cap, int32_t* count, int32_t* sorted_idx, void* stream) {
+    using namespace kf;
+    if (!geom || !hits || !binned) return fail(KF_ERR_NULL_PTR, "kf_window_lookup: NULL struct argument");
+    int rc = check_geom(geom, "kf_window_lookup");
+    if (rc) return rc;
+    int64_t n_bins;
+    rc = check_bins(geom, hits, binned->n_phi, binned->n_z, "kf_window_lookup", &n_bins);
+    if (rc) return rc;
+    if (n_query < 0 || cap < 0) return fail(KF_ERR_INVALID_ARG, "kf_window_lookup: n_query < 0 or cap < 0");
+    if (n_query == 0) return KF_OK;
+    if (!event || !layer || !phi_c || !dphi || !z_c || !dz || !count || (cap > 0 && !sorted_idx) || !binned->bin_off)
+        return fail(KF_ERR_NULL_PTR, "kf_window_lookup: NULL array");
+    LookupArgs a;
+    a.n_layers = geom->n_layers; a.n_phi = binned->n_phi; a.n_z = binned->n_z; a.cap = cap; a.n_query = n_query;
+    a.event = event; a.layer = layer; a.phi_c = phi_c; a.dphi = dphi; a.z_c = z_c; a.dz = dz;
+    a.bin_off = binned->bin_off; a.count = count; a.sorted_idx = sorted_idx;
+    a.inv_dphi = host_inv_dphi(binned->n_phi);
+    for (int l = 0; l < KF_MAX_LAYERS; ++l) {
+        const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
+        a.zmax[l] = y.zmax;
+        a.inv_dz[l] = (float)binned->n_z / (2.0f * y.zmax);
+    }
+    kf_window_lookup_kernel<<<(unsigned)((n_query + BIN_BLOCK - 1) / BIN_BLOCK), BIN_BLOCK, 0, (cudaStream_t)stream>>>(a);
+    return check_launch("kf_window_lookup");
+}

@@ -1,0 +1,52 @@
+// kf_binmath.cuh -- bit-exact bin arithmetic (X1-X3): IEEE fp32 single operations and integer work only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kf {
+
+// X1: azimuthal bin from comparisons against the tangent table tab[k] = fl32(tan(2 pi k / n_phi)), k = 0..n_phi/8
+// (strictly increasing, tab[0] = 0): no atan2, hence no dependence on a math library.
+__device__ __forceinline__ int phi_bin(float x, float y, int n_phi, const float* __restrict__ tab) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const bool swap = ay > ax;
+    const float lo = swap ? ax : ay, hi = swap ? ay : ax;
+    const float t = hi > 0.0f ? __fdiv_rn(lo, hi) : 0.0f;
+    int j = 0, end = n_phi >> 3;                     // largest j in [0, n_phi/8 - 1] with tab[j] <= t
+    while (end - j > 1) {
+        const int mid = (j + end) >> 1;
+        if (tab[mid] <= t) j = mid; else end = mid;
+    }
+    const int a = swap ? (n_phi >> 2) - 1 - j : j;
+    if (x >= 0.0f) return (y >= 0.0f) ? a : n_phi - 1 - a;
+    return (y >= 0.0f) ? (n_phi >> 1) - 1 - a : (n_phi >> 1) + a;
+}
+
+// X2: z row; inv_dz = fl32(n_z / (2 zmax))
+__device__ __forceinline__ int z_bin(float z, float zmax, float inv_dz, int n_z) {
+    const float f = floorf(__fmul_rn(__fadd_rn(z, zmax), inv_dz));
+    return (f >= (float)n_z) ? n_z - 1 : (f < 0.0f ? 0 : (int)f);
+}
+
+// X3: window -> first phi bin, number of phi bins (wrapping), z rows
+struct WindowBins { int first, n_b, iz_lo, iz_hi; };
+
+__device__ __forceinline__ WindowBins window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, float inv_dz,
+                                                  float inv_dphi, int n_phi, int n_z) {
+    WindowBins w;
+    const int b_lo = (int)floorf(__fmul_rn(__fsub_rn(phi_c, dphi), inv_dphi));
+    const int b_hi = (int)floorf(__fmul_rn(__fadd_rn(phi_c, dphi), inv_dphi));
+    int nb = b_hi - b_lo + 1;
+    nb = nb > n_phi ? n_phi : nb;
+    w.n_b = nb < 0 ? 0 : nb;
+    int f = b_lo % n_phi;
+    w.first = f < 0 ? f + n_phi : f;
+    w.iz_lo = z_bin(__fsub_rn(z_c, dz), zmax, inv_dz, n_z);
+    w.iz_hi = z_bin(__fadd_rn(z_c, dz), zmax, inv_dz, n_z);
+    return w;
+}
+
+// inv_dphi = fl32(n_phi / (2 pi)), the division carried out in double
+inline float host_inv_dphi(int n_phi) { return (float)((double)n_phi / 6.283185307179586476925286766559); }
+
+}  // namespace kf
