@@ -1,13 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the KF hot path on B200 (contract: see DESIGN.md sec. 7).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload fit_c1|fit_c2|build_c3] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload fit_c1|fit_c2|fit_c0|build_c3|build_c4]
+                  [--impl ours|reference]
 
-A "step" is one pass of the whole hot path over one batch of synthetic input (for the fit workloads: one kf_fit
-call over all tracks).  `value` is whole-job throughput with inputs resident in HBM; `e2e` is the same through the
-C-ABI call with pinned HOST buffers, H2D and D2H copies inside the timed region.  `--impl reference` times the fp64
-CPU oracle (oracle/) on a bounded sample of the same workload on the host cores.
-Under torchrun every rank fits its own shard of the same size (weak scaling, no collective on the data path).
+A "step" is one pass of the hot path over one batch of synthetic input: for the fit workloads one kf_fit call over
+all tracks (steps F1-F9), for the build workloads kf_bin_hits + kf_build over all events (steps B0-B6).  The default
+line is fit_c1 = BASELINE.json configs[1] (the configuration the roofline target is quoted on) and carries, under
+"build", the seeds/s of configs[3] measured the same way in the same run.  `value` is whole-job throughput with
+inputs resident in HBM; `e2e` is the same through the C-ABI call with pinned HOST buffers, H2D and D2H copies inside
+the timed region.  `--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload
+on the host cores.  Under torchrun every rank works on its own shard of the same size (weak scaling, no collective
+on the data path).
 """
 from __future__ import annotations
 
@@ -28,12 +32,17 @@ sys.path.insert(0, ROOT)
 from paper_1711_06571_b200 import synth  # noqa: E402
 
 # Algorithmic work per unit (frozen before tuning).
-FIT_FLOP_PER_TRACK_LAYER = 800.0
+FIT_FLOP_PER_TRACK_LAYER = 700.0          # re-count from the sec. 3 formulas
+FIT_FLOP_PER_TRACK_LAYER_SURVEY = 800.0   # SURVEY.md sec. 8d hand count (reported as frac_survey_count)
 FIT_BYTES_SEED_IN = 6 * 4 + 21 * 4 + 1            # par + cov + q
 FIT_BYTES_OUT = 6 * 4 + 21 * 4 + 4 + 4 + 4        # par + cov + chi2 + nhits + status
 FIT_BYTES_PER_HIT = 12
 FIT_BYTES_PER_IDX = 4
+BUILD_FLOP = dict(n_prop=458.0, n_scan=15.0, n_window=40.0, n_upd=250.0)
+BIN_BYTES_PER_HIT = 44.0
 SM_COUNT, FP32_LANES = 148, 128
+FIT_CFG = {"fit_c0": 0, "fit_c1": 1, "fit_c2": 2}
+BUILD_CFG = {"build_c3": 3, "build_c4": 4}
 
 
 def peaks():
@@ -42,6 +51,10 @@ def peaks():
         d = json.load(open(path))
         return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def fp32_peak_tflops(pk) -> float:
+    return SM_COUNT * FP32_LANES * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
 
 
 class ClockSampler:
@@ -93,19 +106,32 @@ class ClockSampler:
                     reasons=sorted(reasons), samples=len(sm))
 
 
+# ----------------------------------------------------------------------------------------------------------------
+# algorithmic work
+# ----------------------------------------------------------------------------------------------------------------
 def fit_units(fi) -> dict:
     """Algorithmic flops / bytes of one kf_fit call over `fi`."""
     n_upd = int(fi.valid.sum())
     by = fi.n * (FIT_BYTES_SEED_IN + FIT_BYTES_OUT) + n_upd * FIT_BYTES_PER_HIT
     if fi.hit_idx is not None:
         by += fi.n * fi.geom.n_layers * FIT_BYTES_PER_IDX
-    return dict(track_layers=n_upd, flops=n_upd * FIT_FLOP_PER_TRACK_LAYER, bytes=by)
+    return dict(track_layers=n_upd, flops=n_upd * FIT_FLOP_PER_TRACK_LAYER, flops_survey=n_upd * FIT_FLOP_PER_TRACK_LAYER_SURVEY, bytes=by)
 
 
-def run_reference(args, fi, workload):
+def build_units(counters: dict, n_seeds: int, K: int, L: int, scale: float = 1.0) -> dict:
+    """Algorithmic flops / bytes of one kf_build call from the oracle's own counters."""
+    c = {k: v * scale for k, v in counters.items()}
+    fl = sum(BUILD_FLOP[k] * c[k] for k in BUILD_FLOP)
+    by = 16.0 * c["n_scan"] + 8.0 * c["n_rows"] + 113.0 * n_seeds + (117.0 + 4.0 * L) * K * n_seeds
+    return dict(flops=fl, bytes=by, counters={k: int(v) for k, v in c.items()})
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_fit(fi, n_s, steps, warmup):
     from oracle import kf_oracle as o
-    n_s = min(fi.n, args.ref_sample)
-    idx = np.arange(n_s)
+    n_s = min(fi.n, n_s)
     L, ld = fi.geom.n_layers, fi.ld
     hx = np.ascontiguousarray(fi.hit_x.reshape(L, ld)[:, :n_s]).reshape(-1).astype(np.float64)
     hy = np.ascontiguousarray(fi.hit_y.reshape(L, ld)[:, :n_s]).reshape(-1).astype(np.float64)
@@ -114,57 +140,121 @@ def run_reference(args, fi, workload):
     par = np.ascontiguousarray(fi.par[:, :n_s]); cov = np.ascontiguousarray(fi.cov[:, :n_s]); q = fi.q[:n_s]
     seg = np.arange(L + 1) * n_s
     call = lambda: o.fit(fi.geom.layer_table(), fi.geom.bz, par, cov, q, hx, hy, hz, seg, hi)
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         call()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         call()
-    dt = (time.perf_counter() - t0) / args.steps
-    v = n_s / dt
-    sample = f"first {n_s} tracks of the {fi.n}-track workload per step"
-    return dict(impl="reference", metric="tracks_fitted_per_s", value=v, unit="tracks/s", n_gpus=args.gpus, steps=args.steps,
-                warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f64", data="synthetic", config=dict(workload=workload, tracks=fi.n, layers=L),
-                cpu_baseline=dict(value=v, unit="tracks/s", cores=o.num_threads(), kind="oracle", sample=sample),
-                e2e=dict(value=v, unit="tracks/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    dt = (time.perf_counter() - t0) / steps
+    return dict(value=n_s / dt, unit="tracks/s", cores=o.num_threads(), kind="oracle",
+                sample=f"first {n_s} tracks of the {fi.n}-track workload per step", ms_per_step=dt * 1e3)
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="fit_c1", choices=["fit_c1", "fit_c2", "fit_c0"])
-    ap.add_argument("--tracks", type=int, default=None, help="override the track count (debug only; invalidates the metric)")
-    ap.add_argument("--ref-sample", type=int, default=100_000)
-    ap.add_argument("--cpu-sample", type=int, default=200_000)
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
+def oracle_build(bi, n_ev, steps, warmup):
+    """kfo_bin_hits + kfo_build on the first n_ev events (whole events: seeds only see hits of their own event)."""
+    from oracle import kf_oracle as o
+    L = bi.geom.n_layers
+    n_ev = min(n_ev, bi.n_events)
+    n_h = int(bi.seg_off[n_ev * L])
+    sel = np.nonzero(bi.seed_event < n_ev)[0]
+    n_s = len(sel)
+    assert n_s == 0 or sel[-1] == n_s - 1, "seeds are stored event by event"
+    seg = bi.seg_off[: n_ev * L + 1]
+    lt = bi.geom.layer_table()
+    res = {}
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    cfg_id = {"fit_c0": 0, "fit_c1": 1, "fit_c2": 2}[args.workload]
+    def call():
+        rb = o.bin_hits(lt, n_ev, seg, bi.hit_x[:n_h], bi.hit_y[:n_h], bi.hit_z[:n_h], bi.n_phi, bi.n_z)
+        res["r"] = o.kf_build(lt, bi.geom.bz, rb, seg, bi.par, bi.cov, bi.q[:n_s], bi.seed_event[:n_s], bi.seed_hit_idx, bi.first_layer,
+                              bi.K, bi.chi2_cut, bi.n_sigma, n=n_s)
+    for _ in range(warmup):
+        call()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        call()
+    dt = (time.perf_counter() - t0) / steps
+    return dict(value=n_s / dt, unit="seeds/s", cores=o.num_threads(), kind="oracle",
+                sample=f"first {n_ev} of {bi.n_events} events ({n_s} of {bi.n_seeds} seeds, {n_h} hits), binning + building, per step",
+                ms_per_step=dt * 1e3), res["r"]["counters"], n_s
 
-    if args.impl == "reference":
-        if rank != 0:
-            return 0
-        fi = synth.fit_inputs(cfg_id, n=args.tracks)
-        print(json.dumps(run_reference(args, fi, args.workload)), flush=True)
-        return 0
 
+def run_reference(args, workload):
+    if workload in FIT_CFG:
+        fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks)
+        cb = oracle_fit(fi, args.ref_sample, args.steps, args.warmup)
+        metric, cfg = "tracks_fitted_per_s", dict(workload=workload, tracks=fi.n, layers=fi.geom.n_layers)
+    else:
+        bi = synth.build_inputs(BUILD_CFG[workload], n_events=args.events)
+        cb, _, _ = oracle_build(bi, args.ref_events, args.steps, args.warmup)
+        metric, cfg = "seeds_built_per_s", dict(workload=workload, events=bi.n_events, seeds=bi.n_seeds, layers=bi.geom.n_layers, K=bi.K)
+    ms = cb.pop("ms_per_step")
+    return dict(impl="reference", metric=metric, value=cb["value"], unit=cb["unit"], n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", config=cfg, cpu_baseline=cb,
+                e2e=dict(value=cb["value"], unit=cb["unit"], h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# GPU legs
+# ----------------------------------------------------------------------------------------------------------------
+class Dist:
+    def __init__(self):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    def barrier(self):
+        import torch
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_ms(self, ms: float) -> float:
+        from paper_1711_06571_b200 import shard
+        return shard.max_over_ranks(ms, device="cuda")
+
+
+def time_steps(step, steps, warmup, stream, d: Dist, marks=0):
+    """W warm-up steps, then K steps between barrier + synchronize, CUDA events on the launching stream.
+    `step(rec)` may call rec(i) to drop intermediate events (i < marks) for per-kernel shares.
+    -> (ms per step as max over ranks, per-step ms list, per-mark ms lists, wall t0, t1)"""
     import torch
-    import torch.distributed as dist
-    from paper_1711_06571_b200 import binding as b
+    for _ in range(warmup):
+        step(lambda i: None)
+    d.barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    mk = [[torch.cuda.Event(enable_timing=True) for _ in range(marks)] for _ in range(steps)]
+    t0 = time.time()
+    ev[0].record(stream)
+    for i in range(steps):
+        step(lambda j, i=i: mk[i][j].record(stream))
+        ev[i + 1].record(stream)
+    d.barrier()
+    t1 = time.time()
+    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+    seg = []
+    for j in range(marks + 1 if marks else 0):
+        a = [(ev[i] if j == 0 else mk[i][j - 1]) for i in range(steps)]
+        b_ = [(mk[i][j] if j < marks else ev[i + 1]) for i in range(steps)]
+        seg.append([x.elapsed_time(y) for x, y in zip(a, b_)])
+    return d.max_ms(ev[0].elapsed_time(ev[-1]) / steps), per, seg, t0, t1
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+def pin(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+
+
+def nbytes(ts):
+    return int(sum(t.numel() * t.element_size() for t in ts if t is not None))
+
+
+def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
+    import torch
+    from paper_1711_06571_b200 import binding as b
     # every rank: its own shard of the configured size (weak scaling); events differ by rank
-    fi = synth.fit_inputs(cfg_id, n=args.tracks, event=rank)
+    fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks, event=d.rank)
     units = fit_units(fi)
     geom = b.Geom(fi.geom.layer_table(), fi.geom.bz)
     hits = b.Hits(fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, 1)
@@ -174,47 +264,26 @@ def main():
     out.q = seeds.q
     stream = torch.cuda.current_stream()
 
-    def step():
+    def step(rec):
         b.kf_fit(geom, hits, hit_idx, None, seeds, out=out, stream=stream)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    t0 = time.time()
-    ev[0].record(stream)
-    for i in range(args.steps):
-        step()
-        ev[i + 1].record(stream)
-    barrier()
-    t1 = time.time()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    W = max(args.warmup, 3)
+    sampler = ClockSampler(d.local) if d.rank == 0 else None
+    ms_per_step, per, _, t0, t1 = time_steps(step, args.steps, W, stream, d)
     clocks = sampler.stop(t0, t1) if sampler else None
-    ms = torch.tensor([total_ms / args.steps], device="cuda")
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_per_step = float(ms.item())
-    value = fi.n * world / (ms_per_step * 1e-3)
+    value = fi.n * d.world / (ms_per_step * 1e-3)
 
     # ---- end to end: pinned host buffers -> H2D -> kf_fit -> D2H, all inside the timed region ----
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_par, h_cov, h_q = pin(fi.par), pin(fi.cov), pin(fi.q)
     h_x, h_y, h_z = pin(fi.hit_x), pin(fi.hit_y), pin(fi.hit_z)
     h_idx = None if fi.hit_idx is None else pin(fi.hit_idx)
     o_par = torch.empty((6, seeds.ld), dtype=torch.float32).pin_memory(); o_cov = torch.empty((21, seeds.ld), dtype=torch.float32).pin_memory()
     o_chi2 = torch.empty(fi.n, dtype=torch.float32).pin_memory(); o_nh = torch.empty(fi.n, dtype=torch.int32).pin_memory()
     o_st = torch.empty(fi.n, dtype=torch.int32).pin_memory()
-    h2d = sum(t.numel() * t.element_size() for t in (h_par, h_cov, h_q, h_x, h_y, h_z) + ((h_idx,) if h_idx is not None else ()))
-    d2h = sum(t.numel() * t.element_size() for t in (o_par, o_cov, o_chi2, o_nh, o_st))
+    h2d = nbytes((h_par, h_cov, h_q, h_x, h_y, h_z, h_idx))
+    d2h = nbytes((o_par, o_cov, o_chi2, o_nh, o_st))
 
-    def e2e_step():
+    def e2e_step(rec):
         seeds.par.copy_(h_par, non_blocking=True); seeds.cov.copy_(h_cov, non_blocking=True); seeds.q.copy_(h_q, non_blocking=True)
         hits.x.copy_(h_x, non_blocking=True); hits.y.copy_(h_y, non_blocking=True); hits.z.copy_(h_z, non_blocking=True)
         if h_idx is not None:
@@ -223,58 +292,184 @@ def main():
         o_par.copy_(out.par, non_blocking=True); o_cov.copy_(out.cov, non_blocking=True); o_chi2.copy_(out.chi2, non_blocking=True)
         o_nh.copy_(out.nhits, non_blocking=True); o_st.copy_(out.status, non_blocking=True)
 
-    e2e_steps = max(3, min(args.steps, 10))
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(e2e_steps):
-        e2e_step()
-    e1.record(stream)
-    barrier()
-    ems = torch.tensor([e0.elapsed_time(e1) / e2e_steps], device="cuda")
-    if world > 1:
-        dist.all_reduce(ems, op=dist.ReduceOp.MAX)
-    e2e_value = fi.n * world / (float(ems.item()) * 1e-3)
-
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+    e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
+    e2e_value = fi.n * d.world / (e2e_ms * 1e-3)
+    if d.rank != 0:
+        return None
 
     pk = peaks()
     kern_ms = statistics.mean(per)                    # one kernel per step: CUDA events on the launching stream
-    fp32_peak = SM_COUNT * FP32_LANES * 2 * pk["sm_max_mhz"] * 1e6 / 1e12     # TFLOP/s
-    t_alu = units["flops"] / (fp32_peak * 1e12)
+    peak = fp32_peak_tflops(pk)
+    t_alu = units["flops"] / (peak * 1e12)
     t_hbm = units["bytes"] / (pk["hbm_gbs"] * 1e9)
-    achieved_tflops = units["flops"] / (kern_ms * 1e-3) / 1e12
-    roofline = dict(bound="alu", achieved=achieved_tflops, peak=fp32_peak, unit="TFLOP/s", frac=achieved_tflops / fp32_peak,
-                    traffic=None, kernel="kf_fit_kernel", kernel_ms=kern_ms, kernel_ms_min=min(per),
+    ach = units["flops"] / (kern_ms * 1e-3) / 1e12
+    roofline = dict(bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None,
+                    kernel="kf_fit_kernel", kernel_ms=kern_ms, kernel_ms_min=min(per), kernel_share_of_step=1.0,
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (clocks.max.sm, {pk['source']})",
                     alg_flops_per_launch=units["flops"], alg_bytes_per_launch=units["bytes"],
+                    alg_flop_per_track_layer=FIT_FLOP_PER_TRACK_LAYER,
+                    frac_survey_count=units["flops_survey"] / (kern_ms * 1e-3) / 1e12 / peak,
                     hbm_achieved_gbs=units["bytes"] / (kern_ms * 1e-3) / 1e9, hbm_peak_gbs=pk["hbm_gbs"],
                     frac_of_slower_roof=max(t_alu, t_hbm) / (kern_ms * 1e-3))
+    roofline["traffic"] = stored_traffic(workload)
+    line = dict(metric="tracks_fitted_per_s", value=value, unit="tracks/s", n_gpus=d.world, steps=args.steps, warmup=W,
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=units["track_layers"],
+                            l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (units["bytes"] / 1e6)),
+                clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms),
+                gpu_launches=args.steps, roofline=roofline)
+    if not args.no_cpu_baseline:
+        cb = oracle_fit(fi, args.cpu_sample, 1, 0)
+        cb.pop("ms_per_step")
+        line["cpu_baseline"] = cb
+    return line
+
+
+def stored_traffic(workload):
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tr):
         try:
-            roofline["traffic"] = json.load(open(tr)).get(args.workload)
+            return json.load(open(tr)).get(workload)
         except Exception:
-            pass
-    line = dict(metric="tracks_fitted_per_s", value=value, unit="tracks/s", n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
-                config=dict(workload=args.workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=units["track_layers"],
-                            l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (units["bytes"] / 1e6)),
-                clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                                        ms_per_step=float(ems.item())),
-                gpu_launches=args.steps, roofline=roofline)
+            return None
+    return None
+
+
+BUILD_LAUNCHES_PER_STEP = 7   # count, 3 x scan, scatter, place, build (the two memsets and the table copy are not kernels)
+
+
+def bench_build(args, d: Dist, workload: str, sample_clocks=True):
+    import torch
+    from paper_1711_06571_b200 import binding as b
+    cfg = BUILD_CFG[workload]
+    bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000)
+    L, K = bi.geom.n_layers, bi.K
+    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    n_bins = bi.n_events * L * bi.n_phi * bi.n_z
+    binned = b.Binned(hits.n_hits, n_bins, bi.n_phi, bi.n_z)
+    ws = torch.empty(max(b.kf_bin_workspace_bytes(geom, hits, bi.n_phi, bi.n_z), 1), dtype=torch.uint8, device="cuda")
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    sev = torch.from_numpy(bi.seed_event).cuda(); shi = torch.from_numpy(bi.seed_hit_idx).cuda()
+    out = b.Cands(bi.n_seeds, K, L)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda") if hits.n_hits * 28 < (160 << 20) else None
+
+    def step(rec):
+        if flush is not None:
+            flush.fill_(1)        # working set below the 126 MB L2: flush between timed iterations
+        rec(0)
+        b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
+        rec(1)
+        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, stream=stream)
+
+    W = max(args.warmup, 3)
+    sampler = ClockSampler(d.local) if (d.rank == 0 and sample_clocks) else None
+    _, _, seg, t0, t1 = time_steps(step, args.steps, W, stream, d, marks=2)
+    clocks = sampler.stop(t0, t1) if sampler else None
+    bin_ms, build_ms = statistics.mean(seg[1]), statistics.mean(seg[2])
+    ms_per_step = d.max_ms(bin_ms + build_ms)          # the L2 flush is not part of the step
+    value = bi.n_seeds * d.world / (ms_per_step * 1e-3)
+
+    # ---- end to end: hits + seeds H2D, bin + build, candidates D2H ----
+    h = [pin(a) for a in (bi.hit_x, bi.hit_y, bi.hit_z, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx)]
+    dev = [hits.x, hits.y, hits.z, seeds.par, seeds.cov, seeds.q, sev, shi]
+    outs = [out.tracks.par, out.tracks.cov, out.tracks.chi2, out.tracks.nhits, out.tracks.status, out.hit_idx, out.n_cand]
+    ho = [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in outs]
+
+    def e2e_step(rec):
+        for dst, src in zip(dev, h):
+            dst.copy_(src, non_blocking=True)
+        b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
+        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, stream=stream)
+        for dst, src in zip(ho, outs):
+            dst.copy_(src, non_blocking=True)
+
+    e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
+    if d.rank != 0:
+        return None
+    pk = peaks()
+    res = dict(metric="seeds_built_per_s", value=value, unit="seeds/s", ms_per_step=ms_per_step, bin_ms=bin_ms, build_ms=build_ms,
+               hits_binned_per_s=hits.n_hits / (bin_ms * 1e-3),
+               config=dict(workload=workload, events_per_gpu=bi.n_events, seeds_per_gpu=bi.n_seeds, hits_per_gpu=hits.n_hits, layers=L, K=K,
+                           n_phi=bi.n_phi, n_z=bi.n_z, chi2_cut=bi.chi2_cut, n_sigma=bi.n_sigma,
+                           l2="192 MB fill between timed iterations (outside the timed segments)" if flush is not None else
+                              "hits + sorted copy + candidates per step exceed the 126 MB L2; no explicit flush"),
+               e2e=dict(value=bi.n_seeds * d.world / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=nbytes(h), d2h_bytes_per_step=nbytes(ho),
+                        ms_per_step=e2e_ms),
+               gpu_launches=args.steps * BUILD_LAUNCHES_PER_STEP, clocks=clocks)
+    bin_bytes = BIN_BYTES_PER_HIT * hits.n_hits + 8.0 * n_bins
+    res["bin_roofline"] = dict(bound="hbm", achieved=bin_bytes / (bin_ms * 1e-3) / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
+                               frac=bin_bytes / (bin_ms * 1e-3) / 1e9 / pk["hbm_gbs"], alg_bytes_per_step=bin_bytes, kernels="kf_bin_* (6 launches)")
     if not args.no_cpu_baseline:
-        from oracle import kf_oracle as o
-        sub = argparse.Namespace(**vars(args)); sub.steps = 1; sub.warmup = 0; sub.ref_sample = args.cpu_sample
-        ref = run_reference(sub, fi, args.workload)
-        line["cpu_baseline"] = ref["cpu_baseline"]
-    print(json.dumps(line), flush=True)
-    if world > 1:
+        cb, counters, n_s = oracle_build(bi, args.cpu_events, 1, 0)
+        cb.pop("ms_per_step")
+        u = build_units(counters, bi.n_seeds, K, L, scale=bi.n_seeds / max(n_s, 1))
+        peak = fp32_peak_tflops(pk)
+        t_alu, t_hbm = u["flops"] / (peak * 1e12), u["bytes"] / (pk["hbm_gbs"] * 1e9)
+        if t_alu >= t_hbm:
+            ach = u["flops"] / (build_ms * 1e-3) / 1e12
+            rf = dict(bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak)
+        else:
+            ach = u["bytes"] / (build_ms * 1e-3) / 1e9
+            rf = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"])
+        rf.update(traffic=stored_traffic(workload), kernel="kf_build_kernel", kernel_ms=build_ms, kernel_share_of_step=build_ms / (bin_ms + build_ms),
+                  alg_flops_per_launch=u["flops"], alg_bytes_per_launch=u["bytes"], counters=u["counters"],
+                  counters_source="oracle run of the cpu_baseline sample, scaled by seeds")
+        res["roofline"] = rf
+        res["cpu_baseline"] = cb
+    return res
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="fit_c1", choices=list(FIT_CFG) + list(BUILD_CFG))
+    ap.add_argument("--tracks", type=int, default=None, help="override the track count (debug only; invalidates the metric)")
+    ap.add_argument("--events", type=int, default=None, help="override the event count of a build workload (debug only)")
+    ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: tracks per step")
+    ap.add_argument("--ref-events", type=int, default=16, help="--impl reference: events per step (build workloads)")
+    ap.add_argument("--cpu-sample", type=int, default=200_000)
+    ap.add_argument("--cpu-events", type=int, default=16, help="events the oracle builds for cpu_baseline and the build counters")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-build", action="store_true", help="default line without the configs[3] build leg")
+    args = ap.parse_args()
+    d = Dist()
+
+    if args.impl == "reference":
+        if d.rank == 0:
+            print(json.dumps(run_reference(args, args.workload)), flush=True)
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(d.local)
+    if d.world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", d.local))
+
+    if args.workload in FIT_CFG:
+        line = bench_fit(args, d, args.workload)
+        if not args.no_build and args.tracks is None:
+            bl = bench_build(args, d, "build_c3", sample_clocks=False)
+            if line is not None:
+                line["build"] = bl
+                line["gpu_launches"] += bl["gpu_launches"]
+    else:
+        r = bench_build(args, d, args.workload)
+        line = None
+        if r is not None:
+            line = dict(metric=r.pop("metric"), value=r.pop("value"), unit=r.pop("unit"), n_gpus=d.world, steps=args.steps,
+                        warmup=max(args.warmup, 3), ms_per_step=r.pop("ms_per_step"), higher_is_better=True, scaling="weak",
+                        vs_baseline=None, dtype="f32", data="synthetic", **r)
+    if d.rank == 0:
+        print(json.dumps(line), flush=True)
+    if d.world > 1:
+        import torch.distributed as dist
         dist.destroy_process_group()
     return 0
 

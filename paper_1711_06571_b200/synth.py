@@ -384,7 +384,7 @@ def _three_point_seed(p1, p2, p3, bz):
 def build_inputs(config: int, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
                  K: int = 10, chi2_cut: float = 30.0, n_sigma: float = 3.0, noise: float | None = None,
                  fake_frac: float | None = None, n_phi: int | None = None, n_z: int | None = None,
-                 smear: bool = True, ms: bool = True) -> BuildInputs:
+                 smear: bool = True, ms: bool = True, event0: int = 0) -> BuildInputs:
     """Inputs of kf_bin_hits / kf_build for BASELINE.json configs 3-4 (sizes can be overridden for tests).
 
     Per event: truth tracks from the particle gun; hits per layer = truth hits + `noise` x (number of truth
@@ -406,7 +406,7 @@ def build_inputs(config: int, n_events: int | None = None, tracks: int | None = 
     seeds, sigs, qs, sev, struth, shit = [], [], [], [], [], []
     truth_hit_idx = np.full((L, n_events * tracks), -1, dtype=np.int32)
     for ev in range(n_events):
-        rng = rng_for(config, ev)
+        rng = rng_for(config, ev + event0)     # event0: a rank's own events (weak scaling)
         gun = particle_gun(rng, tracks, cfg["gun"])
         sim = simulate(geom, gun, rng, ms=ms, smear=smear)
         ev_hits = []
@@ -440,9 +440,14 @@ def build_inputs(config: int, n_events: int | None = None, tracks: int | None = 
         if n_fake:
             f_sd, f_q, f_hit = [], [], []
             h0, h1, h2 = ev_hits[0], ev_hits[1], ev_hits[2]
-            az1 = np.arctan2(h1[1], h1[0]); az2 = np.arctan2(h2[1], h2[0])
             dphi = 3.0 * 2.0 * np.pi / n_phi / 2.0      # "3x3 bin neighbourhood": +-1.5 bins
             dz = 3.0 * (2.0 * geom.zmax[0] / n_z) / 2.0
+            # hits of layers 1, 2 ordered by azimuth, so that a phi window is one (wrapping) slice
+            srt = []
+            for hh in (h1, h2):
+                az = np.arctan2(hh[1], hh[0])
+                o = np.argsort(az, kind="stable")
+                srt.append((az[o], o, hh[2][o]))
             tries = 0
             while len(f_sd) < n_fake and tries < 200 * n_fake:
                 tries += 1
@@ -450,10 +455,16 @@ def build_inputs(config: int, n_events: int | None = None, tracks: int | None = 
                 a0 = np.arctan2(h0[1][i0], h0[0][i0]); z0 = h0[2][i0]
                 picks = [i0]
                 fail = False
-                for (hh, azs, l) in ((h1, az1, 1), (h2, az2, 2)):
+                for (azs, order, zsrt), l in zip(srt, (1, 2)):
                     zexp = z0 * geom.r[l] / geom.r[0]
-                    dd = np.abs(np.mod(azs - a0 + np.pi, 2 * np.pi) - np.pi)
-                    cand = np.nonzero((dd <= dphi) & (np.abs(hh[2] - zexp) <= dz))[0]
+                    lo, hi = a0 - dphi, a0 + dphi
+                    parts = []
+                    for (u, v) in ((lo, hi), (lo + 2 * np.pi, hi + 2 * np.pi), (lo - 2 * np.pi, hi - 2 * np.pi)):
+                        i, j = np.searchsorted(azs, u, side="left"), np.searchsorted(azs, v, side="right")
+                        if j > i:
+                            parts.append(np.arange(i, j))
+                    sl = np.concatenate(parts) if parts else np.zeros(0, dtype=np.int64)
+                    cand = np.sort(order[sl[np.abs(zsrt[sl] - zexp) <= dz]])
                     if len(cand) == 0:
                         fail = True; break
                     picks.append(int(cand[rng.integers(len(cand))]))
