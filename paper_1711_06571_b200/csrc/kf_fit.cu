@@ -18,16 +18,26 @@ struct FitArgs {
     const int32_t* hit_idx; const int32_t* trk_event;
     float* par_o; float* cov_o; float* chi2_o; int32_t* nhits_o; uint32_t* status_o;
     LayerC layer[KF_MAX_LAYERS];
-    int64_t seg0[KF_MAX_LAYERS];   // segment offsets of event 0 (used when trk_event == NULL)
+    const float *hxl[KF_MAX_LAYERS], *hyl[KF_MAX_LAYERS], *hzl[KF_MAX_LAYERS];   // hx + seg_off[l] ... of event 0 (trk_event == NULL)
 };
 
-constexpr int FIT_BLOCK = 128;
+#ifndef KF_FIT_BLOCK
+#define KF_FIT_BLOCK 128
+#endif
+#ifndef KF_FIT_MINB
+#define KF_FIT_MINB 4
+#endif
+constexpr int FIT_BLOCK = KF_FIT_BLOCK;
 
-__global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant__ FitArgs a) {
+// IDX: explicit hit_idx (else identity), EVT: per-track event (else event 0), ISO: sig_r == sig_rphi on every layer.
+// The layer loop leaves through `break` when the track ends (failed propagation: the state of the last updated layer
+// is final) or when the update went numerically wrong (rare: the track is then redone up to the layer before).
+template <bool IDX, bool EVT, bool ISO>
+__global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {
     const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
     if (t >= a.n) return;
     const float cw = -(float)a.q[t] * a.kb;
-    const int ev = a.trk_event ? a.trk_event[t] : 0;
+    const int64_t seg = EVT ? (int64_t)a.trk_event[t] * a.n_layers : 0;
     float p[6], C[21];
     float chi2 = 0.0f;
     int nh = 0;
@@ -45,37 +55,41 @@ __global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant
         chi2 = 0.0f;
         nh = 0;
         int bad = -1;
-        bool alive = true;
 #pragma unroll 1
         for (int l = 0; l < limit; ++l) {
-            const int64_t idx = a.hit_idx ? (int64_t)a.hit_idx[l * a.ld_idx + t] : t;
-            // idx < 0: layer skipped entirely (R8).  One structured if-block, no break / continue inside
-            // the loop, so that diverged lanes reconverge at the end of every layer.
-            if (alive && idx >= 0) {
-                const int64_t h = (a.trk_event ? a.seg_off_dev[(int64_t)ev * a.n_layers + l] : a.seg0[l]) + idx;
-                const float mx = a.hx[h], my = a.hy[h], mz = a.hz[h];   // F6: issued before the arithmetic
-                const uint32_t flag = predict(p, C, g, cw, a.layer[l]);  // F2-F5
-                if (flag) {
-                    st |= flag;
-                    alive = false;
-                } else {
-                    Ldl3 Si;
-                    float r[3], c2;
-                    const HitCov V = hit_cov(mx, my, a.layer[l]);
-                    bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);            // F7
-                    if (ok) {
-                        gain_update(p, C, g, Si, V, r);                              // F8
-                        ok = step_finite(p, c2) && p[3] > 0.0f && (!careful || all_finite(p, C));
-                    }
-                    if (ok) {
-                        chi2 += c2;
-                        nh += 1;
-                    } else {
-                        bad = l;
-                        alive = false;
-                    }
-                }
+            int64_t idx = t;
+            if (IDX) {
+                idx = a.hit_idx[l * a.ld_idx + t];
+                if (idx < 0) continue;           // layer skipped entirely (R8)
             }
+            // F6: issued before the arithmetic
+            float mx, my, mz;
+            if (EVT) {
+                const int64_t h = a.seg_off_dev[seg + l] + idx;
+                mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
+            } else {
+                mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+            }
+            const LayerC ly = a.layer[l];
+            const uint32_t flag = predict(p, C, g, cw, ly);                    // F2-F5
+            if (flag) {
+                st |= flag;
+                break;
+            }
+            Ldl3 Si;
+            float r[3], c2;
+            HitCov V;
+            if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
+            else V = hit_cov(mx, my, ly);
+            bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);               // F7 (branch-free; garbage when !ok)
+            gain_update<ISO>(p, C, g, Si, V, r);                                // F8
+            ok = ok && step_finite(p, c2) && p[3] > 0.0f && (!careful || all_finite(p, C));
+            if (!ok) {
+                bad = l;
+                break;
+            }
+            chi2 += c2;
+            nh += 1;
         }
         if (bad < 0) {
             if (careful || all_finite(p, C)) break;
@@ -96,6 +110,12 @@ __global__ void __launch_bounds__(FIT_BLOCK) kf_fit_kernel(const __grid_constant
     a.chi2_o[t] = chi2;
     a.nhits_o[t] = nh;
     a.status_o[t] = st;
+}
+
+template <bool IDX, bool EVT>
+static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t st) {
+    if (iso) kf_fit_kernel<IDX, EVT, true><<<blocks, FIT_BLOCK, 0, st>>>(a);
+    else kf_fit_kernel<IDX, EVT, false><<<blocks, FIT_BLOCK, 0, st>>>(a);
 }
 
 }  // namespace kf
@@ -122,16 +142,22 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     a.hx = hits->x; a.hy = hits->y; a.hz = hits->z;
     a.seg_off_dev = hits->seg_off_dev; a.hit_idx = hit_idx; a.trk_event = trk_event;
     a.par_o = out->par; a.cov_o = out->cov; a.chi2_o = out->chi2; a.nhits_o = out->nhits; a.status_o = out->status;
+    bool iso = true;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
-        a.layer[l] = make_layer(l < geom->n_layers ? geom->layers[l] : geom->layers[geom->n_layers - 1]);
-        a.seg0[l] = l < geom->n_layers ? hits->seg_off[l] : 0;
+        const int ll = l < geom->n_layers ? l : geom->n_layers - 1;
+        a.layer[l] = make_layer(geom->layers[ll]);
+        iso = iso && geom->layers[ll].sig_r == geom->layers[ll].sig_rphi;
+        const int64_t o = hits->seg_off[ll];
+        a.hxl[l] = hits->x + o; a.hyl[l] = hits->y + o; a.hzl[l] = hits->z + o;
     }
     if (!hit_idx) {   // identity indexing: every segment of event 0 must hold n hits
         for (int l = 0; l < geom->n_layers; ++l)
             if (!trk_event && hits->seg_off[l + 1] - hits->seg_off[l] < seeds->n)
                 return fail(KF_ERR_INVALID_ARG, "kf_fit: hit_idx == NULL needs >= n hits in every segment");
     }
-    const int64_t blocks = (a.n + FIT_BLOCK - 1) / FIT_BLOCK;
-    kf_fit_kernel<<<(unsigned)blocks, FIT_BLOCK, 0, (cudaStream_t)stream>>>(a);
+    const unsigned blocks = (unsigned)((a.n + FIT_BLOCK - 1) / FIT_BLOCK);
+    cudaStream_t cs = (cudaStream_t)stream;
+    if (hit_idx) { if (trk_event) launch_fit<true, true>(a, iso, blocks, cs); else launch_fit<true, false>(a, iso, blocks, cs); }
+    else { if (trk_event) launch_fit<false, true>(a, iso, blocks, cs); else launch_fit<false, false>(a, iso, blocks, cs); }
     return check_launch("kf_fit");
 }

@@ -16,11 +16,10 @@ constexpr float CMIN = 0.1f;             // grazing guard on cos(incidence)
 
 enum : uint32_t { ST_UNREACHABLE = 1u, ST_LEFT_Z = 2u, ST_GRAZING = 4u, ST_NUMERIC = 8u };
 
-// per-layer constants, prepared on the host
-struct LayerC {
-    float r, r2, zmax, xx0r;          // radius, radius^2, half length, xx0 * r
-    float var_rphi, var_z, var_r;     // hit variances
-    float rcmin;                      // r * CMIN
+// per-layer constants, prepared on the host; two 16-byte vectors so that a layer is two constant-bank loads
+struct alignas(16) LayerC {
+    float r2, rcmin, xx0r, var_z;     // radius^2, r * CMIN, xx0 * r, hit variance along z
+    float var_r, var_rphi, zmax, r;   // hit variances along r and r-phi, half length, radius
 };
 
 // 1-ulp hardware approximations (MUFU.RCP / MUFU.RSQ / MUFU.LG2): no IEEE slow paths, no branches.
@@ -37,43 +36,59 @@ __device__ __forceinline__ void trig_init(Trig& g, float phi, float theta) {
     sincosf(theta, &g.st, &g.ct);
 }
 
-// rotate (c, s) by d; polynomial for |d| < 0.06 (truncation < 6e-11), library call otherwise (angle = full value)
+// rotate (c, s) by d: polynomial for |d| < 0.06 (truncation < 6e-11) followed by one Newton step back to unit norm
+__device__ __forceinline__ void rotate_poly(float& c, float& s, float d) {
+    const float d2 = d * d;
+    const float sd = d * fmaf(d2, fmaf(d2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    const float cd = fmaf(d2, fmaf(d2, 1.0f / 24.0f, -0.5f), 1.0f);
+    const float cn = fmaf(c, cd, -s * sd), sn = fmaf(s, cd, c * sd);
+    const float k = fmaf(-0.5f, fmaf(cn, cn, sn * sn), 1.5f);
+    c = cn * k; s = sn * k;
+}
+
+// library call otherwise (angle = full value)
 __device__ __forceinline__ void rotate_small(float& c, float& s, float d, float angle) {
-    if (fabsf(d) < 0.06f) {
-        const float d2 = d * d;
-        const float sd = d * fmaf(d2, fmaf(d2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
-        const float cd = fmaf(d2, fmaf(d2, 1.0f / 24.0f, -0.5f), 1.0f);
-        const float cn = fmaf(c, cd, -s * sd), sn = fmaf(s, cd, c * sd);
-        const float k = fmaf(-0.5f, fmaf(cn, cn, sn * sn), 1.5f);     // one Newton step back to unit norm
-        c = cn * k; s = sn * k;
+    if (fabsf(d) < 0.06f) rotate_poly(c, s, d);
+    else sincosf(angle, &s, &c);
+}
+
+// both angles of the state after an update; one test for the (rare) large correction
+__device__ __forceinline__ void rotate_pair(Trig& g, float dphi, float dth, float phi, float theta) {
+    if (fmaxf(fabsf(dphi), fabsf(dth)) < 0.06f) {
+        rotate_poly(g.cp, g.sp, dphi);
+        rotate_poly(g.ct, g.st, dth);
     } else {
-        sincosf(angle, &s, &c);
+        sincosf(phi, &g.sp, &g.cp);
+        sincosf(theta, &g.st, &g.ct);
     }
 }
 
 // packed lower-triangular index
 __host__ __device__ constexpr int pk(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
 
-// atan(t)/t, |t| <= ~1: odd minimax-free Taylor for small t, library atan otherwise
-__device__ __forceinline__ float atan_over_t(float t) {
-    float t2 = t * t;
-    if (t2 < 0.09f) {   // |t| < 0.3 (turning angle < 0.58 rad per layer): truncation < t^14/15 = 3e-9
-        return fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 13.0f, -1.0f / 11.0f), 1.0f / 9.0f), -1.0f / 7.0f), 0.2f),
-                             -1.0f / 3.0f), 1.0f);
-    }
-    return atanf(t) * frcp(t);
-}
-
-// f1(a) = (cos a - sin a / a)/a, f2(a) = (sin a - (1 - cos a)/a)/a ; series below |a| = 0.5 (cancellation-free)
-__device__ __forceinline__ void curv_partials(float a, float sa, float ca, float& f1, float& f2) {
-    float a2 = a * a;
-    if (a2 < 0.25f) {
-        f1 = a * (-1.0f / 3.0f + a2 * (1.0f / 30.0f + a2 * (-1.0f / 840.0f + a2 * (1.0f / 45360.0f))));
-        f2 = 0.5f + a2 * (-0.125f + a2 * (1.0f / 144.0f + a2 * (-1.0f / 5760.0f + a2 * (1.0f / 403200.0f))));
+// Turning-angle functions of t = tan(alpha/2):  f = atan(t)/t  (alpha = 2 t f, s = 2 tau f) and the curvature partials
+// f1(a) = (cos a - sin a / a)/a, f2(a) = (sin a - (1 - cos a)/a)/a of a = alpha.  One test selects the series for all
+// three (|t| < 0.245, i.e. |alpha| < 0.48 per layer: every track above ~0.2 GeV on these geometries except near its
+// turning point); truncation < 4e-9 relative.  The other side uses the library atan and the closed forms.
+__device__ __forceinline__ void angle_functions(float t, float t2, float sa, float ca, float& f, float& alpha, float& f1, float& f2) {
+    if (t2 < 0.06f) {
+        f = fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 11.0f, 1.0f / 9.0f), -1.0f / 7.0f), 0.2f), -1.0f / 3.0f), 1.0f);
+        alpha = 2.0f * t * f;
+        const float a2 = alpha * alpha;
+        f1 = alpha * fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 45360.0f, -1.0f / 840.0f), 1.0f / 30.0f), -1.0f / 3.0f);
+        f2 = fmaf(a2, fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 403200.0f, -1.0f / 5760.0f), 1.0f / 144.0f), -0.125f), 0.5f);
     } else {
-        float ia = frcp(a);
-        f1 = (ca - sa * ia) * ia;
-        f2 = (sa - (1.0f - ca) * ia) * ia;
+        f = atanf(t) * frcp(t);
+        alpha = 2.0f * t * f;
+        const float a2 = alpha * alpha;
+        if (a2 < 0.25f) {
+            f1 = alpha * fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 45360.0f, -1.0f / 840.0f), 1.0f / 30.0f), -1.0f / 3.0f);
+            f2 = fmaf(a2, fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 403200.0f, -1.0f / 5760.0f), 1.0f / 144.0f), -0.125f), 0.5f);
+        } else {
+            const float ia = frcp(alpha);
+            f1 = (ca - sa * ia) * ia;
+            f2 = (sa - (1.0f - ca) * ia) * ia;
+        }
     }
 }
 
@@ -86,6 +101,7 @@ struct Transport {
     float cpn, spn;      // cos / sin of phi'
     float up;            // x' cos phi' + y' sin phi' = r cos(incidence)
     float w;             // curvature
+    float f1, f2;        // curvature partials (angle_functions)
 };
 
 // Closed-form first crossing of the cylinder r (R2): with u, v the position along / across the direction,
@@ -109,16 +125,16 @@ __device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, flo
     const float th = w * tau;                     // tan(alpha/2)
     const float th2 = th * th;
     const float inv = frcp(1.0f + th2);
-    t.sa = 2.0f * th * inv;
+    const float X = 2.0f * tau * inv;             // sin(alpha)/w
+    const float Y = X * th;                       // (1 - cos(alpha))/w
+    t.sa = w * X;
     t.ca = (1.0f - th2) * inv;
-    const float X = 2.0f * tau * inv;
-    const float Y = X * th;
     t.dx = fmaf(cp, X, -sp * Y);
     t.dy = fmaf(sp, X, cp * Y);
     t.xn = x + t.dx;
     t.yn = y + t.dy;
-    const float f = atan_over_t(th);
-    t.alpha = 2.0f * th * f;
+    float f;
+    angle_functions(th, th2, t.sa, t.ca, f, t.alpha, t.f1, t.f2);
     t.s = 2.0f * tau * f;
     t.zn = fmaf(t.s, cot, p[2]);
     t.cpn = fmaf(cp, t.ca, -sp * t.sa);
@@ -140,8 +156,7 @@ __device__ __forceinline__ uint32_t predict(float (&p)[6], float (&C)[21], Trig&
     if (flag) return flag;
 
     // ---- Jacobian entries (R3) ----
-    float f1, f2;
-    curv_partials(t.alpha, t.sa, t.ca, f1, f2);
+    const float f1 = t.f1, f2 = t.f2;
     const float cs2 = cw * t.s * t.s;
     const float dXdi = cs2 * f1, dYdi = cs2 * f2;
     const float Fxi = fmaf(cp, dXdi, -sp * dYdi), Fyi = fmaf(sp, dXdi, cp * dYdi);
@@ -230,20 +245,19 @@ __device__ __forceinline__ HitCov hit_cov(float mx, float my, const LayerC& ly) 
 struct Sym3 { float m00, m10, m11, m20, m21, m22; };
 struct Ldl3 { float l10, l20, l21, i0, i1, i2; };
 
+// Branch-free: a non-positive pivot makes the later entries garbage (Inf / NaN), never a trap; the caller must not use
+// F when the result is false.
 __device__ __forceinline__ bool ldl3(const Sym3& S, Ldl3& F) {
-    if (!(S.m00 > 0.0f)) return false;
     F.i0 = frcp(S.m00);
     F.l10 = S.m10 * F.i0;
     F.l20 = S.m20 * F.i0;
     const float d1 = fmaf(-F.l10, S.m10, S.m11);
-    if (!(d1 > 0.0f)) return false;
     F.i1 = frcp(d1);
     const float t21 = fmaf(-F.l20, S.m10, S.m21);
     F.l21 = t21 * F.i1;
     const float d2 = fmaf(-F.l21, t21, fmaf(-F.l20, S.m20, S.m22));
-    if (!(d2 > 0.0f)) return false;
     F.i2 = frcp(d2);
-    return true;
+    return (S.m00 > 0.0f) && (d1 > 0.0f) && (d2 > 0.0f);
 }
 
 // x = S^-1 b
@@ -261,12 +275,12 @@ __device__ __forceinline__ bool innovation(const float (&p)[6], const float (&C)
     Sym3 S;
     S.m00 = C[pk(0, 0)] + V.xx; S.m10 = C[pk(1, 0)] + V.xy; S.m11 = C[pk(1, 1)] + V.yy;
     S.m20 = C[pk(2, 0)]; S.m21 = C[pk(2, 1)]; S.m22 = C[pk(2, 2)] + V.zz;
-    if (!ldl3(S, F)) return false;
+    const bool ok = ldl3(S, F);
     r[0] = mx - p[0]; r[1] = my - p[1]; r[2] = mz - p[2];
     const float y1 = fmaf(-F.l10, r[0], r[1]);
     const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, r[0], r[2]));
     chi2 = fmaf(r[0] * r[0], F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-    return true;
+    return ok;
 }
 
 // Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C <- C - K C[0:3,:].
@@ -274,6 +288,8 @@ __device__ __forceinline__ bool innovation(const float (&p)[6], const float (&C)
 //   (C - K H C) H^T = C H^T - K (S - V) = K V          (because K S = C H^T),
 // which matters in fp32: for low-pT tracks at shallow incidence the predicted position variance exceeds the hit
 // variance by 1e3-1e4 and C - K C would lose every significant digit of the updated position block.
+// ISO: V = diag(V.xx, V.xx, V.zz) known at compile time (sig_r == sig_rphi on every layer).
+template <bool ISO = false>
 __device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], Trig& g, const Ldl3& F, const HitCov& V,
                                             const float (&r)[3]) {
     float K[6][3];
@@ -285,8 +301,7 @@ __device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], Trig&
     const float dth = fmaf(K[5][0], r[0], fmaf(K[5][1], r[1], K[5][2] * r[2]));
     p[4] += dphi;
     p[5] += dth;
-    rotate_small(g.cp, g.sp, dphi, p[4]);
-    rotate_small(g.ct, g.st, dth, p[5]);
+    rotate_pair(g, dphi, dth, p[4], p[5]);
     // momentum block (rows/cols 3..5): C_ab -= sum_k K_ak C_kb, with the still-intact old C[b][k]
 #pragma unroll
     for (int a = 3; a < 6; ++a)
@@ -296,8 +311,13 @@ __device__ __forceinline__ void gain_update(float (&p)[6], float (&C)[21], Trig&
     // columns 0..2: K V
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-        C[pk(i, 0)] = fmaf(K[i][0], V.xx, K[i][1] * V.xy);
-        if (i >= 1) C[pk(i, 1)] = fmaf(K[i][0], V.xy, K[i][1] * V.yy);
+        if (ISO) {
+            C[pk(i, 0)] = K[i][0] * V.xx;
+            if (i >= 1) C[pk(i, 1)] = K[i][1] * V.xx;
+        } else {
+            C[pk(i, 0)] = fmaf(K[i][0], V.xx, K[i][1] * V.xy);
+            if (i >= 1) C[pk(i, 1)] = fmaf(K[i][0], V.xy, K[i][1] * V.yy);
+        }
         if (i >= 2) C[pk(i, 2)] = K[i][2] * V.zz;
     }
 }
