@@ -13,7 +13,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libkf_b200.so")
+_SO = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so")   # KF_B200_LIB: another build of the same library (A/B timing)
 _lib = None
 
 KF_MAX_LAYERS = 32

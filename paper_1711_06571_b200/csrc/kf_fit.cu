@@ -5,6 +5,7 @@
 // and the coalesced store of the result (F9).  Per-layer constants arrive as a __grid_constant__ kernel
 // parameter, i.e. through the constant bank: warp-uniform, no global loads.
 #include "kf_common.cuh"
+#include "kf_state.cuh"
 
 namespace kf {
 
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
     if (t >= a.n) return;
     const float cw = -(float)a.q[t] * a.kb;
     const int64_t seg = EVT ? (int64_t)a.trk_event[t] * a.n_layers : 0;
-    float p[6], C[21];
+    State s;
     float chi2 = 0.0f;
     int nh = 0;
     uint32_t st = 0u;
@@ -46,15 +47,13 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
     bool careful = false;
     for (int attempt = 0; attempt < 3; ++attempt) {
         // F1: coalesced SoA load
-#pragma unroll
-        for (int i = 0; i < 6; ++i) p[i] = a.par[i * a.ld_in + t];
-#pragma unroll
-        for (int i = 0; i < 21; ++i) C[i] = a.cov[i * a.ld_in + t];
-        Trig g;
-        trig_init(g, p[4], p[5]);
+        state_load(s, [&](int i) { return a.par[i * a.ld_in + t]; }, [&](int k) { return a.cov[k * a.ld_in + t]; });
         chi2 = 0.0f;
         nh = 0;
         int bad = -1;
+        // F6 with identity indexing: the hit of the next layer is requested one layer ahead
+        float nx = 0.f, ny = 0.f, nz = 0.f;
+        if (!IDX && !EVT && limit > 0) { nx = a.hxl[0][t]; ny = a.hyl[0][t]; nz = a.hzl[0][t]; }
 #pragma unroll 1
         for (int l = 0; l < limit; ++l) {
             int64_t idx = t;
@@ -68,10 +67,15 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
                 const int64_t h = a.seg_off_dev[seg + l] + idx;
                 mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
             } else {
-                mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+                if (!IDX) {
+                    mx = nx; my = ny; mz = nz;
+                    if (l + 1 < limit) { nx = a.hxl[l + 1][t]; ny = a.hyl[l + 1][t]; nz = a.hzl[l + 1][t]; }
+                } else {
+                    mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+                }
             }
             const LayerC ly = a.layer[l];
-            const uint32_t flag = predict(p, C, g, cw, ly);                    // F2-F5
+            const uint32_t flag = predict(s, cw, ly);                          // F2-F5
             if (flag) {
                 st |= flag;
                 break;
@@ -81,9 +85,9 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
             HitCov V;
             if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
             else V = hit_cov(mx, my, ly);
-            bool ok = innovation(p, C, mx, my, mz, V, Si, r, c2);               // F7 (branch-free; garbage when !ok)
-            gain_update<ISO>(p, C, g, Si, V, r);                                // F8
-            ok = ok && step_finite(p, c2) && p[3] > 0.0f && (!careful || all_finite(p, C));
+            bool ok = innovation(s, mx, my, mz, V, Si, r, c2);                  // F7 (branch-free; garbage when !ok)
+            gain_update<ISO>(s, Si, V, r);                                      // F8
+            ok = ok && step_finite(s, c2) && s.IT.x > 0.0f && (!careful || state_finite(s));
             if (!ok) {
                 bad = l;
                 break;
@@ -92,7 +96,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
             nh += 1;
         }
         if (bad < 0) {
-            if (careful || all_finite(p, C)) break;
+            if (careful || state_finite(s)) break;
             careful = true;          // something non-finite slipped through the cheap per-layer check: find the layer
             st = 0u;
             continue;
@@ -102,11 +106,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
         limit = bad;
     }
     // F9: coalesced store
-    p[4] = wrap_phi(p[4]);
-#pragma unroll
-    for (int i = 0; i < 6; ++i) a.par_o[i * a.ld_out + t] = p[i];
-#pragma unroll
-    for (int i = 0; i < 21; ++i) a.cov_o[i * a.ld_out + t] = C[i];
+    state_store(s, [&](int i, float v) { a.par_o[i * a.ld_out + t] = v; }, [&](int k, float v) { a.cov_o[k * a.ld_out + t] = v; });
     a.chi2_o[t] = chi2;
     a.nhits_o[t] = nh;
     a.status_o[t] = st;

@@ -1,0 +1,248 @@
+// kf_state.cuh -- the per-layer Kalman-filter step on a register-resident state laid out for Blackwell's packed
+// fp32 arithmetic (FFMA2 / FMUL2 / FADD2: two fp32 lanes per instruction; sm_100a).
+//
+// Why: on B200 a scalar three-register FFMA issues at best every ~1.7 cycles per SM sub-partition (measured), a
+// packed FFMA2 every ~2.2 cycles for two FMAs, and FFMA2 takes any scalar register as a free broadcast operand.
+// The 148 x 128 x 2 FP32 peak is therefore only reachable with packed instructions.  The 6x6 algebra of the
+// step is arranged so that its long, regular chains run two rows (or two columns) of a matrix at a time:
+//   rows (x, y) and rows (z, phi) of T = J C and of J C J^T,        columns (1/pT, theta) of T,
+//   rows (0,1), (2,4), (3,5) of the gain K = C H^T S^-1 and of the covariance update.
+// The covariance is stored in exactly the pairs those chains consume and produce, so no repacking is needed between
+// layers; three elements are held twice (C01, C20, C21) and kept identical by copies.
+// Jacobian sparsity ("patterns of elements known ... to be zero or one", sec. 2.1) is written out as in
+// kf_math.cuh.  Formulas: DESIGN.md sec. 3 (R2 helix/cylinder solve, R3 surface Jacobian, R4 Highland noise,
+// R5 3-D update).  Shares nothing with oracle/.
+#pragma once
+#include "kf_math.cuh"
+
+namespace kf {
+
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 fma2(float2 a, float s, float2 c) { return __ffma2_rn(a, make_float2(s, s), c); }   // s: broadcast
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 mul2(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+
+// Track state: 6 parameters, carried sin/cos of both angles, 21 covariance elements (+3 duplicates).
+struct State {
+    float2 XY;           // x, y
+    float2 ZP;           // z, phi
+    float2 IT;           // 1/pT, theta
+    float2 CC, SS;       // (cos phi, cos theta), (sin phi, sin theta)
+    float2 P0, P1, P2;   // (C00, C10), (C01, C11), (C02, C12): rows 0,1 x columns 0,1,2
+    float2 Q0, Q1, Q2;   // (C20, C40), (C21, C41), (C22, C42): rows 2,4 x columns 0,1,2
+    float2 R0, R1, R2;   // (C30, C50), (C31, C51), (C32, C52): rows 3,5 x columns 0,1,2
+    float2 M3, M4;       // (C33, C53), (C43, C54)
+    float C44, C55;
+};
+
+// packed lower-triangular storage <-> State (k = i(i+1)/2 + j)
+template <typename LoadP, typename LoadC>
+__device__ __forceinline__ void state_load(State& s, LoadP par, LoadC cov) {
+    s.XY = f2(par(0), par(1)); s.ZP = f2(par(2), par(4)); s.IT = f2(par(3), par(5));
+    const float c10 = cov(pk(1, 0)), c20 = cov(pk(2, 0)), c21 = cov(pk(2, 1));
+    s.P0 = f2(cov(pk(0, 0)), c10); s.P1 = f2(c10, cov(pk(1, 1))); s.P2 = f2(c20, c21);
+    s.Q0 = f2(c20, cov(pk(4, 0))); s.Q1 = f2(c21, cov(pk(4, 1))); s.Q2 = f2(cov(pk(2, 2)), cov(pk(4, 2)));
+    s.R0 = f2(cov(pk(3, 0)), cov(pk(5, 0))); s.R1 = f2(cov(pk(3, 1)), cov(pk(5, 1))); s.R2 = f2(cov(pk(3, 2)), cov(pk(5, 2)));
+    s.M3 = f2(cov(pk(3, 3)), cov(pk(5, 3))); s.M4 = f2(cov(pk(4, 3)), cov(pk(5, 4)));
+    s.C44 = cov(pk(4, 4)); s.C55 = cov(pk(5, 5));
+    float sp, cp, st, ct;
+    sincosf(s.ZP.y, &sp, &cp);
+    sincosf(s.IT.y, &st, &ct);
+    s.CC = f2(cp, ct); s.SS = f2(sp, st);
+}
+
+template <typename StoreP, typename StoreC>
+__device__ __forceinline__ void state_store(const State& s, StoreP par, StoreC cov) {
+    par(0, s.XY.x); par(1, s.XY.y); par(2, s.ZP.x); par(3, s.IT.x); par(4, wrap_phi(s.ZP.y)); par(5, s.IT.y);
+    cov(pk(0, 0), s.P0.x);
+    cov(pk(1, 0), s.P0.y); cov(pk(1, 1), s.P1.y);
+    cov(pk(2, 0), s.P2.x); cov(pk(2, 1), s.P2.y); cov(pk(2, 2), s.Q2.x);
+    cov(pk(3, 0), s.R0.x); cov(pk(3, 1), s.R1.x); cov(pk(3, 2), s.R2.x); cov(pk(3, 3), s.M3.x);
+    cov(pk(4, 0), s.Q0.y); cov(pk(4, 1), s.Q1.y); cov(pk(4, 2), s.Q2.y); cov(pk(4, 3), s.M4.x); cov(pk(4, 4), s.C44);
+    cov(pk(5, 0), s.R0.y); cov(pk(5, 1), s.R1.y); cov(pk(5, 2), s.R2.y); cov(pk(5, 3), s.M3.y); cov(pk(5, 4), s.M4.y); cov(pk(5, 5), s.C55);
+}
+
+// 0 * inf = NaN, 0 * NaN = NaN: one fused chain over everything
+__device__ __forceinline__ bool state_finite(const State& s) {
+    float2 a = mul2(s.XY, 0.0f);
+    a = fma2(s.ZP, 0.0f, a); a = fma2(s.IT, 0.0f, a);
+    a = fma2(s.P0, 0.0f, a); a = fma2(s.P1, 0.0f, a); a = fma2(s.P2, 0.0f, a);
+    a = fma2(s.Q0, 0.0f, a); a = fma2(s.Q1, 0.0f, a); a = fma2(s.Q2, 0.0f, a);
+    a = fma2(s.R0, 0.0f, a); a = fma2(s.R1, 0.0f, a); a = fma2(s.R2, 0.0f, a);
+    a = fma2(s.M3, 0.0f, a); a = fma2(s.M4, 0.0f, a);
+    return fmaf(0.0f, s.C44, fmaf(0.0f, s.C55, a.x + a.y)) == 0.0f;
+}
+
+// cheap per-layer check: NaN/Inf anywhere in S or the gain reaches chi2 or the parameters
+__device__ __forceinline__ bool step_finite(const State& s, float chi2) {
+    const float2 a = fma2(s.XY, 0.0f, fma2(s.ZP, 0.0f, mul2(s.IT, 0.0f)));
+    return fmaf(0.0f, chi2, a.x + a.y) == 0.0f;
+}
+
+// Predict: transport the state to layer ly, C <- J C J^T + Q (R2-R4).  On a non-zero return s is untouched.
+// cw = -q k Bz.
+__device__ __forceinline__ uint32_t predict(State& s, float cw, const LayerC& ly) {
+    const float cp = s.CC.x, ct = s.CC.y, sp = s.SS.x, st = s.SS.y;
+    const float ist = frcp(st);
+    const float cot = ct * ist;
+    const float pp[6] = {s.XY.x, s.XY.y, s.ZP.x, s.IT.x, s.ZP.y, s.IT.y};
+    Transport t;
+    const uint32_t flag = transport(pp, cw, cp, sp, cot, ly, t);
+    if (flag) return flag;
+
+    // ---- Jacobian (R3): rows x', y' as pairs ab_k = (a_k, b_k), rows z', phi' as pairs cd_k = (c_k, d_k) ----
+    const float cs2 = cw * t.s * t.s;
+    const float dXdi = cs2 * t.f1, dYdi = cs2 * t.f2;
+    const float Fxi = fmaf(cp, dXdi, -sp * dYdi), Fyi = fmaf(sp, dXdi, cp * dYdi);
+    const float iup = frcp(t.up);
+    const float sx = -t.xn * iup, sy = -t.yn * iup;
+    const float si = -fmaf(t.xn, Fxi, t.yn * Fyi) * iup;
+    const float sph = -fmaf(t.yn, t.dx, -t.xn * t.dy) * iup;       // F_x,phi = -dy, F_y,phi = dx
+    const float2 G = f2(t.cpn, t.spn);
+    const float2 ab0 = f2(fmaf(t.cpn, sx, 1.0f), t.spn * sx), ab1 = f2(t.cpn * sy, fmaf(t.spn, sy, 1.0f));
+    const float2 ab3 = fma2(G, si, f2(Fxi, Fyi)), ab4 = fma2(G, sph, f2(-t.dy, t.dx));
+    const float2 H = f2(cot, t.w);
+    const float2 cd0 = mul2(H, sx), cd1 = mul2(H, sy);
+    const float2 cd3 = f2(cot * si, fmaf(t.w, si, cw * t.s)), cd4 = f2(cot * sph, fmaf(t.w, sph, 1.0f));
+    const float c5 = -t.s * ist * ist;
+
+    // ---- T = J C ----
+    // columns 0, 1, 4 of T for the row pairs: T_k = sum_m J_m * C_mk (m = 0, 1, 3, 4); row z' also takes C_2k + c5 C_5k
+#define KF_ROWS(v0, v1, v3, v4, e0, e1, e3, e4) fma2(v0, e0, fma2(v1, e1, fma2(v3, e3, mul2(v4, e4))))
+    const float2 Tab0 = KF_ROWS(ab0, ab1, ab3, ab4, s.P0.x, s.P0.y, s.R0.x, s.Q0.y);
+    float2 Tcd0 = KF_ROWS(cd0, cd1, cd3, cd4, s.P0.x, s.P0.y, s.R0.x, s.Q0.y);
+    Tcd0.x += fmaf(c5, s.R0.y, s.P2.x);
+    const float2 Tab1 = KF_ROWS(ab0, ab1, ab3, ab4, s.P0.y, s.P1.y, s.R1.x, s.Q1.y);
+    float2 Tcd1 = KF_ROWS(cd0, cd1, cd3, cd4, s.P0.y, s.P1.y, s.R1.x, s.Q1.y);
+    Tcd1.x += fmaf(c5, s.R1.y, s.P2.y);
+    const float2 Tab4 = KF_ROWS(ab0, ab1, ab3, ab4, s.Q0.y, s.Q1.y, s.M4.x, s.C44);
+    float2 Tcd4 = KF_ROWS(cd0, cd1, cd3, cd4, s.Q0.y, s.Q1.y, s.M4.x, s.C44);
+    Tcd4.x += fmaf(c5, s.M4.y, s.Q2.y);
+    // columns (3, 5) of T as pairs, one per row: (T_j3, T_j5) = sum_m J_jm * (C_m3, C_m5)
+    const float2 RTa = KF_ROWS(s.R0, s.R1, s.M3, s.M4, ab0.x, ab1.x, ab3.x, ab4.x);
+    const float2 RTb = KF_ROWS(s.R0, s.R1, s.M3, s.M4, ab0.y, ab1.y, ab3.y, ab4.y);
+    const float2 RTd = KF_ROWS(s.R0, s.R1, s.M3, s.M4, cd0.y, cd1.y, cd3.y, cd4.y);
+    float2 RTc = fma2(s.R0, cd0.x, fma2(s.R1, cd1.x, fma2(s.M3, cd3.x, fma2(s.M4, cd4.x, s.R2))));
+    RTc.x = fmaf(c5, s.M3.y, RTc.x);
+    RTc.y = fmaf(c5, s.C55, RTc.y);
+    const float T22 = fmaf(cd0.x, s.P2.x, fmaf(cd1.x, s.P2.y, fmaf(cd3.x, s.R2.x, fmaf(cd4.x, s.Q2.y, fmaf(c5, s.R2.y, s.Q2.x)))));
+    const float2 Tab3 = f2(RTa.x, RTb.x), Tcd3 = f2(RTc.x, RTd.x);
+    // ---- C' = T J^T (rows 1/pT and theta of J are unit rows) ----
+    const float2 nP0 = KF_ROWS(Tab0, Tab1, Tab3, Tab4, ab0.x, ab1.x, ab3.x, ab4.x);          // (C00, C10)
+    const float n11 = fmaf(Tab0.y, ab0.y, fmaf(Tab1.y, ab1.y, fmaf(Tab3.y, ab3.y, Tab4.y * ab4.y)));
+    const float2 nQ0 = KF_ROWS(Tcd0, Tcd1, Tcd3, Tcd4, ab0.x, ab1.x, ab3.x, ab4.x);          // (C20, C40)
+    const float2 nQ1 = KF_ROWS(Tcd0, Tcd1, Tcd3, Tcd4, ab0.y, ab1.y, ab3.y, ab4.y);          // (C21, C41)
+    float2 nQ2 = KF_ROWS(cd0, cd1, cd3, cd4, Tcd0.x, Tcd1.x, Tcd3.x, Tcd4.x);                // (C22 - ..., C42)
+    nQ2.x += fmaf(RTc.y, c5, T22);
+    const float n44 = fmaf(Tcd0.y, cd0.y, fmaf(Tcd1.y, cd1.y, fmaf(Tcd3.y, cd3.y, Tcd4.y * cd4.y)));
+#undef KF_ROWS
+    // ---- multiple scattering (R4), evaluated at the arriving state ----
+    float q33 = 0.0f, q53 = 0.0f, q44 = 0.0f, q55 = 0.0f;
+    if (ly.xx0r > 0.0f) {
+        const float iota = s.IT.x;
+        const float tms = ly.xx0r * ist * iup;                 // xx0 / (sin(theta) cos(inc))
+        const float lg = fmaf(0.038f, flog(tms), 1.0f);
+        const float h = 0.0136f * iota * st * lg;
+        const float v = h * h * tms;                           // theta0^2
+        const float icot = iota * cot;
+        q55 = v;
+        q44 = v * ist * ist;
+        q33 = icot * icot * v;
+        q53 = -icot * v;
+    }
+    // ---- commit ----
+    s.P0 = nP0; s.P1 = f2(nP0.y, n11); s.P2 = f2(nQ0.x, nQ1.x);
+    s.Q0 = nQ0; s.Q1 = nQ1; s.Q2 = nQ2;
+    s.R0 = RTa; s.R1 = RTb; s.R2 = RTc;
+    s.M4 = RTd;
+    s.M3.x += q33; s.M3.y += q53;
+    s.C44 = n44 + q44;
+    s.C55 += q55;
+    s.XY = f2(t.xn, t.yn);
+    s.ZP = f2(t.zn, s.ZP.y + t.alpha);
+    s.CC.x = t.cpn; s.SS.x = t.spn;
+    return 0u;
+}
+
+// Innovation of hit m against the predicted state: factor S = C_pos + V, r = m - pos, chi2 = r^T S^-1 r.
+// Branch-free: when the result is false F, r, chi2 are garbage.
+__device__ __forceinline__ bool innovation(const State& s, float mx, float my, float mz, const HitCov& V, Ldl3& F, float (&r)[3],
+                                           float& chi2) {
+    Sym3 S;
+    S.m00 = s.P0.x + V.xx; S.m10 = s.P0.y + V.xy; S.m11 = s.P1.y + V.yy;
+    S.m20 = s.P2.x; S.m21 = s.P2.y; S.m22 = s.Q2.x + V.zz;
+    const bool ok = ldl3(S, F);
+    r[0] = mx - s.XY.x; r[1] = my - s.XY.y; r[2] = mz - s.ZP.x;
+    const float y1 = fmaf(-F.l10, r[0], r[1]);
+    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, r[0], r[2]));
+    chi2 = fmaf(r[0] * r[0], F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
+    return ok;
+}
+
+// two rows of K = C[:,0:3] S^-1 at once: x = S^-1 b for the pairs (b0, b1, b2)
+__device__ __forceinline__ void ldl3_solve2(const Ldl3& F, float2 b0, float2 b1, float2 b2, float2& x0, float2& x1, float2& x2) {
+    const float2 y1 = fma2(neg2(b0), F.l10, b1);
+    const float2 y2 = fma2(neg2(y1), F.l21, fma2(neg2(b0), F.l20, b2));
+    x2 = mul2(y2, F.i2);
+    x1 = fma2(neg2(x2), F.l21, mul2(y1, F.i1));
+    x0 = fma2(neg2(x2), F.l20, fma2(neg2(x1), F.l10, mul2(b0, F.i0)));
+}
+
+// rotate (c, s) by d for both angles at once: polynomial for |d| < 0.06 (truncation < 6e-11) followed by one Newton
+// step back to unit norm
+__device__ __forceinline__ void rotate_poly2(float2& c, float2& sn_, float2 d) {
+    const float2 d2 = mul2(d, d);
+    const float2 sd = mul2(d, fma2(d2, fma2(d2, 1.0f / 120.0f, f2(-1.0f / 6.0f, -1.0f / 6.0f)), f2(1.0f, 1.0f)));
+    const float2 cd = fma2(d2, fma2(d2, 1.0f / 24.0f, f2(-0.5f, -0.5f)), f2(1.0f, 1.0f));
+    const float2 cn = fma2(c, cd, neg2(mul2(sn_, sd))), sn = fma2(sn_, cd, mul2(c, sd));
+    const float2 k = fma2(fma2(cn, cn, mul2(sn, sn)), -0.5f, f2(1.5f, 1.5f));
+    c = mul2(cn, k); sn_ = mul2(sn, k);
+}
+
+// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C <- C - K C[0:3,:], the columns that touch the
+// measured block in the cancellation-free form K V (see kf_math.cuh).  ISO: V = diag(V.xx, V.xx, V.zz).
+template <bool ISO>
+__device__ __forceinline__ void gain_update(State& s, const Ldl3& F, const HitCov& V, const float (&r)[3]) {
+    float2 KP0, KP1, KP2, KQ0, KQ1, KQ2, KR0, KR1, KR2;      // K rows (0,1), (2,4), (3,5); index = column
+    ldl3_solve2(F, s.P0, s.P1, s.P2, KP0, KP1, KP2);
+    ldl3_solve2(F, s.Q0, s.Q1, s.Q2, KQ0, KQ1, KQ2);
+    ldl3_solve2(F, s.R0, s.R1, s.R2, KR0, KR1, KR2);
+    // state
+    s.XY = fma2(KP0, r[0], fma2(KP1, r[1], fma2(KP2, r[2], s.XY)));
+    const float2 dZP = fma2(KQ0, r[0], fma2(KQ1, r[1], mul2(KQ2, r[2])));
+    const float2 dIT = fma2(KR0, r[0], fma2(KR1, r[1], mul2(KR2, r[2])));
+    s.ZP = add2(s.ZP, dZP);
+    s.IT = add2(s.IT, dIT);
+    const float dphi = dZP.y, dth = dIT.y;
+    if (fmaxf(fabsf(dphi), fabsf(dth)) < 0.06f) {
+        rotate_poly2(s.CC, s.SS, f2(dphi, dth));
+    } else {
+        float sp, cp, st, ct;
+        sincosf(s.ZP.y, &sp, &cp);
+        sincosf(s.IT.y, &st, &ct);
+        s.CC = f2(cp, ct); s.SS = f2(sp, st);
+    }
+    // momentum block: C_ab -= sum_k K_ak C_bk with the still-intact old columns 0..2
+    s.M3 = fma2(neg2(KR0), s.R0.x, fma2(neg2(KR1), s.R1.x, fma2(neg2(KR2), s.R2.x, s.M3)));     // (C33, C53) -= (K3k, K5k) C3k
+    s.M4 = fma2(neg2(s.R0), KQ0.y, fma2(neg2(s.R1), KQ1.y, fma2(neg2(s.R2), KQ2.y, s.M4)));     // (C43, C54) -= K4k (C3k, C5k)
+    s.C44 = fmaf(-KQ0.y, s.Q0.y, fmaf(-KQ1.y, s.Q1.y, fmaf(-KQ2.y, s.Q2.y, s.C44)));
+    s.C55 = fmaf(-KR0.y, s.R0.y, fmaf(-KR1.y, s.R1.y, fmaf(-KR2.y, s.R2.y, s.C55)));
+    // columns 0..2: K V
+    if (ISO) {
+        s.P0 = mul2(KP0, V.xx); s.P1 = mul2(KP1, V.xx);
+        s.Q0 = mul2(KQ0, V.xx); s.Q1 = mul2(KQ1, V.xx);
+        s.R0 = mul2(KR0, V.xx); s.R1 = mul2(KR1, V.xx);
+    } else {
+        s.P0 = fma2(KP0, V.xx, mul2(KP1, V.xy)); s.P1 = fma2(KP0, V.xy, mul2(KP1, V.yy));
+        s.Q0 = fma2(KQ0, V.xx, mul2(KQ1, V.xy)); s.Q1 = fma2(KQ0, V.xy, mul2(KQ1, V.yy));
+        s.R0 = fma2(KR0, V.xx, mul2(KR1, V.xy)); s.R1 = fma2(KR0, V.xy, mul2(KR1, V.yy));
+    }
+    s.Q2 = mul2(KQ2, V.zz); s.R2 = mul2(KR2, V.zz);
+    s.P1.x = s.P0.y;                      // the three duplicates follow the lower triangle
+    s.P2 = f2(s.Q0.x, s.Q1.x);
+}
+
+}  // namespace kf
