@@ -352,6 +352,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
     sev = torch.from_numpy(bi.seed_event).cuda(); shi = torch.from_numpy(bi.seed_hit_idx).cuda()
     out = b.Cands(bi.n_seeds, K, L)
+    bws = torch.empty(max(b.kf_build_workspace_bytes(geom, bi.n_seeds, K), 1), dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda") if hits.n_hits * 28 < (160 << 20) else None
 
@@ -361,7 +362,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
         rec(0)
         b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
         rec(1)
-        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, stream=stream)
+        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, ws=bws, stream=stream)
 
     W = max(args.warmup, 3)
     sampler = ClockSampler(d.local) if (d.rank == 0 and sample_clocks) else None
@@ -381,7 +382,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
         for dst, src in zip(dev, h):
             dst.copy_(src, non_blocking=True)
         b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
-        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, stream=stream)
+        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, ws=bws, stream=stream)
         for dst, src in zip(ho, outs):
             dst.copy_(src, non_blocking=True)
 

@@ -146,11 +146,14 @@ typedef struct {
  * Slots k >= n_cand[s] get nhits = 0, chi2 = 0, status = 0 and hit_idx = -2; their par / cov are not written.
  * cand.q is filled with the seed's charge.  A candidate that cannot be propagated to a layer, leaves
  * |z| <= zmax + window, or fails numerically is finished (status bit set) and carried unchanged.
- * K in 1..32.  kf_build_workspace_bytes() is 0 in this version (candidates live in shared memory); ws may be NULL.
- * kf_build_set_lanes(g): tuning hook, lanes of a warp that cooperate on one seed (4, 8, 16, 32; 0 = automatic);
- * the result does not depend on it. */
+ * K in 1..32.  ws: device workspace of at least kf_build_workspace_bytes(geom, n_seeds, K) bytes (candidate records
+ * and per-layer links of the tiles in flight; ~0.45 MB per resident block, a few hundred blocks); it is only used
+ * while the enqueued kernel runs and may be reused by the next call on the same stream.
+ * kf_build_set_tile(n): tuning hook, seeds owned by one thread block (multiple of 16 in 16..256; 0 = automatic);
+ * the result does not depend on it, the workspace size does (query it after setting the tile).
+ * Errors: NULL pointers, K / first_layer / cuts out of range, bad bin counts, workspace too small (-4), CUDA failure. */
 size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K);
-int kf_build_set_lanes(int32_t lanes);
+int kf_build_set_tile(int32_t seeds_per_block);
 int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
              float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream);

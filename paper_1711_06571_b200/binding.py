@@ -20,7 +20,7 @@ KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
 EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
-           "kf_build", "kf_build_set_lanes", "kf_last_error", "kf_version"]
+           "kf_build", "kf_build_set_tile", "kf_last_error", "kf_version"]
 
 
 class KfError(RuntimeError):
@@ -71,7 +71,7 @@ def lib() -> C.CDLL:
         l.kf_fit.argtypes = [C.c_void_p] * 7
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
-        l.kf_build_set_lanes.argtypes = [C.c_int32]
+        l.kf_build_set_tile.argtypes = [C.c_int32]
         l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = l
     return _lib
@@ -263,20 +263,28 @@ class Cands:
         return d
 
 
-def kf_build_set_lanes(lanes: int):
-    _check(lib().kf_build_set_lanes(C.c_int32(lanes)), "kf_build_set_lanes")
+def kf_build_set_tile(seeds_per_block: int):
+    _check(lib().kf_build_set_tile(C.c_int32(seeds_per_block)), "kf_build_set_tile")
+
+
+def kf_build_workspace_bytes(geom: Geom, n_seeds: int, K: int) -> int:
+    return int(lib().kf_build_workspace_bytes(C.byref(geom.c), n_seeds, K))
 
 
 def kf_build(geom: Geom, hits: Hits, binned: Binned, seeds: Tracks, seed_event, seed_hit_idx, first_layer: int, K: int, chi2_cut: float,
-             n_sigma: float, out: Cands | None = None, stream=None) -> Cands:
-    """include/kf.h kf_build.  seed_event [n] int32 device tensor (or None), seed_hit_idx [first_layer, seeds.ld] int32 (or None)."""
+             n_sigma: float, out: Cands | None = None, ws: torch.Tensor | None = None, stream=None) -> Cands:
+    """include/kf.h kf_build.  seed_event [n] int32 device tensor (or None), seed_hit_idx [first_layer, seeds.ld] int32 (or None).
+    Allocates the output and the workspace with torch when not given."""
     _require_cuda()
     if out is None:
         out = Cands(seeds.n, K, geom.n_layers, seeds.par.device)
     if seed_hit_idx is not None:
         assert tuple(seed_hit_idx.shape) == (first_layer, seeds.ld)
+    if ws is None:
+        ws = torch.empty(max(kf_build_workspace_bytes(geom, seeds.n, K), 1), dtype=torch.uint8, device=seeds.par.device)
     sc = seeds.c()
     rc = lib().kf_build(C.byref(geom.c), C.byref(hits.c), C.byref(binned.c), C.byref(sc), _ptr(seed_event, torch.int32), _ptr(seed_hit_idx, torch.int32),
-                        first_layer, K, chi2_cut, n_sigma, C.byref(out.c), None, 0, _stream(stream))
+                        first_layer, K, chi2_cut, n_sigma, C.byref(out.c), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
     _check(rc, "kf_build")
+    out._ws = ws    # keep the workspace alive until the stream has consumed it
     return out

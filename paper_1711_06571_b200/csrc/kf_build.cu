@@ -4,397 +4,466 @@
 // hits represent the most likely continuation ... branching to explore multiple candidate tracks per seed"
 // (sec. 2); "a fixed number of slots for each track seed" (sec. 4.3).
 //
-// One kernel for all layers.  A group of G lanes (G = 4, 8, 16 or 32, a template parameter) owns one seed; the <= K
-// candidates of the seed live in shared memory (33 words each: 6 parameters, 21 packed covariance elements, chi2,
-// nhits/status word, carried sin/cos of phi and theta) and never touch HBM between layers.  Per layer:
-//   phase 1  lanes loop over the parents: predict (F2-F5), window -> bin ranges (B2), LDL^T factor of S
-//   phase 2  the group walks the window runs of every parent with unit-stride lanes over the sorted hits: strict
-//            window test + chi2 (B3); passing children are appended to a small buffer that is pruned to the best K
-//            (rank by counting inside the group, B4) whenever it fills
-//   phase 3  one hit-less / finished child per parent that produced no hit child; final ranking
-//   phase 4  lanes loop over the kept children: Kalman update (B5), per-layer link (parent slot, hit)
-// At the end the links are traced back into per-candidate hit lists and everything is stored SoA (B6).
+// One kernel for all layers.  A block of 256 threads owns a tile of S seeds and walks the layers with block-level
+// phases; inside every phase one THREAD owns one live candidate (or one seed), so the long dependent chains of the
+// Kalman arithmetic run at full lane occupancy however few candidates a seed has:
+//   phase 1  thread per live candidate: predict (F2-F5), window -> bin ranges (B2), LDL^T factor of S, then the
+//            window scan (B3): strict window test + chi2 per hit, the passing hits kept as the candidate's own
+//            best-K list (sorted insert, shared memory)
+//   phase 2  thread per seed: K-way merge of the lists of its <= K parents -> the best K children (B4, total order
+//            R10); block scan of the child counts -> dense child positions
+//   phase 3  thread per surviving child: Kalman update (B5), per-layer link (parent slot, hit)
+// Candidate records (33 words: 6 parameters, 21 packed covariance elements, carried sin/cos, chi2, meta) live in
+// a block-private global workspace that stays L2-resident: record c of the current layer at a DENSE index (seed
+// offset + slot), struct-of-arrays over the index, so every record load and store is coalesced.  Two buffers: A
+// (updated states) and B (predicted states).  When the tile has more live candidates than the list area holds, the
+// seeds are taken in rounds.  At the end the links are traced back into hit lists and stored SoA (B6).
+#include <algorithm>
 #include "kf_common.cuh"
+#include "kf_state.cuh"
 #include "kf_binmath.cuh"
 
 namespace kf {
 
-constexpr int BUILD_BLOCK = 128;
-constexpr int NS = 33;          // words per candidate record
-constexpr int NW = 20;          // words per parent window record
+#ifndef KF_BUILD_MINB
+#define KF_BUILD_MINB 2
+#endif
+constexpr int BUILD_NT = 256;
+constexpr int NREC = 33;                  // words per candidate record
 constexpr int HITPOS_NONE = 0x7fffffff;
-
-// candidate record
-enum { R_PAR = 0, R_COV = 6, R_CHI2 = 27, R_META = 28, R_TRIG = 29 };
-// meta word: bits 0-7 nhits, bit 8 finished, bits 16-19 status
-__device__ __forceinline__ int meta_pack(int nhits, bool fin, uint32_t st) { return nhits | (fin ? 256 : 0) | (int)(st << 16); }
-// window record
-enum { W_KIND = 0, W_X = 1, W_Y = 2, W_Z = 3, W_THR2 = 4, W_DZ = 5, W_LDL = 6, W_FOK = 12, W_FIRST = 13, W_NB = 14, W_ZLO = 15, W_ZHI = 16,
-       W_CHI2 = 17, W_NH = 18, W_SBAD = 19 };
-enum { KIND_OPEN = 0, KIND_FIN = 1 };
+constexpr int LIST_BYTES = 48 * 1024;     // shared memory for the per-candidate child lists
+enum { W_TRIG = 27, W_CHI2 = 31, W_META = 32 };
+// meta word of a record: bits 0-7 nhits, bit 8 finished, bits 16-19 status
+// info word of a parent in a round: bits 0-7 nhits, bit 8 finished (child inherits the unchanged state), bits 16-19 status to add
 
 struct BuildArgs {
-    int32_t n_layers, first_layer, K, n_phi, n_z, cap;
+    int32_t n_layers, first_layer, K, n_phi, n_z, S, ncap;
     float kb, chi2_cut, n_sigma, inv_dphi;
-    int64_t n_seeds, ld_seed, ld_out;
+    int64_t n_seeds, ld_seed, ld_out, n_tiles;
     const float *par, *cov; const int8_t* q;
     const int32_t *seed_event, *seed_hit_idx;
     const float *sx, *sy, *sz; const int32_t *perm, *bin_off;
     float *par_o, *cov_o, *chi2_o; int8_t* q_o; int32_t* nhits_o; uint32_t* status_o; int32_t *hit_idx_o, *n_cand_o;
+    float* ws_rec;            // [grid][2][NREC][S*K]
+    int32_t* ws_link_hit;     // [grid][n_layers][S*K]
+    uint8_t* ws_link_par;     // [grid][n_layers][S*K]
     LayerC layer[KF_MAX_LAYERS];
     float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax); (sig_rphi/r)^2
 };
 
-// words of shared memory per seed
-__host__ __device__ inline int seed_words(int K, int L, int cap) {
-    return 2 * K * NS + K * NW + L * K + (L * K + 3) / 4 + 2 * 4 * cap;
+// record <-> State; buf points at word 0 of the buffer, stride SK between words
+__device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const float* buf, int SK, int c) {
+    state_set(s, [&](int i) { return buf[i * SK + c]; }, [&](int k) { return buf[(6 + k) * SK + c]; });
+    s.CC = f2(buf[(W_TRIG + 0) * SK + c], buf[(W_TRIG + 2) * SK + c]);
+    s.SS = f2(buf[(W_TRIG + 1) * SK + c], buf[(W_TRIG + 3) * SK + c]);
+    chi2 = buf[W_CHI2 * SK + c];
+    meta = __float_as_int(buf[W_META * SK + c]);
 }
 
-struct Key { float chi2; int nh, parent, hitpos; };
-__device__ __forceinline__ bool key_less(const Key& a, const Key& b) {   // a ranks before b (R10)
-    if (a.nh != b.nh) return a.nh > b.nh;
-    if (a.chi2 != b.chi2) return a.chi2 < b.chi2;
-    if (a.parent != b.parent) return a.parent < b.parent;
-    return a.hitpos < b.hitpos;
+__device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, float* buf, int SK, int c) {
+    state_store<false>(s, [&](int i, float v) { buf[i * SK + c] = v; }, [&](int k, float v) { buf[(6 + k) * SK + c] = v; });
+    buf[(W_TRIG + 0) * SK + c] = s.CC.x; buf[(W_TRIG + 1) * SK + c] = s.SS.x;
+    buf[(W_TRIG + 2) * SK + c] = s.CC.y; buf[(W_TRIG + 3) * SK + c] = s.SS.y;
+    buf[W_CHI2 * SK + c] = chi2;
+    buf[W_META * SK + c] = __int_as_float(meta);
 }
 
-template <int G>
-__device__ __forceinline__ int group_sum(int v, unsigned gmask) {
+__device__ __forceinline__ void rec_copy(const float* src, int cs, float* dst, int cd, int SK) {
 #pragma unroll
-    for (int d = G / 2; d >= 1; d >>= 1) v += __shfl_xor_sync(gmask, v, d);
-    return v;
+    for (int w = 0; w < NREC; ++w) dst[w * SK + cd] = src[w * SK + cs];
 }
 
-// Keep the best min(K, #valid) entries of src[0..n) in rank order in dst; entries of parents flagged sbad are dropped.
-template <int G>
-__device__ __forceinline__ int prune(const int* src, int* dst, int n, int cap, int K, const float* W, int lane, unsigned gmask) {
-    const float* s_chi2 = (const float*)src;
-    const int *s_nh = src + cap, *s_par = src + 2 * cap, *s_hit = src + 3 * cap;
-    int nvalid = 0;
-    for (int e = lane; e < n; e += G) {
-        Key a = {s_chi2[e], s_nh[e], s_par[e], s_hit[e]};
-        const bool valid = a.hitpos == HITPOS_NONE || __float_as_int(W[a.parent * NW + W_SBAD]) == 0;
-        if (!valid) continue;
-        ++nvalid;
-        int rank = 0;
-        for (int f = 0; f < n; ++f) {
-            Key b = {s_chi2[f], s_nh[f], s_par[f], s_hit[f]};
-            const bool vb = b.hitpos == HITPOS_NONE || __float_as_int(W[b.parent * NW + W_SBAD]) == 0;
-            rank += (vb && key_less(b, a)) ? 1 : 0;
-        }
-        if (rank < K) {
-            ((float*)dst)[rank] = a.chi2; dst[cap + rank] = a.nh; dst[2 * cap + rank] = a.parent; dst[3 * cap + rank] = a.hitpos;
-        }
+// ascending (chi2, hit) list of at most K entries, entry j of candidate i at [j * ncap + i] (conflict-free)
+__device__ __forceinline__ void list_insert(float* lc, int* lh, int ncap, int K, int& n, float c, int h) {
+    int pos;
+    if (n == K) {
+        const float cl = lc[(K - 1) * ncap]; const int hl = lh[(K - 1) * ncap];
+        if (!(c < cl || (c == cl && h < hl))) return;
+        pos = K - 1;
+    } else {
+        pos = n++;
     }
-    nvalid = group_sum<G>(nvalid, gmask);
-    __syncwarp(gmask);
-    return nvalid < K ? nvalid : K;
+    while (pos > 0) {
+        const float cp = lc[(pos - 1) * ncap]; const int hp = lh[(pos - 1) * ncap];
+        if (!(c < cp || (c == cp && h < hp))) break;
+        lc[pos * ncap] = cp; lh[pos * ncap] = hp;
+        --pos;
+    }
+    lc[pos * ncap] = c; lh[pos * ncap] = h;
 }
 
-template <int G>
-__global__ void __launch_bounds__(BUILD_BLOCK) kf_build_kernel(const __grid_constant__ BuildArgs a) {
-    extern __shared__ float smem[];
-    const int lane = threadIdx.x % G;
-    const int grp = threadIdx.x / G;
-    const unsigned gmask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
-    const int64_t s = (int64_t)blockIdx.x * (BUILD_BLOCK / G) + grp;
-    if (s >= a.n_seeds) return;          // whole group leaves together
-    const int K = a.K, L = a.n_layers, cap = a.cap;
-    float* A = smem + (size_t)grp * seed_words(K, L, cap);
-    float* B = A + K * NS;
-    float* W = B + K * NS;
-    int* link_hit = (int*)(W + K * NW);
-    unsigned char* link_par = (unsigned char*)(link_hit + L * K);
-    int* buf0 = link_hit + L * K + (L * K + 3) / 4;
-    int* buf1 = buf0 + 4 * cap;
-
-    const float cw = -(float)a.q[s] * a.kb;
-    const int ev = a.seed_event ? a.seed_event[s] : 0;
-    // seed -> slot 0
-    for (int i = lane; i < 27; i += G) A[i] = (i < 6) ? a.par[(int64_t)i * a.ld_seed + s] : a.cov[(int64_t)(i - 6) * a.ld_seed + s];
-    __syncwarp(gmask);
-    if (lane == 0) {
-        Trig g;
-        trig_init(g, A[R_PAR + 4], A[R_PAR + 5]);
-        A[R_CHI2] = 0.0f;
-        A[R_META] = __int_as_float(meta_pack(a.first_layer, false, 0u));
-        A[R_TRIG] = g.cp; A[R_TRIG + 1] = g.sp; A[R_TRIG + 2] = g.st; A[R_TRIG + 3] = g.ct;
+// exclusive scan of one int per thread over the block (BUILD_NT threads); returns the exclusive prefix, total in *total
+__device__ __forceinline__ int block_exclusive_scan(int v, int* s_warp, int* total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
     }
-    __syncwarp(gmask);
-    int nc = 1;
+    if (lane == 31) s_warp[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int t = lane < BUILD_NT / 32 ? s_warp[lane] : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, t, d);
+            if (lane >= d) t += o;
+        }
+        s_warp[lane] = t;
+    }
+    __syncthreads();
+    const int base = w > 0 ? s_warp[w - 1] : 0;
+    *total = s_warp[BUILD_NT / 32 - 1];
+    __syncthreads();
+    return base + inc - v;
+}
 
-    for (int l = a.first_layer; l < L; ++l) {
-        const LayerC& ly = a.layer[l];
-        const bool iso = ly.var_r == ly.var_rphi;
-        const int64_t seg = (int64_t)ev * L + l;
-        // ---------------- phase 1: predict + window ----------------
-        for (int c = lane; c < nc; c += G) {
-            const float* rec = A + c * NS;
-            float* out = B + c * NS;
-            float* w = W + c * NW;
-            float p[6], C[21];
-#pragma unroll
-            for (int i = 0; i < 6; ++i) p[i] = rec[R_PAR + i];
-#pragma unroll
-            for (int i = 0; i < 21; ++i) C[i] = rec[R_COV + i];
-            Trig g = {rec[R_TRIG], rec[R_TRIG + 1], rec[R_TRIG + 2], rec[R_TRIG + 3]};
-            const int meta = __float_as_int(rec[R_META]);
-            uint32_t flag = 0u;
-            bool fin = (meta & 256) != 0;
-            float thr2 = 0.f, dzw = 0.f;
-            Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-            bool fok = false;
-            WindowBins wb = {0, 0, 0, -1};
-            if (!fin) {
-                flag = predict(p, C, g, cw, ly);
-                if (!flag) {
-                    const float x = p[0], y = p[1];
-                    const float r2 = fmaf(x, x, y * y);
-                    const float num = fmaf(x * x, C[pk(1, 1)], fmaf(-2.0f * x * y, C[pk(1, 0)], y * y * C[pk(0, 0)]));
-                    const float varphi = fmaxf(num / (r2 * r2), 0.0f);
-                    const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
-                    dzw = a.n_sigma * sqrtf(C[pk(2, 2)] + ly.var_z);
-                    if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
-                    else if (fabsf(p[2]) > ly.zmax + dzw) flag = ST_LEFT_Z;
-                    else {
-                        thr2 = dphi * dphi * r2;
-                        wb = window_bins(atan2f(y, x), dphi, p[2], dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
-                        if (iso) {
-                            Sym3 S;
-                            S.m00 = C[pk(0, 0)] + ly.var_r; S.m10 = C[pk(1, 0)]; S.m11 = C[pk(1, 1)] + ly.var_r;
-                            S.m20 = C[pk(2, 0)]; S.m21 = C[pk(2, 1)]; S.m22 = C[pk(2, 2)] + ly.var_z;
-                            fok = ldl3(S, F);
-                        }
+// shared memory carve-up (bytes), identical on host and device
+struct BuildSmem { int nc, off, nnew, offn, sel_chi2, sel_hit, sel_pk, cseed, l_chi2, l_hit, l_cnt, l_head, p_chi2, p_info, misc, total; };
+__host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap) {
+    BuildSmem m;
+    int o = 0;
+    auto take = [&](int bytes) { const int at = o; o += (bytes + 15) & ~15; return at; };
+    m.nc = take(4 * S); m.off = take(4 * (S + 1)); m.nnew = take(4 * S); m.offn = take(4 * (S + 1));
+    m.sel_chi2 = take(4 * S * K); m.sel_hit = take(4 * S * K); m.sel_pk = take(4 * S * K); m.cseed = take(2 * S * K);
+    m.l_chi2 = take(4 * ncap * K); m.l_hit = take(4 * ncap * K); m.l_cnt = take(ncap); m.l_head = take(ncap);
+    m.p_chi2 = take(4 * ncap); m.p_info = take(4 * ncap);
+    m.misc = take(4 * 40);
+    m.total = o;
+    return m;
+}
+
+template <bool ISO>
+__global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const __grid_constant__ BuildArgs a) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int S = a.S, K = a.K, L = a.n_layers, ncap = a.ncap, SK = S * K;
+    const BuildSmem m = build_smem(S, K, ncap);
+    int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off);
+    int* s_nnew = (int*)(smem + m.nnew); int* s_offn = (int*)(smem + m.offn);
+    float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit);
+    int* sel_pk = (int*)(smem + m.sel_pk);
+    unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
+    float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
+    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
+    float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
+    int* s_misc = (int*)(smem + m.misc);          // [0..31] warp sums of the scan, [32] round end
+    const int tid = threadIdx.x;
+
+    float* recA = a.ws_rec + (size_t)blockIdx.x * 2 * NREC * SK;
+    float* recB = recA + (size_t)NREC * SK;
+    int32_t* link_hit = a.ws_link_hit + (size_t)blockIdx.x * L * SK;
+    uint8_t* link_par = a.ws_link_par + (size_t)blockIdx.x * L * SK;
+
+    for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+        const int64_t s0 = tile * S;
+        const int ns = (int)min((int64_t)S, a.n_seeds - s0);
+        // ---- seeds -> one candidate each, dense index = seed ----
+        if (tid < S) {
+            if (tid < ns) {
+                const int64_t sg = s0 + tid;
+                State st;
+                state_load(st, [&](int i) { return a.par[(int64_t)i * a.ld_seed + sg]; }, [&](int k) { return a.cov[(int64_t)k * a.ld_seed + sg]; });
+                rec_store(st, 0.0f, a.first_layer, recA, SK, tid);
+            }
+            s_nc[tid] = tid < ns ? 1 : 0;
+            s_off[tid] = tid < ns ? tid : ns;
+            if (tid < ns) s_cseed[tid] = (unsigned short)tid;
+        }
+        if (tid == 0) s_off[S] = ns;
+        __syncthreads();
+
+        for (int l = a.first_layer; l < L; ++l) {
+            const LayerC& ly = a.layer[l];
+            // ---------------- rounds of whole seeds whose candidates fit the list area ----------------
+            int r0 = 0;
+            while (r0 < ns) {
+                const int base = s_off[r0];
+                int r1 = ns;
+                if (s_off[ns] - base > ncap) {
+                    if (tid >= r0 && tid < ns) {
+                        const bool fits = s_off[tid + 1] - base <= ncap;
+                        const bool next_fits = tid + 1 < ns && s_off[tid + 2] - base <= ncap;
+                        if (fits && !next_fits) s_misc[32] = tid + 1;
                     }
+                    __syncthreads();
+                    r1 = s_misc[32];
                 }
-                fin = flag != 0u;
-            }
-            if (fin) {   // finished now or before: the child inherits the unchanged state
-#pragma unroll
-                for (int i = 0; i < NS; ++i) out[i] = rec[i];
-                w[W_KIND] = __int_as_float(KIND_FIN | (int)(flag << 8));
-            } else {
-#pragma unroll
-                for (int i = 0; i < 6; ++i) out[R_PAR + i] = p[i];
-#pragma unroll
-                for (int i = 0; i < 21; ++i) out[R_COV + i] = C[i];
-                out[R_CHI2] = rec[R_CHI2]; out[R_META] = rec[R_META];
-                out[R_TRIG] = g.cp; out[R_TRIG + 1] = g.sp; out[R_TRIG + 2] = g.st; out[R_TRIG + 3] = g.ct;
-                w[W_KIND] = __int_as_float(KIND_OPEN);
-                w[W_X] = p[0]; w[W_Y] = p[1]; w[W_Z] = p[2]; w[W_THR2] = thr2; w[W_DZ] = dzw;
-                w[W_LDL] = F.l10; w[W_LDL + 1] = F.l20; w[W_LDL + 2] = F.l21; w[W_LDL + 3] = F.i0; w[W_LDL + 4] = F.i1; w[W_LDL + 5] = F.i2;
-                w[W_FOK] = __int_as_float(fok ? 1 : 0);
-                w[W_FIRST] = __int_as_float(wb.first); w[W_NB] = __int_as_float(wb.n_b);
-                w[W_ZLO] = __int_as_float(wb.iz_lo); w[W_ZHI] = __int_as_float(wb.iz_hi);
-            }
-            w[W_CHI2] = rec[R_CHI2];
-            w[W_NH] = __int_as_float(meta & 255);
-            w[W_SBAD] = __int_as_float(0);
-        }
-        __syncwarp(gmask);
-        // ---------------- phase 2: window scan ----------------
-        int* buf = buf0;
-        int* alt = buf1;
-        int n_buf = 0;
-        unsigned has_child = 0u;
-        for (int c = 0; c < nc; ++c) {
-            const float* w = W + c * NW;
-            if ((__float_as_int(w[W_KIND]) & 255) != KIND_OPEN) continue;
-            const float px = w[W_X], py = w[W_Y], pz = w[W_Z], thr2 = w[W_THR2], dzw = w[W_DZ];
-            Ldl3 F = {w[W_LDL], w[W_LDL + 1], w[W_LDL + 2], w[W_LDL + 3], w[W_LDL + 4], w[W_LDL + 5]};
-            const bool fok = __float_as_int(w[W_FOK]) != 0;
-            const int first = __float_as_int(w[W_FIRST]), nb = __float_as_int(w[W_NB]);
-            const int zlo = __float_as_int(w[W_ZLO]), zhi = __float_as_int(w[W_ZHI]);
-            const float chi2_par = w[W_CHI2];
-            const int nh_child = __float_as_int(w[W_NH]) + 1;
-            const float* Bc = B + c * NS;
-            for (int iz = zlo; iz <= zhi; ++iz) {
-                const int64_t row = (seg * a.n_z + iz) * a.n_phi;
-                for (int run = 0; run < 2; ++run) {
-                    int b0, b1;
-                    if (run == 0) { b0 = first; b1 = min(first + nb, a.n_phi); }
-                    else { b0 = 0; b1 = first + nb - a.n_phi; }
-                    if (b1 <= b0) continue;
-                    const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
-                    for (int hb = h0; hb < h1; hb += G) {
-                        const int h = hb + lane;
-                        bool pass = false;
-                        float c2 = 0.f;
-                        if (h < h1) {
-                            const float mx = a.sx[h], my = a.sy[h], mz = a.sz[h];
-                            const float cr = fmaf(px, my, -py * mx);
-                            const bool in_win = (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) && (fabsf(mz - pz) <= dzw);
-                            if (in_win) {
-                                bool ok = fok;
-                                if (!iso) {
-                                    const HitCov V = hit_cov(mx, my, ly);
-                                    Sym3 S;
-                                    S.m00 = Bc[R_COV + 0] + V.xx; S.m10 = Bc[R_COV + 1] + V.xy; S.m11 = Bc[R_COV + 2] + V.yy;
-                                    S.m20 = Bc[R_COV + 3]; S.m21 = Bc[R_COV + 4]; S.m22 = Bc[R_COV + 5] + V.zz;
-                                    ok = ldl3(S, F);
-                                }
-                                if (!ok) W[c * NW + W_SBAD] = __int_as_float(1);
-                                else {
-                                    const float r0 = mx - px, r1 = my - py, r2 = mz - pz;
-                                    const float y1 = fmaf(-F.l10, r0, r1);
-                                    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, r0, r2));
-                                    c2 = fmaf(r0 * r0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                    pass = c2 < a.chi2_cut;
+                const int nround = s_off[r1] - base;
+                // ---------------- phase 1: predict + window + scan, thread per candidate ----------------
+                for (int i = tid; i < nround; i += BUILD_NT) {
+                    const int c = base + i;
+                    const int64_t sg = s0 + s_cseed[c];
+                    const float cw = -(float)a.q[sg] * a.kb;
+                    const int ev = a.seed_event ? a.seed_event[sg] : 0;
+                    State st;
+                    float chi2;
+                    int meta;
+                    rec_load(st, chi2, meta, recA, SK, c);
+                    uint32_t flag = 0u;
+                    bool fin = (meta & 256) != 0;
+                    float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
+                    float c00 = 0.f, c10 = 0.f, c11 = 0.f, c20 = 0.f, c21 = 0.f, c22 = 0.f;
+                    Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                    bool fok = false;
+                    WindowBins wb = {0, 0, 0, -1};
+                    if (!fin) {
+                        flag = predict(st, cw, ly);
+                        if (!flag) {
+                            px = st.XY.x; py = st.XY.y; pz = st.ZP.x;
+                            c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
+                            const float r2 = fmaf(px, px, py * py);
+                            const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
+                            const float varphi = fmaxf(num / (r2 * r2), 0.0f);
+                            const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
+                            dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+                            if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
+                            else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
+                            else {
+                                thr2 = dphi * dphi * r2;
+                                wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+                                if (ISO) {
+                                    Sym3 Sm;
+                                    Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
+                                    Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
+                                    fok = ldl3(Sm, F);
                                 }
                             }
                         }
-                        const unsigned m = __ballot_sync(gmask, pass);
-                        if (m) {
-                            const int n_new = __popc(m);
-                            if (n_buf + n_new > cap) {
-                                __syncwarp(gmask);
-                                n_buf = prune<G>(buf, alt, n_buf, cap, K, W, lane, gmask);
-                                int* t = buf; buf = alt; alt = t;
+                        fin = flag != 0u;
+                    }
+                    int cnt = 0;
+                    if (!fin) {
+                        rec_store(st, chi2, meta, recB, SK, c);
+                        // ---- window scan (B3) ----
+                        bool sbad = false;
+                        float* lc = s_lchi2 + i;
+                        int* lh = s_lhit + i;
+                        const int64_t seg = (int64_t)ev * L + l;
+                        for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
+                            const int64_t row = (seg * a.n_z + iz) * a.n_phi;
+                            for (int run = 0; run < 2; ++run) {
+                                int b0, b1;
+                                if (run == 0) { b0 = wb.first; b1 = min(wb.first + wb.n_b, a.n_phi); }
+                                else { b0 = 0; b1 = wb.first + wb.n_b - a.n_phi; }
+                                if (b1 <= b0) continue;
+                                const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
+                                for (int h = h0; h < h1; ++h) {
+                                    const float mx = a.sx[h], my = a.sy[h], mz = a.sz[h];
+                                    const float cr = fmaf(px, my, -py * mx);
+                                    const bool in_win = (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                                        (fabsf(mz - pz) <= dzw);
+                                    if (!in_win) continue;
+                                    bool ok = fok;
+                                    if (!ISO) {
+                                        const HitCov V = hit_cov(mx, my, ly);
+                                        Sym3 Sm;
+                                        Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
+                                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
+                                        ok = ldl3(Sm, F);
+                                    }
+                                    if (!ok) { sbad = true; continue; }
+                                    const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
+                                    const float y1 = fmaf(-F.l10, q0, q1);
+                                    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
+                                    const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
+                                    if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
+                                }
                             }
-                            if (pass) {
-                                const int idx = n_buf + __popc(m & ((1u << (threadIdx.x & 31)) - 1u));
-                                ((float*)buf)[idx] = chi2_par + c2; buf[cap + idx] = nh_child; buf[2 * cap + idx] = c; buf[3 * cap + idx] = h;
-                            }
-                            n_buf += n_new;
-                            has_child |= 1u << c;
+                        }
+                        if (sbad) {      // S not positive definite: one finished child with the unchanged state
+                            fin = true;
+                            flag = ST_NUMERIC;
+                            cnt = 0;
                         }
                     }
+                    if (fin) rec_copy(recA, c, recB, c, SK);
+                    s_lcnt[i] = (unsigned char)cnt;
+                    s_lhead[i] = 0;
+                    s_pchi2[i] = chi2;
+                    s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
                 }
+                __syncthreads();
+                // ---------------- phase 2: best K children of a seed, thread per seed (B4) ----------------
+                if (tid >= r0 && tid < r1) {
+                    const int s = tid;
+                    const int nc = s_nc[s], ib = s_off[s] - base;
+                    int n_out = 0;
+                    for (; n_out < K; ++n_out) {
+                        int bk = -1, bnh = -1, bhit = 0, binfo = 0;
+                        float bchi = 0.f;
+                        for (int k = 0; k < nc; ++k) {
+                            const int i = ib + k;
+                            const int info = s_pinfo[i], head = s_lhead[i], cnt = s_lcnt[i];
+                            int nh, hit;
+                            float cc;
+                            if (cnt == 0) {              // finished or hit-less parent: exactly one child
+                                if (head) continue;
+                                nh = info & 255; cc = s_pchi2[i]; hit = HITPOS_NONE;
+                            } else {
+                                if (head >= cnt) continue;
+                                nh = (info & 255) + 1; cc = s_lchi2[head * ncap + i]; hit = s_lhit[head * ncap + i];
+                            }
+                            if (bk < 0 || nh > bnh || (nh == bnh && cc < bchi)) { bk = k; bnh = nh; bchi = cc; bhit = hit; binfo = info; }
+                        }
+                        if (bk < 0) break;
+                        s_lhead[ib + bk] += 1;
+                        sel_chi2[s * K + n_out] = bchi;
+                        sel_hit[s * K + n_out] = bhit;
+                        sel_pk[s * K + n_out] = bk | (bnh << 8) | (binfo & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
+                    }
+                    s_nnew[s] = n_out;
+                }
+                __syncthreads();
+                r0 = r1;
             }
-        }
-        __syncwarp(gmask);
-        // ---------------- phase 3: hit-less / finished children, final ranking ----------------
-        for (int c = 0; c < nc; ++c) {
-            const float* w = W + c * NW;
-            const bool open = (__float_as_int(w[W_KIND]) & 255) == KIND_OPEN;
-            const bool sbad = __float_as_int(w[W_SBAD]) != 0;
-            if (open && !sbad && ((has_child >> c) & 1u)) continue;
-            if (open && sbad)      // S not positive definite: the finished child inherits the unchanged state, not the prediction
-                for (int i = lane; i < NS; i += G) B[c * NS + i] = A[c * NS + i];
-            if (n_buf + 1 > cap) {
-                __syncwarp(gmask);
-                n_buf = prune<G>(buf, alt, n_buf, cap, K, W, lane, gmask);
-                int* t = buf; buf = alt; alt = t;
+            // ---------------- dense positions of the children ----------------
+            {
+                const int v = tid < ns ? s_nnew[tid] : 0;
+                int tot;
+                const int ex = block_exclusive_scan(v, s_misc, &tot);
+                if (tid < S) s_offn[tid] = tid < ns ? ex : tot;
+                if (tid == 0) s_offn[S] = tot;
+                for (int j = 0; j < v; ++j) s_cseed[ex + j] = (unsigned short)tid;
+                __syncthreads();
             }
-            if (lane == 0) {
-                ((float*)buf)[n_buf] = w[W_CHI2]; buf[cap + n_buf] = __float_as_int(w[W_NH]); buf[2 * cap + n_buf] = c; buf[3 * cap + n_buf] = HITPOS_NONE;
-            }
-            ++n_buf;
-        }
-        __syncwarp(gmask);
-        const int n_new = prune<G>(buf, alt, n_buf, cap, K, W, lane, gmask);
-        const int* sel = alt;
-        // ---------------- phase 4: update the survivors ----------------
-        for (int j = lane; j < n_new; j += G) {
-            const int parent = sel[2 * cap + j], hitpos = sel[3 * cap + j];
-            const float* rec = B + parent * NS;
-            const float* w = W + parent * NW;
-            float* out = A + j * NS;
-            int meta = __float_as_int(rec[R_META]);
-            int link;
-            if (hitpos == HITPOS_NONE) {
-                const int kind = __float_as_int(w[W_KIND]);
-                const bool sbad = __float_as_int(w[W_SBAD]) != 0;
-#pragma unroll
-                for (int i = 0; i < NS; ++i) out[i] = rec[i];
-                if ((kind & 255) == KIND_FIN || sbad) {
-                    meta |= 256 | (int)(((uint32_t)(kind >> 8) | (sbad ? ST_NUMERIC : 0u)) << 16);
-                    out[R_META] = __int_as_float(meta);
-                    link = -2;
+            // ---------------- phase 3: update the survivors, thread per child (B5) ----------------
+            const int nchild = s_offn[S];
+            for (int cn = tid; cn < nchild; cn += BUILD_NT) {
+                const int s = s_cseed[cn];
+                const int j = cn - s_offn[s];
+                const float chi2c = sel_chi2[s * K + j];
+                const int hitpos = sel_hit[s * K + j], pkd = sel_pk[s * K + j];
+                const int k = pkd & 255, nh = (pkd >> 8) & 255;
+                const int cp = s_off[s] + k;
+                int link;
+                if (hitpos == HITPOS_NONE) {
+                    rec_copy(recB, cp, recA, cn, SK);
+                    if (pkd & (1 << 16)) {
+                        const int meta = __float_as_int(recB[W_META * SK + cp]) | 256 | (((pkd >> 24) & 15) << 16);
+                        recA[W_META * SK + cn] = __int_as_float(meta);
+                        link = -2;
+                    } else {
+                        link = -1;
+                    }
                 } else {
-                    link = -1;
+                    State st;
+                    float chi2p;
+                    int meta;
+                    rec_load(st, chi2p, meta, recB, SK, cp);
+                    const float mx = a.sx[hitpos], my = a.sy[hitpos], mz = a.sz[hitpos];
+                    HitCov V;
+                    if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
+                    else V = hit_cov(mx, my, ly);
+                    Ldl3 F;
+                    float r[3], c2;
+                    bool ok = innovation(st, mx, my, mz, V, F, r, c2);
+                    gain_update<ISO>(st, F, V, r);
+                    ok = ok && state_finite(st) && st.IT.x > 0.0f;
+                    if (ok) {
+                        rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
+                    } else {     // failed update: keep the predicted state, finish the candidate
+                        rec_copy(recB, cp, recA, cn, SK);
+                        recA[W_CHI2 * SK + cn] = chi2c;
+                        recA[W_META * SK + cn] = __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16));
+                    }
+                    link = a.perm[hitpos];
                 }
+                link_hit[l * SK + s * K + j] = link;
+                link_par[l * SK + s * K + j] = (uint8_t)k;
+            }
+            __syncthreads();
+            if (tid < S) { s_nc[tid] = tid < ns ? s_nnew[tid] : 0; s_off[tid] = s_offn[tid]; }
+            if (tid == 0) s_off[S] = s_offn[S];
+            __syncthreads();
+        }
+
+        // ---------------- B6: back-trace + store ----------------
+        if (tid < ns) a.n_cand_o[s0 + tid] = s_nc[tid];
+        for (int idx = tid; idx < ns * K; idx += BUILD_NT) {
+            const int s = idx / K, j = idx - s * K;
+            const int64_t sg = s0 + s;
+            const int64_t slot = sg * K + j;
+            a.q_o[slot] = a.q[sg];
+            if (j < s_nc[s]) {
+                const int c = s_off[s] + j;
+                State st;
+                float chi2;
+                int meta;
+                rec_load(st, chi2, meta, recA, SK, c);
+                state_store(st, [&](int i, float v) { a.par_o[(int64_t)i * a.ld_out + slot] = v; },
+                            [&](int kk, float v) { a.cov_o[(int64_t)kk * a.ld_out + slot] = v; });
+                a.chi2_o[slot] = chi2;
+                a.nhits_o[slot] = meta & 255;
+                a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
+                int k = j;
+                for (int l = L - 1; l >= a.first_layer; --l) {
+                    a.hit_idx_o[(int64_t)l * a.ld_out + slot] = link_hit[l * SK + s * K + k];
+                    k = link_par[l * SK + s * K + k];
+                }
+                for (int l = 0; l < a.first_layer; ++l)
+                    a.hit_idx_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + sg] : -1;
             } else {
-                float p[6], C[21];
-#pragma unroll
-                for (int i = 0; i < 6; ++i) p[i] = rec[R_PAR + i];
-#pragma unroll
-                for (int i = 0; i < 21; ++i) C[i] = rec[R_COV + i];
-                Trig g = {rec[R_TRIG], rec[R_TRIG + 1], rec[R_TRIG + 2], rec[R_TRIG + 3]};
-                const float mx = a.sx[hitpos], my = a.sy[hitpos], mz = a.sz[hitpos];
-                const HitCov V = hit_cov(mx, my, ly);
-                Ldl3 F;
-                float r[3], c2;
-                bool ok = innovation(p, C, mx, my, mz, V, F, r, c2);
-                if (ok) {
-                    gain_update(p, C, g, F, V, r);
-                    ok = all_finite(p, C) && p[3] > 0.0f;
-                }
-                const int nh = sel[cap + j];
-                if (ok) {
-#pragma unroll
-                    for (int i = 0; i < 6; ++i) out[R_PAR + i] = p[i];
-#pragma unroll
-                    for (int i = 0; i < 21; ++i) out[R_COV + i] = C[i];
-                    out[R_TRIG] = g.cp; out[R_TRIG + 1] = g.sp; out[R_TRIG + 2] = g.st; out[R_TRIG + 3] = g.ct;
-                    meta = (meta & ~255) | nh;
-                } else {     // failed update: keep the predicted state, finish the candidate
-#pragma unroll
-                    for (int i = 0; i < NS; ++i) out[i] = rec[i];
-                    meta = ((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16);
-                }
-                out[R_CHI2] = ((const float*)sel)[j];
-                out[R_META] = __int_as_float(meta);
-                link = a.perm[hitpos];
+                a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
+                for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
             }
-            link_hit[l * K + j] = link;
-            link_par[l * K + j] = (unsigned char)parent;
         }
-        nc = n_new;
-        __syncwarp(gmask);
-    }
-
-    // ---------------- B6: back-trace + store ----------------
-    if (lane == 0) a.n_cand_o[s] = nc;
-    for (int j = lane; j < K; j += G) {
-        const int64_t slot = s * K + j;
-        a.q_o[slot] = a.q[s];
-        if (j < nc) {
-            const float* rec = A + j * NS;
-#pragma unroll
-            for (int i = 0; i < 6; ++i) a.par_o[(int64_t)i * a.ld_out + slot] = (i == 4) ? wrap_phi(rec[R_PAR + i]) : rec[R_PAR + i];
-#pragma unroll
-            for (int i = 0; i < 21; ++i) a.cov_o[(int64_t)i * a.ld_out + slot] = rec[R_COV + i];
-            const int meta = __float_as_int(rec[R_META]);
-            a.chi2_o[slot] = rec[R_CHI2];
-            a.nhits_o[slot] = meta & 255;
-            a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
-            int k = j;
-            for (int l = L - 1; l >= a.first_layer; --l) {
-                a.hit_idx_o[(int64_t)l * a.ld_out + slot] = link_hit[l * K + k];
-                k = link_par[l * K + k];
-            }
-            for (int l = 0; l < a.first_layer; ++l)
-                a.hit_idx_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + s] : -1;
-        } else {
-            a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
-            for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
-        }
+        __syncthreads();     // the workspace and the shared arrays are reused by the next tile
     }
 }
 
-template <int G>
-static int launch_build(const BuildArgs& a, cudaStream_t st) {
-    const int seeds_per_block = BUILD_BLOCK / G;
-    const size_t smem = (size_t)seeds_per_block * seed_words(a.K, a.n_layers, a.cap) * sizeof(float);
-    if (smem > 227 * 1024) return fail(KF_ERR_INVALID_ARG, "kf_build: K = %d needs %zu bytes of shared memory per block (> 227 KB)", a.K, smem);
-    cudaError_t e = cudaFuncSetAttribute(kf_build_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
-    const int64_t blocks = (a.n_seeds + seeds_per_block - 1) / seeds_per_block;
-    kf_build_kernel<G><<<(unsigned)blocks, BUILD_BLOCK, smem, st>>>(a);
-    return check_launch("kf_build");
+// ---- host side: tile size, grid and workspace layout (one function, used by the size query and by the launch) ----
+static int g_build_tile = 0;   // 0 = automatic
+
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+            cudaGetLastError();
+            n = 148;
+        }
+    }
+    return n;
 }
 
-static int g_build_lanes = 0;   // 0 = automatic
+struct BuildPlan { int S, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o_lh, o_lp, total; };
+
+static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
+    BuildPlan p;
+    const int resident = 2 * sm_count();
+    int S = g_build_tile;
+    if (S == 0) {    // a full wave of tiles when the job is small (latency-sized), 128 seeds otherwise
+        const int64_t per = (n_seeds + resident - 1) / resident;
+        S = (int)std::min<int64_t>(128, std::max<int64_t>(32, (per + 15) / 16 * 16));
+    }
+    p.S = S;
+    const int SK = S * K;
+    p.ncap = std::min(SK, std::max(K, (LIST_BYTES / (8 * K)) & ~31));
+    p.n_tiles = (n_seeds + S - 1) / S;
+    p.grid = (int)std::min<int64_t>(std::max<int64_t>(p.n_tiles, 1), resident);
+    p.smem = (size_t)build_smem(S, K, p.ncap).total;
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    size_t o = 0;
+    p.o_rec = o; o += up((size_t)p.grid * 2 * NREC * SK * sizeof(float));
+    p.o_lh = o; o += up((size_t)p.grid * n_layers * SK * sizeof(int32_t));
+    p.o_lp = o; o += up((size_t)p.grid * n_layers * SK);
+    p.total = o;
+    return p;
+}
 
 }  // namespace kf
 
-extern "C" size_t kf_build_workspace_bytes(const kf_geom*, int64_t, int32_t) { return 0; }   // candidates stay in shared memory
+extern "C" size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K) {
+    if (!geom || geom->n_layers < 1 || geom->n_layers > KF_MAX_LAYERS || n_seeds < 0 || K < 1 || K > 32) return 0;
+    return kf::build_plan(geom->n_layers, n_seeds, K).total;
+}
 
-// tuning / test hook: lanes per seed (4, 8, 16, 32; 0 = automatic)
-extern "C" int kf_build_set_lanes(int32_t g) {
-    if (g != 0 && g != 4 && g != 8 && g != 16 && g != 32) return kf::fail(KF_ERR_INVALID_ARG, "kf_build_set_lanes: %d not in {0, 4, 8, 16, 32}", g);
-    kf::g_build_lanes = g;
+// tuning / test hook: seeds per block (16..256, multiple of 16; 0 = automatic).  The result does not depend on it.
+extern "C" int kf_build_set_tile(int32_t seeds_per_block) {
+    if (seeds_per_block != 0 && (seeds_per_block < 16 || seeds_per_block > kf::BUILD_NT || seeds_per_block % 16))
+        return kf::fail(KF_ERR_INVALID_ARG, "kf_build_set_tile: %d not 0 or a multiple of 16 in 16..256", seeds_per_block);
+    kf::g_build_tile = seeds_per_block;
     return KF_OK;
 }
 
@@ -402,7 +471,6 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
                         const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
                         float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream) {
     using namespace kf;
-    (void)ws; (void)ws_bytes;
     if (!geom || !hits || !binned || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_build: NULL struct argument");
     int rc = check_geom(geom, "kf_build");
     if (rc) return rc;
@@ -420,27 +488,32 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     const kf_tracks& c = out->cand;
     if (!c.par || !c.cov || !c.q || !c.chi2 || !c.nhits || !c.status || !out->hit_idx || !out->n_cand)
         return fail(KF_ERR_NULL_PTR, "kf_build: NULL output array");
+    const BuildPlan p = build_plan(geom->n_layers, seeds->n, K);
+    if (!ws || ws_bytes < p.total) return fail(KF_ERR_WORKSPACE_TOO_SMALL, "kf_build: workspace %zu < %zu bytes", ws_bytes, p.total);
+    if (p.smem > 227 * 1024) return fail(KF_ERR_INVALID_ARG, "kf_build: tile of %d seeds with K = %d needs %zu bytes of shared memory (> 227 KB)", p.S, K, p.smem);
     BuildArgs a;
     a.n_layers = geom->n_layers; a.first_layer = first_layer; a.K = K; a.n_phi = binned->n_phi; a.n_z = binned->n_z;
+    a.S = p.S; a.ncap = p.ncap; a.n_tiles = p.n_tiles;
     a.kb = KCURV * geom->bz_tesla; a.chi2_cut = chi2_cut; a.n_sigma = n_sigma; a.inv_dphi = host_inv_dphi(binned->n_phi);
     a.n_seeds = seeds->n; a.ld_seed = seeds->ld; a.ld_out = out->ld;
     a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.seed_event = seed_event; a.seed_hit_idx = seed_hit_idx;
     a.sx = binned->x; a.sy = binned->y; a.sz = binned->z; a.perm = binned->perm; a.bin_off = binned->bin_off;
     a.par_o = c.par; a.cov_o = c.cov; a.chi2_o = c.chi2; a.q_o = c.q; a.nhits_o = c.nhits; a.status_o = c.status;
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;
+    a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh); a.ws_link_par = (uint8_t*)((char*)ws + p.o_lp);
+    bool iso = true;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
         a.layer[l] = make_layer(y);
         a.inv_dz[l] = (float)binned->n_z / (2.0f * y.zmax);
         a.sphi_over_r2[l] = (y.sig_rphi / y.r) * (y.sig_rphi / y.r);
+        iso = iso && y.sig_r == y.sig_rphi;
     }
-    int G = g_build_lanes ? g_build_lanes : 8;
-    a.cap = K + G > 32 ? K + G : 32;
     cudaStream_t st = (cudaStream_t)stream;
-    switch (G) {
-        case 4: return launch_build<4>(a, st);
-        case 8: return launch_build<8>(a, st);
-        case 16: return launch_build<16>(a, st);
-        default: return launch_build<32>(a, st);
-    }
+    cudaError_t e = iso ? cudaFuncSetAttribute(kf_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem)
+                        : cudaFuncSetAttribute(kf_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
+    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+    if (iso) kf_build_kernel<true><<<p.grid, BUILD_NT, p.smem, st>>>(a);
+    else kf_build_kernel<false><<<p.grid, BUILD_NT, p.smem, st>>>(a);
+    return check_launch("kf_build");
 }

@@ -40,7 +40,7 @@ struct State {
 
 // packed lower-triangular storage <-> State (k = i(i+1)/2 + j)
 template <typename LoadP, typename LoadC>
-__device__ __forceinline__ void state_load(State& s, LoadP par, LoadC cov) {
+__device__ __forceinline__ void state_set(State& s, LoadP par, LoadC cov) {
     s.XY = f2(par(0), par(1)); s.ZP = f2(par(2), par(4)); s.IT = f2(par(3), par(5));
     const float c10 = cov(pk(1, 0)), c20 = cov(pk(2, 0)), c21 = cov(pk(2, 1));
     s.P0 = f2(cov(pk(0, 0)), c10); s.P1 = f2(c10, cov(pk(1, 1))); s.P2 = f2(c20, c21);
@@ -48,15 +48,26 @@ __device__ __forceinline__ void state_load(State& s, LoadP par, LoadC cov) {
     s.R0 = f2(cov(pk(3, 0)), cov(pk(5, 0))); s.R1 = f2(cov(pk(3, 1)), cov(pk(5, 1))); s.R2 = f2(cov(pk(3, 2)), cov(pk(5, 2)));
     s.M3 = f2(cov(pk(3, 3)), cov(pk(5, 3))); s.M4 = f2(cov(pk(4, 3)), cov(pk(5, 4)));
     s.C44 = cov(pk(4, 4)); s.C55 = cov(pk(5, 5));
+}
+
+// sin / cos of both angles from the angles themselves (start of a track; afterwards they are carried)
+__device__ __forceinline__ void state_trig(State& s) {
     float sp, cp, st, ct;
     sincosf(s.ZP.y, &sp, &cp);
     sincosf(s.IT.y, &st, &ct);
     s.CC = f2(cp, ct); s.SS = f2(sp, st);
 }
 
-template <typename StoreP, typename StoreC>
+template <typename LoadP, typename LoadC>
+__device__ __forceinline__ void state_load(State& s, LoadP par, LoadC cov) {
+    state_set(s, par, cov);
+    state_trig(s);
+}
+
+// WRAP: phi wrapped to (-pi, pi] (final output) or left as accumulated (intermediate record)
+template <bool WRAP = true, typename StoreP, typename StoreC>
 __device__ __forceinline__ void state_store(const State& s, StoreP par, StoreC cov) {
-    par(0, s.XY.x); par(1, s.XY.y); par(2, s.ZP.x); par(3, s.IT.x); par(4, wrap_phi(s.ZP.y)); par(5, s.IT.y);
+    par(0, s.XY.x); par(1, s.XY.y); par(2, s.ZP.x); par(3, s.IT.x); par(4, WRAP ? wrap_phi(s.ZP.y) : s.ZP.y); par(5, s.IT.y);
     cov(pk(0, 0), s.P0.x);
     cov(pk(1, 0), s.P0.y); cov(pk(1, 1), s.P1.y);
     cov(pk(2, 0), s.P2.x); cov(pk(2, 1), s.P2.y); cov(pk(2, 2), s.Q2.x);

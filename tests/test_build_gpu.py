@@ -94,18 +94,18 @@ def test_window_lookup_bit_exact():
     assert rc.max() > cap and (rc == 0).any()
 
 
-def run_build(bi, K=None, lanes=0, first_layer=None):
+def run_build(bi, K=None, tile=0, first_layer=None):
     from paper_1711_06571_b200 import binding as b
     geom, hits, binned = gpu_bin(bi)
     seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    b.kf_build_set_lanes(lanes)
+    b.kf_build_set_tile(tile)
     try:
         out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K if K is None else K,
                          bi.chi2_cut, bi.n_sigma)
         torch.cuda.synchronize()
     finally:
-        b.kf_build_set_lanes(0)
+        b.kf_build_set_tile(0)
     return out.to_host()
 
 
@@ -155,19 +155,21 @@ def compare_build(g, r, n_seeds, K, max_mismatch_frac, band_frac=0.02):
     return rep
 
 
-@pytest.mark.parametrize("lanes", [4, 8, 16, 32])
-def test_build_config3_small(lanes):
+@pytest.mark.parametrize("tile", [0, 16, 112, 256])
+def test_build_config3_small(tile):
     bi = synth.build_inputs(3, n_events=2, tracks=2000)
-    compare_build(run_build(bi, lanes=lanes), ref_build(bi), bi.n_seeds, bi.K, 2e-3)
+    compare_build(run_build(bi, tile=tile), ref_build(bi), bi.n_seeds, bi.K, 2e-3)
 
 
-def test_build_lanes_do_not_change_the_result():
+def test_build_tile_does_not_change_the_result():
+    """Seeds per block (and with it the number of rounds a layer takes: 256 seeds x up to 10 candidates exceed the list
+    area on the outer layers) must not change a single bit of the result."""
     bi = synth.build_inputs(4, n_events=1, tracks=2000, fake_frac=0.2)
-    base = run_build(bi, lanes=8)
-    for lanes in (4, 16, 32):
-        other = run_build(bi, lanes=lanes)
+    base = run_build(bi, tile=128)
+    for tile in (16, 48, 256):
+        other = run_build(bi, tile=tile)
         for k in ("n_cand", "hit_idx", "nhits", "status", "chi2"):
-            assert np.array_equal(base[k], other[k]), (lanes, k)
+            assert np.array_equal(base[k], other[k]), (tile, k)
         v = base["nhits"] > 0
         assert np.array_equal(base["par"][:, v], other["par"][:, v]) and np.array_equal(base["cov"][:, v], other["cov"][:, v])
 
@@ -192,7 +194,7 @@ def test_build_dense_windows_exceed_the_child_buffer():
     bi = synth.build_inputs(3, n_events=1, tracks=300, noise=40.0, n_sigma=30.0, chi2_cut=3000.0)
     r = ref_build(bi)
     assert r["counters"]["n_children"] / r["counters"]["n_seed_layers"] > 20
-    compare_build(run_build(bi, lanes=4), r, bi.n_seeds, bi.K, 5e-2)
+    compare_build(run_build(bi, tile=64), r, bi.n_seeds, bi.K, 5e-2)
 
 
 def test_build_edge_cases():
@@ -217,6 +219,10 @@ def test_build_edge_cases():
         b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 33, 30.0, 3.0)
     with pytest.raises(b.KfError, match="-1"):
         b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 10, -1.0, 3.0)
+    with pytest.raises(b.KfError, match="-4"):
+        b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 10, 30.0, 3.0, ws=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(b.KfError, match="-1"):
+        b.kf_build_set_tile(24)
 
 
 def test_build_config3_full():
