@@ -25,13 +25,11 @@
 
 namespace kf {
 
-#ifndef KF_BUILD_MINB
-#define KF_BUILD_MINB 2
-#endif
-constexpr int BUILD_NT = 256;
+constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (twice the seeds of the tile)
+constexpr int BUILD_THREADS_PER_SM = 512; // 128 registers per thread
 constexpr int NREC = 33;                  // words per candidate record
 constexpr int HITPOS_NONE = 0x7fffffff;
-constexpr int LIST_BYTES = 48 * 1024;     // shared memory for the per-candidate child lists
+constexpr int LIST_BYTES_PER_THREAD = 192; // shared memory for the per-candidate child lists, per thread of the block
 enum { W_TRIG = 27, W_CHI2 = 31, W_META = 32 };
 // meta word of a record: bits 0-7 nhits, bit 8 finished, bits 16-19 status
 // info word of a parent in a round: bits 0-7 nhits, bit 8 finished (child inherits the unchanged state), bits 16-19 status to add
@@ -46,7 +44,6 @@ struct BuildArgs {
     float *par_o, *cov_o, *chi2_o; int8_t* q_o; int32_t* nhits_o; uint32_t* status_o; int32_t *hit_idx_o, *n_cand_o;
     float* ws_rec;            // [grid][2][NREC][S*K]
     int32_t* ws_link_hit;     // [grid][n_layers][S*K]
-    uint8_t* ws_link_par;     // [grid][n_layers][S*K]
     LayerC layer[KF_MAX_LAYERS];
     float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax); (sig_rphi/r)^2
 };
@@ -92,7 +89,8 @@ __device__ __forceinline__ void list_insert(float* lc, int* lh, int ncap, int K,
     lc[pos * ncap] = c; lh[pos * ncap] = h;
 }
 
-// exclusive scan of one int per thread over the block (BUILD_NT threads); returns the exclusive prefix, total in *total
+// exclusive scan of one int per thread over the block (NT threads); returns the exclusive prefix, total in *total
+template <int NT>
 __device__ __forceinline__ int block_exclusive_scan(int v, int* s_warp, int* total) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int inc = v;
@@ -104,7 +102,7 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* s_warp, int* tot
     if (lane == 31) s_warp[w] = inc;
     __syncthreads();
     if (w == 0) {
-        int t = lane < BUILD_NT / 32 ? s_warp[lane] : 0;
+        int t = lane < NT / 32 ? s_warp[lane] : 0;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const int o = __shfl_up_sync(0xffffffffu, t, d);
@@ -114,14 +112,14 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* s_warp, int* tot
     }
     __syncthreads();
     const int base = w > 0 ? s_warp[w - 1] : 0;
-    *total = s_warp[BUILD_NT / 32 - 1];
+    *total = s_warp[NT / 32 - 1];
     __syncthreads();
     return base + inc - v;
 }
 
 // shared memory carve-up (bytes), identical on host and device
-struct BuildSmem { int nc, off, nnew, offn, sel_chi2, sel_hit, sel_pk, cseed, l_chi2, l_hit, l_cnt, l_head, p_chi2, p_info, misc, total; };
-__host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap) {
+struct BuildSmem { int nc, off, nnew, offn, sel_chi2, sel_hit, sel_pk, cseed, l_chi2, l_hit, l_cnt, l_head, p_chi2, p_info, link_par, misc, total; };
+__host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap, int L) {
     BuildSmem m;
     int o = 0;
     auto take = [&](int bytes) { const int at = o; o += (bytes + 15) & ~15; return at; };
@@ -129,16 +127,24 @@ __host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap) {
     m.sel_chi2 = take(4 * S * K); m.sel_hit = take(4 * S * K); m.sel_pk = take(4 * S * K); m.cseed = take(2 * S * K);
     m.l_chi2 = take(4 * ncap * K); m.l_hit = take(4 * ncap * K); m.l_cnt = take(ncap); m.l_head = take(ncap);
     m.p_chi2 = take(4 * ncap); m.p_info = take(4 * ncap);
+    m.link_par = take(L * S * K);
     m.misc = take(4 * 40);
     m.total = o;
     return m;
 }
 
-template <bool ISO>
-__global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const __grid_constant__ BuildArgs a) {
+#ifdef KF_BUILD_TIMING
+__device__ unsigned long long g_build_timing[8];
+#define KF_TICK(i) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_build_timing[i], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
+#else
+#define KF_TICK(i) do { } while (0)
+#endif
+
+template <int NT, bool ISO>
+__global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel(const __grid_constant__ BuildArgs a) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int S = a.S, K = a.K, L = a.n_layers, ncap = a.ncap, SK = S * K;
-    const BuildSmem m = build_smem(S, K, ncap);
+    const BuildSmem m = build_smem(S, K, ncap, L);
     int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off);
     int* s_nnew = (int*)(smem + m.nnew); int* s_offn = (int*)(smem + m.offn);
     float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit);
@@ -153,8 +159,11 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
     float* recA = a.ws_rec + (size_t)blockIdx.x * 2 * NREC * SK;
     float* recB = recA + (size_t)NREC * SK;
     int32_t* link_hit = a.ws_link_hit + (size_t)blockIdx.x * L * SK;
-    uint8_t* link_par = a.ws_link_par + (size_t)blockIdx.x * L * SK;
+    uint8_t* link_par = smem + m.link_par;
 
+#ifdef KF_BUILD_TIMING
+    long long tick_ = clock64();
+#endif
     for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t s0 = tile * S;
         const int ns = (int)min((int64_t)S, a.n_seeds - s0);
@@ -172,6 +181,7 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
         }
         if (tid == 0) s_off[S] = ns;
         __syncthreads();
+        KF_TICK(0);
 
         for (int l = a.first_layer; l < L; ++l) {
             const LayerC& ly = a.layer[l];
@@ -191,7 +201,7 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
                 }
                 const int nround = s_off[r1] - base;
                 // ---------------- phase 1: predict + window + scan, thread per candidate ----------------
-                for (int i = tid; i < nround; i += BUILD_NT) {
+                for (int i = tid; i < nround; i += NT) {
                     const int c = base + i;
                     const int64_t sg = s0 + s_cseed[c];
                     const float cw = -(float)a.q[sg] * a.kb;
@@ -248,26 +258,36 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
                                 else { b0 = 0; b1 = wb.first + wb.n_b - a.n_phi; }
                                 if (b1 <= b0) continue;
                                 const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
-                                for (int h = h0; h < h1; ++h) {
-                                    const float mx = a.sx[h], my = a.sy[h], mz = a.sz[h];
-                                    const float cr = fmaf(px, my, -py * mx);
-                                    const bool in_win = (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
-                                                        (fabsf(mz - pz) <= dzw);
-                                    if (!in_win) continue;
-                                    bool ok = fok;
-                                    if (!ISO) {
-                                        const HitCov V = hit_cov(mx, my, ly);
-                                        Sym3 Sm;
-                                        Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
-                                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
-                                        ok = ldl3(Sm, F);
+                                for (int hb = h0; hb < h1; hb += 4) {      // four hits per memory round trip
+                                    float hx[4], hy[4], hz[4];
+#pragma unroll
+                                    for (int u = 0; u < 4; ++u) {
+                                        const int hh = min(hb + u, h1 - 1);
+                                        hx[u] = a.sx[hh]; hy[u] = a.sy[hh]; hz[u] = a.sz[hh];
                                     }
-                                    if (!ok) { sbad = true; continue; }
-                                    const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
-                                    const float y1 = fmaf(-F.l10, q0, q1);
-                                    const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
-                                    const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                    if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
+#pragma unroll
+                                    for (int u = 0; u < 4; ++u) {
+                                        const int h = hb + u;
+                                        const float mx = hx[u], my = hy[u], mz = hz[u];
+                                        const float cr = fmaf(px, my, -py * mx);
+                                        const bool in_win = (h < h1) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                                            (fabsf(mz - pz) <= dzw);
+                                        if (!in_win) continue;
+                                        bool ok = fok;
+                                        if (!ISO) {
+                                            const HitCov V = hit_cov(mx, my, ly);
+                                            Sym3 Sm;
+                                            Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
+                                            Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
+                                            ok = ldl3(Sm, F);
+                                        }
+                                        if (!ok) { sbad = true; continue; }
+                                        const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
+                                        const float y1 = fmaf(-F.l10, q0, q1);
+                                        const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
+                                        const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
+                                        if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
+                                    }
                                 }
                             }
                         }
@@ -284,6 +304,7 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
                     s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
                 }
                 __syncthreads();
+                KF_TICK(1);
                 // ---------------- phase 2: best K children of a seed, thread per seed (B4) ----------------
                 if (tid >= r0 && tid < r1) {
                     const int s = tid;
@@ -315,21 +336,23 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
                     s_nnew[s] = n_out;
                 }
                 __syncthreads();
+                KF_TICK(2);
                 r0 = r1;
             }
             // ---------------- dense positions of the children ----------------
             {
                 const int v = tid < ns ? s_nnew[tid] : 0;
                 int tot;
-                const int ex = block_exclusive_scan(v, s_misc, &tot);
+                const int ex = block_exclusive_scan<NT>(v, s_misc, &tot);
                 if (tid < S) s_offn[tid] = tid < ns ? ex : tot;
                 if (tid == 0) s_offn[S] = tot;
                 for (int j = 0; j < v; ++j) s_cseed[ex + j] = (unsigned short)tid;
                 __syncthreads();
             }
+            KF_TICK(3);
             // ---------------- phase 3: update the survivors, thread per child (B5) ----------------
             const int nchild = s_offn[S];
-            for (int cn = tid; cn < nchild; cn += BUILD_NT) {
+            for (int cn = tid; cn < nchild; cn += NT) {
                 const int s = s_cseed[cn];
                 const int j = cn - s_offn[s];
                 const float chi2c = sel_chi2[s * K + j];
@@ -376,11 +399,12 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
             if (tid < S) { s_nc[tid] = tid < ns ? s_nnew[tid] : 0; s_off[tid] = s_offn[tid]; }
             if (tid == 0) s_off[S] = s_offn[S];
             __syncthreads();
+            KF_TICK(4);
         }
 
         // ---------------- B6: back-trace + store ----------------
         if (tid < ns) a.n_cand_o[s0 + tid] = s_nc[tid];
-        for (int idx = tid; idx < ns * K; idx += BUILD_NT) {
+        for (int idx = tid; idx < ns * K; idx += NT) {
             const int s = idx / K, j = idx - s * K;
             const int64_t sg = s0 + s;
             const int64_t slot = sg * K + j;
@@ -409,11 +433,15 @@ __global__ void __launch_bounds__(BUILD_NT, KF_BUILD_MINB) kf_build_kernel(const
             }
         }
         __syncthreads();     // the workspace and the shared arrays are reused by the next tile
+        KF_TICK(5);
     }
 }
 
 // ---- host side: tile size, grid and workspace layout (one function, used by the size query and by the launch) ----
-static int g_build_tile = 0;   // 0 = automatic
+#ifndef KF_BUILD_DEFAULT_TILE
+#define KF_BUILD_DEFAULT_TILE 128
+#endif
+static int g_build_tile = 0;   // 0 = default
 
 static int sm_count() {
     static int n = 0;
@@ -427,32 +455,48 @@ static int sm_count() {
     return n;
 }
 
-struct BuildPlan { int S, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o_lh, o_lp, total; };
+struct BuildPlan { int S, NT, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o_lh, total; };
 
 static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
     BuildPlan p;
-    const int resident = 2 * sm_count();
     int S = g_build_tile;
-    if (S == 0) {    // a full wave of tiles when the job is small (latency-sized), 128 seeds otherwise
-        const int64_t per = (n_seeds + resident - 1) / resident;
-        S = (int)std::min<int64_t>(128, std::max<int64_t>(32, (per + 15) / 16 * 16));
-    }
+    if (S == 0) S = KF_BUILD_DEFAULT_TILE;
     p.S = S;
+    p.NT = S <= 32 ? 64 : (S <= 64 ? 128 : 256);
     const int SK = S * K;
-    p.ncap = std::min(SK, std::max(K, (LIST_BYTES / (8 * K)) & ~31));
+    p.ncap = std::min(SK, std::max(std::max(K, 32), (LIST_BYTES_PER_THREAD * p.NT / (8 * K)) & ~31));
     p.n_tiles = (n_seeds + S - 1) / S;
+    p.smem = (size_t)build_smem(S, K, p.ncap, n_layers).total;
+    const int by_smem = (int)std::max<size_t>(1, (size_t)(227 * 1024) / (p.smem + 1024));
+    const int resident = sm_count() * std::min(BUILD_THREADS_PER_SM / p.NT, by_smem);
     p.grid = (int)std::min<int64_t>(std::max<int64_t>(p.n_tiles, 1), resident);
-    p.smem = (size_t)build_smem(S, K, p.ncap).total;
     auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
     size_t o = 0;
     p.o_rec = o; o += up((size_t)p.grid * 2 * NREC * SK * sizeof(float));
     p.o_lh = o; o += up((size_t)p.grid * n_layers * SK * sizeof(int32_t));
-    p.o_lp = o; o += up((size_t)p.grid * n_layers * SK);
     p.total = o;
     return p;
 }
 
+template <int NT>
+static int launch_build(const BuildArgs& a, const BuildPlan& p, bool iso, cudaStream_t st) {
+    cudaError_t e = iso ? cudaFuncSetAttribute(kf_build_kernel<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem)
+                        : cudaFuncSetAttribute(kf_build_kernel<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
+    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+    if (iso) kf_build_kernel<NT, true><<<p.grid, NT, p.smem, st>>>(a);
+    else kf_build_kernel<NT, false><<<p.grid, NT, p.smem, st>>>(a);
+    return check_launch("kf_build");
+}
+
 }  // namespace kf
+
+#ifdef KF_BUILD_TIMING
+extern "C" void kf_build_timing(unsigned long long* out, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, kf::g_build_timing, sizeof(unsigned long long) * 8);
+    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(kf::g_build_timing, z, sizeof z); }
+}
+#endif
 
 extern "C" size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K) {
     if (!geom || geom->n_layers < 1 || geom->n_layers > KF_MAX_LAYERS || n_seeds < 0 || K < 1 || K > 32) return 0;
@@ -461,7 +505,7 @@ extern "C" size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds,
 
 // tuning / test hook: seeds per block (16..256, multiple of 16; 0 = automatic).  The result does not depend on it.
 extern "C" int kf_build_set_tile(int32_t seeds_per_block) {
-    if (seeds_per_block != 0 && (seeds_per_block < 16 || seeds_per_block > kf::BUILD_NT || seeds_per_block % 16))
+    if (seeds_per_block != 0 && (seeds_per_block < 16 || seeds_per_block > kf::BUILD_MAX_NT || seeds_per_block % 16))
         return kf::fail(KF_ERR_INVALID_ARG, "kf_build_set_tile: %d not 0 or a multiple of 16 in 16..256", seeds_per_block);
     kf::g_build_tile = seeds_per_block;
     return KF_OK;
@@ -500,7 +544,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     a.sx = binned->x; a.sy = binned->y; a.sz = binned->z; a.perm = binned->perm; a.bin_off = binned->bin_off;
     a.par_o = c.par; a.cov_o = c.cov; a.chi2_o = c.chi2; a.q_o = c.q; a.nhits_o = c.nhits; a.status_o = c.status;
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;
-    a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh); a.ws_link_par = (uint8_t*)((char*)ws + p.o_lp);
+    a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh);
     bool iso = true;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
@@ -510,10 +554,9 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
         iso = iso && y.sig_r == y.sig_rphi;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = iso ? cudaFuncSetAttribute(kf_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem)
-                        : cudaFuncSetAttribute(kf_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
-    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
-    if (iso) kf_build_kernel<true><<<p.grid, BUILD_NT, p.smem, st>>>(a);
-    else kf_build_kernel<false><<<p.grid, BUILD_NT, p.smem, st>>>(a);
-    return check_launch("kf_build");
+    switch (p.NT) {
+        case 64: return launch_build<64>(a, p, iso, st);
+        case 128: return launch_build<128>(a, p, iso, st);
+        default: return launch_build<256>(a, p, iso, st);
+    }
 }
