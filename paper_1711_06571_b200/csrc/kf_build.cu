@@ -65,9 +65,18 @@ __device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, 
     buf[W_META * SK + c] = __int_as_float(meta);
 }
 
-__device__ __forceinline__ void rec_copy(const float* src, int cs, float* dst, int cd, int SK) {
+// src and dst never overlap (different buffers): all loads of a chunk are issued before its stores, so a copy costs two
+// memory round trips instead of one per word
+__device__ __forceinline__ void rec_copy(const float* __restrict__ src, int cs, float* __restrict__ dst, int cd, int SK) {
+    float v[17];
 #pragma unroll
-    for (int w = 0; w < NREC; ++w) dst[w * SK + cd] = src[w * SK + cs];
+    for (int w = 0; w < 17; ++w) v[w] = __ldcg(src + w * SK + cs);
+#pragma unroll
+    for (int w = 0; w < 17; ++w) dst[w * SK + cd] = v[w];
+#pragma unroll
+    for (int w = 17; w < NREC; ++w) v[w - 17] = __ldcg(src + w * SK + cs);
+#pragma unroll
+    for (int w = 17; w < NREC; ++w) dst[w * SK + cd] = v[w - 17];
 }
 
 // ascending (chi2, hit) list of at most K entries, entry j of candidate i at [j * ncap + i] (conflict-free)
@@ -140,6 +149,228 @@ __device__ unsigned long long g_build_timing[8];
 #define KF_TICK(i) do { } while (0)
 #endif
 
+// per-block context: sizes, workspace and shared-memory arrays (built once, passed by reference to the phase bodies)
+struct Tile {
+    int S, K, L, ncap, SK;
+    float *recA, *recB; int32_t* link_hit; uint8_t* link_par;
+    int *s_nc, *s_off, *s_nnew, *s_offn;
+    float* sel_chi2; int *sel_hit, *sel_pk; unsigned short* s_cseed;
+    float* s_lchi2; int* s_lhit; unsigned char *s_lcnt, *s_lhead; float* s_pchi2; int* s_pinfo;
+};
+
+// The three per-thread bodies are separate functions (not inlined) so that each gets its own register allocation:
+// inlined into one kernel they need 228 registers and spill ~480 bytes at the 128 the launch bounds allow.
+
+// phase 1, one live candidate: dense index base + i, round-local index i
+template <bool ISO>
+__device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, int l, int base, int i, int64_t s0) {
+    const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
+    float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
+    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
+    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
+    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
+    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
+    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
+    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
+    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
+    const LayerC& ly = a.layer[l];
+                    const int c = base + i;
+                        const int64_t sg = s0 + s_cseed[c];
+                        const float cw = -(float)a.q[sg] * a.kb;
+                        const int ev = a.seed_event ? a.seed_event[sg] : 0;
+                        State st;
+                        float chi2;
+                        int meta;
+                        rec_load(st, chi2, meta, recA, SK, c);
+                        uint32_t flag = 0u;
+                        bool fin = (meta & 256) != 0;
+                        float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
+                        float c00 = 0.f, c10 = 0.f, c11 = 0.f, c20 = 0.f, c21 = 0.f, c22 = 0.f;
+                        Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                        bool fok = false;
+                        WindowBins wb = {0, 0, 0, -1};
+                        if (!fin) {
+                            flag = predict(st, cw, ly);
+                            if (!flag) {
+                                px = st.XY.x; py = st.XY.y; pz = st.ZP.x;
+                                c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
+                                const float r2 = fmaf(px, px, py * py);
+                                const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
+                                const float varphi = fmaxf(num / (r2 * r2), 0.0f);
+                                const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
+                                dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+                                if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
+                                else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
+                                else {
+                                    thr2 = dphi * dphi * r2;
+                                    wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+                                    if (ISO) {
+                                        Sym3 Sm;
+                                        Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
+                                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
+                                        fok = ldl3(Sm, F);
+                                    }
+                                }
+                            }
+                            fin = flag != 0u;
+                        }
+                        int cnt = 0;
+                        if (!fin) {
+                            rec_store(st, chi2, meta, recB, SK, c);
+                            // ---- window scan (B3) ----
+                            bool sbad = false;
+                            float* lc = s_lchi2 + i;
+                            int* lh = s_lhit + i;
+                            const int64_t seg = (int64_t)ev * L + l;
+                            for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
+                                const int64_t row = (seg * a.n_z + iz) * a.n_phi;
+                                for (int run = 0; run < 2; ++run) {
+                                    int b0, b1;
+                                    if (run == 0) { b0 = wb.first; b1 = min(wb.first + wb.n_b, a.n_phi); }
+                                    else { b0 = 0; b1 = wb.first + wb.n_b - a.n_phi; }
+                                    if (b1 <= b0) continue;
+                                    const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
+                                    for (int hb = h0; hb < h1; hb += 4) {      // four hits per memory round trip
+                                        float hx[4], hy[4], hz[4];
+    #pragma unroll
+                                        for (int u = 0; u < 4; ++u) {
+                                            const int hh = min(hb + u, h1 - 1);
+                                            hx[u] = a.sx[hh]; hy[u] = a.sy[hh]; hz[u] = a.sz[hh];
+                                        }
+    #pragma unroll
+                                        for (int u = 0; u < 4; ++u) {
+                                            const int h = hb + u;
+                                            const float mx = hx[u], my = hy[u], mz = hz[u];
+                                            const float cr = fmaf(px, my, -py * mx);
+                                            const bool in_win = (h < h1) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                                                (fabsf(mz - pz) <= dzw);
+                                            if (!in_win) continue;
+                                            bool ok = fok;
+                                            if (!ISO) {
+                                                const HitCov V = hit_cov(mx, my, ly);
+                                                Sym3 Sm;
+                                                Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
+                                                Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
+                                                ok = ldl3(Sm, F);
+                                            }
+                                            if (!ok) { sbad = true; continue; }
+                                            const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
+                                            const float y1 = fmaf(-F.l10, q0, q1);
+                                            const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
+                                            const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
+                                            if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
+                                        }
+                                    }
+                                }
+                            }
+                            if (sbad) {      // S not positive definite: one finished child with the unchanged state
+                                fin = true;
+                                flag = ST_NUMERIC;
+                                cnt = 0;
+                            }
+                        }
+                        if (fin) rec_copy(recA, c, recB, c, SK);
+                        s_lcnt[i] = (unsigned char)cnt;
+                        s_lhead[i] = 0;
+                        s_pchi2[i] = chi2;
+                        s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
+}
+
+// phase 3, one surviving child: dense index cn among the children of the tile
+template <bool ISO>
+__device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int l, int cn) {
+    const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
+    float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
+    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
+    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
+    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
+    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
+    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
+    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
+    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
+    const LayerC& ly = a.layer[l];
+    const int s = s_cseed[cn];
+    const int j = cn - s_offn[s];
+    const float chi2c = sel_chi2[s * K + j];
+    const int hitpos = sel_hit[s * K + j], pkd = sel_pk[s * K + j];
+    const int k = pkd & 255, nh = (pkd >> 8) & 255;
+    const int cp = s_off[s] + k;
+    int link;
+    if (hitpos == HITPOS_NONE) {
+        rec_copy(recB, cp, recA, cn, SK);
+        if (pkd & (1 << 16)) {
+            const int meta = __float_as_int(recB[W_META * SK + cp]) | 256 | (((pkd >> 24) & 15) << 16);
+            recA[W_META * SK + cn] = __int_as_float(meta);
+            link = -2;
+        } else {
+            link = -1;
+        }
+    } else {
+        State st;
+        float chi2p;
+        int meta;
+        rec_load(st, chi2p, meta, recB, SK, cp);
+        const float mx = a.sx[hitpos], my = a.sy[hitpos], mz = a.sz[hitpos];
+        HitCov V;
+        if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
+        else V = hit_cov(mx, my, ly);
+        Ldl3 F;
+        float r[3], c2;
+        bool ok = innovation(st, mx, my, mz, V, F, r, c2);
+        gain_update<ISO>(st, F, V, r);
+        ok = ok && state_finite(st) && st.IT.x > 0.0f;
+        if (ok) {
+            rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
+        } else {     // failed update: keep the predicted state, finish the candidate
+            rec_copy(recB, cp, recA, cn, SK);
+            recA[W_CHI2 * SK + cn] = chi2c;
+            recA[W_META * SK + cn] = __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16));
+        }
+        link = a.perm[hitpos];
+    }
+    link_hit[l * SK + s * K + j] = link;
+    link_par[l * SK + s * K + j] = (uint8_t)k;
+}
+
+// B6, one output slot idx = seed * K + j of the tile
+__device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int idx) {
+    const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
+    float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
+    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
+    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
+    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
+    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
+    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
+    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
+    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
+    const int s = idx / K, j = idx - s * K;
+    const int64_t sg = s0 + s;
+    const int64_t slot = sg * K + j;
+    a.q_o[slot] = a.q[sg];
+    if (j < s_nc[s]) {
+        const int c = s_off[s] + j;
+        State st;
+        float chi2;
+        int meta;
+        rec_load(st, chi2, meta, recA, SK, c);
+        state_store(st, [&](int i, float v) { a.par_o[(int64_t)i * a.ld_out + slot] = v; },
+                    [&](int kk, float v) { a.cov_o[(int64_t)kk * a.ld_out + slot] = v; });
+        a.chi2_o[slot] = chi2;
+        a.nhits_o[slot] = meta & 255;
+        a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
+        int k = j;
+        for (int l = L - 1; l >= a.first_layer; --l) {
+            a.hit_idx_o[(int64_t)l * a.ld_out + slot] = link_hit[l * SK + s * K + k];
+            k = link_par[l * SK + s * K + k];
+        }
+        for (int l = 0; l < a.first_layer; ++l)
+            a.hit_idx_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + sg] : -1;
+    } else {
+        a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
+        for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
+    }
+}
+
 template <int NT, bool ISO>
 __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel(const __grid_constant__ BuildArgs a) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -160,6 +391,12 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     float* recB = recA + (size_t)NREC * SK;
     int32_t* link_hit = a.ws_link_hit + (size_t)blockIdx.x * L * SK;
     uint8_t* link_par = smem + m.link_par;
+    Tile T;
+    T.S = S; T.K = K; T.L = L; T.ncap = ncap; T.SK = SK;
+    T.recA = recA; T.recB = recB; T.link_hit = link_hit; T.link_par = link_par;
+    T.s_nc = s_nc; T.s_off = s_off; T.s_nnew = s_nnew; T.s_offn = s_offn;
+    T.sel_chi2 = sel_chi2; T.sel_hit = sel_hit; T.sel_pk = sel_pk; T.s_cseed = s_cseed;
+    T.s_lchi2 = s_lchi2; T.s_lhit = s_lhit; T.s_lcnt = s_lcnt; T.s_lhead = s_lhead; T.s_pchi2 = s_pchi2; T.s_pinfo = s_pinfo;
 
 #ifdef KF_BUILD_TIMING
     long long tick_ = clock64();
@@ -202,106 +439,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 const int nround = s_off[r1] - base;
                 // ---------------- phase 1: predict + window + scan, thread per candidate ----------------
                 for (int i = tid; i < nround; i += NT) {
-                    const int c = base + i;
-                    const int64_t sg = s0 + s_cseed[c];
-                    const float cw = -(float)a.q[sg] * a.kb;
-                    const int ev = a.seed_event ? a.seed_event[sg] : 0;
-                    State st;
-                    float chi2;
-                    int meta;
-                    rec_load(st, chi2, meta, recA, SK, c);
-                    uint32_t flag = 0u;
-                    bool fin = (meta & 256) != 0;
-                    float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
-                    float c00 = 0.f, c10 = 0.f, c11 = 0.f, c20 = 0.f, c21 = 0.f, c22 = 0.f;
-                    Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                    bool fok = false;
-                    WindowBins wb = {0, 0, 0, -1};
-                    if (!fin) {
-                        flag = predict(st, cw, ly);
-                        if (!flag) {
-                            px = st.XY.x; py = st.XY.y; pz = st.ZP.x;
-                            c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
-                            const float r2 = fmaf(px, px, py * py);
-                            const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
-                            const float varphi = fmaxf(num / (r2 * r2), 0.0f);
-                            const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
-                            dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
-                            if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
-                            else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
-                            else {
-                                thr2 = dphi * dphi * r2;
-                                wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
-                                if (ISO) {
-                                    Sym3 Sm;
-                                    Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
-                                    Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
-                                    fok = ldl3(Sm, F);
-                                }
-                            }
-                        }
-                        fin = flag != 0u;
-                    }
-                    int cnt = 0;
-                    if (!fin) {
-                        rec_store(st, chi2, meta, recB, SK, c);
-                        // ---- window scan (B3) ----
-                        bool sbad = false;
-                        float* lc = s_lchi2 + i;
-                        int* lh = s_lhit + i;
-                        const int64_t seg = (int64_t)ev * L + l;
-                        for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
-                            const int64_t row = (seg * a.n_z + iz) * a.n_phi;
-                            for (int run = 0; run < 2; ++run) {
-                                int b0, b1;
-                                if (run == 0) { b0 = wb.first; b1 = min(wb.first + wb.n_b, a.n_phi); }
-                                else { b0 = 0; b1 = wb.first + wb.n_b - a.n_phi; }
-                                if (b1 <= b0) continue;
-                                const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
-                                for (int hb = h0; hb < h1; hb += 4) {      // four hits per memory round trip
-                                    float hx[4], hy[4], hz[4];
-#pragma unroll
-                                    for (int u = 0; u < 4; ++u) {
-                                        const int hh = min(hb + u, h1 - 1);
-                                        hx[u] = a.sx[hh]; hy[u] = a.sy[hh]; hz[u] = a.sz[hh];
-                                    }
-#pragma unroll
-                                    for (int u = 0; u < 4; ++u) {
-                                        const int h = hb + u;
-                                        const float mx = hx[u], my = hy[u], mz = hz[u];
-                                        const float cr = fmaf(px, my, -py * mx);
-                                        const bool in_win = (h < h1) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
-                                                            (fabsf(mz - pz) <= dzw);
-                                        if (!in_win) continue;
-                                        bool ok = fok;
-                                        if (!ISO) {
-                                            const HitCov V = hit_cov(mx, my, ly);
-                                            Sym3 Sm;
-                                            Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
-                                            Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
-                                            ok = ldl3(Sm, F);
-                                        }
-                                        if (!ok) { sbad = true; continue; }
-                                        const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
-                                        const float y1 = fmaf(-F.l10, q0, q1);
-                                        const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
-                                        const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                        if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
-                                    }
-                                }
-                            }
-                        }
-                        if (sbad) {      // S not positive definite: one finished child with the unchanged state
-                            fin = true;
-                            flag = ST_NUMERIC;
-                            cnt = 0;
-                        }
-                    }
-                    if (fin) rec_copy(recA, c, recB, c, SK);
-                    s_lcnt[i] = (unsigned char)cnt;
-                    s_lhead[i] = 0;
-                    s_pchi2[i] = chi2;
-                    s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
+                    build_candidate<ISO>(a, T, l, base, i, s0);
                 }
                 __syncthreads();
                 KF_TICK(1);
@@ -353,47 +491,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
             // ---------------- phase 3: update the survivors, thread per child (B5) ----------------
             const int nchild = s_offn[S];
             for (int cn = tid; cn < nchild; cn += NT) {
-                const int s = s_cseed[cn];
-                const int j = cn - s_offn[s];
-                const float chi2c = sel_chi2[s * K + j];
-                const int hitpos = sel_hit[s * K + j], pkd = sel_pk[s * K + j];
-                const int k = pkd & 255, nh = (pkd >> 8) & 255;
-                const int cp = s_off[s] + k;
-                int link;
-                if (hitpos == HITPOS_NONE) {
-                    rec_copy(recB, cp, recA, cn, SK);
-                    if (pkd & (1 << 16)) {
-                        const int meta = __float_as_int(recB[W_META * SK + cp]) | 256 | (((pkd >> 24) & 15) << 16);
-                        recA[W_META * SK + cn] = __int_as_float(meta);
-                        link = -2;
-                    } else {
-                        link = -1;
-                    }
-                } else {
-                    State st;
-                    float chi2p;
-                    int meta;
-                    rec_load(st, chi2p, meta, recB, SK, cp);
-                    const float mx = a.sx[hitpos], my = a.sy[hitpos], mz = a.sz[hitpos];
-                    HitCov V;
-                    if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
-                    else V = hit_cov(mx, my, ly);
-                    Ldl3 F;
-                    float r[3], c2;
-                    bool ok = innovation(st, mx, my, mz, V, F, r, c2);
-                    gain_update<ISO>(st, F, V, r);
-                    ok = ok && state_finite(st) && st.IT.x > 0.0f;
-                    if (ok) {
-                        rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
-                    } else {     // failed update: keep the predicted state, finish the candidate
-                        rec_copy(recB, cp, recA, cn, SK);
-                        recA[W_CHI2 * SK + cn] = chi2c;
-                        recA[W_META * SK + cn] = __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16));
-                    }
-                    link = a.perm[hitpos];
-                }
-                link_hit[l * SK + s * K + j] = link;
-                link_par[l * SK + s * K + j] = (uint8_t)k;
+                build_child<ISO>(a, T, l, cn);
             }
             __syncthreads();
             if (tid < S) { s_nc[tid] = tid < ns ? s_nnew[tid] : 0; s_off[tid] = s_offn[tid]; }
@@ -405,32 +503,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
         // ---------------- B6: back-trace + store ----------------
         if (tid < ns) a.n_cand_o[s0 + tid] = s_nc[tid];
         for (int idx = tid; idx < ns * K; idx += NT) {
-            const int s = idx / K, j = idx - s * K;
-            const int64_t sg = s0 + s;
-            const int64_t slot = sg * K + j;
-            a.q_o[slot] = a.q[sg];
-            if (j < s_nc[s]) {
-                const int c = s_off[s] + j;
-                State st;
-                float chi2;
-                int meta;
-                rec_load(st, chi2, meta, recA, SK, c);
-                state_store(st, [&](int i, float v) { a.par_o[(int64_t)i * a.ld_out + slot] = v; },
-                            [&](int kk, float v) { a.cov_o[(int64_t)kk * a.ld_out + slot] = v; });
-                a.chi2_o[slot] = chi2;
-                a.nhits_o[slot] = meta & 255;
-                a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
-                int k = j;
-                for (int l = L - 1; l >= a.first_layer; --l) {
-                    a.hit_idx_o[(int64_t)l * a.ld_out + slot] = link_hit[l * SK + s * K + k];
-                    k = link_par[l * SK + s * K + k];
-                }
-                for (int l = 0; l < a.first_layer; ++l)
-                    a.hit_idx_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + sg] : -1;
-            } else {
-                a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
-                for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
-            }
+            build_output(a, T, s0, idx);
         }
         __syncthreads();     // the workspace and the shared arrays are reused by the next tile
         KF_TICK(5);
