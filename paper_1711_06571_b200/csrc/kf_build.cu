@@ -49,12 +49,15 @@ struct BuildArgs {
 };
 
 // record <-> State; buf points at word 0 of the buffer, stride SK between words
-__device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const float* buf, int SK, int c) {
-    state_set(s, [&](int i) { return buf[i * SK + c]; }, [&](int k) { return buf[(6 + k) * SK + c]; });
-    s.CC = f2(buf[(W_TRIG + 0) * SK + c], buf[(W_TRIG + 2) * SK + c]);
-    s.SS = f2(buf[(W_TRIG + 1) * SK + c], buf[(W_TRIG + 3) * SK + c]);
-    chi2 = buf[W_CHI2 * SK + c];
-    meta = __float_as_int(buf[W_META * SK + c]);
+__device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const float* __restrict__ buf, int SK, int c) {
+    float v[NREC];
+#pragma unroll
+    for (int w = 0; w < NREC; ++w) v[w] = __ldcg(buf + w * SK + c);      // all 33 requests in flight together
+    state_set(s, [&](int i) { return v[i]; }, [&](int k) { return v[6 + k]; });
+    s.CC = f2(v[W_TRIG + 0], v[W_TRIG + 2]);
+    s.SS = f2(v[W_TRIG + 1], v[W_TRIG + 3]);
+    chi2 = v[W_CHI2];
+    meta = __float_as_int(v[W_META]);
 }
 
 __device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, float* buf, int SK, int c) {
@@ -224,25 +227,28 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                             const int64_t seg = (int64_t)ev * L + l;
                             for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
                                 const int64_t row = (seg * a.n_z + iz) * a.n_phi;
-                                for (int run = 0; run < 2; ++run) {
-                                    int b0, b1;
-                                    if (run == 0) { b0 = wb.first; b1 = min(wb.first + wb.n_b, a.n_phi); }
-                                    else { b0 = 0; b1 = wb.first + wb.n_b - a.n_phi; }
-                                    if (b1 <= b0) continue;
-                                    const int h0 = a.bin_off[row + b0], h1 = a.bin_off[row + b1];
-                                    for (int hb = h0; hb < h1; hb += 4) {      // four hits per memory round trip
+                                // both runs of the row (the window may wrap at phi = pi) in one pass: four bin offsets in
+                                // one memory round trip, then four hits per round trip over the concatenated ranges
+                                const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
+                                const int h0a = a.bin_off[row + wb.first], h1a = a.bin_off[row + e0];
+                                const int h0b = a.bin_off[row], h1b = a.bin_off[row + e1];
+                                const int na = h1a - h0a, nab = na + (h1b - h0b);
+                                {
+                                    for (int t0 = 0; t0 < nab; t0 += 4) {
                                         float hx[4], hy[4], hz[4];
+                                        int hpos[4];
     #pragma unroll
                                         for (int u = 0; u < 4; ++u) {
-                                            const int hh = min(hb + u, h1 - 1);
-                                            hx[u] = a.sx[hh]; hy[u] = a.sy[hh]; hz[u] = a.sz[hh];
+                                            const int t = min(t0 + u, nab - 1);
+                                            hpos[u] = t < na ? h0a + t : h0b + (t - na);
+                                            hx[u] = a.sx[hpos[u]]; hy[u] = a.sy[hpos[u]]; hz[u] = a.sz[hpos[u]];
                                         }
-    #pragma unroll
+#pragma unroll
                                         for (int u = 0; u < 4; ++u) {
-                                            const int h = hb + u;
+                                            const int h = hpos[u];
                                             const float mx = hx[u], my = hy[u], mz = hz[u];
                                             const float cr = fmaf(px, my, -py * mx);
-                                            const bool in_win = (h < h1) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                            const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
                                                                 (fabsf(mz - pz) <= dzw);
                                             if (!in_win) continue;
                                             bool ok = fok;
@@ -334,40 +340,46 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
 
 // B6, one output slot idx = seed * K + j of the tile
 __device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int idx) {
-    const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
-    float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
-    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
-    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
-    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
-    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
-    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
-    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
-    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
+    const int K = T.K, L = T.L, SK = T.SK;
+    const float* __restrict__ recA = T.recA;
+    const int32_t* __restrict__ link_hit = T.link_hit;
+    const uint8_t* link_par = T.link_par;
+    float* __restrict__ par_o = a.par_o; float* __restrict__ cov_o = a.cov_o; int32_t* __restrict__ hit_o = a.hit_idx_o;
     const int s = idx / K, j = idx - s * K;
     const int64_t sg = s0 + s;
     const int64_t slot = sg * K + j;
     a.q_o[slot] = a.q[sg];
-    if (j < s_nc[s]) {
-        const int c = s_off[s] + j;
+    if (j < T.s_nc[s]) {
+        const int c = T.s_off[s] + j;
         State st;
         float chi2;
         int meta;
         rec_load(st, chi2, meta, recA, SK, c);
-        state_store(st, [&](int i, float v) { a.par_o[(int64_t)i * a.ld_out + slot] = v; },
-                    [&](int kk, float v) { a.cov_o[(int64_t)kk * a.ld_out + slot] = v; });
+        // back-trace: the parent chain runs through shared memory, so the hit links of four layers are requested together
+        int k = j;
+        for (int l = L - 1; l >= a.first_layer; l -= 4) {
+            int v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (l - u >= a.first_layer) {
+                    v[u] = __ldcg(link_hit + (l - u) * SK + s * K + k);
+                    k = link_par[(l - u) * SK + s * K + k];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (l - u >= a.first_layer) hit_o[(int64_t)(l - u) * a.ld_out + slot] = v[u];
+        }
+        for (int l = 0; l < a.first_layer; ++l)
+            hit_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + sg] : -1;
+        state_store(st, [&](int i, float v) { par_o[(int64_t)i * a.ld_out + slot] = v; },
+                    [&](int kk, float v) { cov_o[(int64_t)kk * a.ld_out + slot] = v; });
         a.chi2_o[slot] = chi2;
         a.nhits_o[slot] = meta & 255;
         a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
-        int k = j;
-        for (int l = L - 1; l >= a.first_layer; --l) {
-            a.hit_idx_o[(int64_t)l * a.ld_out + slot] = link_hit[l * SK + s * K + k];
-            k = link_par[l * SK + s * K + k];
-        }
-        for (int l = 0; l < a.first_layer; ++l)
-            a.hit_idx_o[(int64_t)l * a.ld_out + slot] = a.seed_hit_idx ? a.seed_hit_idx[(int64_t)l * a.ld_seed + sg] : -1;
     } else {
         a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
-        for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
+        for (int l = 0; l < L; ++l) hit_o[(int64_t)l * a.ld_out + slot] = -2;
     }
 }
 
@@ -443,35 +455,47 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 }
                 __syncthreads();
                 KF_TICK(1);
-                // ---------------- phase 2: best K children of a seed, thread per seed (B4) ----------------
-                if (tid >= r0 && tid < r1) {
-                    const int s = tid;
-                    const int nc = s_nc[s], ib = s_off[s] - base;
-                    int n_out = 0;
-                    for (; n_out < K; ++n_out) {
-                        int bk = -1, bnh = -1, bhit = 0, binfo = 0;
-                        float bchi = 0.f;
-                        for (int k = 0; k < nc; ++k) {
-                            const int i = ib + k;
-                            const int info = s_pinfo[i], head = s_lhead[i], cnt = s_lcnt[i];
-                            int nh, hit;
-                            float cc;
-                            if (cnt == 0) {              // finished or hit-less parent: exactly one child
-                                if (head) continue;
-                                nh = info & 255; cc = s_pchi2[i]; hit = HITPOS_NONE;
-                            } else {
-                                if (head >= cnt) continue;
-                                nh = (info & 255) + 1; cc = s_lchi2[head * ncap + i]; hit = s_lhit[head * ncap + i];
+                // ---------------- phase 2: best K children of a seed (B4), thread per PARENT ----------------
+                // rank of a child = number of children of the same seed that precede it in the total order R10
+                // (nhits desc, chi2 asc, parent slot asc, sorted hit position asc); the lists are ascending, so counting
+                // in another parent's list stops at the first entry that does not precede.  Ranks are unique.
+                for (int i = tid; i < nround; i += NT) {
+                    const int s = s_cseed[base + i];
+                    const int ib = s_off[s] - base, k = i - ib, nc = s_nc[s];
+                    const int info = s_pinfo[i], cnt = s_lcnt[i];
+                    const int nh = (info & 255) + (cnt ? 1 : 0);
+                    const int nmine = cnt ? cnt : 1;             // a finished or hit-less parent has exactly one child
+                    for (int j = 0; j < nmine; ++j) {
+                        const float cc = cnt ? s_lchi2[j * ncap + i] : s_pchi2[i];
+                        int rank = j;
+                        for (int k2 = 0; k2 < nc && rank < K; ++k2) {
+                            if (k2 == k) continue;
+                            const int i2 = ib + k2;
+                            const int cnt2 = s_lcnt[i2];
+                            const int nh2 = (s_pinfo[i2] & 255) + (cnt2 ? 1 : 0);
+                            if (nh2 > nh) rank += cnt2 ? cnt2 : 1;
+                            else if (nh2 == nh) {
+                                if (cnt2 == 0) {
+                                    const float c2 = s_pchi2[i2];
+                                    rank += (c2 < cc || (c2 == cc && k2 < k)) ? 1 : 0;
+                                } else {
+                                    for (int j2 = 0; j2 < cnt2; ++j2) {
+                                        const float c2 = s_lchi2[j2 * ncap + i2];
+                                        if (c2 < cc || (c2 == cc && k2 < k)) ++rank; else break;
+                                    }
+                                }
                             }
-                            if (bk < 0 || nh > bnh || (nh == bnh && cc < bchi)) { bk = k; bnh = nh; bchi = cc; bhit = hit; binfo = info; }
                         }
-                        if (bk < 0) break;
-                        s_lhead[ib + bk] += 1;
-                        sel_chi2[s * K + n_out] = bchi;
-                        sel_hit[s * K + n_out] = bhit;
-                        sel_pk[s * K + n_out] = bk | (bnh << 8) | (binfo & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
+                        if (rank >= K) break;                    // own entries ascend: the rest ranks later still
+                        sel_chi2[s * K + rank] = cc;
+                        sel_hit[s * K + rank] = cnt ? s_lhit[j * ncap + i] : HITPOS_NONE;
+                        sel_pk[s * K + rank] = k | (nh << 8) | (info & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
                     }
-                    s_nnew[s] = n_out;
+                    if (k == 0) {
+                        int tot = 0;
+                        for (int k2 = 0; k2 < nc; ++k2) { const int c2 = s_lcnt[ib + k2]; tot += c2 ? c2 : 1; }
+                        s_nnew[s] = min(tot, K);
+                    }
                 }
                 __syncthreads();
                 KF_TICK(2);
