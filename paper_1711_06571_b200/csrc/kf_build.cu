@@ -61,11 +61,11 @@ __device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const
 }
 
 __device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, float* buf, int SK, int c) {
-    state_store<false>(s, [&](int i, float v) { buf[i * SK + c] = v; }, [&](int k, float v) { buf[(6 + k) * SK + c] = v; });
-    buf[(W_TRIG + 0) * SK + c] = s.CC.x; buf[(W_TRIG + 1) * SK + c] = s.SS.x;
-    buf[(W_TRIG + 2) * SK + c] = s.CC.y; buf[(W_TRIG + 3) * SK + c] = s.SS.y;
-    buf[W_CHI2 * SK + c] = chi2;
-    buf[W_META * SK + c] = __int_as_float(meta);
+    state_store<false>(s, [&](int i, float v) { __stcg(buf + i * SK + c, v); }, [&](int k, float v) { __stcg(buf + (6 + k) * SK + c, v); });
+    __stcg(buf + (W_TRIG + 0) * SK + c, s.CC.x); __stcg(buf + (W_TRIG + 1) * SK + c, s.SS.x);
+    __stcg(buf + (W_TRIG + 2) * SK + c, s.CC.y); __stcg(buf + (W_TRIG + 3) * SK + c, s.SS.y);
+    __stcg(buf + W_CHI2 * SK + c, chi2);
+    __stcg(buf + W_META * SK + c, __int_as_float(meta));
 }
 
 // src and dst never overlap (different buffers): all loads of a chunk are issued before its stores, so a copy costs two
@@ -75,11 +75,11 @@ __device__ __forceinline__ void rec_copy(const float* __restrict__ src, int cs, 
 #pragma unroll
     for (int w = 0; w < 17; ++w) v[w] = __ldcg(src + w * SK + cs);
 #pragma unroll
-    for (int w = 0; w < 17; ++w) dst[w * SK + cd] = v[w];
+    for (int w = 0; w < 17; ++w) __stcg(dst + w * SK + cd, v[w]);
 #pragma unroll
     for (int w = 17; w < NREC; ++w) v[w - 17] = __ldcg(src + w * SK + cs);
 #pragma unroll
-    for (int w = 17; w < NREC; ++w) dst[w * SK + cd] = v[w - 17];
+    for (int w = 17; w < NREC; ++w) __stcg(dst + w * SK + cd, v[w - 17]);
 }
 
 // ascending (chi2, hit) list of at most K entries, entry j of candidate i at [j * ncap + i] (conflict-free)
@@ -155,10 +155,7 @@ __device__ unsigned long long g_build_timing[8];
 // per-block context: sizes, workspace and shared-memory arrays (built once, passed by reference to the phase bodies)
 struct Tile {
     int S, K, L, ncap, SK;
-    float *recA, *recB; int32_t* link_hit; uint8_t* link_par;
-    int *s_nc, *s_off, *s_nnew, *s_offn;
-    float* sel_chi2; int *sel_hit, *sel_pk; unsigned short* s_cseed;
-    float* s_lchi2; int* s_lhit; unsigned char *s_lcnt, *s_lhead; float* s_pchi2; int* s_pinfo;
+    float *recA, *recB; int32_t* link_hit;
 };
 
 // The three per-thread bodies are separate functions (not inlined) so that each gets its own register allocation:
@@ -167,13 +164,18 @@ struct Tile {
 // phase 1, one live candidate: dense index base + i, round-local index i
 template <bool ISO>
 __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, int l, int base, int i, int64_t s0) {
+    // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
+    extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
+    const BuildSmem m = build_smem(T.S, K, ncap, L);
     float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
-    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
-    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
-    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
-    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
-    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
+    int32_t* link_hit = T.link_hit; uint8_t* link_par = smem + m.link_par;
+    int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off); int* s_offn = (int*)(smem + m.offn);
+    float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit); int* sel_pk = (int*)(smem + m.sel_pk);
+    unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
+    float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
+    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
+    float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
     (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
     (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
     const LayerC& ly = a.layer[l];
@@ -230,8 +232,8 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                 // both runs of the row (the window may wrap at phi = pi) in one pass: four bin offsets in
                                 // one memory round trip, then four hits per round trip over the concatenated ranges
                                 const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
-                                const int h0a = a.bin_off[row + wb.first], h1a = a.bin_off[row + e0];
-                                const int h0b = a.bin_off[row], h1b = a.bin_off[row + e1];
+                                const int h0a = __ldg(a.bin_off + row + wb.first), h1a = __ldg(a.bin_off + row + e0);
+                                const int h0b = __ldg(a.bin_off + row), h1b = __ldg(a.bin_off + row + e1);
                                 const int na = h1a - h0a, nab = na + (h1b - h0b);
                                 {
                                     for (int t0 = 0; t0 < nab; t0 += 4) {
@@ -241,7 +243,7 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                         for (int u = 0; u < 4; ++u) {
                                             const int t = min(t0 + u, nab - 1);
                                             hpos[u] = t < na ? h0a + t : h0b + (t - na);
-                                            hx[u] = a.sx[hpos[u]]; hy[u] = a.sy[hpos[u]]; hz[u] = a.sz[hpos[u]];
+                                            hx[u] = __ldg(a.sx + hpos[u]); hy[u] = __ldg(a.sy + hpos[u]); hz[u] = __ldg(a.sz + hpos[u]);
                                         }
 #pragma unroll
                                         for (int u = 0; u < 4; ++u) {
@@ -285,13 +287,18 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
 // phase 3, one surviving child: dense index cn among the children of the tile
 template <bool ISO>
 __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int l, int cn) {
+    // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
+    extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
+    const BuildSmem m = build_smem(T.S, K, ncap, L);
     float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
-    int32_t* link_hit = T.link_hit; uint8_t* link_par = T.link_par;
-    int* s_nc = T.s_nc; int* s_off = T.s_off; int* s_offn = T.s_offn;
-    float* sel_chi2 = T.sel_chi2; int* sel_hit = T.sel_hit; int* sel_pk = T.sel_pk; unsigned short* s_cseed = T.s_cseed;
-    float* s_lchi2 = T.s_lchi2; int* s_lhit = T.s_lhit; unsigned char* s_lcnt = T.s_lcnt; unsigned char* s_lhead = T.s_lhead;
-    float* s_pchi2 = T.s_pchi2; int* s_pinfo = T.s_pinfo;
+    int32_t* link_hit = T.link_hit; uint8_t* link_par = smem + m.link_par;
+    int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off); int* s_offn = (int*)(smem + m.offn);
+    float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit); int* sel_pk = (int*)(smem + m.sel_pk);
+    unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
+    float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
+    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
+    float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
     (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
     (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
     const LayerC& ly = a.layer[l];
@@ -316,7 +323,7 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
         float chi2p;
         int meta;
         rec_load(st, chi2p, meta, recB, SK, cp);
-        const float mx = a.sx[hitpos], my = a.sy[hitpos], mz = a.sz[hitpos];
+        const float mx = __ldg(a.sx + hitpos), my = __ldg(a.sy + hitpos), mz = __ldg(a.sz + hitpos);
         HitCov V;
         if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
         else V = hit_cov(mx, my, ly);
@@ -329,28 +336,31 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
             rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
         } else {     // failed update: keep the predicted state, finish the candidate
             rec_copy(recB, cp, recA, cn, SK);
-            recA[W_CHI2 * SK + cn] = chi2c;
-            recA[W_META * SK + cn] = __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16));
+            __stcg(recA + W_CHI2 * SK + cn, chi2c);
+            __stcg(recA + W_META * SK + cn, __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16)));
         }
-        link = a.perm[hitpos];
+        link = __ldg(a.perm + hitpos);
     }
-    link_hit[l * SK + s * K + j] = link;
+    __stcg(link_hit + l * SK + s * K + j, link);
     link_par[l * SK + s * K + j] = (uint8_t)k;
 }
 
 // B6, one output slot idx = seed * K + j of the tile
 __device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int idx) {
+    extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, SK = T.SK;
+    const BuildSmem m = build_smem(T.S, K, T.ncap, L);
     const float* __restrict__ recA = T.recA;
     const int32_t* __restrict__ link_hit = T.link_hit;
-    const uint8_t* link_par = T.link_par;
+    const uint8_t* link_par = smem + m.link_par;
+    const int* s_nc = (const int*)(smem + m.nc); const int* s_off = (const int*)(smem + m.off);
     float* __restrict__ par_o = a.par_o; float* __restrict__ cov_o = a.cov_o; int32_t* __restrict__ hit_o = a.hit_idx_o;
     const int s = idx / K, j = idx - s * K;
     const int64_t sg = s0 + s;
     const int64_t slot = sg * K + j;
     a.q_o[slot] = a.q[sg];
-    if (j < T.s_nc[s]) {
-        const int c = T.s_off[s] + j;
+    if (j < s_nc[s]) {
+        const int c = s_off[s] + j;
         State st;
         float chi2;
         int meta;
@@ -405,10 +415,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     uint8_t* link_par = smem + m.link_par;
     Tile T;
     T.S = S; T.K = K; T.L = L; T.ncap = ncap; T.SK = SK;
-    T.recA = recA; T.recB = recB; T.link_hit = link_hit; T.link_par = link_par;
-    T.s_nc = s_nc; T.s_off = s_off; T.s_nnew = s_nnew; T.s_offn = s_offn;
-    T.sel_chi2 = sel_chi2; T.sel_hit = sel_hit; T.sel_pk = sel_pk; T.s_cseed = s_cseed;
-    T.s_lchi2 = s_lchi2; T.s_lhit = s_lhit; T.s_lcnt = s_lcnt; T.s_lhead = s_lhead; T.s_pchi2 = s_pchi2; T.s_pinfo = s_pinfo;
+    T.recA = recA; T.recB = recB; T.link_hit = link_hit;
 
 #ifdef KF_BUILD_TIMING
     long long tick_ = clock64();
