@@ -42,17 +42,24 @@ struct BuildArgs {
     const int32_t *seed_event, *seed_hit_idx;
     const float *sx, *sy, *sz; const int32_t *perm, *bin_off;
     float *par_o, *cov_o, *chi2_o; int8_t* q_o; int32_t* nhits_o; uint32_t* status_o; int32_t *hit_idx_o, *n_cand_o;
-    float* ws_rec;            // [grid][2][NREC][S*K]
+    float* ws_rec;            // [grid][2][NREC4][S*K] float4
     int32_t* ws_link_hit;     // [grid][n_layers][S*K]
     LayerC layer[KF_MAX_LAYERS];
     float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax); (sig_rphi/r)^2
 };
 
-// record <-> State; buf points at word 0 of the buffer, stride SK between words
+// Records are stored as NREC4 = 9 groups of four words, group g of record c at float4 index g * SK + c: a record moves
+// with 9 coalesced 16-byte accesses per thread.  buf points at group 0 of the buffer.
+constexpr int NREC4 = (NREC + 3) / 4;
+
 __device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const float* __restrict__ buf, int SK, int c) {
-    float v[NREC];
+    float v[4 * NREC4];
+    const float4* __restrict__ b4 = reinterpret_cast<const float4*>(buf);
 #pragma unroll
-    for (int w = 0; w < NREC; ++w) v[w] = __ldcg(buf + w * SK + c);      // all 33 requests in flight together
+    for (int g = 0; g < NREC4; ++g) {                                   // all requests in flight together
+        const float4 t = __ldcg(b4 + g * SK + c);
+        v[4 * g] = t.x; v[4 * g + 1] = t.y; v[4 * g + 2] = t.z; v[4 * g + 3] = t.w;
+    }
     state_set(s, [&](int i) { return v[i]; }, [&](int k) { return v[6 + k]; });
     s.CC = f2(v[W_TRIG + 0], v[W_TRIG + 2]);
     s.SS = f2(v[W_TRIG + 1], v[W_TRIG + 3]);
@@ -60,26 +67,30 @@ __device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const
     meta = __float_as_int(v[W_META]);
 }
 
-__device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, float* buf, int SK, int c) {
-    state_store<false>(s, [&](int i, float v) { __stcg(buf + i * SK + c, v); }, [&](int k, float v) { __stcg(buf + (6 + k) * SK + c, v); });
-    __stcg(buf + (W_TRIG + 0) * SK + c, s.CC.x); __stcg(buf + (W_TRIG + 1) * SK + c, s.SS.x);
-    __stcg(buf + (W_TRIG + 2) * SK + c, s.CC.y); __stcg(buf + (W_TRIG + 3) * SK + c, s.SS.y);
-    __stcg(buf + W_CHI2 * SK + c, chi2);
-    __stcg(buf + W_META * SK + c, __int_as_float(meta));
+__device__ __forceinline__ void rec_store(const State& s, float chi2, int meta, float* __restrict__ buf, int SK, int c) {
+    float v[4 * NREC4];
+    state_store<false>(s, [&](int i, float x) { v[i] = x; }, [&](int k, float x) { v[6 + k] = x; });
+    v[W_TRIG + 0] = s.CC.x; v[W_TRIG + 1] = s.SS.x; v[W_TRIG + 2] = s.CC.y; v[W_TRIG + 3] = s.SS.y;
+    v[W_CHI2] = chi2; v[W_META] = __int_as_float(meta);
+    v[33] = 0.0f; v[34] = 0.0f; v[35] = 0.0f;
+    float4* __restrict__ b4 = reinterpret_cast<float4*>(buf);
+#pragma unroll
+    for (int g = 0; g < NREC4; ++g) __stcg(b4 + g * SK + c, make_float4(v[4 * g], v[4 * g + 1], v[4 * g + 2], v[4 * g + 3]));
 }
 
-// src and dst never overlap (different buffers): all loads of a chunk are issued before its stores, so a copy costs two
-// memory round trips instead of one per word
+// one word of a record
+__device__ __forceinline__ float rec_word(const float* buf, int SK, int c, int w) { return __ldcg(buf + ((w >> 2) * SK + c) * 4 + (w & 3)); }
+__device__ __forceinline__ void rec_set_word(float* buf, int SK, int c, int w, float x) { __stcg(buf + ((w >> 2) * SK + c) * 4 + (w & 3), x); }
+
+// src and dst never overlap (different buffers): all loads are issued before the stores
 __device__ __forceinline__ void rec_copy(const float* __restrict__ src, int cs, float* __restrict__ dst, int cd, int SK) {
-    float v[17];
+    const float4* __restrict__ s4 = reinterpret_cast<const float4*>(src);
+    float4* __restrict__ d4 = reinterpret_cast<float4*>(dst);
+    float4 v[NREC4];
 #pragma unroll
-    for (int w = 0; w < 17; ++w) v[w] = __ldcg(src + w * SK + cs);
+    for (int g = 0; g < NREC4; ++g) v[g] = __ldcg(s4 + g * SK + cs);
 #pragma unroll
-    for (int w = 0; w < 17; ++w) __stcg(dst + w * SK + cd, v[w]);
-#pragma unroll
-    for (int w = 17; w < NREC; ++w) v[w - 17] = __ldcg(src + w * SK + cs);
-#pragma unroll
-    for (int w = 17; w < NREC; ++w) __stcg(dst + w * SK + cd, v[w - 17]);
+    for (int g = 0; g < NREC4; ++g) __stcg(d4 + g * SK + cd, v[g]);
 }
 
 // ascending (chi2, hit) list of at most K entries, entry j of candidate i at [j * ncap + i] (conflict-free)
@@ -312,8 +323,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
     if (hitpos == HITPOS_NONE) {
         rec_copy(recB, cp, recA, cn, SK);
         if (pkd & (1 << 16)) {
-            const int meta = __float_as_int(recB[W_META * SK + cp]) | 256 | (((pkd >> 24) & 15) << 16);
-            recA[W_META * SK + cn] = __int_as_float(meta);
+            const int meta = __float_as_int(rec_word(recB, SK, cp, W_META)) | 256 | (((pkd >> 24) & 15) << 16);
+            rec_set_word(recA, SK, cn, W_META, __int_as_float(meta));
             link = -2;
         } else {
             link = -1;
@@ -336,8 +347,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
             rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
         } else {     // failed update: keep the predicted state, finish the candidate
             rec_copy(recB, cp, recA, cn, SK);
-            __stcg(recA + W_CHI2 * SK + cn, chi2c);
-            __stcg(recA + W_META * SK + cn, __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16)));
+            rec_set_word(recA, SK, cn, W_CHI2, chi2c);
+            rec_set_word(recA, SK, cn, W_META, __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16)));
         }
         link = __ldg(a.perm + hitpos);
     }
@@ -409,8 +420,8 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     int* s_misc = (int*)(smem + m.misc);          // [0..31] warp sums of the scan, [32] round end
     const int tid = threadIdx.x;
 
-    float* recA = a.ws_rec + (size_t)blockIdx.x * 2 * NREC * SK;
-    float* recB = recA + (size_t)NREC * SK;
+    float* recA = a.ws_rec + (size_t)blockIdx.x * 2 * (4 * NREC4) * SK;
+    float* recB = recA + (size_t)(4 * NREC4) * SK;
     int32_t* link_hit = a.ws_link_hit + (size_t)blockIdx.x * L * SK;
     uint8_t* link_par = smem + m.link_par;
     Tile T;
@@ -576,7 +587,7 @@ static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
     p.grid = (int)std::min<int64_t>(std::max<int64_t>(p.n_tiles, 1), resident);
     auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
     size_t o = 0;
-    p.o_rec = o; o += up((size_t)p.grid * 2 * NREC * SK * sizeof(float));
+    p.o_rec = o; o += up((size_t)p.grid * 2 * (4 * NREC4) * SK * sizeof(float));
     p.o_lh = o; o += up((size_t)p.grid * n_layers * SK * sizeof(int32_t));
     p.total = o;
     return p;
