@@ -39,7 +39,7 @@ FIT_BYTES_OUT = 6 * 4 + 21 * 4 + 4 + 4 + 4        # par + cov + chi2 + nhits + s
 FIT_BYTES_PER_HIT = 12
 FIT_BYTES_PER_IDX = 4
 BUILD_FLOP = dict(n_prop=458.0, n_scan=15.0, n_window=40.0, n_upd=250.0)
-BIN_BYTES_PER_HIT = 44.0
+BIN_BYTES_PER_HIT = 60.0   # read 12, key 4 + 4, tmp 8 + 8, write x, y, z, perm 16 + packed record 16 (the place kernel re-reads 8)
 SM_COUNT, FP32_LANES = 148, 128
 FIT_CFG = {"fit_c0": 0, "fit_c1": 1, "fit_c2": 2}
 BUILD_CFG = {"build_c3": 3, "build_c4": 4}

@@ -109,6 +109,8 @@ typedef struct {
     float *x, *y, *z;     /* [n_hits] hits in sorted order                                                 */
     int32_t* perm;        /* [n_hits] sorted position -> original index within its segment                 */
     int32_t* bin_off;     /* [n_events*n_layers*n_z*n_phi + 1] offsets into the sorted arrays              */
+    float* xyzp;          /* [n_hits][4] the same hits as 16-byte records (x, y, z, bits of perm): what the */
+                          /* window scan of kf_build reads, one load per hit; 16-byte aligned; required     */
 } kf_binned;
 
 size_t kf_bin_workspace_bytes(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z);

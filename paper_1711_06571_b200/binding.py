@@ -47,7 +47,7 @@ class kf_hits(C.Structure):
 
 class kf_binned(C.Structure):
     _fields_ = [("n_phi", C.c_int32), ("n_z", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p),
-                ("perm", C.c_void_p), ("bin_off", C.c_void_p)]
+                ("perm", C.c_void_p), ("bin_off", C.c_void_p), ("xyzp", C.c_void_p)]
 
 
 class kf_cands(C.Structure):
@@ -204,12 +204,14 @@ class Binned:
         self.z = torch.empty(m, dtype=torch.float32, device=device)
         self.perm = torch.empty(m, dtype=torch.int32, device=device)
         self.bin_off = torch.empty(n_bins + 1, dtype=torch.int32, device=device)
-        self.c = kf_binned(n_phi, n_z, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(), self.perm.data_ptr(), self.bin_off.data_ptr())
+        self.xyzp = torch.empty((m, 4), dtype=torch.float32, device=device)
+        self.c = kf_binned(n_phi, n_z, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(), self.perm.data_ptr(), self.bin_off.data_ptr(),
+                           self.xyzp.data_ptr())
 
     def to_host(self) -> dict:
         n = self.n_hits
         return dict(x=self.x[:n].cpu().numpy(), y=self.y[:n].cpu().numpy(), z=self.z[:n].cpu().numpy(), perm=self.perm[:n].cpu().numpy(),
-                    bin_off=self.bin_off.cpu().numpy(), n_phi=self.n_phi, n_z=self.n_z)
+                    bin_off=self.bin_off.cpu().numpy(), n_phi=self.n_phi, n_z=self.n_z, xyzp=self.xyzp[:n].cpu().numpy())
 
 
 def kf_bin_workspace_bytes(geom: Geom, hits: Hits, n_phi: int, n_z: int) -> int:

@@ -33,6 +33,7 @@ struct BinArgs {
     int2* tmp;                   // [n_hits] (key, original index within segment)
     float *sx, *sy, *sz;
     int32_t* perm;
+    float4* xyzp;
     float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
 };
 
@@ -137,10 +138,12 @@ __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_place_kernel(const __grid_co
     const int seg = me.x / (a.n_z * a.n_phi);
     const int64_t src = a.seg_off[seg] + me.y;
     const int dst = o0 + rank;
+    const float x = a.hx[src], y = a.hy[src], z = a.hz[src];
     a.perm[dst] = me.y;
-    a.sx[dst] = a.hx[src];
-    a.sy[dst] = a.hy[src];
-    a.sz[dst] = a.hz[src];
+    a.sx[dst] = x;
+    a.sy[dst] = y;
+    a.sz[dst] = z;
+    a.xyzp[dst] = make_float4(x, y, z, __int_as_float(me.y));
 }
 
 // ---- window lookup (diagnostic entry; the build kernel walks the same ranges) ----
@@ -225,7 +228,7 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
     if (!hits->seg_off || !hits->seg_off_dev) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: hits->seg_off / seg_off_dev is NULL");
     if (!out->bin_off) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: out->bin_off is NULL");
     const int64_t n_hits = hits->n_hits;
-    if (n_hits > 0 && (!hits->x || !hits->y || !hits->z || !out->x || !out->y || !out->z || !out->perm))
+    if (n_hits > 0 && (!hits->x || !hits->y || !hits->z || !out->x || !out->y || !out->z || !out->perm || !out->xyzp))
         return fail(KF_ERR_NULL_PTR, "kf_bin_hits: NULL hit array");
     const int n_seg = hits->n_events * geom->n_layers;
     if (hits->seg_off[0] != 0 || hits->seg_off[n_seg] != n_hits) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits: seg_off must run from 0 to n_hits");
@@ -253,7 +256,7 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
     a.hx = hits->x; a.hy = hits->y; a.hz = hits->z; a.seg_off = hits->seg_off_dev;
     a.tan_tab = (const float*)(base + w.tab);
     a.key = (int32_t*)(base + w.key); a.bin_off = out->bin_off; a.cursor = (int32_t*)(base + w.cursor); a.tmp = (int2*)(base + w.tmp);
-    a.sx = out->x; a.sy = out->y; a.sz = out->z; a.perm = out->perm;
+    a.sx = out->x; a.sy = out->y; a.sz = out->z; a.perm = out->perm; a.xyzp = (float4*)out->xyzp;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
         a.zmax[l] = y.zmax;

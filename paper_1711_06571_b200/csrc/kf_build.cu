@@ -40,7 +40,7 @@ struct BuildArgs {
     int64_t n_seeds, ld_seed, ld_out, n_tiles;
     const float *par, *cov; const int8_t* q;
     const int32_t *seed_event, *seed_hit_idx;
-    const float *sx, *sy, *sz; const int32_t *perm, *bin_off;
+    const float4* xyzp; const int32_t* bin_off;
     float *par_o, *cov_o, *chi2_o; int8_t* q_o; int32_t* nhits_o; uint32_t* status_o; int32_t *hit_idx_o, *n_cand_o;
     float* ws_rec;            // [grid][2][NREC4][S*K] float4
     int32_t* ws_link_hit;     // [grid][n_layers][S*K]
@@ -248,18 +248,18 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                 const int na = h1a - h0a, nab = na + (h1b - h0b);
                                 {
                                     for (int t0 = 0; t0 < nab; t0 += 4) {
-                                        float hx[4], hy[4], hz[4];
+                                        float4 hv[4];
                                         int hpos[4];
     #pragma unroll
                                         for (int u = 0; u < 4; ++u) {
                                             const int t = min(t0 + u, nab - 1);
                                             hpos[u] = t < na ? h0a + t : h0b + (t - na);
-                                            hx[u] = __ldg(a.sx + hpos[u]); hy[u] = __ldg(a.sy + hpos[u]); hz[u] = __ldg(a.sz + hpos[u]);
+                                            hv[u] = __ldg(a.xyzp + hpos[u]);
                                         }
 #pragma unroll
                                         for (int u = 0; u < 4; ++u) {
                                             const int h = hpos[u];
-                                            const float mx = hx[u], my = hy[u], mz = hz[u];
+                                            const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
                                             const float cr = fmaf(px, my, -py * mx);
                                             const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
                                                                 (fabsf(mz - pz) <= dzw);
@@ -334,7 +334,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
         float chi2p;
         int meta;
         rec_load(st, chi2p, meta, recB, SK, cp);
-        const float mx = __ldg(a.sx + hitpos), my = __ldg(a.sy + hitpos), mz = __ldg(a.sz + hitpos);
+        const float4 hv = __ldg(a.xyzp + hitpos);
+            const float mx = hv.x, my = hv.y, mz = hv.z;
         HitCov V;
         if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
         else V = hit_cov(mx, my, ly);
@@ -350,7 +351,7 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
             rec_set_word(recA, SK, cn, W_CHI2, chi2c);
             rec_set_word(recA, SK, cn, W_META, __int_as_float(((meta & ~255) | nh) | 256 | (int)(ST_NUMERIC << 16)));
         }
-        link = __ldg(a.perm + hitpos);
+        link = __float_as_int(hv.w);
     }
     __stcg(link_hit + l * SK + s * K + j, link);
     link_par[l * SK + s * K + j] = (uint8_t)k;
@@ -642,7 +643,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     out->K = K; out->n_layers = geom->n_layers; out->n_seeds = seeds->n; out->cand.n = seeds->n * K;
     if (seeds->n == 0) return KF_OK;
     if (!seeds->par || !seeds->cov || !seeds->q) return fail(KF_ERR_NULL_PTR, "kf_build: NULL seed array");
-    if (!binned->x || !binned->y || !binned->z || !binned->perm || !binned->bin_off) return fail(KF_ERR_NULL_PTR, "kf_build: NULL binned array");
+    if (!binned->xyzp || !binned->bin_off) return fail(KF_ERR_NULL_PTR, "kf_build: NULL binned array (xyzp, bin_off)");
     if (hits->n_events > 1 && !seed_event) return fail(KF_ERR_NULL_PTR, "kf_build: seed_event is NULL with n_events > 1");
     const kf_tracks& c = out->cand;
     if (!c.par || !c.cov || !c.q || !c.chi2 || !c.nhits || !c.status || !out->hit_idx || !out->n_cand)
@@ -656,7 +657,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     a.kb = KCURV * geom->bz_tesla; a.chi2_cut = chi2_cut; a.n_sigma = n_sigma; a.inv_dphi = host_inv_dphi(binned->n_phi);
     a.n_seeds = seeds->n; a.ld_seed = seeds->ld; a.ld_out = out->ld;
     a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.seed_event = seed_event; a.seed_hit_idx = seed_hit_idx;
-    a.sx = binned->x; a.sy = binned->y; a.sz = binned->z; a.perm = binned->perm; a.bin_off = binned->bin_off;
+    a.xyzp = (const float4*)binned->xyzp; a.bin_off = binned->bin_off;
     a.par_o = c.par; a.cov_o = c.cov; a.chi2_o = c.chi2; a.q_o = c.q; a.nhits_o = c.nhits; a.status_o = c.status;
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;
     a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh);

@@ -32,6 +32,10 @@ def ref_bin(bi):
 def assert_binned_equal(g, r):
     for k in ("bin_off", "perm", "x", "y", "z"):
         assert np.array_equal(g[k], r[k]), k
+    # the 16-byte records the build kernel reads: same hits, perm carried as bits
+    p4 = g["xyzp"]
+    assert np.array_equal(p4[:, 0], r["x"]) and np.array_equal(p4[:, 1], r["y"]) and np.array_equal(p4[:, 2], r["z"])
+    assert np.array_equal(np.ascontiguousarray(p4[:, 3]).view(np.int32), r["perm"])
 
 
 @pytest.mark.parametrize("config,kw", [(3, dict(n_events=1, tracks=1)), (3, dict(n_events=3, tracks=777)), (3, {}),
