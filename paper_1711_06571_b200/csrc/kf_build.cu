@@ -28,6 +28,10 @@ namespace kf {
 constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (twice the seeds of the tile)
 constexpr int BUILD_THREADS_PER_SM = 512; // 128 registers per thread
 constexpr int NREC = 33;                  // words per candidate record
+#ifndef KF_SCAN_BATCH
+#define KF_SCAN_BATCH 4
+#endif
+constexpr int SCAN_BATCH = KF_SCAN_BATCH;  // hits requested together in the window scan
 constexpr int HITPOS_NONE = 0x7fffffff;
 constexpr int LIST_BYTES_PER_THREAD = 192; // shared memory for the per-candidate child lists, per thread of the block
 enum { W_TRIG = 27, W_CHI2 = 31, W_META = 32 };
@@ -93,23 +97,31 @@ __device__ __forceinline__ void rec_copy(const float* __restrict__ src, int cs, 
     for (int g = 0; g < NREC4; ++g) __stcg(d4 + g * SK + cd, v[g]);
 }
 
-// ascending (chi2, hit) list of at most K entries, entry j of candidate i at [j * ncap + i] (conflict-free)
-__device__ __forceinline__ void list_insert(float* lc, int* lh, int ncap, int K, int& n, float c, int h) {
-    int pos;
-    if (n == K) {
-        const float cl = lc[(K - 1) * ncap]; const int hl = lh[(K - 1) * ncap];
-        if (!(c < cl || (c == cl && h < hl))) return;
-        pos = K - 1;
-    } else {
-        pos = n++;
+// Child list of a candidate: at most K entries (chi2, hit), entry j of candidate i at [j * ncap + i] (conflict-free).
+// During the scan entries are appended unsorted; a full list (more than K compatible hits: rare) keeps the best K by
+// replacing its worst entry; list_sort orders it ascending by (chi2, hit) once the scan is over.
+__device__ __noinline__ void list_replace_worst(float* lc, int* lh, int ncap, int K, float c, int h) {
+    int w = 0;
+    float cw = lc[0]; int hw = lh[0];
+    for (int j = 1; j < K; ++j) {
+        const float cj = lc[j * ncap]; const int hj = lh[j * ncap];
+        if (cj > cw || (cj == cw && hj > hw)) { w = j; cw = cj; hw = hj; }
     }
-    while (pos > 0) {
-        const float cp = lc[(pos - 1) * ncap]; const int hp = lh[(pos - 1) * ncap];
-        if (!(c < cp || (c == cp && h < hp))) break;
-        lc[pos * ncap] = cp; lh[pos * ncap] = hp;
-        --pos;
+    if (c < cw || (c == cw && h < hw)) { lc[w * ncap] = c; lh[w * ncap] = h; }
+}
+
+__device__ __forceinline__ void list_sort(float* lc, int* lh, int ncap, int n) {
+    for (int a = 1; a < n; ++a) {
+        const float c = lc[a * ncap]; const int h = lh[a * ncap];
+        int pos = a;
+        while (pos > 0) {
+            const float cp = lc[(pos - 1) * ncap]; const int hp = lh[(pos - 1) * ncap];
+            if (!(c < cp || (c == cp && h < hp))) break;
+            lc[pos * ncap] = cp; lh[pos * ncap] = hp;
+            --pos;
+        }
+        lc[pos * ncap] = c; lh[pos * ncap] = h;
     }
-    lc[pos * ncap] = c; lh[pos * ncap] = h;
 }
 
 // exclusive scan of one int per thread over the block (NT threads); returns the exclusive prefix, total in *total
@@ -157,10 +169,17 @@ __host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap, int L) {
 }
 
 #ifdef KF_BUILD_TIMING
-__device__ unsigned long long g_build_timing[8];
+__device__ unsigned long long g_build_timing[16];
 #define KF_TICK(i) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_build_timing[i], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
 #else
 #define KF_TICK(i) do { } while (0)
+#endif
+#ifdef KF_BUILD_TIMING
+#define KF_CTICK(i) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_build_timing[i], (unsigned long long)(now_ - ctick_)); ctick_ = now_; } } while (0)
+#define KF_CTICK_INIT long long ctick_ = clock64()
+#else
+#define KF_CTICK(i) do { } while (0)
+#define KF_CTICK_INIT do { } while (0)
 #endif
 
 // per-block context: sizes, workspace and shared-memory arrays (built once, passed by reference to the phase bodies)
@@ -194,10 +213,12 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                         const int64_t sg = s0 + s_cseed[c];
                         const float cw = -(float)a.q[sg] * a.kb;
                         const int ev = a.seed_event ? a.seed_event[sg] : 0;
+                        KF_CTICK_INIT;
                         State st;
                         float chi2;
                         int meta;
                         rec_load(st, chi2, meta, recA, SK, c);
+                        KF_CTICK(8);
                         uint32_t flag = 0u;
                         bool fin = (meta & 256) != 0;
                         float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
@@ -232,38 +253,45 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                         }
                         int cnt = 0;
                         if (!fin) {
+                            KF_CTICK(9);
                             rec_store(st, chi2, meta, recB, SK, c);
+                            KF_CTICK(10);
                             // ---- window scan (B3) ----
                             bool sbad = false;
                             float* lc = s_lchi2 + i;
                             int* lh = s_lhit + i;
                             const int64_t seg = (int64_t)ev * L + l;
+                            // Both runs of a row (the window may wrap at phi = pi) are scanned as one range.  Memory round
+                            // trips are what this loop costs (the hits are cold): the four bin offsets of the NEXT row are
+                            // requested before the hits of the current row, and SCAN_BATCH hits are requested together.
+                            const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
+                            const int32_t* bo = a.bin_off + (seg * a.n_z + wb.iz_lo) * a.n_phi;
+                            int h0a = 0, h1a = 0, h0b = 0, h1b = 0;
+                            if (wb.iz_lo <= wb.iz_hi) { h0a = __ldg(bo + wb.first); h1a = __ldg(bo + e0); h0b = __ldg(bo); h1b = __ldg(bo + e1); }
                             for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
-                                const int64_t row = (seg * a.n_z + iz) * a.n_phi;
-                                // both runs of the row (the window may wrap at phi = pi) in one pass: four bin offsets in
-                                // one memory round trip, then four hits per round trip over the concatenated ranges
-                                const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
-                                const int h0a = __ldg(a.bin_off + row + wb.first), h1a = __ldg(a.bin_off + row + e0);
-                                const int h0b = __ldg(a.bin_off + row), h1b = __ldg(a.bin_off + row + e1);
+                                bo += a.n_phi;
+                                int n0a = 0, n1a = 0, n0b = 0, n1b = 0;
+                                if (iz < wb.iz_hi) { n0a = __ldg(bo + wb.first); n1a = __ldg(bo + e0); n0b = __ldg(bo); n1b = __ldg(bo + e1); }
                                 const int na = h1a - h0a, nab = na + (h1b - h0b);
                                 {
-                                    for (int t0 = 0; t0 < nab; t0 += 4) {
-                                        float4 hv[4];
-                                        int hpos[4];
+                                    for (int t0 = 0; t0 < nab; t0 += SCAN_BATCH) {
+                                        float4 hv[SCAN_BATCH];
+                                        int hpos[SCAN_BATCH];
     #pragma unroll
-                                        for (int u = 0; u < 4; ++u) {
+                                        for (int u = 0; u < SCAN_BATCH; ++u) {
                                             const int t = min(t0 + u, nab - 1);
                                             hpos[u] = t < na ? h0a + t : h0b + (t - na);
                                             hv[u] = __ldg(a.xyzp + hpos[u]);
                                         }
 #pragma unroll
-                                        for (int u = 0; u < 4; ++u) {
+                                        for (int u = 0; u < SCAN_BATCH; ++u) {
                                             const int h = hpos[u];
                                             const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
                                             const float cr = fmaf(px, my, -py * mx);
                                             const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
                                                                 (fabsf(mz - pz) <= dzw);
-                                            if (!in_win) continue;
+                                            // branch-free up to the verdict: a divergent path per slot would be run by the
+                                            // whole warp whenever a single lane takes it
                                             bool ok = fok;
                                             if (!ISO) {
                                                 const HitCov V = hit_cov(mx, my, ly);
@@ -272,27 +300,37 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                                 Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
                                                 ok = ldl3(Sm, F);
                                             }
-                                            if (!ok) { sbad = true; continue; }
+                                            sbad = sbad || (in_win && !ok);
                                             const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
                                             const float y1 = fmaf(-F.l10, q0, q1);
                                             const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
                                             const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                            if (c2 < a.chi2_cut) list_insert(lc, lh, ncap, K, cnt, chi2 + c2, h);
+                                            if (in_win && ok && c2 < a.chi2_cut) {
+                                                if (cnt < K) {           // unsorted append (two predicated stores)
+                                                    lc[cnt * ncap] = chi2 + c2; lh[cnt * ncap] = h; ++cnt;
+                                                } else {
+                                                    list_replace_worst(lc, lh, ncap, K, chi2 + c2, h);
+                                                }
+                                            }
                                         }
                                     }
                                 }
+                                h0a = n0a; h1a = n1a; h0b = n0b; h1b = n1b;
                             }
+                            list_sort(lc, lh, ncap, cnt);
                             if (sbad) {      // S not positive definite: one finished child with the unchanged state
                                 fin = true;
                                 flag = ST_NUMERIC;
                                 cnt = 0;
                             }
                         }
+                        KF_CTICK(11);
                         if (fin) rec_copy(recA, c, recB, c, SK);
                         s_lcnt[i] = (unsigned char)cnt;
                         s_lhead[i] = 0;
                         s_pchi2[i] = chi2;
                         s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
+                        KF_CTICK(12);
 }
 
 // phase 3, one surviving child: dense index cn among the children of the tile
@@ -554,9 +592,6 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
 }
 
 // ---- host side: tile size, grid and workspace layout (one function, used by the size query and by the launch) ----
-#ifndef KF_BUILD_DEFAULT_TILE
-#define KF_BUILD_DEFAULT_TILE 128
-#endif
 static int g_build_tile = 0;   // 0 = default
 
 static int sm_count() {
@@ -576,7 +611,9 @@ struct BuildPlan { int S, NT, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o
 static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
     BuildPlan p;
     int S = g_build_tile;
-    if (S == 0) S = KF_BUILD_DEFAULT_TILE;
+    if (S == 0)      // one wave of 128-seed tiles when the job is that small (latency-sized), otherwise small tiles: more
+                     // independent blocks per SM, so that the block-level barriers of one tile overlap work of another
+        S = n_seeds <= (int64_t)128 * 2 * sm_count() ? 128 : 32;
     p.S = S;
     p.NT = S <= 32 ? 64 : (S <= 64 ? 128 : 256);
     const int SK = S * K;
@@ -609,8 +646,8 @@ static int launch_build(const BuildArgs& a, const BuildPlan& p, bool iso, cudaSt
 #ifdef KF_BUILD_TIMING
 extern "C" void kf_build_timing(unsigned long long* out, int reset) {
     cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out, kf::g_build_timing, sizeof(unsigned long long) * 8);
-    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(kf::g_build_timing, z, sizeof z); }
+    cudaMemcpyFromSymbol(out, kf::g_build_timing, sizeof(unsigned long long) * 16);
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(kf::g_build_timing, z, sizeof z); }
 }
 #endif
 
