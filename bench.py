@@ -326,12 +326,14 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
 
 
 def stored_traffic(workload):
-    tr = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tr):
-        try:
-            return json.load(open(tr)).get(workload)
-        except Exception:
-            return None
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.csv)."""
+    import csv
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tr):
+        return None
+    for row in csv.DictReader(open(tr)):
+        if row["workload"] == workload and row["dram_bytes_per_launch"]:
+            return float(row["dram_bytes_per_launch"])
     return None
 
 

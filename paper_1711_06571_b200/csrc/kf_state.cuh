@@ -3,14 +3,15 @@
 //
 // Why: on B200 a scalar three-register FFMA issues at best every ~1.7 cycles per SM sub-partition (measured), a
 // packed FFMA2 every ~2.2 cycles for two FMAs, and FFMA2 takes any scalar register as a free broadcast operand.
-// The 148 x 128 x 2 FP32 peak is therefore only reachable with packed instructions.  The 6x6 algebra of the
+// The 148 x 128 x 2 FP32 peak is therefore only reachable with packed instructions, and a candidate's step takes
+// 452 instead of 560 warp instructions.  The 6x6 algebra of the
 // step is arranged so that its long, regular chains run two rows (or two columns) of a matrix at a time:
 //   rows (x, y) and rows (z, phi) of T = J C and of J C J^T,        columns (1/pT, theta) of T,
 //   rows (0,1), (2,4), (3,5) of the gain K = C H^T S^-1 and of the covariance update.
 // The covariance is stored in exactly the pairs those chains consume and produce, so no repacking is needed between
 // layers; three elements are held twice (C01, C20, C21) and kept identical by copies.
-// Jacobian sparsity ("patterns of elements known ... to be zero or one", sec. 2.1) is written out as in
-// kf_math.cuh.  Formulas: DESIGN.md sec. 3 (R2 helix/cylinder solve, R3 surface Jacobian, R4 Highland noise,
+// Jacobian sparsity (20 non-zeros, 3 of them == 1; "patterns of elements known ... to be zero or one", PAPER.md:L40
+// sec. 2.1) is written out by hand.  Formulas: DESIGN.md sec. 3 (R2 helix/cylinder solve, R3 surface Jacobian, R4 Highland noise,
 // R5 3-D update).  Shares nothing with oracle/.
 #pragma once
 #include "kf_math.cuh"
@@ -213,8 +214,12 @@ __device__ __forceinline__ void rotate_poly2(float2& c, float2& sn_, float2 d) {
     c = mul2(cn, k); sn_ = mul2(sn, k);
 }
 
-// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C <- C - K C[0:3,:], the columns that touch the
-// measured block in the cancellation-free form K V (see kf_math.cuh).  ISO: V = diag(V.xx, V.xx, V.zz).
+// Gain and update (R5): K = C[:,0:3] S^-1, p += K r, C <- C - K C[0:3,:].
+// The columns that touch the measured block are written in the algebraically identical, cancellation-free form
+//   (C - K H C) H^T = C H^T - K (S - V) = K V          (because K S = C H^T),
+// which matters in fp32: for low-pT tracks at shallow incidence the predicted position variance exceeds the hit
+// variance by 1e3-1e4 and C - K C would lose every significant digit of the updated position block.
+// ISO: V = diag(V.xx, V.xx, V.zz) (sig_r == sig_rphi on every layer).
 template <bool ISO>
 __device__ __forceinline__ void gain_update(State& s, const Ldl3& F, const HitCov& V, const float (&r)[3]) {
     float2 KP0, KP1, KP2, KQ0, KQ1, KQ2, KR0, KR1, KR2;      // K rows (0,1), (2,4), (3,5); index = column
