@@ -160,6 +160,17 @@ int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, 
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
              float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * kf_select_best -- hand-over from building to the final fit ("When a complete track has been
+ * reconstructed, a final fit using the KF is performed").  hit_idx[l*ld + s] = hit of the best candidate (slot s*K)
+ * of seed s on layer l, in the layout kf_fit reads; layers without hit, layers not crossed and layers < first_layer
+ * (already behind the seed state) are -1.  The final fit is then
+ *   kf_fit(geom, hits, hit_idx, seed_event, seeds, out, stream)       with ld == seeds->ld.
+ * Note: kf_fit skips a layer without hit entirely (R8) whereas kf_build transports the candidate through it
+ * (adding its scattering), so the refit equals the built candidate only for hit lists without holes.
+ * Errors: NULL pointers, ld < n_seeds, first_layer outside 0..n_layers, CUDA failure. */
+int kf_select_best(const kf_cands* cands, int32_t first_layer, int32_t* hit_idx, int64_t ld, void* stream);
+
 const char* kf_last_error(void);
 int kf_version(void);
 

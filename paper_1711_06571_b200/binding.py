@@ -20,7 +20,7 @@ KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
 EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
-           "kf_build", "kf_build_set_tile", "kf_last_error", "kf_version"]
+           "kf_build", "kf_build_set_tile", "kf_select_best", "kf_last_error", "kf_version"]
 
 
 class KfError(RuntimeError):
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_build_set_tile.argtypes = [C.c_int32]
+        l.kf_select_best.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p]
         l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = l
     return _lib
@@ -289,4 +290,15 @@ def kf_build(geom: Geom, hits: Hits, binned: Binned, seeds: Tracks, seed_event, 
                         first_layer, K, chi2_cut, n_sigma, C.byref(out.c), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
     _check(rc, "kf_build")
     out._ws = ws    # keep the workspace alive until the stream has consumed it
+    return out
+
+
+def kf_select_best(cands: Cands, first_layer: int, ld: int, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """include/kf.h kf_select_best -> [n_layers, ld] int32 hit indices of the best candidate per seed, for kf_fit."""
+    _require_cuda()
+    if out is None:
+        out = torch.full((cands.n_layers, ld), -1, dtype=torch.int32, device=cands.hit_idx.device)
+    assert tuple(out.shape) == (cands.n_layers, ld)
+    rc = lib().kf_select_best(C.byref(cands.c), first_layer, _ptr(out, torch.int32), ld, _stream(stream))
+    _check(rc, "kf_select_best")
     return out
