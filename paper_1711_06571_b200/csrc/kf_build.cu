@@ -25,6 +25,9 @@
 
 namespace kf {
 
+#ifndef KF_BUILD_TPS
+#define KF_BUILD_TPS 2     // threads per seed of the tile
+#endif
 constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (twice the seeds of the tile)
 constexpr int BUILD_THREADS_PER_SM = 512; // 128 registers per thread
 constexpr int NREC = 33;                  // words per candidate record
@@ -124,6 +127,10 @@ __device__ __forceinline__ void list_sort(float* lc, int* lh, int ncap, int n) {
     }
 }
 
+__device__ __forceinline__ unsigned long long child_key(int nh, float chi2, int k, int j) {
+    return ((unsigned long long)(63 - nh) << 42) | ((unsigned long long)__float_as_uint(chi2) << 10) | (unsigned long long)((k << 5) | j);
+}
+
 // exclusive scan of one int per thread over the block (NT threads); returns the exclusive prefix, total in *total
 template <int NT>
 __device__ __forceinline__ int block_exclusive_scan(int v, int* s_warp, int* total) {
@@ -160,7 +167,7 @@ __host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap, int L) {
     auto take = [&](int bytes) { const int at = o; o += (bytes + 15) & ~15; return at; };
     m.nc = take(4 * S); m.off = take(4 * (S + 1)); m.nnew = take(4 * S); m.offn = take(4 * (S + 1));
     m.sel_chi2 = take(4 * S * K); m.sel_hit = take(4 * S * K); m.sel_pk = take(4 * S * K); m.cseed = take(2 * S * K);
-    m.l_chi2 = take(4 * ncap * K); m.l_hit = take(4 * ncap * K); m.l_cnt = take(ncap); m.l_head = take(ncap);
+    m.l_chi2 = take(4 * ncap * K); m.l_hit = take(4 * ncap * K); m.l_cnt = take(ncap); m.l_head = take(8 * ncap);
     m.p_chi2 = take(4 * ncap); m.p_info = take(4 * ncap);
     m.link_par = take(L * S * K);
     m.misc = take(4 * 40);
@@ -327,7 +334,6 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                         KF_CTICK(11);
                         if (fin) rec_copy(recA, c, recB, c, SK);
                         s_lcnt[i] = (unsigned char)cnt;
-                        s_lhead[i] = 0;
                         s_pchi2[i] = chi2;
                         s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
                         KF_CTICK(12);
@@ -454,7 +460,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     int* sel_pk = (int*)(smem + m.sel_pk);
     unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
     float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
-    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
+    unsigned char* s_lcnt = smem + m.l_cnt; unsigned long long* s_hkey = (unsigned long long*)(smem + m.l_head);
     float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
     int* s_misc = (int*)(smem + m.misc);          // [0..31] warp sums of the scan, [32] round end
     const int tid = threadIdx.x;
@@ -512,47 +518,33 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 }
                 __syncthreads();
                 KF_TICK(1);
-                // ---------------- phase 2: best K children of a seed (B4), thread per PARENT ----------------
-                // rank of a child = number of children of the same seed that precede it in the total order R10
-                // (nhits desc, chi2 asc, parent slot asc, sorted hit position asc); the lists are ascending, so counting
-                // in another parent's list stops at the first entry that does not precede.  Ranks are unique.
-                for (int i = tid; i < nround; i += NT) {
-                    const int s = s_cseed[base + i];
-                    const int ib = s_off[s] - base, k = i - ib, nc = s_nc[s];
-                    const int info = s_pinfo[i], cnt = s_lcnt[i];
-                    const int nh = (info & 255) + (cnt ? 1 : 0);
-                    const int nmine = cnt ? cnt : 1;             // a finished or hit-less parent has exactly one child
-                    for (int j = 0; j < nmine; ++j) {
-                        const float cc = cnt ? s_lchi2[j * ncap + i] : s_pchi2[i];
-                        int rank = j;
-                        for (int k2 = 0; k2 < nc && rank < K; ++k2) {
-                            if (k2 == k) continue;
-                            const int i2 = ib + k2;
-                            const int cnt2 = s_lcnt[i2];
-                            const int nh2 = (s_pinfo[i2] & 255) + (cnt2 ? 1 : 0);
-                            if (nh2 > nh) rank += cnt2 ? cnt2 : 1;
-                            else if (nh2 == nh) {
-                                if (cnt2 == 0) {
-                                    const float c2 = s_pchi2[i2];
-                                    rank += (c2 < cc || (c2 == cc && k2 < k)) ? 1 : 0;
-                                } else {
-                                    for (int j2 = 0; j2 < cnt2; ++j2) {
-                                        const float c2 = s_lchi2[j2 * ncap + i2];
-                                        if (c2 < cc || (c2 == cc && k2 < k)) ++rank; else break;
-                                    }
-                                }
-                            }
-                        }
-                        if (rank >= K) break;                    // own entries ascend: the rest ranks later still
-                        sel_chi2[s * K + rank] = cc;
-                        sel_hit[s * K + rank] = cnt ? s_lhit[j * ncap + i] : HITPOS_NONE;
-                        sel_pk[s * K + rank] = k | (nh << 8) | (info & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
+                // ---------------- phase 2: best K children of a seed (B4), thread per seed ----------------
+                // K-way merge of the sorted child lists of the <= K parents.  The head of every list is a 48-bit key whose
+                // integer order is the total order R10: (63 - nhits) | chi2 bits (chi2 >= 0, so the bit pattern is
+                // monotonic) | parent slot | position in the parent's list (ascending in (chi2, hit)); exhausted = all ones.
+                if (tid >= r0 && tid < r1) {
+                    const int s = tid;
+                    const int nc = s_nc[s], ib = s_off[s] - base;
+                    for (int k = 0; k < nc; ++k) {
+                        const int i = ib + k;
+                        const int cnt = s_lcnt[i];
+                        const int nh = (s_pinfo[i] & 255) + (cnt ? 1 : 0);     // a finished or hit-less parent: one child, no hit
+                        s_hkey[i] = child_key(nh, cnt ? s_lchi2[i] : s_pchi2[i], k, 0);
                     }
-                    if (k == 0) {
-                        int tot = 0;
-                        for (int k2 = 0; k2 < nc; ++k2) { const int c2 = s_lcnt[ib + k2]; tot += c2 ? c2 : 1; }
-                        s_nnew[s] = min(tot, K);
+                    int n_out = 0;
+                    for (; n_out < K; ++n_out) {
+                        unsigned long long best = ~0ull;
+                        for (int k = 0; k < nc; ++k) best = min(best, s_hkey[ib + k]);
+                        if (best == ~0ull) break;
+                        const int k = (int)(best >> 5) & 31, j = (int)best & 31, nh = 63 - (int)(best >> 42);
+                        const int i = ib + k;
+                        const int cnt = s_lcnt[i];
+                        sel_chi2[s * K + n_out] = __uint_as_float((unsigned)(best >> 10));
+                        sel_hit[s * K + n_out] = cnt ? s_lhit[j * ncap + i] : HITPOS_NONE;
+                        sel_pk[s * K + n_out] = k | (nh << 8) | (s_pinfo[i] & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
+                        s_hkey[i] = (j + 1 < cnt) ? child_key(nh, s_lchi2[(j + 1) * ncap + i], k, j + 1) : ~0ull;
                     }
+                    s_nnew[s] = n_out;
                 }
                 __syncthreads();
                 KF_TICK(2);
@@ -615,7 +607,7 @@ static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
                      // independent blocks per SM, so that the block-level barriers of one tile overlap work of another
         S = n_seeds <= (int64_t)128 * 2 * sm_count() ? 128 : 32;
     p.S = S;
-    p.NT = S <= 32 ? 64 : (S <= 64 ? 128 : 256);
+    p.NT = S * KF_BUILD_TPS <= 64 ? 64 : (S * KF_BUILD_TPS <= 128 ? 128 : 256);
     const int SK = S * K;
     p.ncap = std::min(SK, std::max(std::max(K, 32), (LIST_BYTES_PER_THREAD * p.NT / (8 * K)) & ~31));
     p.n_tiles = (n_seeds + S - 1) / S;
