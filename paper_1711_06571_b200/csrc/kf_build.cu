@@ -401,8 +401,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
     link_par[l * SK + s * K + j] = (uint8_t)k;
 }
 
-// B6, one output slot idx = seed * K + j of the tile
-__device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int idx) {
+// B6, one live candidate (dense index c) -> its output slot; unused slots are filled by the caller
+__device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int c) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, SK = T.SK;
     const BuildSmem m = build_smem(T.S, K, T.ncap, L);
@@ -411,12 +411,12 @@ __device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int
     const uint8_t* link_par = smem + m.link_par;
     const int* s_nc = (const int*)(smem + m.nc); const int* s_off = (const int*)(smem + m.off);
     float* __restrict__ par_o = a.par_o; float* __restrict__ cov_o = a.cov_o; int32_t* __restrict__ hit_o = a.hit_idx_o;
-    const int s = idx / K, j = idx - s * K;
+    const unsigned short* s_cseed = (const unsigned short*)(smem + m.cseed);
+    const int s = s_cseed[c], j = c - s_off[s];
     const int64_t sg = s0 + s;
     const int64_t slot = sg * K + j;
-    a.q_o[slot] = a.q[sg];
-    if (j < s_nc[s]) {
-        const int c = s_off[s] + j;
+    (void)s_nc;
+    {
         State st;
         float chi2;
         int meta;
@@ -443,9 +443,6 @@ __device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int
         a.chi2_o[slot] = chi2;
         a.nhits_o[slot] = meta & 255;
         a.status_o[slot] = (uint32_t)(meta >> 16) & 15u;
-    } else {
-        a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
-        for (int l = 0; l < L; ++l) hit_o[(int64_t)l * a.ld_out + slot] = -2;
     }
 }
 
@@ -575,8 +572,15 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
 
         // ---------------- B6: back-trace + store ----------------
         if (tid < ns) a.n_cand_o[s0 + tid] = s_nc[tid];
-        for (int idx = tid; idx < ns * K; idx += NT) {
-            build_output(a, T, s0, idx);
+        for (int c = tid; c < s_off[ns]; c += NT) build_output(a, T, s0, c);       // live candidates, densely
+        for (int idx = tid; idx < ns * K; idx += NT) {                            // every slot: charge; unused slots: empty
+            const int s = idx / K, j = idx - s * K;
+            const int64_t slot = (s0 + s) * K + j;
+            a.q_o[slot] = a.q[s0 + s];
+            if (j >= s_nc[s]) {
+                a.chi2_o[slot] = 0.0f; a.nhits_o[slot] = 0; a.status_o[slot] = 0u;
+                for (int l = 0; l < L; ++l) a.hit_idx_o[(int64_t)l * a.ld_out + slot] = -2;
+            }
         }
         __syncthreads();     // the workspace and the shared arrays are reused by the next tile
         KF_TICK(5);
