@@ -274,23 +274,50 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
     value = fi.n * d.world / (ms_per_step * 1e-3)
 
     # ---- end to end: pinned host buffers -> H2D -> kf_fit -> D2H, all inside the timed region ----
-    h_par, h_cov, h_q = pin(fi.par), pin(fi.cov), pin(fi.q)
-    h_x, h_y, h_z = pin(fi.hit_x), pin(fi.hit_y), pin(fi.hit_z)
-    h_idx = None if fi.hit_idx is None else pin(fi.hit_idx)
-    o_par = torch.empty((6, seeds.ld), dtype=torch.float32).pin_memory(); o_cov = torch.empty((21, seeds.ld), dtype=torch.float32).pin_memory()
-    o_chi2 = torch.empty(fi.n, dtype=torch.float32).pin_memory(); o_nh = torch.empty(fi.n, dtype=torch.int32).pin_memory()
-    o_st = torch.empty(fi.n, dtype=torch.int32).pin_memory()
-    h2d = nbytes((h_par, h_cov, h_q, h_x, h_y, h_z, h_idx))
-    d2h = nbytes((o_par, o_cov, o_chi2, o_nh, o_st))
+    # The tracks are split into `args.e2e_streams` independent sub-batches, each with its own stream, pinned host
+    # buffers and device buffers, so that the copies of one sub-batch overlap the fit of another ("multiple events in
+    # flight ... to overlap expensive copy operations").
+    L = fi.geom.n_layers
+    n_sub = max(1, min(args.e2e_streams, fi.n))
+    bounds = [fi.n * i // n_sub for i in range(n_sub + 1)]
+    subs = []
+    for c in range(n_sub):
+        lo, hi = bounds[c], bounds[c + 1]
+        m = hi - lo
+        ldc = max(32, (m + 31) // 32 * 32)
+        hp = np.zeros((6, ldc), np.float32); hp[:, :m] = fi.par[:, lo:hi]
+        hc = np.zeros((21, ldc), np.float32); hc[:, :m] = fi.cov[:, lo:hi]
+        hxs = [np.ascontiguousarray(a_.reshape(L, fi.ld)[:, lo:hi]).reshape(-1) for a_ in (fi.hit_x, fi.hit_y, fi.hit_z)]
+        hidx = None
+        if fi.hit_idx is not None:
+            hidx = np.full((L, ldc), -1, np.int32)
+            hidx[:, :m] = np.where(fi.hit_idx[:, lo:hi] >= 0, np.arange(m, dtype=np.int32)[None, :], -1)
+        sub = dict(m=m, stream=torch.cuda.Stream(), h_in=[pin(hp), pin(hc), pin(fi.q[lo:hi])] + [pin(x) for x in hxs] + ([pin(hidx)] if hidx is not None else []))
+        sub["seeds"] = b.Tracks.empty(m, ldc)
+        sub["hits"] = b.Hits(hxs[0], hxs[1], hxs[2], np.arange(L + 1, dtype=np.int64) * m, 1)
+        sub["hit_idx"] = None if hidx is None else torch.from_numpy(hidx).cuda()
+        sub["out"] = b.Tracks.empty(m, ldc)
+        sub["out"].q = sub["seeds"].q
+        sub["d_in"] = [sub["seeds"].par, sub["seeds"].cov, sub["seeds"].q, sub["hits"].x, sub["hits"].y, sub["hits"].z] + ([sub["hit_idx"]] if hidx is not None else [])
+        sub["d_out"] = [sub["out"].par, sub["out"].cov, sub["out"].chi2, sub["out"].nhits, sub["out"].status]
+        sub["h_out"] = [torch.empty(t_.shape, dtype=t_.dtype).pin_memory() for t_ in sub["d_out"]]
+        subs.append(sub)
+    h2d = sum(nbytes(sb["h_in"]) for sb in subs)
+    d2h = sum(nbytes(sb["h_out"]) for sb in subs)
 
     def e2e_step(rec):
-        seeds.par.copy_(h_par, non_blocking=True); seeds.cov.copy_(h_cov, non_blocking=True); seeds.q.copy_(h_q, non_blocking=True)
-        hits.x.copy_(h_x, non_blocking=True); hits.y.copy_(h_y, non_blocking=True); hits.z.copy_(h_z, non_blocking=True)
-        if h_idx is not None:
-            hit_idx.copy_(h_idx, non_blocking=True)
-        b.kf_fit(geom, hits, hit_idx, None, seeds, out=out, stream=stream)
-        o_par.copy_(out.par, non_blocking=True); o_cov.copy_(out.cov, non_blocking=True); o_chi2.copy_(out.chi2, non_blocking=True)
-        o_nh.copy_(out.nhits, non_blocking=True); o_st.copy_(out.status, non_blocking=True)
+        start = torch.cuda.Event(); start.record(stream)
+        for sb in subs:
+            st_ = sb["stream"]
+            st_.wait_event(start)
+            with torch.cuda.stream(st_):
+                for dst, src in zip(sb["d_in"], sb["h_in"]):
+                    dst.copy_(src, non_blocking=True)
+                b.kf_fit(geom, sb["hits"], sb["hit_idx"], None, sb["seeds"], out=sb["out"], stream=st_)
+                for dst, src in zip(sb["h_out"], sb["d_out"]):
+                    dst.copy_(src, non_blocking=True)
+            done = torch.cuda.Event(); done.record(st_)
+            stream.wait_event(done)
 
     e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
     e2e_value = fi.n * d.world / (e2e_ms * 1e-3)
@@ -316,7 +343,7 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 config=dict(workload=workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=units["track_layers"],
                             l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (units["bytes"] / 1e6)),
-                clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms),
+                clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms, streams=n_sub),
                 gpu_launches=args.steps, roofline=roofline)
     if not args.no_cpu_baseline:
         cb = oracle_fit(fi, args.cpu_sample, 1, 0)
@@ -437,6 +464,7 @@ def main():
     ap.add_argument("--ref-events", type=int, default=16, help="--impl reference: events per step (build workloads)")
     ap.add_argument("--cpu-sample", type=int, default=200_000)
     ap.add_argument("--cpu-events", type=int, default=16, help="events the oracle builds for cpu_baseline and the build counters")
+    ap.add_argument("--e2e-streams", type=int, default=4, help="sub-batches in flight in the end-to-end leg (copies overlap compute)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-build", action="store_true", help="default line without the configs[3] build leg")
     args = ap.parse_args()
