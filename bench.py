@@ -402,18 +402,54 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     value = bi.n_seeds * d.world / (ms_per_step * 1e-3)
 
     # ---- end to end: hits + seeds H2D, bin + build, candidates D2H ----
-    h = [pin(a) for a in (bi.hit_x, bi.hit_y, bi.hit_z, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx)]
-    dev = [hits.x, hits.y, hits.z, seeds.par, seeds.cov, seeds.q, sev, shi]
-    outs = [out.tracks.par, out.tracks.cov, out.tracks.chi2, out.tracks.nhits, out.tracks.status, out.hit_idx, out.n_cand]
-    ho = [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in outs]
+    # The events are split into `args.e2e_streams` groups, each with its own stream and buffers: several events in flight,
+    # copies of one group overlapping the building of another.
+    n_sub = max(1, min(args.e2e_streams, bi.n_events))
+    ev_b = [bi.n_events * i // n_sub for i in range(n_sub + 1)]
+    subs = []
+    for c in range(n_sub):
+        e0, e1 = ev_b[c], ev_b[c + 1]
+        h0, h1 = int(bi.seg_off[e0 * L]), int(bi.seg_off[e1 * L])
+        sel = np.nonzero((bi.seed_event >= e0) & (bi.seed_event < e1))[0]
+        s0_, s1_ = (int(sel[0]), int(sel[-1]) + 1) if len(sel) else (0, 0)
+        m = s1_ - s0_
+        ldc = max(32, (m + 31) // 32 * 32)
+        hp = np.zeros((6, ldc), np.float32); hp[:, :m] = bi.par[:, s0_:s1_]
+        hc = np.zeros((21, ldc), np.float32); hc[:, :m] = bi.cov[:, s0_:s1_]
+        hs = np.full((bi.first_layer, ldc), -1, np.int32); hs[:, :m] = bi.seed_hit_idx[:, s0_:s1_]
+        sub = dict(stream=torch.cuda.Stream(), n_ev=e1 - e0, m=m)
+        sub["hits"] = b.Hits(bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], bi.seg_off[e0 * L: e1 * L + 1] - h0, e1 - e0)
+        sub["binned"] = b.Binned(h1 - h0, (e1 - e0) * L * bi.n_phi * bi.n_z, bi.n_phi, bi.n_z)
+        sub["ws"] = torch.empty(max(b.kf_bin_workspace_bytes(geom, sub["hits"], bi.n_phi, bi.n_z), 1), dtype=torch.uint8, device="cuda")
+        sub["seeds"] = b.Tracks.empty(m, ldc)
+        sub["sev"] = torch.zeros(max(m, 1), dtype=torch.int32, device="cuda")[:m]
+        sub["shi"] = torch.empty((bi.first_layer, ldc), dtype=torch.int32, device="cuda")
+        sub["out"] = b.Cands(m, K, L)
+        sub["bws"] = torch.empty(max(b.kf_build_workspace_bytes(geom, m, K), 1), dtype=torch.uint8, device="cuda")
+        sub["h_in"] = [pin(a_) for a_ in (bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], hp, hc, bi.q[s0_:s1_], bi.seed_event[s0_:s1_] - e0, hs)]
+        sub["d_in"] = [sub["hits"].x, sub["hits"].y, sub["hits"].z, sub["seeds"].par, sub["seeds"].cov, sub["seeds"].q, sub["sev"], sub["shi"]]
+        o_ = sub["out"]
+        sub["d_out"] = [o_.tracks.par, o_.tracks.cov, o_.tracks.chi2, o_.tracks.nhits, o_.tracks.status, o_.hit_idx, o_.n_cand]
+        sub["h_out"] = [torch.empty(t_.shape, dtype=t_.dtype).pin_memory() for t_ in sub["d_out"]]
+        subs.append(sub)
+    h = [x for sb in subs for x in sb["h_in"]]
+    ho = [x for sb in subs for x in sb["h_out"]]
 
     def e2e_step(rec):
-        for dst, src in zip(dev, h):
-            dst.copy_(src, non_blocking=True)
-        b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
-        b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, ws=bws, stream=stream)
-        for dst, src in zip(ho, outs):
-            dst.copy_(src, non_blocking=True)
+        start = torch.cuda.Event(); start.record(stream)
+        for sb in subs:
+            st_ = sb["stream"]
+            st_.wait_event(start)
+            with torch.cuda.stream(st_):
+                for dst, src in zip(sb["d_in"], sb["h_in"]):
+                    dst.copy_(src, non_blocking=True)
+                b.kf_bin_hits(geom, sb["hits"], bi.n_phi, bi.n_z, out=sb["binned"], ws=sb["ws"], stream=st_)
+                b.kf_build(geom, sb["hits"], sb["binned"], sb["seeds"], sb["sev"], sb["shi"], bi.first_layer, K, bi.chi2_cut, bi.n_sigma,
+                           out=sb["out"], ws=sb["bws"], stream=st_)
+                for dst, src in zip(sb["h_out"], sb["d_out"]):
+                    dst.copy_(src, non_blocking=True)
+            done = torch.cuda.Event(); done.record(st_)
+            stream.wait_event(done)
 
     e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
     if d.rank != 0:
@@ -426,7 +462,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
                            l2="192 MB fill between timed iterations (outside the timed segments)" if flush is not None else
                               "hits + sorted copy + candidates per step exceed the 126 MB L2; no explicit flush"),
                e2e=dict(value=bi.n_seeds * d.world / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=nbytes(h), d2h_bytes_per_step=nbytes(ho),
-                        ms_per_step=e2e_ms),
+                        ms_per_step=e2e_ms, streams=n_sub),
                gpu_launches=args.steps * BUILD_LAUNCHES_PER_STEP, clocks=clocks)
     bin_bytes = BIN_BYTES_PER_HIT * hits.n_hits + 8.0 * n_bins
     res["bin_roofline"] = dict(bound="hbm", achieved=bin_bytes / (bin_ms * 1e-3) / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
