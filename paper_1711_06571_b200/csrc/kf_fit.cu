@@ -26,13 +26,90 @@ struct FitArgs {
 #define KF_FIT_BLOCK 128
 #endif
 #ifndef KF_FIT_MINB
-#define KF_FIT_MINB 4
+#define KF_FIT_MINB 5
 #endif
 constexpr int FIT_BLOCK = KF_FIT_BLOCK;
 
 // IDX: explicit hit_idx (else identity), EVT: per-track event (else event 0), ISO: sig_r == sig_rphi on every layer.
-// The layer loop leaves through `break` when the track ends (failed propagation: the state of the last updated layer
-// is final) or when the update went numerically wrong (rare: the track is then redone up to the layer before).
+
+// The layer loop of one track, layers [0, limit).  Leaves through `break` when the track ends (failed propagation: the
+// state of the last updated layer is final; status bit set) or when an update went numerically wrong: then the index
+// of that layer is returned (-1 otherwise) and the state is garbage.  CAREFUL: every element of the state is checked
+// after every layer (the fast path checks what reaches chi2 and the parameters, and the whole state once at the end).
+template <bool IDX, bool EVT, bool ISO, bool CAREFUL>
+__device__ __forceinline__ int fit_layers(const FitArgs& a, int64_t t, float cw, int64_t seg, int limit, State& s, float& chi2, int& nh,
+                                          uint32_t& st) {
+    // F1: coalesced SoA load
+    state_load(s, [&](int i) { return a.par[i * a.ld_in + t]; }, [&](int k) { return a.cov[k * a.ld_in + t]; });
+    chi2 = 0.0f;
+    nh = 0;
+    int bad = -1;
+    // F6 with identity indexing: the hit of the next layer is requested one layer ahead
+    float nx = 0.f, ny = 0.f, nz = 0.f;
+    if (!IDX && !EVT && limit > 0) { nx = a.hxl[0][t]; ny = a.hyl[0][t]; nz = a.hzl[0][t]; }
+#pragma unroll 1
+    for (int l = 0; l < limit; ++l) {
+        int64_t idx = t;
+        if (IDX) {
+            idx = a.hit_idx[l * a.ld_idx + t];
+            if (idx < 0) continue;           // layer skipped entirely (R8)
+        }
+        // F6: issued before the arithmetic
+        float mx, my, mz;
+        if (EVT) {
+            const int64_t h = a.seg_off_dev[seg + l] + idx;
+            mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
+        } else {
+            if (!IDX) {
+                mx = nx; my = ny; mz = nz;
+                if (l + 1 < limit) { nx = a.hxl[l + 1][t]; ny = a.hyl[l + 1][t]; nz = a.hzl[l + 1][t]; }
+            } else {
+                mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+            }
+        }
+        const LayerC ly = a.layer[l];
+        const uint32_t flag = predict(s, cw, ly);                          // F2-F5
+        if (flag) {
+            st |= flag;
+            break;
+        }
+        Ldl3 Si;
+        float r[3], c2;
+        HitCov V;
+        if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
+        else V = hit_cov(mx, my, ly);
+        bool ok = innovation(s, mx, my, mz, V, Si, r, c2);                  // F7 (branch-free; garbage when !ok)
+        gain_update<ISO>(s, Si, V, r);                                      // F8
+        ok = ok && step_finite(s, c2) && s.IT.x > 0.0f && (!CAREFUL || state_finite(s));
+        if (!ok) {
+            bad = l;
+            break;
+        }
+        chi2 += c2;
+        nh += 1;
+    }
+    return bad;
+}
+
+// Numeric failure (rare): the track keeps the state of the last good layer, i.e. it is redone up to the layer before the
+// one that failed.  A separate function so that the fast path keeps its registers.
+template <bool IDX, bool EVT, bool ISO>
+__device__ __noinline__ void fit_redo(const FitArgs& a, int64_t t, float cw, int64_t seg, State& s, float& chi2, int& nh, uint32_t& st) {
+    int limit = a.n_layers;
+    st = 0u;
+    for (int attempt = 0; attempt < 3; ++attempt) {
+        const uint32_t keep = st;
+        const int bad = fit_layers<IDX, EVT, ISO, true>(a, t, cw, seg, limit, s, chi2, nh, st);
+        if (bad < 0) return;
+        st = keep | ST_NUMERIC;
+        limit = bad;
+    }
+    // three failing layers in a row: the seed itself
+    state_load(s, [&](int i) { return a.par[i * a.ld_in + t]; }, [&](int k) { return a.cov[k * a.ld_in + t]; });
+    chi2 = 0.0f;
+    nh = 0;
+}
+
 template <bool IDX, bool EVT, bool ISO>
 __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {
     const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
@@ -40,71 +117,11 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
     const float cw = -(float)a.q[t] * a.kb;
     const int64_t seg = EVT ? (int64_t)a.trk_event[t] * a.n_layers : 0;
     State s;
-    float chi2 = 0.0f;
-    int nh = 0;
+    float chi2;
+    int nh;
     uint32_t st = 0u;
-    int limit = a.n_layers;
-    bool careful = false;
-    for (int attempt = 0; attempt < 3; ++attempt) {
-        // F1: coalesced SoA load
-        state_load(s, [&](int i) { return a.par[i * a.ld_in + t]; }, [&](int k) { return a.cov[k * a.ld_in + t]; });
-        chi2 = 0.0f;
-        nh = 0;
-        int bad = -1;
-        // F6 with identity indexing: the hit of the next layer is requested one layer ahead
-        float nx = 0.f, ny = 0.f, nz = 0.f;
-        if (!IDX && !EVT && limit > 0) { nx = a.hxl[0][t]; ny = a.hyl[0][t]; nz = a.hzl[0][t]; }
-#pragma unroll 1
-        for (int l = 0; l < limit; ++l) {
-            int64_t idx = t;
-            if (IDX) {
-                idx = a.hit_idx[l * a.ld_idx + t];
-                if (idx < 0) continue;           // layer skipped entirely (R8)
-            }
-            // F6: issued before the arithmetic
-            float mx, my, mz;
-            if (EVT) {
-                const int64_t h = a.seg_off_dev[seg + l] + idx;
-                mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
-            } else {
-                if (!IDX) {
-                    mx = nx; my = ny; mz = nz;
-                    if (l + 1 < limit) { nx = a.hxl[l + 1][t]; ny = a.hyl[l + 1][t]; nz = a.hzl[l + 1][t]; }
-                } else {
-                    mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
-                }
-            }
-            const LayerC ly = a.layer[l];
-            const uint32_t flag = predict(s, cw, ly);                          // F2-F5
-            if (flag) {
-                st |= flag;
-                break;
-            }
-            Ldl3 Si;
-            float r[3], c2;
-            HitCov V;
-            if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
-            else V = hit_cov(mx, my, ly);
-            bool ok = innovation(s, mx, my, mz, V, Si, r, c2);                  // F7 (branch-free; garbage when !ok)
-            gain_update<ISO>(s, Si, V, r);                                      // F8
-            ok = ok && step_finite(s, c2) && s.IT.x > 0.0f && (!careful || state_finite(s));
-            if (!ok) {
-                bad = l;
-                break;
-            }
-            chi2 += c2;
-            nh += 1;
-        }
-        if (bad < 0) {
-            if (careful || state_finite(s)) break;
-            careful = true;          // something non-finite slipped through the cheap per-layer check: find the layer
-            st = 0u;
-            continue;
-        }
-        // numeric failure (rare): the track keeps the state of the last good layer -> redo the layers before it
-        st |= ST_NUMERIC;
-        limit = bad;
-    }
+    const int bad = fit_layers<IDX, EVT, ISO, false>(a, t, cw, seg, a.n_layers, s, chi2, nh, st);
+    if (bad >= 0 || !state_finite(s)) fit_redo<IDX, EVT, ISO>(a, t, cw, seg, s, chi2, nh, st);
     // F9: coalesced store
     state_store(s, [&](int i, float v) { a.par_o[i * a.ld_out + t] = v; }, [&](int k, float v) { a.cov_o[k * a.ld_out + t] = v; });
     a.chi2_o[t] = chi2;
