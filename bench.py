@@ -183,6 +183,19 @@ def run_reference(args, workload):
         fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks)
         cb = oracle_fit(fi, args.ref_sample, args.steps, args.warmup)
         metric, cfg = "tracks_fitted_per_s", dict(workload=workload, tracks=fi.n, layers=fi.geom.n_layers)
+    elif workload == "mplex":
+        from oracle import kf_oracle as o
+        m = 2_000_000
+        rng = np.random.default_rng(66)
+        a_ = rng.normal(size=(m, 6, 6)).astype(np.float32); b_ = rng.normal(size=(m, 6, 6)).astype(np.float32)
+        for _ in range(args.warmup):
+            o.mat66_multiply(a_, b_)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            o.mat66_multiply(a_, b_)
+        dt = (time.perf_counter() - t0) / args.steps
+        cb = dict(value=m / dt, unit="multiplies/s", cores=1, kind="oracle", sample=f"{m} matrices per step, numpy fp64 matmul", ms_per_step=dt * 1e3)
+        metric, cfg = "mat66_multiplies_per_s", dict(workload=workload, matrices=args.tracks or 4_000_000)
     else:
         bi = synth.build_inputs(BUILD_CFG[workload], n_events=args.events)
         cb, _, _ = oracle_build(bi, args.ref_events, args.steps, args.warmup)
@@ -487,13 +500,65 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     return res
 
 
+def bench_mplex(args, d: Dist):
+    """Layout micro-benchmark (sec. 4.3, Fig. 5): n 6x6 products per step in
+    matrix-major layout (`value`), as an array of matrices, and through the library (cuBLAS batched GEMM via torch.bmm)."""
+    import torch
+    from paper_1711_06571_b200 import binding as b
+    n = args.tracks or 4_000_000
+    g = torch.Generator(device="cuda"); g.manual_seed(66 + d.rank)
+    A1 = torch.randn((n, 36), generator=g, device="cuda"); B1 = torch.randn((n, 36), generator=g, device="cuda")
+    A0 = A1.t().contiguous(); B0 = B1.t().contiguous()
+    C0 = torch.empty_like(A0); C1 = torch.empty_like(A1); C2 = torch.empty((n, 6, 6), device="cuda")
+    stream = torch.cuda.current_stream()
+    W = max(args.warmup, 3)
+    res = {}
+    for name, fn in (("matrix_major", lambda rec: b.kf_mat66_multiply(0, A0, B0, out=C0, stream=stream)),
+                     ("array_of_matrices", lambda rec: b.kf_mat66_multiply(1, A1, B1, out=C1, stream=stream)),
+                     ("cublas_bmm", lambda rec: torch.bmm(A1.view(n, 6, 6), B1.view(n, 6, 6), out=C2))):
+        sampler = ClockSampler(d.local) if (d.rank == 0 and name == "matrix_major") else None
+        ms, per, _, t0, t1 = time_steps(fn, args.steps, W, stream, d)
+        if sampler:
+            clocks = sampler.stop(t0, t1)
+        res[name] = dict(ms=ms, per_s=n * d.world / (ms * 1e-3))
+    # end to end (matrix-major): pinned host A, B -> device, multiply, C -> pinned host
+    hA, hB = A0.cpu().pin_memory(), B0.cpu().pin_memory(); hC = torch.empty_like(hA).pin_memory()
+
+    def e2e_step(rec):
+        A0.copy_(hA, non_blocking=True); B0.copy_(hB, non_blocking=True)
+        b.kf_mat66_multiply(0, A0, B0, out=C0, stream=stream)
+        hC.copy_(C0, non_blocking=True)
+
+    e2e_ms, _, _, _, _ = time_steps(e2e_step, 3, 1, stream, d)
+    if d.rank != 0:
+        return None
+    pk = peaks()
+    by = 3 * 144.0 * n
+    ach = by / (res["matrix_major"]["ms"] * 1e-3) / 1e9
+    line = dict(metric="mat66_multiplies_per_s", value=res["matrix_major"]["per_s"], unit="multiplies/s", n_gpus=d.world, steps=args.steps, warmup=W,
+                ms_per_step=res["matrix_major"]["ms"], higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload="mplex", matrices_per_gpu=n, l2="3 x %.0f MB per step exceed the 126 MB L2; no explicit flush" % (144.0 * n / 1e6)),
+                clocks=clocks, layouts=res,
+                e2e=dict(value=n * d.world / (e2e_ms * 1e-3), unit="multiplies/s", h2d_bytes_per_step=2 * 144 * n, d2h_bytes_per_step=144 * n, ms_per_step=e2e_ms),
+                gpu_launches=args.steps,
+                roofline=dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=None, kernel="kf_mat66_soa_kernel",
+                              alg_bytes_per_launch=by, alg_flops_per_launch=432.0 * n))
+    if not args.no_cpu_baseline:
+        from oracle import kf_oracle as o
+        m = min(n, 2_000_000)
+        a_ = A1[:m].cpu().numpy().reshape(m, 6, 6); b_ = B1[:m].cpu().numpy().reshape(m, 6, 6)
+        t0 = time.perf_counter(); o.mat66_multiply(a_, b_); dt = time.perf_counter() - t0
+        line["cpu_baseline"] = dict(value=m / dt, unit="multiplies/s", cores=1, kind="oracle", sample=f"first {m} matrices, numpy fp64 matmul")
+    return line
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="fit_c1", choices=list(FIT_CFG) + list(BUILD_CFG))
+    ap.add_argument("--workload", default="fit_c1", choices=list(FIT_CFG) + list(BUILD_CFG) + ["mplex"])
     ap.add_argument("--tracks", type=int, default=None, help="override the track count (debug only; invalidates the metric)")
     ap.add_argument("--events", type=int, default=None, help="override the event count of a build workload (debug only)")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: tracks per step")
@@ -519,7 +584,9 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", d.local))
 
-    if args.workload in FIT_CFG:
+    if args.workload == "mplex":
+        line = bench_mplex(args, d)
+    elif args.workload in FIT_CFG:
         line = bench_fit(args, d, args.workload)
         if not args.no_build and args.tracks is None:
             bl = bench_build(args, d, "build_c3", sample_clocks=False)

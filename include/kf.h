@@ -171,6 +171,13 @@ int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, 
  * Errors: NULL pointers, ld < n_seeds, first_layer outside 0..n_layers, CUDA failure. */
 int kf_select_best(const kf_cands* cands, int32_t first_layer, int32_t* hit_idx, int64_t ld, void* stream);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * kf_mat66_multiply -- the paper's layout micro-benchmark (sec. 4.3, Fig. 5): C_i = A_i B_i for n
+ * general 6x6 fp32 matrices.  layout 0 = matrix-major ("Matriplex"): element (r, c) of matrix i at [(6r + c)*ld + i],
+ * ld >= n; layout 1 = array of matrices: matrix i at [36 i + 6r + c] (ld ignored; arrays 16-byte aligned).
+ * C must not overlap A or B.  Errors: bad layout, n < 0, ld < n, NULL or misaligned arrays, CUDA failure. */
+int kf_mat66_multiply(int32_t layout, int64_t n, int64_t ld, const float* A, const float* B, float* C, void* stream);
+
 const char* kf_last_error(void);
 int kf_version(void);
 

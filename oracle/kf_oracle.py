@@ -217,3 +217,13 @@ def kf_build(layers, bz, binned, seg_off, par, cov21, q, seed_event, seed_hit_id
     m = n * K
     return dict(par=po[:, :m], cov=co[:, :m].T.reshape(m, 6, 6), chi2=c2[:m], nhits=nh[:m], status=st[:m], hit_idx=hi[:, :m], n_cand=nc[:n],
                 counters=dict(zip(COUNTERS, (int(v) for v in cnt))))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# layout micro-benchmark (sec. 4.3, Fig. 5): n independent 6x6 products, the plain definition
+# ---------------------------------------------------------------------------------------------------------
+def mat66_multiply(A, B):
+    """C_i = A_i B_i, A and B [n][6][6] (any float dtype) -> [n][6][6] float64; C_i[r][c] = sum_k A_i[r][k] B_i[k][c]."""
+    A = np.asarray(A, dtype=np.float64); B = np.asarray(B, dtype=np.float64)
+    assert A.shape == B.shape and A.shape[1:] == (6, 6)
+    return np.matmul(A, B)

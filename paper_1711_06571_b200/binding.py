@@ -20,7 +20,7 @@ KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
 EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
-           "kf_build", "kf_build_set_tile", "kf_select_best", "kf_last_error", "kf_version"]
+           "kf_build", "kf_build_set_tile", "kf_select_best", "kf_mat66_multiply", "kf_last_error", "kf_version"]
 
 
 class KfError(RuntimeError):
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_build_set_tile.argtypes = [C.c_int32]
+        l.kf_mat66_multiply.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_select_best.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p]
         l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = l
@@ -301,4 +302,15 @@ def kf_select_best(cands: Cands, first_layer: int, ld: int, out: torch.Tensor | 
     assert tuple(out.shape) == (cands.n_layers, ld)
     rc = lib().kf_select_best(C.byref(cands.c), first_layer, _ptr(out, torch.int32), ld, _stream(stream))
     _check(rc, "kf_select_best")
+    return out
+
+
+def kf_mat66_multiply(layout: int, A: torch.Tensor, B: torch.Tensor, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """include/kf.h kf_mat66_multiply.  layout 0: A, B [36, ld] (matrix-major); layout 1: A, B [n, 36] (array of matrices)."""
+    _require_cuda()
+    if out is None:
+        out = torch.empty_like(A)
+    n, ld = (A.shape[1], A.shape[1]) if layout == 0 else (A.shape[0], 0)
+    rc = lib().kf_mat66_multiply(layout, n, ld, _ptr(A, torch.float32), _ptr(B, torch.float32), _ptr(out, torch.float32), _stream(stream))
+    _check(rc, "kf_mat66_multiply")
     return out

@@ -498,3 +498,17 @@ def test_fit_skips_and_stops():
     assert np.array_equal(r3["par"][:, low], r9["par"][:, low]) and np.array_equal(r3["cov"][low], r9["cov"][low])
     assert ((r3["status"][high] & o.UNREACHABLE) == 0).all()
     assert np.array_equal(base["nhits"], np.full(64, 10))
+
+
+def test_mat66_multiply_definition():
+    """Layout micro-benchmark oracle: element-wise triple loop, identity, and (AB)^T = B^T A^T."""
+    rng = np.random.default_rng(66)
+    A = rng.normal(size=(5, 6, 6)); B = rng.normal(size=(5, 6, 6))
+    C = o.mat66_multiply(A, B)
+    for i in range(5):
+        for r in range(6):
+            for c in range(6):
+                assert abs(C[i, r, c] - sum(A[i, r, k] * B[i, k, c] for k in range(6))) < 1e-13
+    I = np.broadcast_to(np.eye(6), (5, 6, 6))
+    assert np.array_equal(o.mat66_multiply(A, I), A) and np.array_equal(o.mat66_multiply(I, B), B)
+    assert np.allclose(o.mat66_multiply(A, B).transpose(0, 2, 1), o.mat66_multiply(B.transpose(0, 2, 1), A.transpose(0, 2, 1)), atol=1e-13)
