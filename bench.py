@@ -541,7 +541,7 @@ def bench_mplex(args, d: Dist):
                 clocks=clocks, layouts=res,
                 e2e=dict(value=n * d.world / (e2e_ms * 1e-3), unit="multiplies/s", h2d_bytes_per_step=2 * 144 * n, d2h_bytes_per_step=144 * n, ms_per_step=e2e_ms),
                 gpu_launches=args.steps,
-                roofline=dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=None, kernel="kf_mat66_soa_kernel",
+                roofline=dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=stored_traffic("mplex") if n == 4_000_000 else None, kernel="kf_mat66_soa_kernel",
                               alg_bytes_per_launch=by, alg_flops_per_launch=432.0 * n))
     if not args.no_cpu_baseline:
         from oracle import kf_oracle as o

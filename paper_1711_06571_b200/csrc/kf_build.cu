@@ -4,20 +4,22 @@
 // hits represent the most likely continuation ... branching to explore multiple candidate tracks per seed"
 // (sec. 2); "a fixed number of slots for each track seed" (sec. 4.3).
 //
-// One kernel for all layers.  A block of 256 threads owns a tile of S seeds and walks the layers with block-level
-// phases; inside every phase one THREAD owns one live candidate (or one seed), so the long dependent chains of the
-// Kalman arithmetic run at full lane occupancy however few candidates a seed has:
-//   phase 1  thread per live candidate: predict (F2-F5), window -> bin ranges (B2), LDL^T factor of S, then the
-//            window scan (B3): strict window test + chi2 per hit, the passing hits kept as the candidate's own
-//            best-K list (sorted insert, shared memory)
-//   phase 2  thread per seed: K-way merge of the lists of its <= K parents -> the best K children (B4, total order
-//            R10); block scan of the child counts -> dense child positions
-//   phase 3  thread per surviving child: Kalman update (B5), per-layer link (parent slot, hit)
-// Candidate records (33 words: 6 parameters, 21 packed covariance elements, carried sin/cos, chi2, meta) live in
-// a block-private global workspace that stays L2-resident: record c of the current layer at a DENSE index (seed
-// offset + slot), struct-of-arrays over the index, so every record load and store is coalesced.  Two buffers: A
-// (updated states) and B (predicted states).  When the tile has more live candidates than the list area holds, the
-// seeds are taken in rounds.  At the end the links are traced back into hit lists and stored SoA (B6).
+// One kernel for all layers.  A block of 64-256 threads owns a tile of S seeds (32 or 128) and walks the layers with
+// block-level phases; inside every phase one THREAD owns one live candidate, one seed or one child, so the long
+// dependent chains of the Kalman arithmetic run at full lane occupancy however few candidates a seed has:
+//   phase 1  thread per live candidate (build_candidate): predict (F2-F5), window -> bin ranges (B2), LDL^T factor
+//            of S, then the window scan (B3): strict window test + chi2 per 16-byte hit record, the passing hits
+//            appended to the candidate's own list (shared memory; best K kept, sorted once the scan is over)
+//   phase 2  thread per seed: K-way merge of the lists of its <= K parents over 48-bit keys whose integer order is
+//            the total order R10 -> the best K children (B4); block scan of the child counts -> dense child positions
+//   phase 3  thread per surviving child (build_child): Kalman update (B5), per-layer link (parent slot, hit)
+// Candidate records (33 words: 6 parameters, 21 packed covariance elements, carried sin/cos, chi2, meta; stored as 9
+// groups of four) live in a block-private global workspace that stays L2-resident: record c of the current layer
+// at a DENSE index (seed offset + slot), group-of-four-major over the index, so every record moves with 9 coalesced
+// 16-byte accesses.  Two buffers: A (updated states) and B (predicted states).  When the tile has more live candidates
+// than the list area holds, the seeds are taken in rounds.  At the end the links are traced back into hit lists and
+// stored SoA, one thread per live candidate (B6).  The three per-thread bodies are separate (not inlined) functions:
+// inlined they need 228 registers and spill 480 bytes at the 128 the launch bounds allow.
 #include <algorithm>
 #include "kf_common.cuh"
 #include "kf_state.cuh"
@@ -28,7 +30,7 @@ namespace kf {
 #ifndef KF_BUILD_TPS
 #define KF_BUILD_TPS 2     // threads per seed of the tile
 #endif
-constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (twice the seeds of the tile)
+constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (KF_BUILD_TPS x the seeds of the tile)
 constexpr int BUILD_THREADS_PER_SM = 512; // 128 registers per thread
 constexpr int NREC = 33;                  // words per candidate record
 #ifndef KF_SCAN_BATCH
