@@ -98,6 +98,11 @@ typedef struct {
  * Output phi is wrapped to (-pi, pi].  Errors: NULL pointers, n < 0, ld < n, bad geometry, CUDA launch failure. */
 int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
            const kf_tracks* seeds, kf_tracks* out, void* stream);
+/* With identity indexing, event 0, sig_r == sig_rphi on every layer and even strides / 8-byte aligned arrays kf_fit runs
+ * two tracks per thread (all arithmetic as packed fp32 pairs); tracks that leave the fast path (failed crossing, large
+ * turning angle or angle correction, numeric trouble) are redone by the one-track code.  kf_fit_set_pairs(0) forces the
+ * one-track kernel, kf_fit_set_pairs(1) restores the default (test / tuning hook; results agree to rounding). */
+int kf_fit_set_pairs(int32_t enable);
 
 /* ---------------------------------------------------------------------------------------------------------
  * Binned hit index (DESIGN.md sec. 2 B0, readings X1-X2).  Filled by kf_bin_hits into

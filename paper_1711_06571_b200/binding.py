@@ -19,7 +19,7 @@ _lib = None
 KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
-EXPORTS = ["kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
+EXPORTS = ["kf_fit", "kf_fit_set_pairs", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
            "kf_build", "kf_build_set_tile", "kf_select_best", "kf_mat66_multiply", "kf_last_error", "kf_version"]
 
 
@@ -178,6 +178,10 @@ class Hits:
 
 def kf_version() -> int:
     return int(lib().kf_version())
+
+
+def kf_fit_set_pairs(enable: int):
+    _check(lib().kf_fit_set_pairs(C.c_int32(enable)), "kf_fit_set_pairs")
 
 
 def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Tracks | None = None, stream=None) -> Tracks:

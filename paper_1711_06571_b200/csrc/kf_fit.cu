@@ -6,6 +6,7 @@
 // parameter, i.e. through the constant bank: warp-uniform, no global loads.
 #include "kf_common.cuh"
 #include "kf_state.cuh"
+#include "kf_pair.cuh"
 
 namespace kf {
 
@@ -129,6 +130,79 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __
     a.status_o[t] = st;
 }
 
+// ---- two tracks per thread (kf_pair.cuh): identity indexing, event 0, isotropic hit covariance ----
+// one track by the one-track code, as a function: the odd tail and the pairs that left the fast path
+__device__ __noinline__ void fit_one(const FitArgs& a, int64_t t) {
+    const float cw = -(float)a.q[t] * a.kb;
+    State s;
+    float chi2;
+    int nh;
+    uint32_t st = 0u;
+    const int bad = fit_layers<false, false, true, false>(a, t, cw, 0, a.n_layers, s, chi2, nh, st);
+    if (bad >= 0 || !state_finite(s)) fit_redo<false, false, true>(a, t, cw, 0, s, chi2, nh, st);
+    state_store(s, [&](int i, float v) { a.par_o[i * a.ld_out + t] = v; }, [&](int k, float v) { a.cov_o[k * a.ld_out + t] = v; });
+    a.chi2_o[t] = chi2;
+    a.nhits_o[t] = nh;
+    a.status_o[t] = st;
+}
+
+#ifndef KF_PAIR_MINB
+#define KF_PAIR_MINB 3
+#endif
+__global__ void __launch_bounds__(FIT_BLOCK, KF_PAIR_MINB) kf_fit_pair_kernel(const __grid_constant__ FitArgs a) {
+    using namespace pair;
+    const int64_t t = 2 * ((int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x);
+    if (t >= a.n) return;
+    if (t + 1 >= a.n) { fit_one(a, t); return; }
+    auto ld2 = [](const float* p_) { V r; r.v = *reinterpret_cast<const float2*>(p_); return r; };
+    const V cw = mk(-(float)a.q[t] * a.kb, -(float)a.q[t + 1] * a.kb);
+    State2 S;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) S.p[i] = ld2(a.par + i * a.ld_in + t);
+#pragma unroll
+    for (int i = 0; i < 21; ++i) S.C[i] = ld2(a.cov + i * a.ld_in + t);
+    {
+        float s0, c0, s1, c1;
+        sincosf(S.p[4].v.x, &s0, &c0); sincosf(S.p[4].v.y, &s1, &c1);
+        S.g.sp = mk(s0, s1); S.g.cp = mk(c0, c1);
+        sincosf(S.p[5].v.x, &s0, &c0); sincosf(S.p[5].v.y, &s1, &c1);
+        S.g.st = mk(s0, s1); S.g.ct = mk(c0, c1);
+    }
+    V chi2 = pair::sp(0.0f);
+    bool good = true;
+    const int L = a.n_layers;
+    V nx = ld2(a.hxl[0] + t), ny = ld2(a.hyl[0] + t), nz = ld2(a.hzl[0] + t);     // F6: one layer ahead
+#pragma unroll 1
+    for (int l = 0; l < L; ++l) {
+        const V mx = nx, my = ny, mz = nz;
+        if (l + 1 < L) { nx = ld2(a.hxl[l + 1] + t); ny = ld2(a.hyl[l + 1] + t); nz = ld2(a.hzl[l + 1] + t); }
+        const LayerC ly = a.layer[l];
+        good = predict(S, cw, ly);                                   // F2-F5
+        if (!good) break;
+        V c2;
+        good = update(S, mx, my, mz, ly.var_r, ly.var_z, c2);        // F7-F8
+        if (!good) break;
+        chi2 = chi2 + c2;
+    }
+    if (!good || !all_finite(S)) {      // not the fast path for one of the two: both by the one-track code
+        fit_one(a, t);
+        fit_one(a, t + 1);
+        return;
+    }
+    // F9
+    auto st2 = [](float* p_, V v) { *reinterpret_cast<float2*>(p_) = v.v; };
+    S.p[4] = mk(wrap_phi(S.p[4].v.x), wrap_phi(S.p[4].v.y));
+#pragma unroll
+    for (int i = 0; i < 6; ++i) st2(a.par_o + i * a.ld_out + t, S.p[i]);
+#pragma unroll
+    for (int i = 0; i < 21; ++i) st2(a.cov_o + i * a.ld_out + t, S.C[i]);
+    st2(a.chi2_o + t, chi2);
+    *reinterpret_cast<int2*>(a.nhits_o + t) = make_int2(L, L);
+    *reinterpret_cast<uint2*>(a.status_o + t) = make_uint2(0u, 0u);
+}
+
+static int g_fit_pairs = 1;   // 1 = two tracks per thread where the arguments allow it, 0 = never (test hook)
+
 template <bool IDX, bool EVT>
 static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t st) {
     if (iso) kf_fit_kernel<IDX, EVT, true><<<blocks, FIT_BLOCK, 0, st>>>(a);
@@ -136,6 +210,13 @@ static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t
 }
 
 }  // namespace kf
+
+// test / tuning hook: 1 = two tracks per thread where the arguments allow it (default), 0 = always one track per thread
+extern "C" int kf_fit_set_pairs(int32_t enable) {
+    if (enable != 0 && enable != 1) return kf::fail(KF_ERR_INVALID_ARG, "kf_fit_set_pairs: %d not 0 or 1", enable);
+    kf::g_fit_pairs = enable;
+    return KF_OK;
+}
 
 extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
                       const kf_tracks* seeds, kf_tracks* out, void* stream) {
@@ -174,6 +255,19 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     }
     const unsigned blocks = (unsigned)((a.n + FIT_BLOCK - 1) / FIT_BLOCK);
     cudaStream_t cs = (cudaStream_t)stream;
+    if (g_fit_pairs && !hit_idx && !trk_event && iso) {
+        // two tracks per thread: 8-byte loads and stores of track pairs, so every array and stride must be even
+        bool even = (a.ld_in % 2 == 0) && (a.ld_out % 2 == 0);
+        const void* ptrs[] = {a.par, a.cov, a.par_o, a.cov_o, a.chi2_o, a.nhits_o, a.status_o};
+        for (const void* q_ : ptrs) even = even && ((uintptr_t)q_ % 8 == 0);
+        for (int l = 0; l < geom->n_layers; ++l)
+            even = even && ((uintptr_t)a.hxl[l] % 8 == 0) && ((uintptr_t)a.hyl[l] % 8 == 0) && ((uintptr_t)a.hzl[l] % 8 == 0);
+        if (even) {
+            const int64_t n_thr = (a.n + 1) / 2;
+            kf_fit_pair_kernel<<<(unsigned)((n_thr + FIT_BLOCK - 1) / FIT_BLOCK), FIT_BLOCK, 0, cs>>>(a);
+            return check_launch("kf_fit");
+        }
+    }
     if (hit_idx) { if (trk_event) launch_fit<true, true>(a, iso, blocks, cs); else launch_fit<true, false>(a, iso, blocks, cs); }
     else { if (trk_event) launch_fit<false, true>(a, iso, blocks, cs); else launch_fit<false, false>(a, iso, blocks, cs); }
     return check_launch("kf_fit");

@@ -70,11 +70,52 @@ def test_fit_config2_small():
 
 
 def test_fit_explicit_index_equals_identity():
+    """One-track kernel: identity indexing and the same indices given explicitly are the same arithmetic, bit for bit."""
+    from paper_1711_06571_b200 import binding as b
     fi = synth.fit_inputs(0, n=4096)
     fj = synth.fit_inputs(0, n=4096, force_index=True)
-    a, b_ = run_gpu(fi), run_gpu(fj)
+    b.kf_fit_set_pairs(0)
+    try:
+        a, b_ = run_gpu(fi), run_gpu(fj)
+    finally:
+        b.kf_fit_set_pairs(1)
     for k in ("par", "cov", "chi2", "nhits", "status"):
         assert np.array_equal(a[k], b_[k]), k
+
+
+@pytest.mark.parametrize("config,n", [(0, 10_001), (2, 20_000)])
+def test_fit_pairs_and_single_agree(config, n):
+    """Two tracks per thread (default for identity indexing) against the one-track kernel on the same input: same
+    decisions, values within a tenth of the parity tolerances of each other; both against the oracle.  Config 2 without
+    its index list (identity): low-pT tracks leave the fast path and are redone by the one-track code inside the kernel."""
+    from paper_1711_06571_b200 import binding as b
+    fi = synth.fit_inputs(config, n=n)
+    if config == 2:          # identity indexing needs a hit on every layer: keep the tracks that have them all
+        full = np.nonzero(fi.valid.all(axis=0))[0]
+        keep = full[: len(full) // 2 * 2 + 1]
+        L = fi.geom.n_layers
+        m = len(keep)
+        ld = m + 1                                     # m is odd: an even stride, and an odd tail for the pair kernel
+        pad = lambda a_: np.ascontiguousarray(np.concatenate([a_[:, keep], a_[:, keep[:1]]], axis=1))
+        hits = [pad(h.reshape(L, fi.ld)).reshape(-1) for h in (fi.hit_x, fi.hit_y, fi.hit_z)]
+        fi.par = pad(fi.par); fi.cov = pad(fi.cov); fi.q = fi.q[keep]
+        fi.hit_x, fi.hit_y, fi.hit_z = hits
+        fi.hit_idx = None; fi.n = m; fi.ld = ld; fi.seg_off = np.arange(L + 1, dtype=np.int64) * ld
+    r = run_ref(fi)
+    g2 = run_gpu(fi)
+    b.kf_fit_set_pairs(0)
+    try:
+        g1 = run_gpu(fi)
+    finally:
+        b.kf_fit_set_pairs(1)
+    check(g2, r, min_frac_strict=0.99)
+    check(g1, r, min_frac_strict=0.99)
+    assert np.array_equal(g1["nhits"], g2["nhits"]) and np.array_equal(g1["status"], g2["status"])
+    sel = g1["nhits"] > 0
+    assert np.allclose(g1["chi2"][sel], g2["chi2"][sel], rtol=5e-4, atol=5e-4)      # each within 1e-3 of the oracle
+    d = g1["par"][:, sel].astype(np.float64) - g2["par"][:, sel]
+    d[4] = np.angle(np.exp(1j * d[4]))
+    assert (np.abs(d) <= np.maximum(5e-5 * np.abs(g1["par"][:, sel]), 1e-5)).all()
 
 
 def test_fit_stops_and_flags():
@@ -132,7 +173,11 @@ def test_fit_multi_event_segments():
     out = b.kf_fit(geom, hits, torch.from_numpy(hit_idx).cuda(), torch.from_numpy(ev).cuda(), b.Tracks.from_host(par, cov, q))
     torch.cuda.synchronize()
     got = out.to_host()
-    a, c = run_gpu(f0), run_gpu(f1)
+    b.kf_fit_set_pairs(0)            # the one-track kernel on both sides: the same arithmetic, bit for bit
+    try:
+        a, c = run_gpu(f0), run_gpu(f1)
+    finally:
+        b.kf_fit_set_pairs(1)
     assert np.array_equal(got["par"][:, :f0.n], a["par"]) and np.array_equal(got["par"][:, f0.n:], c["par"])
     assert np.array_equal(got["chi2"][:f0.n], a["chi2"]) and np.array_equal(got["chi2"][f0.n:], c["chi2"])
 
