@@ -344,7 +344,7 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
     t_hbm = units["bytes"] / (pk["hbm_gbs"] * 1e9)
     ach = units["flops"] / (kern_ms * 1e-3) / 1e12
     roofline = dict(bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None,
-                    kernel="kf_fit_kernel", kernel_ms=kern_ms, kernel_ms_min=min(per), kernel_share_of_step=1.0,
+                    kernel="kf_fit_pair_kernel" if fi.hit_idx is None else "kf_fit_kernel", kernel_ms=kern_ms, kernel_ms_min=min(per), kernel_share_of_step=1.0,
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (clocks.max.sm, {pk['source']})",
                     alg_flops_per_launch=units["flops"], alg_bytes_per_launch=units["bytes"],
                     alg_flop_per_track_layer=FIT_FLOP_PER_TRACK_LAYER,
