@@ -98,34 +98,41 @@ __device__ __forceinline__ bool predict(State2& S, V cw, const LayerC& ly) {
     const V sx = -(xn * iup), sy = -(yn * iup);
     const V si = -(fma(xn, Fxi, yn * Fyi) * iup);
     const V sph = -(fma(xn, Fxp, yn * Fyp) * iup);
-    const V a0 = fma(cpn, sx, 1.0f), a1 = cpn * sy, a3 = fma(cpn, si, Fxi), a4 = fma(cpn, sph, Fxp);
-    const V b0 = spn * sx, b1 = fma(spn, sy, 1.0f), b3 = fma(spn, si, Fyi), b4 = fma(spn, sph, Fyp);
-    const V c0 = cot * sx, c1 = cot * sy, c3 = cot * si, c4 = cot * sph, c5 = -(s * ist * ist);
-    const V d0 = w * sx, d1 = w * sy, d3 = fma(w, si, cw * s), d4 = fma(w, sph, 1.0f);
+    // J = I + E + g s^T with s^T = ds/dp = (sx, sy, 0, si, sph, 0), g = dp'/ds = (cos phi', sin phi', cot, 0, w, 0)^T and the
+    // fixed-path-length part E: E_03 = Fxi, E_04 = Fxp, E_13 = Fyi, E_14 = Fyp, E_25 = c5, E_43 = cw s.  Used in this form
+    // (corrections added to C) the transport costs 30 instructions less than with the 17 Jacobian entries multiplied out.
+    const V c5 = -(s * ist * ist), e43 = cw * s;
 #define CC(i, j) C[pk(i, j)]
-#define ROW4(c0_, c1_, c3_, c4_, j) fma(c0_, CC(0, j), fma(c1_, CC(1, j), fma(c3_, CC(3, j), c4_ * CC(4, j))))
-    const V T00 = ROW4(a0, a1, a3, a4, 0), T01 = ROW4(a0, a1, a3, a4, 1), T03 = ROW4(a0, a1, a3, a4, 3),
-            T04 = ROW4(a0, a1, a3, a4, 4), T05 = ROW4(a0, a1, a3, a4, 5);
-    const V T10 = ROW4(b0, b1, b3, b4, 0), T11 = ROW4(b0, b1, b3, b4, 1), T13 = ROW4(b0, b1, b3, b4, 3),
-            T14 = ROW4(b0, b1, b3, b4, 4), T15 = ROW4(b0, b1, b3, b4, 5);
-    const V T40 = ROW4(d0, d1, d3, d4, 0), T41 = ROW4(d0, d1, d3, d4, 1), T43 = ROW4(d0, d1, d3, d4, 3),
-            T44 = ROW4(d0, d1, d3, d4, 4), T45 = ROW4(d0, d1, d3, d4, 5);
-#define ROW6(j) (fma(c0, CC(0, j), fma(c1, CC(1, j), fma(c3, CC(3, j), fma(c4, CC(4, j), fma(c5, CC(5, j), CC(2, j)))))))
-    const V T20 = ROW6(0), T21 = ROW6(1), T22 = ROW6(2), T23 = ROW6(3), T24 = ROW6(4), T25 = ROW6(5);
-#undef ROW4
-#undef ROW6
-#define DOT4(T0, T1, T3, T4, e0, e1, e3, e4) fma(T0, e0, fma(T1, e1, fma(T3, e3, T4 * e4)))
-    const V n00 = DOT4(T00, T01, T03, T04, a0, a1, a3, a4);
-    const V n10 = DOT4(T10, T11, T13, T14, a0, a1, a3, a4);
-    const V n11 = DOT4(T10, T11, T13, T14, b0, b1, b3, b4);
-    const V n20 = DOT4(T20, T21, T23, T24, a0, a1, a3, a4);
-    const V n21 = DOT4(T20, T21, T23, T24, b0, b1, b3, b4);
-    const V n22 = fma(T20, c0, fma(T21, c1, fma(T23, c3, fma(T24, c4, fma(T25, c5, T22)))));
-    const V n40 = DOT4(T40, T41, T43, T44, a0, a1, a3, a4);
-    const V n41 = DOT4(T40, T41, T43, T44, b0, b1, b3, b4);
-    const V n42 = DOT4(T20, T21, T23, T24, d0, d1, d3, d4);
-    const V n44 = DOT4(T40, T41, T43, T44, d0, d1, d3, d4);
-#undef DOT4
+    // ---- T = J C = C + g (s^T C) + E C ----
+#define RJ(j) fma(sx, CC(0, j), fma(sy, CC(1, j), fma(si, CC(3, j), sph * CC(4, j))))
+    const V r0 = RJ(0), r1 = RJ(1), r2 = RJ(2), r3 = RJ(3), r4 = RJ(4), r5 = RJ(5);
+#undef RJ
+#define T0(j, r) fma(cpn, r, fma(Fxi, CC(3, j), fma(Fxp, CC(4, j), CC(0, j))))
+#define T1(j, r) fma(spn, r, fma(Fyi, CC(3, j), fma(Fyp, CC(4, j), CC(1, j))))
+#define T2(j, r) fma(cot, r, fma(c5, CC(5, j), CC(2, j)))
+#define T4(j, r) fma(w, r, fma(e43, CC(3, j), CC(4, j)))
+    const V T00 = T0(0, r0), T01 = T0(1, r1), T03 = T0(3, r3), T04 = T0(4, r4), T05 = T0(5, r5);
+    const V T10 = T1(0, r0), T11 = T1(1, r1), T13 = T1(3, r3), T14 = T1(4, r4), T15 = T1(5, r5);
+    const V T20 = T2(0, r0), T21 = T2(1, r1), T22 = T2(2, r2), T23 = T2(3, r3), T24 = T2(4, r4), T25 = T2(5, r5);
+    const V T40 = T4(0, r0), T41 = T4(1, r1), T43 = T4(3, r3), T44 = T4(4, r4), T45 = T4(5, r5);
+#undef T0
+#undef T1
+#undef T2
+#undef T4
+    // ---- C' = T J^T = T + (T s) g^T + T E^T, lower triangle; (4,2) through its mirror (2,4) ----
+#define QI(Ta, Tb, Tc, Td) fma(sx, Ta, fma(sy, Tb, fma(si, Tc, sph * Td)))
+    const V q0 = QI(T00, T01, T03, T04), q1 = QI(T10, T11, T13, T14), q2 = QI(T20, T21, T23, T24), q4 = QI(T40, T41, T43, T44);
+#undef QI
+    const V n00 = fma(q0, cpn, fma(Fxi, T03, fma(Fxp, T04, T00)));
+    const V n10 = fma(q1, cpn, fma(Fxi, T13, fma(Fxp, T14, T10)));
+    const V n11 = fma(q1, spn, fma(Fyi, T13, fma(Fyp, T14, T11)));
+    const V n20 = fma(q2, cpn, fma(Fxi, T23, fma(Fxp, T24, T20)));
+    const V n21 = fma(q2, spn, fma(Fyi, T23, fma(Fyp, T24, T21)));
+    const V n22 = fma(q2, cot, fma(c5, T25, T22));
+    const V n40 = fma(q4, cpn, fma(Fxi, T43, fma(Fxp, T44, T40)));
+    const V n41 = fma(q4, spn, fma(Fyi, T43, fma(Fyp, T44, T41)));
+    const V n42 = fma(q2, w, fma(e43, T23, T24));
+    const V n44 = fma(q4, w, fma(e43, T43, T44));
     // ---- multiple scattering (R4) ----
     V q33 = sp(0.0f), q53 = sp(0.0f), q44 = sp(0.0f), q55 = sp(0.0f);
     if (ly.xx0r > 0.0f) {
