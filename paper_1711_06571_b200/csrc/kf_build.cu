@@ -292,15 +292,26 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                             hpos[u] = t < na ? h0a + t : h0b + (t - na);
                                             hv[u] = __ldg(a.xyzp + hpos[u]);
                                         }
+                                        // window test of the batch (cheap, branch-free) -> bit mask; chi2 and the list only for the
+                                        // few hits inside the window, one at a time
+                                        unsigned inside = 0u;
 #pragma unroll
                                         for (int u = 0; u < SCAN_BATCH; ++u) {
-                                            const int h = hpos[u];
                                             const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
                                             const float cr = fmaf(px, my, -py * mx);
                                             const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
                                                                 (fabsf(mz - pz) <= dzw);
-                                            // branch-free up to the verdict: a divergent path per slot would be run by the
-                                            // whole warp whenever a single lane takes it
+                                            inside |= in_win ? (1u << u) : 0u;
+                                        }
+                                        while (inside) {
+                                            const int u = __ffs(inside) - 1;
+                                            inside &= inside - 1u;
+                                            float4 m4 = hv[0];
+                                            int h = hpos[0];
+#pragma unroll
+                                            for (int v = 1; v < SCAN_BATCH; ++v)
+                                                if (u == v) { m4 = hv[v]; h = hpos[v]; }
+                                            const float mx = m4.x, my = m4.y, mz = m4.z;
                                             bool ok = fok;
                                             if (!ISO) {
                                                 const HitCov V = hit_cov(mx, my, ly);
@@ -309,13 +320,13 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, 
                                                 Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
                                                 ok = ldl3(Sm, F);
                                             }
-                                            sbad = sbad || (in_win && !ok);
+                                            if (!ok) { sbad = true; continue; }
                                             const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
                                             const float y1 = fmaf(-F.l10, q0, q1);
                                             const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
                                             const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                            if (in_win && ok && c2 < a.chi2_cut) {
-                                                if (cnt < K) {           // unsorted append (two predicated stores)
+                                            if (c2 < a.chi2_cut) {
+                                                if (cnt < K) {           // unsorted append
                                                     lc[cnt * ncap] = chi2 + c2; lh[cnt * ncap] = h; ++cnt;
                                                 } else {
                                                     list_replace_worst(lc, lh, ncap, K, chi2 + c2, h);
