@@ -112,7 +112,7 @@ __device__ __noinline__ void fit_redo(const FitArgs& a, int64_t t, float cw, int
 }
 
 template <bool IDX, bool EVT, bool ISO>
-__global__ void __launch_bounds__(FIT_BLOCK, KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {
+__global__ void __launch_bounds__(FIT_BLOCK, IDX ? KF_FIT_MINB + 1 : KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {   // gathered hits: one more block
     const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
     if (t >= a.n) return;
     const float cw = -(float)a.q[t] * a.kb;
