@@ -107,9 +107,11 @@ static double g_of(const double p[6], double w, double s, double R, double* dg) 
 /* Propagate the state to the cylinder of radius R: smallest positive root of g(s) = x'^2 + y'^2 - R^2 [R2].
  * J (row-major 6x6) = d p'/d p INCLUDING the path-length term (the state is transported to the surface).
  * Returns 0 or a flag: KFO_UNREACHABLE (start not inside R, or no crossing within half a turn), KFO_GRAZING
- * (cos(incidence) < KFO_CMIN; outputs are still filled).  s_out = transverse path, cosinc_out = u'/R. */
-int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
-                  double* cosinc_out) {
+ * (cos(incidence) < KFO_CMIN; outputs are still filled).  s_out = transverse path, cosinc_out = u'/R.
+ * tangency_out (diagnostics for DESIGN.md R16, may be NULL): how far the helix is from just touching the cylinder --
+ * cos^2(incidence) when it crosses, max(R^2 - r^2)/R^2 over the half turn when it does not, 1e300 when neither applies. */
+static int propagate_ex(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
+                        double* cosinc_out, double* tangency_out) {
     const double w = -(double)q * KFO_KCURV * bz * p[3];
     const double c_w = -(double)q * KFO_KCURV * bz; /* w = c_w * iota */
     double r02 = p[0] * p[0] + p[1] * p[1];
@@ -117,6 +119,7 @@ int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6],
     for (int i = 0; i < 36; ++i) J[i] = (i % 7 == 0) ? 1.0 : 0.0;
     if (s_out) *s_out = 0.0;
     if (cosinc_out) *cosinc_out = 0.0;
+    if (tangency_out) *tangency_out = 1e300;
     if (!(r02 < R * R) || !isfinite(w) || !isfinite(r02)) return KFO_UNREACHABLE;
 
     /* march: a circle of radius rho >= R that starts inside the cylinder leaves it within an arc pi R
@@ -125,12 +128,35 @@ int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6],
     const int NMARCH = 64;
     double smax = (fabs(w) * R <= 1.0) ? KFO_PI * R * (1.0 + 1e-9) : KFO_PI / fabs(w);
     double lo = 0.0, hi = -1.0;
+    int kbest = 0;
+    double gbest = r02 - R * R;
     for (int k = 1; k <= NMARCH; ++k) {
         double sk = smax * (double)k / NMARCH;
-        if (g_of(p, w, sk, R, NULL) >= 0.0) { hi = sk; break; }
+        double gk = g_of(p, w, sk, R, NULL);
+        if (gk >= 0.0) { hi = sk; break; }
+        if (gk > gbest) { gbest = gk; kbest = k; }
         lo = sk;
     }
-    if (hi < 0.0) return KFO_UNREACHABLE;
+    if (hi < 0.0) {
+        /* No sample lies outside, but a helix that only just pokes through the cylinder crosses it twice between two
+           samples.  Along the helix r^2 = a + b cos(w s + delta): at most one maximum within half a turn, bracketed by the
+           neighbours of the largest sample.  Golden-section search for it; if it is >= 0 the first crossing lies between
+           the bracket's start (inside) and the maximum. */
+        double a = smax * (double)(kbest > 0 ? kbest - 1 : 0) / NMARCH, b = smax * (double)(kbest < NMARCH ? kbest + 1 : NMARCH) / NMARCH;
+        const double a0 = a, gr = 0.6180339887498949;
+        double x1 = b - gr * (b - a), x2 = a + gr * (b - a);
+        double f1 = g_of(p, w, x1, R, NULL), f2 = g_of(p, w, x2, R, NULL);
+        for (int it = 0; it < 200 && b - a > 1e-16 * fmax(1.0, b); ++it) {
+            if (f1 < f2) { a = x1; x1 = x2; f1 = f2; x2 = a + gr * (b - a); f2 = g_of(p, w, x2, R, NULL); }
+            else { b = x2; x2 = x1; f2 = f1; x1 = b - gr * (b - a); f1 = g_of(p, w, x1, R, NULL); }
+        }
+        const double sm = f1 > f2 ? x1 : x2, gm = f1 > f2 ? f1 : f2;
+        if (!(gm >= 0.0)) {
+            if (tangency_out) *tangency_out = -gm / (R * R);
+            return KFO_UNREACHABLE;
+        }
+        lo = a0; hi = sm;
+    }
     /* safeguarded Newton inside [lo, hi], g(lo) < 0 <= g(hi) */
     double s = 0.5 * (lo + hi);
     for (int it = 0; it < 200; ++it) {
@@ -148,6 +174,7 @@ int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6],
     const double up = xn * cpn + yn * spn; /* R cos(incidence) */
     if (s_out) *s_out = s;
     if (cosinc_out) *cosinc_out = up / R;
+    if (tangency_out) *tangency_out = (up / R) * (up / R);
 
     /* fixed-s partial derivatives (sec. 8c-3) */
     const double a = w * s;
@@ -179,6 +206,10 @@ int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6],
     J[5 * 6 + 5] = 1.0;
     if (!(up / R >= KFO_CMIN)) return KFO_GRAZING;
     return 0;
+}
+int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
+                  double* cosinc_out) {
+    return propagate_ex(p, q, bz, R, pout, J, s_out, cosinc_out, NULL);
 }
 
 /* remove the rounding-level asymmetry of the dense loops: C <- (C + C^T)/2 */
@@ -330,15 +361,20 @@ int kfo_update(const double p[6], const double C[36], const double m[3], double 
 
 /* One KF step: propagate to layer l, add Q, (optionally) update with hit m.  Used by fit and build.
  * Returns flags; on flags != 0 the outputs are not to be used. */
-static int predict(const double* layers, int l, double bz, const double p[6], const double C[36], int q,
-                   double pp[6], double Cp[36]) {
+static int predict_ci(const double* layers, int l, double bz, const double p[6], const double C[36], int q,
+                      double pp[6], double Cp[36], double* ci_out, double* tangency_out) {
     double J[36], Q[36], s, ci;
-    int f = kfo_propagate(p, q, bz, LR(layers, l), pp, J, &s, &ci);
+    int f = propagate_ex(p, q, bz, LR(layers, l), pp, J, &s, &ci, tangency_out);
+    if (ci_out) *ci_out = ci;
     if (f) return f;
     similarity6(J, C, Cp);
     kfo_ms_noise(pp, ci, LXX0(layers, l), Q);
     for (int i = 0; i < 36; ++i) Cp[i] += Q[i];
     return 0;
+}
+static int predict(const double* layers, int l, double bz, const double p[6], const double C[36], int q,
+                   double pp[6], double Cp[36]) {
+    return predict_ci(layers, l, bz, p, C, q, pp, Cp, NULL, NULL);
 }
 int kfo_predict(const double* layers, int l, double bz, const double p[6], const double C[36], int q, double pp[6],
                 double Cp[36]) {
@@ -346,7 +382,9 @@ int kfo_predict(const double* layers, int l, double bz, const double p[6], const
 }
 
 /* kf_fit_ref [R8]: forward (inside-out) filter over the layers in order of increasing radius.
- * hit_idx[l*ld + t] < 0 -> layer skipped entirely; NULL -> identity.  Hit of track t on layer l is
+ * hit_idx[l*ld + t] >= 0 -> propagate, add Q, update with that hit;  == -1 -> the layer is crossed without a hit:
+ * propagate and add Q (the material is there whether or not a hit was found), no update;  <= -2 -> layer not
+ * crossed: skipped entirely;  NULL -> identity.  Hit of track t on layer l is
  * (hx,hy,hz)[seg_off[ev*L + l] + idx], ev = trk_event ? trk_event[t] : 0.
  * A propagation failure or a failed update sets the status bit, stops the track and keeps the last good state.
  * par [6][ld], cov [36][ld] dense in, outputs alike; chi2/nhits/status [n].  chi2_in/nhits_in may be NULL (=0). */
@@ -365,9 +403,14 @@ int kfo_fit(int n_layers, const double* layers, double bz, int64_t n, int64_t ld
         int ev = trk_event ? trk_event[t] : 0;
         for (int l = 0; l < n_layers; ++l) {
             int64_t idx = hit_idx ? hit_idx[(int64_t)l * ld + t] : t;
-            if (idx < 0) continue;
+            if (idx < -1) continue;
             int f = predict(layers, l, bz, p, C, q[t], pp, Cp);
             if (f) { st |= (uint32_t)f; break; }
+            if (idx == -1) { /* hole: the predicted state (incl. Q) becomes the state */
+                memcpy(p, pp, sizeof p);
+                memcpy(C, Cp, sizeof C);
+                continue;
+            }
             int64_t h = seg_off[(int64_t)ev * n_layers + l] + idx;
             double m[3] = {hx[h], hy[h], hz[h]}, c2;
             f = kfo_update(pp, Cp, m, LSRPHI(layers, l), LSZ(layers, l), LSR(layers, l), pu, Cu, &c2);
@@ -462,13 +505,18 @@ int kfo_bin_hits(int n_layers, const double* layers, int n_events, const int64_t
 void kfo_window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, int n_phi, int n_z, int* first, int* n_b,
                      int* iz_lo, int* iz_hi) {
     float inv_dphi = (float)((double)n_phi / (2.0 * KFO_PI));
-    float f_lo = (phi_c - dphi) * inv_dphi, f_hi = (phi_c + dphi) * inv_dphi;
-    int b_lo = (int)floorf(f_lo), b_hi = (int)floorf(f_hi);
-    int nb = b_hi - b_lo + 1;
-    if (nb > n_phi) nb = n_phi;
-    if (nb < 0) nb = 0;
-    *n_b = nb;
-    *first = ((b_lo % n_phi) + n_phi) % n_phi;
+    if (!(dphi * inv_dphi < (float)n_phi)) { /* half width of a full turn or more: every bin, starting at bin 0 [X3] */
+        *first = 0;
+        *n_b = n_phi;
+    } else {
+        float f_lo = (phi_c - dphi) * inv_dphi, f_hi = (phi_c + dphi) * inv_dphi;
+        int b_lo = (int)floorf(f_lo), b_hi = (int)floorf(f_hi);
+        int nb = b_hi - b_lo + 1;
+        if (nb > n_phi) nb = n_phi;
+        if (nb < 0) nb = 0;
+        *n_b = nb;
+        *first = ((b_lo % n_phi) + n_phi) % n_phi;
+    }
     *iz_lo = kfo_z_bin(z_c - dz, zmax, n_z);
     *iz_hi = kfo_z_bin(z_c + dz, zmax, n_z);
 }
@@ -526,13 +574,24 @@ static int child_cmp(const void* a_, const void* b_) {
  * Outputs, slot = s*K + k: par_o [6][ld_out], cov_o [36][ld_out], chi2_o, nhits_o, status_o [n_seeds*K],
  * hit_idx_o [n_layers][ld_out], n_cand [n_seeds]; unused slots: nhits 0, chi2 0, status 0, hit_idx -2, par/cov 0.
  * counters[8]: 0 propagations, 1 hits scanned, 2 pass strict window, 3 pass chi2 cut (hit children), 4 updates,
- *              5 bin rows touched, 6 seed-layers, 7 children ranked. */
+ *              5 bin rows touched, 6 seed-layers, 7 children ranked.
+ * margins (NULL or [n_seeds][n_layers][5], test diagnostics for DESIGN.md R16): the smallest RELATIVE distance of any
+ * decision taken for that seed on that layer to its threshold (1e300 = no such decision):
+ *   [0] strict window: | |x'm_y - y'm_x| / (dphi r' r_m) - 1 | and | |m_z - z_c| / dz - 1 | of a hit that passes the other
+ *       window tests and would pass (or passes) the chi2 cut;
+ *   [1] chi2 cut: |chi2_h / chi2_cut - 1| of a hit inside the window;
+ *   [2] rank: |chi2_a - chi2_b| / max(chi2_a, chi2_b) of children adjacent in the ranking with equal nhits, at least
+ *       one of them kept;
+ *   [3] propagation: |cos_inc / c_min - 1| (grazing guard) and | |z'| / (zmax + dz) - 1 | (acceptance);
+ *   [4] tangency (a crossing that only just exists / only just does not, i.e. the choice between the "grazing" and the
+ *       "unreachable" bit): cos^2(incidence), resp. max(R^2 - r^2)/R^2 along the half turn. */
 int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z, const float* sx, const float* sy,
               const float* sz, const int32_t* perm, const int32_t* bin_off, const int64_t* seg_off, int64_t n_seeds,
               int64_t ld_seed, const double* par, const double* cov, const int8_t* q, const double* chi2_in,
               const int32_t* seed_event, const int32_t* seed_hit_idx, int first_layer, int K, double chi2_cut,
               double n_sigma, int use_bins, int64_t ld_out, double* par_o, double* cov_o, double* chi2_o,
-              int32_t* nhits_o, uint32_t* status_o, int32_t* hit_idx_o, int32_t* n_cand, int64_t* counters) {
+              int32_t* nhits_o, uint32_t* status_o, int32_t* hit_idx_o, int32_t* n_cand, int64_t* counters,
+              double* margins) {
     if (K < 1 || K > 32 || n_layers > 32 || first_layer < 0 || first_layer > n_layers) return -1;
     int64_t cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : cnt[:8])
@@ -559,11 +618,16 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
             const int64_t seg = (int64_t)ev * n_layers + l;
             n_ch = 0;
             cnt[6] += 1;
+            double mg[5] = {1e300, 1e300, 1e300, 1e300, 1e300};
+#define KFO_MARGIN(k, v) do { double v_ = (v); if (v_ < mg[k]) mg[k] = v_; } while (0)
             for (int c = 0; c < nc; ++c) {
                 kfo_child pass = {c, 2, INT64_MAX, cur[c].chi2, cur[c].nhits};
                 pflag[c] = 0;
-                int f = cur[c].finished ? -1 : predict(layers, l, bz, cur[c].p, cur[c].C, q[sd], pp[c], Cp[c]);
+                double ci = 0.0, tang = 1e300;
+                int f = cur[c].finished ? -1 : predict_ci(layers, l, bz, cur[c].p, cur[c].C, q[sd], pp[c], Cp[c], &ci, &tang);
                 if (!cur[c].finished) cnt[0] += 1;
+                if (!cur[c].finished && (f == 0 || f == KFO_GRAZING)) KFO_MARGIN(3, fabs(ci / KFO_CMIN - 1.0));
+                if (!cur[c].finished) KFO_MARGIN(4, tang);
                 double dphi = 0, dzw = 0;
                 if (f == 0) { /* window (R11) */
                     const double x = pp[c][0], y = pp[c][1], r2 = x * x + y * y;
@@ -572,7 +636,10 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                     dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R));
                     dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz);
                     if (!isfinite(dphi) || !isfinite(dzw)) f = KFO_NUMERIC;
-                    else if (fabs(pp[c][2]) > zmax + dzw) f = KFO_LEFT_Z;
+                    else {
+                        KFO_MARGIN(3, fabs(fabs(pp[c][2]) / (zmax + dzw) - 1.0));
+                        if (fabs(pp[c][2]) > zmax + dzw) f = KFO_LEFT_Z;
+                    }
                 }
                 if (f != 0) { /* finished (or just found unpropagatable): state unchanged */
                     if (f > 0) pflag[c] = (uint32_t)f;
@@ -597,12 +664,25 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                             cnt[1] += 1;
                             const double m[3] = {sx[h], sy[h], sz[h]};
                             const double rm = sqrt(m[0] * m[0] + m[1] * m[1]);
-                            if (!(fabs(x * m[1] - y * m[0]) <= dphi * rp * rm)) continue;
-                            if (!(x * m[0] + y * m[1] > 0.0)) continue;
-                            if (!(fabs(m[2] - zc) <= dzw)) continue;
+                            const int in_phi = fabs(x * m[1] - y * m[0]) <= dphi * rp * rm;
+                            const int in_dot = x * m[0] + y * m[1] > 0.0;
+                            const int in_z = fabs(m[2] - zc) <= dzw;
+                            if (margins && in_dot && (in_phi || in_z)) { /* distance to the window edges (diagnostics only) */
+                                const double mphi = fabs(fabs(x * m[1] - y * m[0]) / (dphi * rp * rm) - 1.0);
+                                const double mz = fabs(fabs(m[2] - zc) / dzw - 1.0);
+                                const double near = fmin(in_z ? mphi : 1e300, in_phi ? mz : 1e300);
+                                if (near < mg[0]) {
+                                    double c2m;
+                                    if (kfo_chi2(pp[c], Cp[c], m, srphi, szz, sr, &c2m) || c2m < chi2_cut) mg[0] = near;
+                                }
+                            }
+                            if (!in_phi) continue;
+                            if (!in_dot) continue;
+                            if (!in_z) continue;
                             cnt[2] += 1;
                             double c2;
                             if (kfo_chi2(pp[c], Cp[c], m, srphi, szz, sr, &c2)) { s_bad = 1; break; }
+                            KFO_MARGIN(1, fabs(c2 / chi2_cut - 1.0));
                             if (!(c2 < chi2_cut)) continue;
                             cnt[3] += 1;
                             kfo_child k = {c, 0, h, cur[c].chi2 + c2, cur[c].nhits + 1};
@@ -626,6 +706,14 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
             cnt[7] += (int64_t)n_ch;
             qsort(ch, n_ch, sizeof(kfo_child), child_cmp);
             int nn = n_ch < (size_t)K ? (int)n_ch : K;
+            for (int j = 0; j + 1 < (int)n_ch && j < nn; ++j)
+                if (ch[j].nhits == ch[j + 1].nhits) {
+                    const double big = fmax(fabs(ch[j].chi2), fabs(ch[j + 1].chi2));
+                    KFO_MARGIN(2, big > 0.0 ? fabs(ch[j].chi2 - ch[j + 1].chi2) / big : 0.0);
+                }
+            if (margins)
+                for (int k = 0; k < 5; ++k) margins[((int64_t)sd * n_layers + l) * 5 + k] = mg[k];
+#undef KFO_MARGIN
             for (int j = 0; j < nn; ++j) {
                 const kfo_child* k = &ch[j];
                 const kfo_cand* pa = &cur[k->parent];

@@ -122,8 +122,9 @@ def cross_cylinder(x, y, z, ipt, phi, theta, q, bz, R):
     signed curvature w = -q K Bz / pT about the centre c = (x - sin(phi)/w, y + cos(phi)/w); the cylinder
     is the circle |p| = R about the origin.  The two intersections sit at polar angle gamma +- beta, with
     gamma the azimuth of c and cos(beta) = (d^2 + R^2 - rho^2) / (2 d R) (law of cosines, d = |c|).
-    The one reached first is the one with the smaller turning angle about c in the sense of rotation.
-    A straight line (w = 0) uses the chord formula instead.
+    The one reached first is the one with the smaller turning angle about c in the sense of rotation; a crossing
+    that needs more than half a turn is not a step to the next layer outwards and counts as not reached (DESIGN.md
+    R2; never the case for a particle that starts moving outwards).  A straight line (w = 0) uses the chord formula.
     """
     x, y, z, ipt, phi, theta = (np.asarray(a, dtype=np.float64) for a in (x, y, z, ipt, phi, theta))
     w = -np.asarray(q, dtype=np.float64) * K_CURV * bz * ipt
@@ -163,7 +164,7 @@ def cross_cylinder(x, y, z, ipt, phi, theta, q, bz, R):
     ys = np.where(straight, ly, by)
     s = np.where(straight, s_l, s_c)
     phn = np.where(straight, phi, phi_c)
-    ok = inside & (straight | reach)
+    ok = inside & (straight | (reach & (best <= np.pi)))
     zn = z + s / np.tan(theta)
     cosinc = (xs * np.cos(phn) + ys * np.sin(phn)) / R
     return ok, xs, ys, zn, phn, s, cosinc
@@ -273,7 +274,7 @@ class FitInputs:
     hit_y: np.ndarray
     hit_z: np.ndarray
     seg_off: np.ndarray    # [L+1] i64
-    hit_idx: np.ndarray | None  # [L][ld] i32 (identity or -1), None = identity everywhere
+    hit_idx: np.ndarray | None  # [L][ld] i32 (identity, or -2 = layer not crossed), None = identity everywhere
     truth: np.ndarray      # [L][n][6] f64 (NaN where no hit)
     valid: np.ndarray      # [L][n] bool
     gun: dict = field(default_factory=dict)
@@ -305,10 +306,10 @@ def fit_inputs(config: int, n: int | None = None, ms: bool = True, smear: bool =
     all_valid = bool(sim["valid"].all())
     hit_idx = None
     if force_index or not all_valid:
-        hit_idx = np.full((L, ld), -1, dtype=np.int32)
+        hit_idx = np.full((L, ld), -2, dtype=np.int32)     # -2: the truth track ended before this layer (not crossed)
         ident = np.arange(n, dtype=np.int32)
         for l in range(L):
-            hit_idx[l, :n] = np.where(sim["valid"][l], ident, -1)
+            hit_idx[l, :n] = np.where(sim["valid"][l], ident, -2)
     seg_off = (np.arange(L + 1, dtype=np.int64) * ld)
     return FitInputs(geom=geom, n=n, ld=ld, par=t["par"], cov=t["cov"], q=t["q"], hit_x=hx.reshape(-1), hit_y=hy.reshape(-1),
                      hit_z=hz.reshape(-1), seg_off=seg_off, hit_idx=hit_idx, truth=sim["truth"], valid=sim["valid"], gun=gun)

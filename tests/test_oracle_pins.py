@@ -84,9 +84,9 @@ def test_P1_generic_start_vs_circle_geometry():
         if not ok:
             assert f == o.UNREACHABLE
             continue
-        if ci < 0.02:   # a grazing double crossing may be stepped over by the 64-step march (flagged anyway)
+        assert f == (o.GRAZING if ci < 0.1 else 0)      # near-tangent double crossings included: none may be stepped over
+        if ci < 1e-4:                                   # the root is then conditioned like 1/cos(incidence)
             continue
-        assert f == (o.GRAZING if ci < 0.1 else 0)
         worst = max(worst, abs(po[0] - x), abs(po[1] - y), abs(po[2] - z), abs(po[4] - ph), abs(s_o - s))
         assert abs(np.hypot(po[0], po[1]) - R) < 1e-11
     assert worst < 1e-8
@@ -474,10 +474,10 @@ def test_P11_hundred_track_cases(event):
 
 
 def test_fit_skips_and_stops():
-    """hit_idx = -1 skips the layer entirely; a failing layer freezes the track with the status bit set."""
+    """hit_idx <= -2 skips the layer entirely; a failing layer freezes the track with the status bit set."""
     fi = synth.fit_inputs(0, n=64, force_index=True)
     base = _run(fi)
-    hi = fi.hit_idx.copy(); hi[4, :] = -1
+    hi = fi.hit_idx.copy(); hi[4, :] = -2
     r = o.fit(fi.geom.layer_table(), fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, hi)
     assert (r["nhits"] == 9).all() and (r["status"] == 0).all()
     # same as removing the layer from the geometry altogether
@@ -498,6 +498,153 @@ def test_fit_skips_and_stops():
     assert np.array_equal(r3["par"][:, low], r9["par"][:, low]) and np.array_equal(r3["cov"][low], r9["cov"][low])
     assert ((r3["status"][high] & o.UNREACHABLE) == 0).all()
     assert np.array_equal(base["nhits"], np.full(64, 10))
+
+
+def test_fit_hole_layer_transports_and_adds_material():
+    """hit_idx == -1 (R8): the layer is crossed without a hit -- the state is transported to it and the
+    layer's scattering is added, only the update is left out.
+    (a) Without material on that layer the intermediate stop changes nothing: transport to r_4 and then to r_5 is
+        the transport to r_5 (the helix maps form a group, so the Jacobians compose) -- equal to the fit with the
+        layer removed from the geometry.  Catches: a Jacobian that does not compose (a wrong ds/dp term), a hole
+        that leaves the state behind or touches chi2 / nhits.
+    (b) With material the covariance can only grow: C(hole) - C(layer removed) is positive semi-definite and not
+        zero, the chi2 of the later hits falls.  Catches: Q subtracted or dropped."""
+    fi = synth.fit_inputs(0, n=64, force_index=True)
+    L, ld = 10, fi.ld
+    hi = fi.hit_idx.copy(); hi[4, :] = -1
+    keep = [l for l in range(10) if l != 4]
+    hx = fi.hit_x.reshape(L, ld)[keep].reshape(-1); hy = fi.hit_y.reshape(L, ld)[keep].reshape(-1); hz = fi.hit_z.reshape(L, ld)[keep].reshape(-1)
+    lt = fi.geom.layer_table()
+    removed = o.fit(np.delete(lt, 4, axis=0), fi.geom.bz, fi.par, fi.cov, fi.q, hx, hy, hz, np.arange(10) * ld)
+    lt0 = lt.copy(); lt0[4, 2] = 0.0
+    r = o.fit(lt0, fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, hi)
+    assert (r["nhits"] == 9).all() and (r["status"] == 0).all()
+    assert np.max(np.abs(r["par"] - removed["par"])) < 1e-9 and np.max(np.abs(r["chi2"] - removed["chi2"])) < 1e-7
+    assert np.max(np.abs(r["cov"] - removed["cov"]) / np.abs(removed["cov"]).max(axis=(1, 2), keepdims=True)) < 1e-8
+    rm = o.fit(lt, fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, hi)
+    assert (rm["nhits"] == 9).all() and (rm["status"] == 0).all()
+    # stop right after the hole (layers 0..5, hit on 5): before later hits mix the information
+    h5 = hi.copy(); h5[6:] = -2
+    a = o.fit(lt, fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, h5)
+    b_ = o.fit(lt0, fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, h5)
+    for t in range(fi.n):
+        lam = np.linalg.eigvalsh(a["cov"][t] - b_["cov"][t])
+        assert lam[0] > -1e-9 * lam[-1] and lam[-1] > 0
+    assert (a["chi2"] < b_["chi2"]).mean() > 0.95
+    # a hole on the last layer leaves the state ON that layer (transported, not updated)
+    hl = fi.hit_idx.copy(); hl[9, :] = -1
+    e = o.fit(lt, fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, hl)
+    assert np.allclose(np.hypot(e["par"][0], e["par"][1]), 40.0, atol=1e-9) and (e["nhits"] == 9).all()
+
+
+def test_fit_hole_layers_keep_unit_pulls():
+    """Statistics pin of R8: 25 % of the inner hits of config-2-like tracks removed and marked as holes (-1).  With the
+    material of the hole layers the pulls stay unit and chi2/ndf = 1; leaving the material out (the round-1 reading,
+    reproduced here with -2) widens the 1/pT pull to ~1.12 and chi2/ndf to ~1.03."""
+    fi = synth.fit_inputs(2, n=20000, force_index=True)
+    L = fi.geom.n_layers
+    rng = np.random.default_rng(5)
+    last = np.where(fi.valid, np.arange(L)[:, None], -1).max(axis=0)
+    lay = np.arange(L)[:, None]
+    drop = (rng.random((L, fi.n)) < 0.25) & fi.valid & (lay < last[None, :]) & (lay > 0)
+    width = {}
+    for mode in (-1, -2):
+        h = fi.hit_idx.copy(); h[:, :fi.n][drop] = mode
+        r = o.fit(fi.geom.layer_table(), fi.geom.bz, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, h)
+        kept = type("V", (), {})()
+        kept.n, kept.geom, kept.truth, kept.valid = fi.n, fi.geom, fi.truth, fi.valid & ~drop
+        pulls, chi2, nh = _pulls(kept, r)
+        assert len(chi2) > 0.9 * fi.n
+        width[mode] = (pulls.std(axis=0), (chi2 / (2 * nh)).mean())
+    assert np.all(np.abs(width[-1][0] - 1) < 0.03) and abs(width[-1][1] - 1) < 0.02, width[-1]
+    assert width[-2][0][2] > 1.06 and width[-2][1] > 1.015, width[-2]
+
+
+def _first_crossing_turn(x, y, phi, w, R):
+    """Turning angle about the centre of curvature up to the first crossing of |p| = R (test-local circle-circle
+    geometry): None when the circles do not intersect."""
+    cx, cy, rho = x - np.sin(phi) / w, y + np.cos(phi) / w, 1 / abs(w)
+    d = np.hypot(cx, cy)
+    cosb = (d * d + R * R - rho * rho) / (2 * d * R)
+    if abs(cosb) > 1:
+        return None
+    beta, gamma, psi0 = np.arccos(cosb), np.arctan2(cy, cx), np.arctan2(y - cy, x - cx)
+    turns = []
+    for pm in (1, -1):
+        psi = np.arctan2(R * np.sin(gamma + pm * beta) - cy, R * np.cos(gamma + pm * beta) - cx)
+        turns.append(np.mod((psi - psi0) * np.sign(w), 2 * np.pi))
+    return min(turns)
+
+
+def test_P1_half_turn_boundary():
+    """DESIGN.md R2: the crossing must come within HALF a turn.  States anywhere inside the cylinder, moving in any
+    direction (inwards included), tight circles: the oracle reports UNREACHABLE exactly when the circles do not
+    intersect or the first crossing needs more than half a turn, and the simulator's cross_cylinder agrees.
+    Catches: a march limit of a full turn (or none), the second crossing taken for inward-moving states."""
+    rng = np.random.default_rng(7)
+    n_far = n_near = 0
+    for _ in range(6000):
+        R = rng.uniform(5, 80)
+        r0, a = rng.uniform(0.05, 0.97) * R, rng.uniform(-np.pi, np.pi)
+        rho = np.exp(rng.uniform(np.log(0.52 * (R - r0)), np.log(3 * R)))      # tight circles: many need a long arc
+        q, bz = rng.choice([-1, 1]), rng.choice([3.8, -3.8])
+        pt = rho * K * abs(bz)
+        phi = rng.uniform(-np.pi, np.pi)
+        p = np.array([r0 * np.cos(a), r0 * np.sin(a), 0.0, 1 / pt, phi, 1.3])
+        w = -q * K * bz / pt
+        turn = _first_crossing_turn(p[0], p[1], phi, w, R)
+        f, po, J, s, ci = o.propagate(p, q, bz, R)
+        ok, xs, ys, *_ = synth.cross_cylinder(p[0], p[1], p[2], p[3], p[4], p[5], q, bz, R)
+        if turn is None:
+            assert f == o.UNREACHABLE and not ok
+            continue
+        if abs(turn - np.pi) < 1e-6:
+            continue
+        if turn > np.pi:
+            n_far += 1
+            assert f == o.UNREACHABLE and not ok, (turn, f)
+            continue
+        cos_inc = (xs * np.cos(phi + turn * np.sign(w)) + ys * np.sin(phi + turn * np.sign(w))) / R
+        n_near += 1
+        assert ok and f == (o.GRAZING if cos_inc < 0.1 else 0), (turn, f, cos_inc)       # near-tangent double crossings included
+        if cos_inc < 1e-3:
+            continue
+        assert abs(abs(w) * s - turn) < 1e-8 and abs(po[0] - xs) < 1e-8 and abs(po[1] - ys) < 1e-8
+    assert n_far > 100 and n_near > 1000
+
+
+def test_fit_numeric_exits():
+    """KFO_NUMERIC in kfo_fit (status bit 3, track frozen at its last good state):
+    (a) an innovation matrix that is not positive definite (hand-made seed covariance with a negative position block):
+        nothing is used, the seed comes back unchanged;
+    (b) an update that drives 1/pT <= 0 (hits of a negative track, seed of positive charge with a wide 1/pT prior):
+        the state is that of the fit truncated before the failing layer.
+    Catches: a failed layer that still updates the state or counts a hit, a missing status bit."""
+    fi = synth.fit_inputs(0, n=8, ms=False)
+    lt = fi.geom.layer_table()
+    cov = fi.cov.copy()
+    cov[synth.pack_index(0, 0), :] = -1.0; cov[synth.pack_index(1, 1), :] = -1.0
+    r = o.fit(lt, fi.geom.bz, fi.par, cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off)
+    assert (r["status"] == o.NUMERIC).all() and (r["nhits"] == 0).all() and (r["chi2"] == 0).all()
+    assert np.array_equal(r["par"], fi.par[:, :8].astype(np.float64))
+    assert np.array_equal(synth.pack_sym(r["cov"]).T, cov[:, :8].astype(np.float64))
+    # (b) wrong charge, stiff seed with a wide curvature prior: 1/pT is pulled through zero
+    par = fi.par.copy(); par[3, :] = 0.02
+    cov = fi.cov.copy(); cov[synth.pack_index(3, 3), :] = 1.0
+    q = (-fi.q).astype(np.int8)
+    r = o.fit(lt, fi.geom.bz, par, cov, q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off)
+    failed = (r["status"] & o.NUMERIC) != 0
+    assert failed.sum() >= 4 and (r["nhits"][failed] < 10).all() and (r["par"][3][failed] > 0).all()
+    for t in np.nonzero(failed)[0]:
+        k = r["nhits"][t]
+        rt = o.fit(lt[:k], fi.geom.bz, par, cov, q, fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off[:k + 1])
+        assert rt["status"][t] == 0 and rt["nhits"][t] == k
+        assert np.array_equal(rt["par"][:, t], r["par"][:, t]) and np.array_equal(rt["cov"][t], r["cov"][t]) and rt["chi2"][t] == r["chi2"][t]
+        # the next update really is the one that fails: 1/pT of the unguarded Kalman step is <= 0
+        f, pp, Cp = o.predict(lt, k, fi.geom.bz, rt["par"][:, t], rt["cov"][t], q[t])
+        m = np.array([fi.hit_x[k * fi.ld + t], fi.hit_y[k * fi.ld + t], fi.hit_z[k * fi.ld + t]], dtype=np.float64)
+        S = Cp[:3, :3] + np.diag([lt[k, 5] ** 2, lt[k, 5] ** 2, lt[k, 4] ** 2])
+        assert f == 0 and (pp + Cp[:, :3] @ np.linalg.solve(S, m - pp[:3]))[3] <= 0
 
 
 def test_mat66_multiply_definition():
