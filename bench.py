@@ -39,7 +39,7 @@ FIT_BYTES_OUT = 6 * 4 + 21 * 4 + 4 + 4 + 4        # par + cov + chi2 + nhits + s
 FIT_BYTES_PER_HIT = 12
 FIT_BYTES_PER_IDX = 4
 BUILD_FLOP = dict(n_prop=458.0, n_scan=15.0, n_window=40.0, n_upd=250.0)
-BIN_BYTES_PER_HIT = 60.0   # read 12, key 4 + 4, tmp 8 + 8, write x, y, z, perm 16 + packed record 16 (the place kernel re-reads 8)
+BIN_BYTES_PER_HIT = 28.0   # algorithmic: read x, y, z (12), write the sorted 16-byte record (16); + 4 per bin for bin_off
 SM_COUNT, FP32_LANES = 148, 128
 FIT_CFG = {"fit_c0": 0, "fit_c1": 1, "fit_c2": 2}
 BUILD_CFG = {"build_c3": 3, "build_c4": 4}
@@ -303,8 +303,8 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
         hxs = [np.ascontiguousarray(a_.reshape(L, fi.ld)[:, lo:hi]).reshape(-1) for a_ in (fi.hit_x, fi.hit_y, fi.hit_z)]
         hidx = None
         if fi.hit_idx is not None:
-            hidx = np.full((L, ldc), -1, np.int32)
-            hidx[:, :m] = np.where(fi.hit_idx[:, lo:hi] >= 0, np.arange(m, dtype=np.int32)[None, :], -1)
+            hidx = np.full((L, ldc), -2, np.int32)
+            hidx[:, :m] = np.where(fi.hit_idx[:, lo:hi] >= 0, np.arange(m, dtype=np.int32)[None, :], fi.hit_idx[:, lo:hi])
         sub = dict(m=m, stream=torch.cuda.Stream(), h_in=[pin(hp), pin(hc), pin(fi.q[lo:hi])] + [pin(x) for x in hxs] + ([pin(hidx)] if hidx is not None else []))
         sub["seeds"] = b.Tracks.empty(m, ldc)
         sub["hits"] = b.Hits(hxs[0], hxs[1], hxs[2], np.arange(L + 1, dtype=np.int64) * m, 1)
@@ -377,7 +377,7 @@ def stored_traffic(workload):
     return None
 
 
-BUILD_LAUNCHES_PER_STEP = 7   # count, 3 x scan, scatter, place, build (the two memsets and the table copy are not kernels)
+BUILD_LAUNCHES_PER_STEP = 5   # bin: count, scan, scatter, place; build (the memset of bin_off is not a kernel)
 
 
 def bench_build(args, d: Dist, workload: str, sample_clocks=True):
@@ -389,7 +389,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     geom = b.Geom(bi.geom.layer_table(), bi.geom.bz)
     hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
     n_bins = bi.n_events * L * bi.n_phi * bi.n_z
-    binned = b.Binned(hits.n_hits, n_bins, bi.n_phi, bi.n_z)
+    binned = b.Binned(hits.n_hits, n_bins, bi.n_phi, bi.n_z, soa=False)     # the records and bin_off: all the build reads
     ws = torch.empty(max(b.kf_bin_workspace_bytes(geom, hits, bi.n_phi, bi.n_z), 1), dtype=torch.uint8, device="cuda")
     seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
     sev = torch.from_numpy(bi.seed_event).cuda(); shi = torch.from_numpy(bi.seed_hit_idx).cuda()
@@ -432,7 +432,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
         hs = np.full((bi.first_layer, ldc), -1, np.int32); hs[:, :m] = bi.seed_hit_idx[:, s0_:s1_]
         sub = dict(stream=torch.cuda.Stream(), n_ev=e1 - e0, m=m)
         sub["hits"] = b.Hits(bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], bi.seg_off[e0 * L: e1 * L + 1] - h0, e1 - e0)
-        sub["binned"] = b.Binned(h1 - h0, (e1 - e0) * L * bi.n_phi * bi.n_z, bi.n_phi, bi.n_z)
+        sub["binned"] = b.Binned(h1 - h0, (e1 - e0) * L * bi.n_phi * bi.n_z, bi.n_phi, bi.n_z, soa=False)
         sub["ws"] = torch.empty(max(b.kf_bin_workspace_bytes(geom, sub["hits"], bi.n_phi, bi.n_z), 1), dtype=torch.uint8, device="cuda")
         sub["seeds"] = b.Tracks.empty(m, ldc)
         sub["sev"] = torch.zeros(max(m, 1), dtype=torch.int32, device="cuda")[:m]
@@ -477,9 +477,9 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
                e2e=dict(value=bi.n_seeds * d.world / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=nbytes(h), d2h_bytes_per_step=nbytes(ho),
                         ms_per_step=e2e_ms, streams=n_sub),
                gpu_launches=args.steps * BUILD_LAUNCHES_PER_STEP, clocks=clocks)
-    bin_bytes = BIN_BYTES_PER_HIT * hits.n_hits + 8.0 * n_bins
+    bin_bytes = BIN_BYTES_PER_HIT * hits.n_hits + 4.0 * n_bins
     res["bin_roofline"] = dict(bound="hbm", achieved=bin_bytes / (bin_ms * 1e-3) / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
-                               frac=bin_bytes / (bin_ms * 1e-3) / 1e9 / pk["hbm_gbs"], alg_bytes_per_step=bin_bytes, kernels="kf_bin_* (6 launches)")
+                               frac=bin_bytes / (bin_ms * 1e-3) / 1e9 / pk["hbm_gbs"], alg_bytes_per_step=bin_bytes, kernels="kf_bin_* (memset + 4 launches)")
     if not args.no_cpu_baseline:
         cb, counters, n_s = oracle_build(bi, args.cpu_events, 1, 0)
         cb.pop("ms_per_step")

@@ -61,6 +61,17 @@ typedef struct { float r, zmax, xx0, sig_rphi, sig_z, sig_r; } kf_layer;
 /* Geometry: n_layers cylinders sorted by increasing r; uniform field bz_tesla along z.  `layers` is a HOST array. */
 typedef struct { int32_t n_layers; float bz_tesla; const kf_layer* layers; } kf_geom;
 
+/* Per-call tuning options (never change a result beyond rounding; kf_build results do not depend on them at all).
+ * Pass NULL for the defaults.  `size` = sizeof(kf_options) of the caller's header (versioning: fields beyond it are
+ * taken as 0 = automatic); kf_options_init fills the defaults.  There is no process-global state in the library. */
+typedef struct {
+    uint32_t size;
+    int32_t fit_tracks_per_thread;   /* 0 = automatic (2 where the arguments allow it), 1 = always one track per thread  */
+    int32_t build_seeds_per_block;   /* seeds owned by one thread block of kf_build: 0 = automatic, else a multiple of 16 in 16..256 */
+    int32_t build_max_blocks;        /* cap on the persistent grid of kf_build: 0 = automatic (fills the device)         */
+} kf_options;
+void kf_options_init(kf_options* opt);
+
 /* SoA track store.  n tracks, stride ld >= n between components. */
 typedef struct {
     int64_t n, ld;
@@ -86,23 +97,25 @@ typedef struct {
 
 /* ---------------------------------------------------------------------------------------------------------
  * kf_fit -- forward (inside-out) Kalman filter over a fixed hit list (DESIGN.md sec. 2 F1-F9).
- * For every track t and every layer l in order of increasing radius with hit_idx[l*ld + t] >= 0:
+ * For every track t and every layer l in order of increasing radius with hit_idx[l*ld + t] >= -1:
  *   propagate the state and covariance along the exact helix to the first crossing of the cylinder r_l (Jacobian
- *   including the path-length term), add the multiple-scattering noise of the layer (Highland), update with the
- *   3-D hit (residual, 3x3 innovation inverse, chi2, gain, state and covariance update).
- * hit_idx: [n_layers][seeds->ld] index of the hit within its segment, < 0 = layer skipped; NULL = identity
- *          (hit of track t on layer l is element t of segment l).
+ *   including the path-length term), add the multiple-scattering noise of the layer (Highland) and, if there is a hit,
+ *   update with the 3-D hit (residual, 3x3 innovation inverse, chi2, gain, state and covariance update).
+ * hit_idx: [n_layers][seeds->ld] index of the hit within its segment; -1 = layer crossed without a hit (transport and
+ *          material, no update: what kf_build does for a candidate without a compatible hit); <= -2 = layer not
+ *          crossed, skipped entirely; NULL = identity (hit of track t on layer l is element t of segment l; needs
+ *          trk_event == NULL).
  * trk_event: [n] event of each track, NULL = event 0.
  * seeds/out: same n; out->ld may differ; out may alias seeds.  out->q is not written.
  * A failing layer sets the status bit, ends the track there and leaves the state of the last updated layer.
- * Output phi is wrapped to (-pi, pi].  Errors: NULL pointers, n < 0, ld < n, bad geometry, CUDA launch failure. */
+ * Output phi is wrapped to (-pi, pi].  Errors: NULL pointers, n < 0, ld < n, bad geometry, hit_idx == NULL together
+ * with trk_event != NULL, CUDA launch failure.
+ * With sig_r == sig_rphi on every layer, event 0 and even strides / 8-byte aligned arrays kf_fit runs two tracks per
+ * thread (all arithmetic as packed fp32 pairs); tracks that leave the fast path (failed crossing, large turning angle
+ * or angle correction, numeric trouble) are redone by the one-track code.  opt->fit_tracks_per_thread = 1 forces the
+ * one-track kernel (results agree to rounding). */
 int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
-           const kf_tracks* seeds, kf_tracks* out, void* stream);
-/* With identity indexing, event 0, sig_r == sig_rphi on every layer and even strides / 8-byte aligned arrays kf_fit runs
- * two tracks per thread (all arithmetic as packed fp32 pairs); tracks that leave the fast path (failed crossing, large
- * turning angle or angle correction, numeric trouble) are redone by the one-track code.  kf_fit_set_pairs(0) forces the
- * one-track kernel, kf_fit_set_pairs(1) restores the default (test / tuning hook; results agree to rounding). */
-int kf_fit_set_pairs(int32_t enable);
+           const kf_tracks* seeds, kf_tracks* out, const kf_options* opt, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------------
  * Binned hit index (DESIGN.md sec. 2 B0, readings X1-X2).  Filled by kf_bin_hits into
@@ -111,7 +124,7 @@ int kf_fit_set_pairs(int32_t enable);
  * Sorted order = ascending (global bin, original index): unique, hence bit-exact testable. */
 typedef struct {
     int32_t n_phi, n_z;   /* n_phi multiple of 8, 8..4096; n_z 1..1024                                     */
-    float *x, *y, *z;     /* [n_hits] hits in sorted order                                                 */
+    float *x, *y, *z;     /* [n_hits] hits in sorted order            } optional: all four NULL = not wanted       */
     int32_t* perm;        /* [n_hits] sorted position -> original index within its segment                 */
     int32_t* bin_off;     /* [n_events*n_layers*n_z*n_phi + 1] offsets into the sorted arrays              */
     float* xyzp;          /* [n_hits][4] the same hits as 16-byte records (x, y, z, bits of perm): what the */
@@ -147,32 +160,31 @@ typedef struct {
     int32_t* n_cand;      /* [n_seeds] */
 } kf_cands;
 
-/* Seeds: state on (or near) layer first_layer-1; their chi2 / nhits inputs are ignored: every seed starts with
- * chi2 = 0 and nhits = first_layer.  seed_event [n] (may be NULL when n_events == 1); seed_hit_idx
+/* Seeds: state on (or near) layer first_layer-1; every seed starts with chi2 = seeds->chi2[s] (0 when seeds->chi2 is
+ * NULL) and nhits = first_layer (seeds->nhits is ignored).  seed_event [n] (may be NULL when n_events == 1); seed_hit_idx
  * [first_layer][seeds->ld] = hits already on the seed (copied to the output lists; NULL = -1).
  * Slots k >= n_cand[s] get nhits = 0, chi2 = 0, status = 0 and hit_idx = -2; their par / cov are not written.
  * cand.q is filled with the seed's charge.  A candidate that cannot be propagated to a layer, leaves
  * |z| <= zmax + window, or fails numerically is finished (status bit set) and carried unchanged.
- * K in 1..32.  ws: device workspace of at least kf_build_workspace_bytes(geom, n_seeds, K) bytes (candidate records
- * and per-layer links of the tiles in flight; ~0.45 MB per resident block, a few hundred blocks); it is only used
- * while the enqueued kernel runs and may be reused by the next call on the same stream.
- * kf_build_set_tile(n): tuning hook, seeds owned by one thread block (multiple of 16 in 16..256; 0 = automatic);
- * the result does not depend on it, the workspace size does (query it after setting the tile).
- * Errors: NULL pointers, K / first_layer / cuts out of range, bad bin counts, workspace too small (-4), CUDA failure. */
-size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K);
-int kf_build_set_tile(int32_t seeds_per_block);
+ * K in 1..32.  ws: device workspace of at least kf_build_workspace_bytes(geom, n_seeds, K, opt) bytes (candidate records
+ * and per-layer hit links of the tiles in flight: (288 + 4 n_layers) K bytes per seed in flight, ~100 MB at most); a
+ * pure function of its arguments; the workspace is only used while the enqueued kernel runs and may be reused by the
+ * next call on the same stream.  opt (NULL = automatic): seeds per thread block and the cap on the persistent grid;
+ * the result does not depend on them, the workspace size does (pass the same opt to both calls).
+ * Errors: NULL pointers, K / first_layer / cuts / options out of range, bad bin counts, workspace too small (-4),
+ * CUDA failure. */
+size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K, const kf_options* opt);
 int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
-             float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream);
+             float n_sigma, kf_cands* out, const kf_options* opt, void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------------
  * kf_select_best -- hand-over from building to the final fit ("When a complete track has been
  * reconstructed, a final fit using the KF is performed").  hit_idx[l*ld + s] = hit of the best candidate (slot s*K)
- * of seed s on layer l, in the layout kf_fit reads; layers without hit, layers not crossed and layers < first_layer
- * (already behind the seed state) are -1.  The final fit is then
- *   kf_fit(geom, hits, hit_idx, seed_event, seeds, out, stream)       with ld == seeds->ld.
- * Note: kf_fit skips a layer without hit entirely (R8) whereas kf_build transports the candidate through it
- * (adding its scattering), so the refit equals the built candidate only for hit lists without holes.
+ * of seed s on layer l, in the layout and with the meaning kf_fit reads: >= 0 hit, -1 layer crossed without a hit,
+ * -2 layer not crossed; layers < first_layer (already behind the seed state) are -2.  The final fit is then
+ *   kf_fit(geom, hits, hit_idx, seed_event, seeds, out, NULL, stream)       with ld == seeds->ld
+ * and goes through exactly the steps the built candidate went through (R8).
  * Errors: NULL pointers, ld < n_seeds, first_layer outside 0..n_layers, CUDA failure. */
 int kf_select_best(const kf_cands* cands, int32_t first_layer, int32_t* hit_idx, int64_t ld, void* stream);
 

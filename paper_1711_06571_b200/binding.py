@@ -13,14 +13,14 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so")   # KF_B200_LIB: another build of the same library (A/B timing)
+_SO = os.path.join(_HERE, "libkf_b200.so")
 _lib = None
 
 KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
-EXPORTS = ["kf_fit", "kf_fit_set_pairs", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
-           "kf_build", "kf_build_set_tile", "kf_select_best", "kf_mat66_multiply", "kf_last_error", "kf_version"]
+EXPORTS = ["kf_options_init", "kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
+           "kf_build", "kf_select_best", "kf_mat66_multiply", "kf_last_error", "kf_version"]
 
 
 class KfError(RuntimeError):
@@ -33,6 +33,10 @@ class kf_layer(C.Structure):
 
 class kf_geom(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("bz_tesla", C.c_float), ("layers", C.POINTER(kf_layer))]
+
+
+class kf_options(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("fit_tracks_per_thread", C.c_int32), ("build_seeds_per_block", C.c_int32), ("build_max_blocks", C.c_int32)]
 
 
 class kf_tracks(C.Structure):
@@ -67,14 +71,15 @@ def lib() -> C.CDLL:
         l.kf_bin_workspace_bytes.restype = C.c_size_t
         l.kf_build_workspace_bytes.restype = C.c_size_t
         l.kf_bin_workspace_bytes.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
-        l.kf_build_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
-        l.kf_fit.argtypes = [C.c_void_p] * 7
+        l.kf_build_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
+        l.kf_options_init.argtypes = [C.c_void_p]
+        l.kf_options_init.restype = None
+        l.kf_fit.argtypes = [C.c_void_p] * 8
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
-        l.kf_build_set_tile.argtypes = [C.c_int32]
         l.kf_mat66_multiply.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_select_best.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p]
-        l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = l
     return _lib
 
@@ -180,12 +185,24 @@ def kf_version() -> int:
     return int(lib().kf_version())
 
 
-def kf_fit_set_pairs(enable: int):
-    _check(lib().kf_fit_set_pairs(C.c_int32(enable)), "kf_fit_set_pairs")
+def options(**fields) -> kf_options:
+    """kf_options with the library's defaults (kf_options_init) and the given fields set, e.g. options(build_seeds_per_block=4)."""
+    o = kf_options()
+    lib().kf_options_init(C.byref(o))
+    for k, v in fields.items():
+        if k not in ("fit_tracks_per_thread", "build_seeds_per_block", "build_max_blocks"):
+            raise KeyError(k)
+        setattr(o, k, int(v))
+    return o
 
 
-def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Tracks | None = None, stream=None) -> Tracks:
-    """include/kf.h kf_fit.  hit_idx: [L, seeds.ld] int32 device tensor or None (identity); trk_event [n] int32 or None."""
+def _opt(opt):
+    return None if opt is None else C.byref(opt)
+
+
+def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Tracks | None = None, opt: kf_options | None = None, stream=None) -> Tracks:
+    """include/kf.h kf_fit.  hit_idx: [L, seeds.ld] int32 device tensor (-1 = hole, -2 = not crossed) or None (identity);
+    trk_event [n] int32 or None."""
     _require_cuda()
     if out is None:
         out = Tracks.empty(seeds.n, seeds.ld, seeds.par.device)
@@ -194,7 +211,7 @@ def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Track
         assert tuple(hit_idx.shape) == (geom.n_layers, seeds.ld)
     sc, oc = seeds.c(), out.c()
     rc = lib().kf_fit(C.byref(geom.c), C.byref(hits.c), _ptr(hit_idx, torch.int32), _ptr(trk_event, torch.int32),
-                      C.byref(sc), C.byref(oc), _stream(stream))
+                      C.byref(sc), C.byref(oc), _opt(opt), _stream(stream))
     _check(rc, "kf_fit")
     return out
 
@@ -202,22 +219,23 @@ def kf_fit(geom: Geom, hits: Hits, hit_idx, trk_event, seeds: Tracks, out: Track
 class Binned:
     """Device arrays of kf_binned, allocated by the caller (here: torch) and filled by kf_bin_hits."""
 
-    def __init__(self, n_hits: int, n_bins: int, n_phi: int, n_z: int, device="cuda"):
+    def __init__(self, n_hits: int, n_bins: int, n_phi: int, n_z: int, device="cuda", soa: bool = True):
+        """soa = False: only bin_off and the 16-byte records xyzp (all kf_build reads); x, y, z, perm stay NULL."""
         self.n_phi, self.n_z, self.n_hits = n_phi, n_z, n_hits
         m = max(n_hits, 1)
-        self.x = torch.empty(m, dtype=torch.float32, device=device)
-        self.y = torch.empty(m, dtype=torch.float32, device=device)
-        self.z = torch.empty(m, dtype=torch.float32, device=device)
-        self.perm = torch.empty(m, dtype=torch.int32, device=device)
+        mk = lambda dt: torch.empty(m, dtype=dt, device=device) if soa else None
+        self.x, self.y, self.z, self.perm = mk(torch.float32), mk(torch.float32), mk(torch.float32), mk(torch.int32)
         self.bin_off = torch.empty(n_bins + 1, dtype=torch.int32, device=device)
         self.xyzp = torch.empty((m, 4), dtype=torch.float32, device=device)
-        self.c = kf_binned(n_phi, n_z, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(), self.perm.data_ptr(), self.bin_off.data_ptr(),
-                           self.xyzp.data_ptr())
+        p = lambda t: t.data_ptr() if t is not None else None
+        self.c = kf_binned(n_phi, n_z, p(self.x), p(self.y), p(self.z), p(self.perm), self.bin_off.data_ptr(), self.xyzp.data_ptr())
 
     def to_host(self) -> dict:
         n = self.n_hits
-        return dict(x=self.x[:n].cpu().numpy(), y=self.y[:n].cpu().numpy(), z=self.z[:n].cpu().numpy(), perm=self.perm[:n].cpu().numpy(),
-                    bin_off=self.bin_off.cpu().numpy(), n_phi=self.n_phi, n_z=self.n_z, xyzp=self.xyzp[:n].cpu().numpy())
+        d = dict(bin_off=self.bin_off.cpu().numpy(), n_phi=self.n_phi, n_z=self.n_z, xyzp=self.xyzp[:n].cpu().numpy())
+        if self.x is not None:
+            d.update(x=self.x[:n].cpu().numpy(), y=self.y[:n].cpu().numpy(), z=self.z[:n].cpu().numpy(), perm=self.perm[:n].cpu().numpy())
+        return d
 
 
 def kf_bin_workspace_bytes(geom: Geom, hits: Hits, n_phi: int, n_z: int) -> int:
@@ -271,16 +289,12 @@ class Cands:
         return d
 
 
-def kf_build_set_tile(seeds_per_block: int):
-    _check(lib().kf_build_set_tile(C.c_int32(seeds_per_block)), "kf_build_set_tile")
-
-
-def kf_build_workspace_bytes(geom: Geom, n_seeds: int, K: int) -> int:
-    return int(lib().kf_build_workspace_bytes(C.byref(geom.c), n_seeds, K))
+def kf_build_workspace_bytes(geom: Geom, n_seeds: int, K: int, opt: kf_options | None = None) -> int:
+    return int(lib().kf_build_workspace_bytes(C.byref(geom.c), n_seeds, K, _opt(opt)))
 
 
 def kf_build(geom: Geom, hits: Hits, binned: Binned, seeds: Tracks, seed_event, seed_hit_idx, first_layer: int, K: int, chi2_cut: float,
-             n_sigma: float, out: Cands | None = None, ws: torch.Tensor | None = None, stream=None) -> Cands:
+             n_sigma: float, out: Cands | None = None, opt: kf_options | None = None, ws: torch.Tensor | None = None, stream=None) -> Cands:
     """include/kf.h kf_build.  seed_event [n] int32 device tensor (or None), seed_hit_idx [first_layer, seeds.ld] int32 (or None).
     Allocates the output and the workspace with torch when not given."""
     _require_cuda()
@@ -289,10 +303,10 @@ def kf_build(geom: Geom, hits: Hits, binned: Binned, seeds: Tracks, seed_event, 
     if seed_hit_idx is not None:
         assert tuple(seed_hit_idx.shape) == (first_layer, seeds.ld)
     if ws is None:
-        ws = torch.empty(max(kf_build_workspace_bytes(geom, seeds.n, K), 1), dtype=torch.uint8, device=seeds.par.device)
+        ws = torch.empty(max(kf_build_workspace_bytes(geom, seeds.n, K, opt), 1), dtype=torch.uint8, device=seeds.par.device)
     sc = seeds.c()
     rc = lib().kf_build(C.byref(geom.c), C.byref(hits.c), C.byref(binned.c), C.byref(sc), _ptr(seed_event, torch.int32), _ptr(seed_hit_idx, torch.int32),
-                        first_layer, K, chi2_cut, n_sigma, C.byref(out.c), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
+                        first_layer, K, chi2_cut, n_sigma, C.byref(out.c), _opt(opt), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
     _check(rc, "kf_build")
     out._ws = ws    # keep the workspace alive until the stream has consumed it
     return out

@@ -38,5 +38,13 @@ int check_geom(const kf_geom* g, const char* who) {
 
 }  // namespace kf
 
+extern "C" void kf_options_init(kf_options* opt) {
+    if (!opt) return;
+    opt->size = (uint32_t)sizeof(kf_options);
+    opt->fit_tracks_per_thread = 0;
+    opt->build_seeds_per_block = 0;
+    opt->build_max_blocks = 0;
+}
+
 extern "C" const char* kf_last_error(void) { return kf::g_err; }
-extern "C" int kf_version(void) { return 100; }
+extern "C" int kf_version(void) { return 200; }

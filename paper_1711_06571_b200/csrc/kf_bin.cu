@@ -5,13 +5,17 @@
 // work specified in IEEE fp32 single operations (__fdiv_rn, __fmul_rn, __fadd_rn: no contraction), so the result
 // is bit-exact against the CPU oracle.
 //
-// Pipeline (all on the caller's stream, HBM-bound: ~44 B per hit):
-//   1. bin_count:   one thread per hit: key = global bin; atomicAdd into bin_off[key + 1]
-//   2. scan:        in-place inclusive scan of bin_off (three small kernels: block sums, scan of sums, add)
-//   3. bin_scatter: pos = bin_off[key] + atomicAdd(cursor[key]); tmp[pos] = (key, original index)   (order within a
-//                   bin is arbitrary here)
-//   4. bin_place:   one thread per position: rank of its original index inside its bin (bins hold a handful of
-//                   hits) -> final position; writes perm and the gathered x, y, z.  Deterministic and stable.
+// Pipeline (one memset + four kernels on the caller's stream, no host-to-device copy: graph-capturable):
+//   0. bin_off <- 0
+//   1. bin_count:   thread per hit: key = global bin; rank = atomicAdd(bin_off[key + 1], 1) is at the same time the
+//                   histogram and the hit's (arbitrary) arrival rank inside its bin; (key, rank) kept, 8 bytes per hit
+//   2. bin_scan:    block per segment: inclusive scan of the segment's bin counts, offset by seg_off[segment] --
+//                   segments are independent, so there is no carry between blocks and one launch does it
+//   3. bin_scatter: thread per hit: record (x, y, z, original index) to bin_off[key] + rank (the hits travel with their
+//                   index: no gather through the index later)
+//   4. bin_place:   thread per bin (a bin holds a handful of hits): order the records of the bin by original index ->
+//                   deterministic, stable; writes the 16-byte records the build scan reads and, if asked for, the
+//                   sorted x, y, z, perm arrays
 #include <cmath>
 #include "kf_common.cuh"
 #include "kf_binmath.cuh"
@@ -19,22 +23,23 @@
 namespace kf {
 
 constexpr int BIN_BLOCK = 256;
-constexpr int SCAN_ITEMS = 16;                       // per thread
-constexpr int SCAN_TILE = BIN_BLOCK * SCAN_ITEMS;    // per block
+constexpr int SCAN_BLOCK = 512;
+constexpr int SCAN_ITEMS = 8;                        // per thread
+constexpr int MAX_TAN_TAB = 4096 / 8 + 1;
 
 struct BinArgs {
     int32_t n_layers, n_phi, n_z, n_seg;
     const float *hx, *hy, *hz;
     const int64_t* seg_off;      // device
-    const float* tan_tab;        // device, n_phi/8 + 1
-    int32_t* key;                // [n_hits]
+    int2* kr;                    // [n_hits] (key, arrival rank within the bin)
     int32_t* bin_off;            // [n_bins + 1]
-    int32_t* cursor;             // [n_bins]
-    int2* tmp;                   // [n_hits] (key, original index within segment)
-    float *sx, *sy, *sz;
+    float4* tmp;                 // [n_hits] records in arrival order within each bin
+    float *sx, *sy, *sz;         // optional (all or none)
     int32_t* perm;
     float4* xyzp;
+    float phi_scale;             // n_phi / (2 pi): first guess of the table search
     float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
+    float tan_tab[MAX_TAN_TAB];  // X1: fl32(tan(2 pi k / n_phi)), k = 0 .. n_phi/8 (evaluated in double on the host), last = 1
 };
 
 __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_constant__ BinArgs a) {
@@ -46,104 +51,86 @@ __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_co
         const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
         const int32_t base = seg * a.n_z * a.n_phi;
         for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
-            const int b = base + z_bin(a.hz[h], a.zmax[l], a.inv_dz[l], a.n_z) * a.n_phi + phi_bin(a.hx[h], a.hy[h], a.n_phi, s_tab);
-            a.key[h] = b;
-            atomicAdd(&a.bin_off[b + 1], 1);
+            const int b = base + z_bin(a.hz[h], a.zmax[l], a.inv_dz[l], a.n_z) * a.n_phi + phi_bin(a.hx[h], a.hy[h], a.n_phi, s_tab, a.phi_scale);
+            a.kr[h] = make_int2(b, atomicAdd(&a.bin_off[b + 1], 1));
         }
     }
 }
 
-// ---- in-place inclusive scan of v[0..n) (int32): block totals, scan of totals by one block, rescan with offsets ----
-__device__ __forceinline__ int block_inclusive_scan(int v, int* s_warp) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const int o = __shfl_up_sync(0xffffffffu, v, d);
-        if (lane >= d) v += o;
-    }
-    if (lane == 31) s_warp[w] = v;
+// block per segment: bin_off[seg*B + b + 1] <- seg_off[seg] + (number of hits in bins 0..b of the segment)
+__global__ void __launch_bounds__(SCAN_BLOCK) kf_bin_scan_kernel(int32_t* __restrict__ bin_off, const int64_t* __restrict__ seg_off, int bins_per_seg) {
+    __shared__ int s_warp[SCAN_BLOCK / 32];
+    __shared__ int s_carry;
+    const int seg = blockIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int32_t* v = bin_off + (int64_t)seg * bins_per_seg + 1;
+    if (threadIdx.x == 0) s_carry = (int)seg_off[seg];
     __syncthreads();
-    if (w == 0) {
-        int t = lane < BIN_BLOCK / 32 ? s_warp[lane] : 0;
+    for (int base = 0; base < bins_per_seg; base += SCAN_BLOCK * SCAN_ITEMS) {
+        const int t0 = base + threadIdx.x * SCAN_ITEMS;
+        int x[SCAN_ITEMS];
+        int acc = 0;
+#pragma unroll
+        for (int i = 0; i < SCAN_ITEMS; ++i) { x[i] = (t0 + i < bins_per_seg) ? v[t0 + i] : 0; acc += x[i]; }
+        int inc = acc;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const int o = __shfl_up_sync(0xffffffffu, t, d);
-            if (lane >= d) t += o;
+            const int o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
         }
-        s_warp[lane] = t;   // inclusive over warps (BIN_BLOCK/32 <= 32)
-    }
-    __syncthreads();
-    if (w > 0) v += s_warp[w - 1];
-    __syncthreads();
-    return v;
-}
-
-__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_tile_sums_kernel(const int32_t* v, int64_t n, int32_t* sums) {
-    __shared__ int s_warp[32];
-    const int64_t t0 = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
-    int acc = 0;
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) acc += (t0 + i < n) ? v[t0 + i] : 0;
-    const int inc = block_inclusive_scan(acc, s_warp);
-    if (threadIdx.x == BIN_BLOCK - 1) sums[blockIdx.x] = inc;
-}
-
-__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_sums_kernel(int32_t* sums, int n_tiles) {   // one block; exclusive, in place
-    __shared__ int s_warp[32];
-    __shared__ int s_carry;
-    if (threadIdx.x == 0) s_carry = 0;
-    __syncthreads();
-    for (int base = 0; base < n_tiles; base += BIN_BLOCK) {
-        const int i = base + threadIdx.x;
-        const int x = i < n_tiles ? sums[i] : 0;
-        const int inc = block_inclusive_scan(x, s_warp);
-        const int carry = s_carry;
-        if (i < n_tiles) sums[i] = carry + inc - x;
+        if (lane == 31) s_warp[w] = inc;
         __syncthreads();
-        if (threadIdx.x == BIN_BLOCK - 1) s_carry = carry + inc;
+        int before = s_carry;
+        for (int j = 0; j < w; ++j) before += s_warp[j];
+        int run = before + inc - acc;
+#pragma unroll
+        for (int i = 0; i < SCAN_ITEMS; ++i) { run += x[i]; if (t0 + i < bins_per_seg) v[t0 + i] = run; }
+        __syncthreads();
+        if (threadIdx.x == SCAN_BLOCK - 1) s_carry = run;
         __syncthreads();
     }
-}
-
-__global__ void __launch_bounds__(BIN_BLOCK) kf_scan_apply_kernel(int32_t* v, int64_t n, const int32_t* sums) {
-    __shared__ int s_warp[32];
-    const int64_t t0 = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
-    int x[SCAN_ITEMS];
-    int acc = 0;
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) { x[i] = (t0 + i < n) ? v[t0 + i] : 0; acc += x[i]; }
-    int run = block_inclusive_scan(acc, s_warp) - acc + sums[blockIdx.x];
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) { run += x[i]; if (t0 + i < n) v[t0 + i] = run; }
 }
 
 __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_scatter_kernel(const __grid_constant__ BinArgs a) {
     for (int seg = blockIdx.y; seg < a.n_seg; seg += gridDim.y) {
         const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
         for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
-            const int b = a.key[h];
-            const int pos = a.bin_off[b] + atomicAdd(&a.cursor[b], 1);
-            a.tmp[pos] = make_int2(b, (int)(h - h0));
+            const int2 kr = a.kr[h];
+            const float x = a.hx[h], y = a.hy[h], z = a.hz[h];
+            const int pos = __ldg(a.bin_off + kr.x) + kr.y;
+            a.tmp[pos] = make_float4(x, y, z, __int_as_float((int)(h - h0)));
         }
     }
 }
 
-__global__ void __launch_bounds__(BIN_BLOCK) kf_bin_place_kernel(const __grid_constant__ BinArgs a, int64_t n_hits) {
-    const int64_t pos = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
-    if (pos >= n_hits) return;
-    const int2 me = a.tmp[pos];
-    const int o0 = a.bin_off[me.x], o1 = a.bin_off[me.x + 1];
+// record i of the bin [o0, o1) to its place: rank of its original index among the bin's records
+template <bool SOA>
+__device__ __forceinline__ void place_one(const BinArgs& a, int o0, int o1, int i) {
+    const float4 me = a.tmp[i];
+    const int idx = __float_as_int(me.w);
     int rank = 0;
-    for (int j = o0; j < o1; ++j) rank += a.tmp[j].y < me.y;
-    const int seg = me.x / (a.n_z * a.n_phi);
-    const int64_t src = a.seg_off[seg] + me.y;
+    for (int j = o0; j < o1; ++j) rank += __float_as_int(a.tmp[j].w) < idx ? 1 : 0;
     const int dst = o0 + rank;
-    const float x = a.hx[src], y = a.hy[src], z = a.hz[src];
-    a.perm[dst] = me.y;
-    a.sx[dst] = x;
-    a.sy[dst] = y;
-    a.sz[dst] = z;
-    a.xyzp[dst] = make_float4(x, y, z, __int_as_float(me.y));
+    a.xyzp[dst] = me;
+    if (SOA) { a.sx[dst] = me.x; a.sy[dst] = me.y; a.sz[dst] = me.z; a.perm[dst] = idx; }
+}
+
+template <bool SOA>
+__global__ void __launch_bounds__(BIN_BLOCK) kf_bin_place_kernel(const __grid_constant__ BinArgs a, int64_t n_bins) {
+    const int64_t b = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
+    int o0 = 0, o1 = 0;
+    if (b < n_bins) { o0 = a.bin_off[b]; o1 = a.bin_off[b + 1]; }
+    const bool big = o1 - o0 > 32;
+    if (!big)
+        for (int i = o0; i < o1; ++i) place_one<SOA>(a, o0, o1, i);
+    // crowded bins (degenerate input): the whole warp shares the work of each of them
+    unsigned todo = __ballot_sync(0xffffffffu, big);
+    const int lane = threadIdx.x & 31;
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const int q0 = __shfl_sync(0xffffffffu, o0, src), q1 = __shfl_sync(0xffffffffu, o1, src);
+        for (int i = q0 + lane; i < q1; i += 32) place_one<SOA>(a, q0, q1, i);
+    }
 }
 
 // ---- window lookup (diagnostic entry; the build kernel walks the same ranges) ----
@@ -193,15 +180,12 @@ static int check_bins(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, i
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct BinWs { size_t tab, key, cursor, tmp, sums, total; };
-static BinWs bin_ws_layout(int64_t n_hits, int64_t n_bins, int n_phi) {
+struct BinWs { size_t kr, tmp, total; };
+static BinWs bin_ws_layout(int64_t n_hits) {
     BinWs w;
     size_t o = 0;
-    w.tab = o; o += align256((size_t)(n_phi / 8 + 1) * sizeof(float));
-    w.key = o; o += align256((size_t)n_hits * sizeof(int32_t));
-    w.cursor = o; o += align256((size_t)n_bins * sizeof(int32_t));
-    w.tmp = o; o += align256((size_t)n_hits * sizeof(int2));
-    w.sums = o; o += align256((size_t)((n_bins + 1 + SCAN_TILE - 1) / SCAN_TILE + 1) * sizeof(int32_t));
+    w.kr = o; o += align256((size_t)n_hits * sizeof(int2));
+    w.tmp = o; o += align256((size_t)n_hits * sizeof(float4));
     w.total = o;
     return w;
 }
@@ -213,7 +197,7 @@ extern "C" size_t kf_bin_workspace_bytes(const kf_geom* geom, const kf_hits* hit
     if (!geom || !hits) return 0;
     int64_t nb;
     if (check_geom(geom, "kf_bin_workspace_bytes") || check_bins(geom, hits, n_phi, n_z, "kf_bin_workspace_bytes", &nb)) return 0;
-    return bin_ws_layout(hits->n_hits, nb, n_phi).total;
+    return bin_ws_layout(hits->n_hits).total;
 }
 
 extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* ws,
@@ -228,8 +212,9 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
     if (!hits->seg_off || !hits->seg_off_dev) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: hits->seg_off / seg_off_dev is NULL");
     if (!out->bin_off) return fail(KF_ERR_NULL_PTR, "kf_bin_hits: out->bin_off is NULL");
     const int64_t n_hits = hits->n_hits;
-    if (n_hits > 0 && (!hits->x || !hits->y || !hits->z || !out->x || !out->y || !out->z || !out->perm || !out->xyzp))
-        return fail(KF_ERR_NULL_PTR, "kf_bin_hits: NULL hit array");
+    const bool soa = out->x || out->y || out->z || out->perm;
+    if (n_hits > 0 && (!hits->x || !hits->y || !hits->z || !out->xyzp || (soa && (!out->x || !out->y || !out->z || !out->perm))))
+        return fail(KF_ERR_NULL_PTR, "kf_bin_hits: NULL hit array (out->x, y, z, perm: all or none)");
     const int n_seg = hits->n_events * geom->n_layers;
     if (hits->seg_off[0] != 0 || hits->seg_off[n_seg] != n_hits) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits: seg_off must run from 0 to n_hits");
     int64_t max_seg = 0;
@@ -238,44 +223,39 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
         if (d < 0) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits: seg_off not monotonic at segment %d", s);
         if (d > max_seg) max_seg = d;
     }
-    const BinWs w = bin_ws_layout(n_hits, n_bins, n_phi);
+    const BinWs w = bin_ws_layout(n_hits);
     if (!ws || ws_bytes < w.total) return fail(KF_ERR_WORKSPACE_TOO_SMALL, "kf_bin_hits: workspace %zu < %zu bytes", ws_bytes, w.total);
     cudaStream_t st = (cudaStream_t)stream;
     char* base = (char*)ws;
     out->n_phi = n_phi; out->n_z = n_z;
 
-    // X1 table: T[k] = fl32(tan(2 pi k / N)) evaluated in double on the host, T[N/8] = 1
-    float tab[4096 / 8 + 1];
-    const double two_pi = 6.283185307179586476925286766559;
-    for (int k = 0; k < n_phi / 8; ++k) tab[k] = (float)std::tan(two_pi * (double)k / (double)n_phi);
-    tab[n_phi / 8] = 1.0f;
-    cudaMemcpyAsync(base + w.tab, tab, (size_t)(n_phi / 8 + 1) * sizeof(float), cudaMemcpyHostToDevice, st);   // pageable source: staged before return
-
     BinArgs a;
     a.n_layers = geom->n_layers; a.n_phi = n_phi; a.n_z = n_z; a.n_seg = n_seg;
     a.hx = hits->x; a.hy = hits->y; a.hz = hits->z; a.seg_off = hits->seg_off_dev;
-    a.tan_tab = (const float*)(base + w.tab);
-    a.key = (int32_t*)(base + w.key); a.bin_off = out->bin_off; a.cursor = (int32_t*)(base + w.cursor); a.tmp = (int2*)(base + w.tmp);
+    a.kr = (int2*)(base + w.kr); a.bin_off = out->bin_off; a.tmp = (float4*)(base + w.tmp);
     a.sx = out->x; a.sy = out->y; a.sz = out->z; a.perm = out->perm; a.xyzp = (float4*)out->xyzp;
+    a.phi_scale = host_inv_dphi(n_phi);
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
         a.zmax[l] = y.zmax;
         a.inv_dz[l] = (float)n_z / (2.0f * y.zmax);      // one IEEE fp32 division of exact operands (X2)
     }
+    // X1 table: T[k] = fl32(tan(2 pi k / N)) evaluated in double on the host, T[N/8] = 1; travels as a kernel argument
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k = 0; k < n_phi / 8; ++k) a.tan_tab[k] = (float)std::tan(two_pi * (double)k / (double)n_phi);
+    a.tan_tab[n_phi / 8] = 1.0f;
+    for (int k = n_phi / 8 + 1; k < MAX_TAN_TAB; ++k) a.tan_tab[k] = 0.0f;
+
     cudaMemsetAsync(out->bin_off, 0, (size_t)(n_bins + 1) * sizeof(int32_t), st);
-    cudaMemsetAsync(a.cursor, 0, (size_t)n_bins * sizeof(int32_t), st);
     if (n_hits > 0) {
         const unsigned gx = (unsigned)std::min<int64_t>((max_seg + BIN_BLOCK - 1) / BIN_BLOCK, 4096);
         const dim3 grid(gx ? gx : 1, (unsigned)std::min(n_seg, 65535));
         kf_bin_count_kernel<<<grid, BIN_BLOCK, (size_t)(n_phi / 8 + 1) * sizeof(float), st>>>(a);
-        const int64_t n_scan = n_bins + 1;
-        const int n_tiles = (int)((n_scan + SCAN_TILE - 1) / SCAN_TILE);
-        int32_t* sums = (int32_t*)(base + w.sums);
-        kf_scan_tile_sums_kernel<<<n_tiles, BIN_BLOCK, 0, st>>>(out->bin_off, n_scan, sums);
-        kf_scan_sums_kernel<<<1, BIN_BLOCK, 0, st>>>(sums, n_tiles);
-        kf_scan_apply_kernel<<<n_tiles, BIN_BLOCK, 0, st>>>(out->bin_off, n_scan, sums);
+        kf_bin_scan_kernel<<<n_seg, SCAN_BLOCK, 0, st>>>(out->bin_off, hits->seg_off_dev, n_phi * n_z);
         kf_bin_scatter_kernel<<<grid, BIN_BLOCK, 0, st>>>(a);
-        kf_bin_place_kernel<<<(unsigned)((n_hits + BIN_BLOCK - 1) / BIN_BLOCK), BIN_BLOCK, 0, st>>>(a, n_hits);
+        const unsigned pb = (unsigned)((n_bins + BIN_BLOCK - 1) / BIN_BLOCK);
+        if (soa) kf_bin_place_kernel<true><<<pb, BIN_BLOCK, 0, st>>>(a, n_bins);
+        else kf_bin_place_kernel<false><<<pb, BIN_BLOCK, 0, st>>>(a, n_bins);
     }
     return check_launch("kf_bin_hits");
 }

@@ -6,17 +6,18 @@
 namespace kf {
 
 // X1: azimuthal bin from comparisons against the tangent table tab[k] = fl32(tan(2 pi k / n_phi)), k = 0..n_phi/8
-// (strictly increasing, tab[0] = 0): no atan2, hence no dependence on a math library.
-__device__ __forceinline__ int phi_bin(float x, float y, int n_phi, const float* __restrict__ tab) {
+// (strictly increasing, tab[0] = 0): no atan2 in the DEFINITION, hence no dependence on a math library -- the bin is
+// j = the largest k <= n_phi/8 - 1 with tab[k] <= t.  atanf only supplies the first guess of the search (scale =
+// n_phi / (2 pi)); the two correction loops make the result the defined one whatever the guess was.
+__device__ __forceinline__ int phi_bin(float x, float y, int n_phi, const float* __restrict__ tab, float scale) {
     const float ax = fabsf(x), ay = fabsf(y);
     const bool swap = ay > ax;
     const float lo = swap ? ax : ay, hi = swap ? ay : ax;
     const float t = hi > 0.0f ? __fdiv_rn(lo, hi) : 0.0f;
-    int j = 0, end = n_phi >> 3;                     // largest j in [0, n_phi/8 - 1] with tab[j] <= t
-    while (end - j > 1) {
-        const int mid = (j + end) >> 1;
-        if (tab[mid] <= t) j = mid; else end = mid;
-    }
+    const int m = n_phi >> 3;
+    int j = min(max((int)(atanf(t) * scale), 0), m - 1);
+    while (j > 0 && tab[j] > t) --j;
+    while (j + 1 < m && tab[j + 1] <= t) ++j;
     const int a = swap ? (n_phi >> 2) - 1 - j : j;
     if (x >= 0.0f) return (y >= 0.0f) ? a : n_phi - 1 - a;
     return (y >= 0.0f) ? (n_phi >> 1) - 1 - a : (n_phi >> 1) + a;
@@ -34,13 +35,17 @@ struct WindowBins { int first, n_b, iz_lo, iz_hi; };
 __device__ __forceinline__ WindowBins window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, float inv_dz,
                                                   float inv_dphi, int n_phi, int n_z) {
     WindowBins w;
-    const int b_lo = (int)floorf(__fmul_rn(__fsub_rn(phi_c, dphi), inv_dphi));
-    const int b_hi = (int)floorf(__fmul_rn(__fadd_rn(phi_c, dphi), inv_dphi));
-    int nb = b_hi - b_lo + 1;
-    nb = nb > n_phi ? n_phi : nb;
-    w.n_b = nb < 0 ? 0 : nb;
-    int f = b_lo % n_phi;
-    w.first = f < 0 ? f + n_phi : f;
+    if (!(__fmul_rn(dphi, inv_dphi) < (float)n_phi)) {      // half width of a full turn or more (or not a number): every bin, from bin 0
+        w.first = 0; w.n_b = n_phi;
+    } else {
+        const int b_lo = (int)floorf(__fmul_rn(__fsub_rn(phi_c, dphi), inv_dphi));
+        const int b_hi = (int)floorf(__fmul_rn(__fadd_rn(phi_c, dphi), inv_dphi));
+        int nb = b_hi - b_lo + 1;
+        nb = nb > n_phi ? n_phi : nb;
+        w.n_b = nb < 0 ? 0 : nb;
+        int f = b_lo % n_phi;
+        w.first = f < 0 ? f + n_phi : f;
+    }
     w.iz_lo = z_bin(__fsub_rn(z_c, dz), zmax, inv_dz, n_z);
     w.iz_hi = z_bin(__fadd_rn(z_c, dz), zmax, inv_dz, n_z);
     return w;

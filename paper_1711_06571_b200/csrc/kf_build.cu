@@ -13,13 +13,16 @@
 //   phase 2  thread per seed: K-way merge of the lists of its <= K parents over 48-bit keys whose integer order is
 //            the total order R10 -> the best K children (B4); block scan of the child counts -> dense child positions
 //   phase 3  thread per surviving child (build_child): Kalman update (B5), per-layer link (parent slot, hit)
-// Candidate records (33 words: 6 parameters, 21 packed covariance elements, carried sin/cos, chi2, meta; stored as 9
-// groups of four) live in a block-private global workspace that stays L2-resident: record c of the current layer
-// at a DENSE index (seed offset + slot), group-of-four-major over the index, so every record moves with 9 coalesced
-// 16-byte accesses.  Two buffers: A (updated states) and B (predicted states).  When the tile has more live candidates
-// than the list area holds, the seeds are taken in rounds.  At the end the links are traced back into hit lists and
-// stored SoA, one thread per live candidate (B6).  The three per-thread bodies are separate (not inlined) functions:
-// inlined they need 228 registers and spill 480 bytes at the 128 the launch bounds allow.
+// Candidate records (33 words: 6 parameters -- phi as a fixed-point angle --, 21 packed covariance elements, carried
+// sin/cos, chi2, meta; stored as 9 groups of four) live in a block-private global workspace that stays L2-resident:
+// record c of the current layer at a DENSE index (seed offset + slot), group-of-four-major over the index, so every
+// record moves with 9 coalesced 16-byte accesses.  Two buffers: A (updated states) and B (predicted states).  When the
+// tile has more live candidates than the list area holds, the seeds are taken in rounds.  At the end the links are
+// traced back into hit lists and stored SoA, one thread per live candidate (B6).  The three per-thread bodies are
+// separate (not inlined) functions: inlined they need 228 registers and spill 480 bytes at the 128 the launch bounds
+// allow.  All warps of a block run the same phase at the same time, which also keeps them in the same ~30 KB of code:
+// a warp-per-tile variant without block barriers (every warp in its own phase) spent a third of its issue slots waiting
+// for instructions (32 KB L1.5 instruction cache; profiles/r03_build.md).
 #include <algorithm>
 #include "kf_common.cuh"
 #include "kf_state.cuh"
@@ -47,7 +50,7 @@ struct BuildArgs {
     int32_t n_layers, first_layer, K, n_phi, n_z, S, ncap;
     float kb, chi2_cut, n_sigma, inv_dphi;
     int64_t n_seeds, ld_seed, ld_out, n_tiles;
-    const float *par, *cov; const int8_t* q;
+    const float *par, *cov, *chi2_in; const int8_t* q;
     const int32_t *seed_event, *seed_hit_idx;
     const float4* xyzp; const int32_t* bin_off;
     float *par_o, *cov_o, *chi2_o; int8_t* q_o; int32_t* nhits_o; uint32_t* status_o; int32_t *hit_idx_o, *n_cand_o;
@@ -69,7 +72,7 @@ __device__ __forceinline__ void rec_load(State& s, float& chi2, int& meta, const
         const float4 t = __ldcg(b4 + g * SK + c);
         v[4 * g] = t.x; v[4 * g + 1] = t.y; v[4 * g + 2] = t.z; v[4 * g + 3] = t.w;
     }
-    state_set(s, [&](int i) { return v[i]; }, [&](int k) { return v[6 + k]; });
+    state_set<true>(s, [&](int i) { return v[i]; }, [&](int k) { return v[6 + k]; });
     s.CC = f2(v[W_TRIG + 0], v[W_TRIG + 2]);
     s.SS = f2(v[W_TRIG + 1], v[W_TRIG + 3]);
     chi2 = v[W_CHI2];
@@ -177,198 +180,180 @@ __host__ __device__ inline BuildSmem build_smem(int S, int K, int ncap, int L) {
     return m;
 }
 
-#ifdef KF_BUILD_TIMING
-__device__ unsigned long long g_build_timing[16];
-#define KF_TICK(i) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_build_timing[i], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
-#else
-#define KF_TICK(i) do { } while (0)
-#endif
-#ifdef KF_BUILD_TIMING
-#define KF_CTICK(i) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_build_timing[i], (unsigned long long)(now_ - ctick_)); ctick_ = now_; } } while (0)
-#define KF_CTICK_INIT long long ctick_ = clock64()
-#else
-#define KF_CTICK(i) do { } while (0)
-#define KF_CTICK_INIT do { } while (0)
-#endif
-
-// per-block context: sizes, workspace and shared-memory arrays (built once, passed by reference to the phase bodies)
+// per-block context: sizes and workspace.  Re-derived inside every phase body from the kernel arguments (constant bank)
+// and the block index: passed by reference it would live in local memory, whose loads miss the small L1 left beside the
+// shared-memory carve-out.
 struct Tile {
     int S, K, L, ncap, SK;
     float *recA, *recB; int32_t* link_hit;
 };
+__device__ __forceinline__ Tile tile_of(const BuildArgs& a) {
+    Tile T;
+    T.S = a.S; T.K = a.K; T.L = a.n_layers; T.ncap = a.ncap; T.SK = a.S * a.K;
+    T.recA = a.ws_rec + (size_t)blockIdx.x * 2 * (4 * NREC4) * T.SK;
+    T.recB = T.recA + (size_t)(4 * NREC4) * T.SK;
+    T.link_hit = a.ws_link_hit + (size_t)blockIdx.x * T.L * T.SK;
+    return T;
+}
 
 // The three per-thread bodies are separate functions (not inlined) so that each gets its own register allocation:
 // inlined into one kernel they need 228 registers and spill ~480 bytes at the 128 the launch bounds allow.
 
 // phase 1, one live candidate: dense index base + i, round-local index i
 template <bool ISO>
-__device__ __noinline__ void build_candidate(const BuildArgs& a, const Tile& T, int l, int base, int i, int64_t s0) {
+__device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base, int i, int64_t s0) {
+    const Tile T = tile_of(a);
     // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
     extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
     const BuildSmem m = build_smem(T.S, K, ncap, L);
     float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
-    int32_t* link_hit = T.link_hit; uint8_t* link_par = smem + m.link_par;
-    int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off); int* s_offn = (int*)(smem + m.offn);
-    float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit); int* sel_pk = (int*)(smem + m.sel_pk);
-    unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
+    const unsigned short* s_cseed = (const unsigned short*)(smem + m.cseed);
     float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
-    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
+    unsigned char* s_lcnt = smem + m.l_cnt;
     float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
-    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
-    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
     const LayerC& ly = a.layer[l];
-                    const int c = base + i;
-                        const int64_t sg = s0 + s_cseed[c];
-                        const float cw = -(float)a.q[sg] * a.kb;
-                        const int ev = a.seed_event ? a.seed_event[sg] : 0;
-                        KF_CTICK_INIT;
-                        State st;
-                        float chi2;
-                        int meta;
-                        rec_load(st, chi2, meta, recA, SK, c);
-                        KF_CTICK(8);
-                        uint32_t flag = 0u;
-                        bool fin = (meta & 256) != 0;
-                        float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
-                        float c00 = 0.f, c10 = 0.f, c11 = 0.f, c20 = 0.f, c21 = 0.f, c22 = 0.f;
-                        Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                        bool fok = false;
-                        WindowBins wb = {0, 0, 0, -1};
-                        if (!fin) {
-                            flag = predict(st, cw, ly);
-                            if (!flag) {
-                                px = st.XY.x; py = st.XY.y; pz = st.ZP.x;
-                                c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
-                                const float r2 = fmaf(px, px, py * py);
-                                const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
-                                const float varphi = fmaxf(num / (r2 * r2), 0.0f);
-                                const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
-                                dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
-                                if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
-                                else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
-                                else {
-                                    thr2 = dphi * dphi * r2;
-                                    wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
-                                    if (ISO) {
-                                        Sym3 Sm;
-                                        Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
-                                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
-                                        fok = ldl3(Sm, F);
-                                    }
-                                }
-                            }
-                            fin = flag != 0u;
+    const int c = base + i;
+    const int64_t sg = s0 + s_cseed[c];
+    const float cw = -(float)a.q[sg] * a.kb;
+    const int ev = a.seed_event ? a.seed_event[sg] : 0;
+    State st;
+    float chi2;
+    int meta;
+    rec_load(st, chi2, meta, recA, SK, c);
+    uint32_t flag = 0u;
+    bool fin = (meta & 256) != 0;
+    float px = 0.f, py = 0.f, pz = 0.f, thr2 = 0.f, dzw = 0.f;
+    float c00 = 0.f, c10 = 0.f, c11 = 0.f, c20 = 0.f, c21 = 0.f, c22 = 0.f;
+    Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    bool fok = false;
+    WindowBins wb = {0, 0, 0, -1};
+    if (!fin) {
+        flag = predict(st, cw, ly);
+        if (!flag) {
+            px = st.XY.x; py = st.XY.y; pz = st.Z;
+            c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
+            const float r2 = fmaf(px, px, py * py);
+            const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
+            const float varphi = fmaxf(num / (r2 * r2), 0.0f);
+            const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
+            dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+            if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
+            else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
+            else {
+                thr2 = dphi * dphi * r2;
+                wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+                if (ISO) {
+                    Sym3 Sm;
+                    Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
+                    Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
+                    fok = ldl3(Sm, F);
+                }
+            }
+        }
+        fin = flag != 0u;
+    }
+    int cnt = 0;
+    if (!fin) {
+        rec_store(st, chi2, meta, recB, SK, c);
+        // ---- window scan (B3) ----
+        bool sbad = false;
+        float* lc = s_lchi2 + i;
+        int* lh = s_lhit + i;
+        const int64_t seg = (int64_t)ev * L + l;
+        // Both runs of a row (the window may wrap at phi = pi) are scanned as one range.  Memory round
+        // trips are what this loop costs (the hits are cold): the four bin offsets of the NEXT row are
+        // requested before the hits of the current row, and SCAN_BATCH hits are requested together.
+        const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
+        const int32_t* bo = a.bin_off + (seg * a.n_z + wb.iz_lo) * a.n_phi;
+        int h0a = 0, h1a = 0, h0b = 0, h1b = 0;
+        if (wb.iz_lo <= wb.iz_hi) { h0a = __ldg(bo + wb.first); h1a = __ldg(bo + e0); h0b = __ldg(bo); h1b = __ldg(bo + e1); }
+        for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
+            bo += a.n_phi;
+            int n0a = 0, n1a = 0, n0b = 0, n1b = 0;
+            if (iz < wb.iz_hi) { n0a = __ldg(bo + wb.first); n1a = __ldg(bo + e0); n0b = __ldg(bo); n1b = __ldg(bo + e1); }
+            const int na = h1a - h0a, nab = na + (h1b - h0b);
+            {
+                for (int t0 = 0; t0 < nab; t0 += SCAN_BATCH) {
+                    float4 hv[SCAN_BATCH];
+                    int hpos[SCAN_BATCH];
+#pragma unroll
+                    for (int u = 0; u < SCAN_BATCH; ++u) {
+                        const int t = min(t0 + u, nab - 1);
+                        hpos[u] = t < na ? h0a + t : h0b + (t - na);
+                        hv[u] = __ldg(a.xyzp + hpos[u]);
+                    }
+                    // window test of the batch (cheap, branch-free) -> bit mask; chi2 and the list only for the
+                    // few hits inside the window, one at a time
+                    unsigned inside = 0u;
+#pragma unroll
+                    for (int u = 0; u < SCAN_BATCH; ++u) {
+                        const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
+                        const float cr = fmaf(px, my, -py * mx);
+                        const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                            (fabsf(mz - pz) <= dzw);
+                        inside |= in_win ? (1u << u) : 0u;
+                    }
+                    while (inside) {
+                        const int u = __ffs(inside) - 1;
+                        inside &= inside - 1u;
+                        float4 m4 = hv[0];
+                        int h = hpos[0];
+#pragma unroll
+                        for (int v = 1; v < SCAN_BATCH; ++v)
+                            if (u == v) { m4 = hv[v]; h = hpos[v]; }
+                        const float mx = m4.x, my = m4.y, mz = m4.z;
+                        bool ok = fok;
+                        if (!ISO) {
+                            const HitCov V = hit_cov(mx, my, ly);
+                            Sym3 Sm;
+                            Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
+                            Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
+                            ok = ldl3(Sm, F);
                         }
-                        int cnt = 0;
-                        if (!fin) {
-                            KF_CTICK(9);
-                            rec_store(st, chi2, meta, recB, SK, c);
-                            KF_CTICK(10);
-                            // ---- window scan (B3) ----
-                            bool sbad = false;
-                            float* lc = s_lchi2 + i;
-                            int* lh = s_lhit + i;
-                            const int64_t seg = (int64_t)ev * L + l;
-                            // Both runs of a row (the window may wrap at phi = pi) are scanned as one range.  Memory round
-                            // trips are what this loop costs (the hits are cold): the four bin offsets of the NEXT row are
-                            // requested before the hits of the current row, and SCAN_BATCH hits are requested together.
-                            const int e0 = min(wb.first + wb.n_b, a.n_phi), e1 = max(wb.first + wb.n_b - a.n_phi, 0);
-                            const int32_t* bo = a.bin_off + (seg * a.n_z + wb.iz_lo) * a.n_phi;
-                            int h0a = 0, h1a = 0, h0b = 0, h1b = 0;
-                            if (wb.iz_lo <= wb.iz_hi) { h0a = __ldg(bo + wb.first); h1a = __ldg(bo + e0); h0b = __ldg(bo); h1b = __ldg(bo + e1); }
-                            for (int iz = wb.iz_lo; iz <= wb.iz_hi; ++iz) {
-                                bo += a.n_phi;
-                                int n0a = 0, n1a = 0, n0b = 0, n1b = 0;
-                                if (iz < wb.iz_hi) { n0a = __ldg(bo + wb.first); n1a = __ldg(bo + e0); n0b = __ldg(bo); n1b = __ldg(bo + e1); }
-                                const int na = h1a - h0a, nab = na + (h1b - h0b);
-                                {
-                                    for (int t0 = 0; t0 < nab; t0 += SCAN_BATCH) {
-                                        float4 hv[SCAN_BATCH];
-                                        int hpos[SCAN_BATCH];
-    #pragma unroll
-                                        for (int u = 0; u < SCAN_BATCH; ++u) {
-                                            const int t = min(t0 + u, nab - 1);
-                                            hpos[u] = t < na ? h0a + t : h0b + (t - na);
-                                            hv[u] = __ldg(a.xyzp + hpos[u]);
-                                        }
-                                        // window test of the batch (cheap, branch-free) -> bit mask; chi2 and the list only for the
-                                        // few hits inside the window, one at a time
-                                        unsigned inside = 0u;
-#pragma unroll
-                                        for (int u = 0; u < SCAN_BATCH; ++u) {
-                                            const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
-                                            const float cr = fmaf(px, my, -py * mx);
-                                            const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
-                                                                (fabsf(mz - pz) <= dzw);
-                                            inside |= in_win ? (1u << u) : 0u;
-                                        }
-                                        while (inside) {
-                                            const int u = __ffs(inside) - 1;
-                                            inside &= inside - 1u;
-                                            float4 m4 = hv[0];
-                                            int h = hpos[0];
-#pragma unroll
-                                            for (int v = 1; v < SCAN_BATCH; ++v)
-                                                if (u == v) { m4 = hv[v]; h = hpos[v]; }
-                                            const float mx = m4.x, my = m4.y, mz = m4.z;
-                                            bool ok = fok;
-                                            if (!ISO) {
-                                                const HitCov V = hit_cov(mx, my, ly);
-                                                Sym3 Sm;
-                                                Sm.m00 = c00 + V.xx; Sm.m10 = c10 + V.xy; Sm.m11 = c11 + V.yy;
-                                                Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + V.zz;
-                                                ok = ldl3(Sm, F);
-                                            }
-                                            if (!ok) { sbad = true; continue; }
-                                            const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
-                                            const float y1 = fmaf(-F.l10, q0, q1);
-                                            const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
-                                            const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
-                                            if (c2 < a.chi2_cut) {
-                                                if (cnt < K) {           // unsorted append
-                                                    lc[cnt * ncap] = chi2 + c2; lh[cnt * ncap] = h; ++cnt;
-                                                } else {
-                                                    list_replace_worst(lc, lh, ncap, K, chi2 + c2, h);
-                                                }
-                                            }
-                                        }
-                                    }
-                                }
-                                h0a = n0a; h1a = n1a; h0b = n0b; h1b = n1b;
-                            }
-                            list_sort(lc, lh, ncap, cnt);
-                            if (sbad) {      // S not positive definite: one finished child with the unchanged state
-                                fin = true;
-                                flag = ST_NUMERIC;
-                                cnt = 0;
+                        if (!ok) { sbad = true; continue; }
+                        const float q0 = mx - px, q1 = my - py, q2 = mz - pz;
+                        const float y1 = fmaf(-F.l10, q0, q1);
+                        const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, q0, q2));
+                        const float c2 = fmaf(q0 * q0, F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
+                        if (c2 < a.chi2_cut) {
+                            if (cnt < K) {           // unsorted append
+                                lc[cnt * ncap] = chi2 + c2; lh[cnt * ncap] = h; ++cnt;
+                            } else {
+                                list_replace_worst(lc, lh, ncap, K, chi2 + c2, h);
                             }
                         }
-                        KF_CTICK(11);
-                        if (fin) rec_copy(recA, c, recB, c, SK);
-                        s_lcnt[i] = (unsigned char)cnt;
-                        s_pchi2[i] = chi2;
-                        s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
-                        KF_CTICK(12);
+                    }
+                }
+            }
+            h0a = n0a; h1a = n1a; h0b = n0b; h1b = n1b;
+        }
+        list_sort(lc, lh, ncap, cnt);
+        if (sbad) {      // S not positive definite: one finished child with the unchanged state
+            fin = true;
+            flag = ST_NUMERIC;
+            cnt = 0;
+        }
+    }
+    if (fin) rec_copy(recA, c, recB, c, SK);
+    s_lcnt[i] = (unsigned char)cnt;
+    s_pchi2[i] = chi2;
+    s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
 }
 
 // phase 3, one surviving child: dense index cn among the children of the tile
 template <bool ISO>
-__device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int l, int cn) {
+__device__ __noinline__ void build_child(const BuildArgs& a, int l, int cn) {
+    const Tile T = tile_of(a);
     // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
     extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, ncap = T.ncap, SK = T.SK;
     const BuildSmem m = build_smem(T.S, K, ncap, L);
     float* __restrict__ recA = T.recA; float* __restrict__ recB = T.recB;
     int32_t* link_hit = T.link_hit; uint8_t* link_par = smem + m.link_par;
-    int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off); int* s_offn = (int*)(smem + m.offn);
-    float* sel_chi2 = (float*)(smem + m.sel_chi2); int* sel_hit = (int*)(smem + m.sel_hit); int* sel_pk = (int*)(smem + m.sel_pk);
-    unsigned short* s_cseed = (unsigned short*)(smem + m.cseed);
-    float* s_lchi2 = (float*)(smem + m.l_chi2); int* s_lhit = (int*)(smem + m.l_hit);
-    unsigned char* s_lcnt = smem + m.l_cnt; unsigned char* s_lhead = smem + m.l_head;
-    float* s_pchi2 = (float*)(smem + m.p_chi2); int* s_pinfo = (int*)(smem + m.p_info);
-    (void)K; (void)L; (void)ncap; (void)SK; (void)recA; (void)recB; (void)link_hit; (void)link_par; (void)s_nc; (void)s_off; (void)s_offn;
-    (void)sel_chi2; (void)sel_hit; (void)sel_pk; (void)s_cseed; (void)s_lchi2; (void)s_lhit; (void)s_lcnt; (void)s_lhead; (void)s_pchi2; (void)s_pinfo;
+    const int* s_off = (const int*)(smem + m.off); const int* s_offn = (const int*)(smem + m.offn);
+    const float* sel_chi2 = (const float*)(smem + m.sel_chi2); const int* sel_hit = (const int*)(smem + m.sel_hit); const int* sel_pk = (const int*)(smem + m.sel_pk);
+    const unsigned short* s_cseed = (const unsigned short*)(smem + m.cseed);
     const LayerC& ly = a.layer[l];
     const int s = s_cseed[cn];
     const int j = cn - s_offn[s];
@@ -392,7 +377,7 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
         int meta;
         rec_load(st, chi2p, meta, recB, SK, cp);
         const float4 hv = __ldg(a.xyzp + hitpos);
-            const float mx = hv.x, my = hv.y, mz = hv.z;
+        const float mx = hv.x, my = hv.y, mz = hv.z;
         HitCov V;
         if (ISO) { V.xx = ly.var_r; V.yy = ly.var_r; V.xy = 0.0f; V.zz = ly.var_z; }
         else V = hit_cov(mx, my, ly);
@@ -415,7 +400,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, const Tile& T, int 
 }
 
 // B6, one live candidate (dense index c) -> its output slot; unused slots are filled by the caller
-__device__ __noinline__ void build_output(const BuildArgs& a, const Tile& T, int64_t s0, int c) {
+__device__ __noinline__ void build_output(const BuildArgs& a, int64_t s0, int c) {
+    const Tile T = tile_of(a);
     extern __shared__ __align__(16) unsigned char smem[];
     const int K = T.K, L = T.L, SK = T.SK;
     const BuildSmem m = build_smem(T.S, K, T.ncap, L);
@@ -475,17 +461,8 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     int* s_misc = (int*)(smem + m.misc);          // [0..31] warp sums of the scan, [32] round end
     const int tid = threadIdx.x;
 
-    float* recA = a.ws_rec + (size_t)blockIdx.x * 2 * (4 * NREC4) * SK;
-    float* recB = recA + (size_t)(4 * NREC4) * SK;
-    int32_t* link_hit = a.ws_link_hit + (size_t)blockIdx.x * L * SK;
-    uint8_t* link_par = smem + m.link_par;
-    Tile T;
-    T.S = S; T.K = K; T.L = L; T.ncap = ncap; T.SK = SK;
-    T.recA = recA; T.recB = recB; T.link_hit = link_hit;
+    float* recA = tile_of(a).recA;
 
-#ifdef KF_BUILD_TIMING
-    long long tick_ = clock64();
-#endif
     for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t s0 = tile * S;
         const int ns = (int)min((int64_t)S, a.n_seeds - s0);
@@ -495,7 +472,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 const int64_t sg = s0 + tid;
                 State st;
                 state_load(st, [&](int i) { return a.par[(int64_t)i * a.ld_seed + sg]; }, [&](int k) { return a.cov[(int64_t)k * a.ld_seed + sg]; });
-                rec_store(st, 0.0f, a.first_layer, recA, SK, tid);
+                rec_store(st, a.chi2_in ? a.chi2_in[sg] : 0.0f, a.first_layer, recA, SK, tid);
             }
             s_nc[tid] = tid < ns ? 1 : 0;
             s_off[tid] = tid < ns ? tid : ns;
@@ -503,7 +480,6 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
         }
         if (tid == 0) s_off[S] = ns;
         __syncthreads();
-        KF_TICK(0);
 
         for (int l = a.first_layer; l < L; ++l) {
             const LayerC& ly = a.layer[l];
@@ -524,10 +500,9 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 const int nround = s_off[r1] - base;
                 // ---------------- phase 1: predict + window + scan, thread per candidate ----------------
                 for (int i = tid; i < nround; i += NT) {
-                    build_candidate<ISO>(a, T, l, base, i, s0);
+                    build_candidate<ISO>(a, l, base, i, s0);
                 }
                 __syncthreads();
-                KF_TICK(1);
                 // ---------------- phase 2: best K children of a seed (B4), thread per seed ----------------
                 // K-way merge of the sorted child lists of the <= K parents.  The head of every list is a 48-bit key whose
                 // integer order is the total order R10: (63 - nhits) | chi2 bits (chi2 >= 0, so the bit pattern is
@@ -557,7 +532,6 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                     s_nnew[s] = n_out;
                 }
                 __syncthreads();
-                KF_TICK(2);
                 r0 = r1;
             }
             // ---------------- dense positions of the children ----------------
@@ -570,22 +544,20 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 for (int j = 0; j < v; ++j) s_cseed[ex + j] = (unsigned short)tid;
                 __syncthreads();
             }
-            KF_TICK(3);
             // ---------------- phase 3: update the survivors, thread per child (B5) ----------------
             const int nchild = s_offn[S];
             for (int cn = tid; cn < nchild; cn += NT) {
-                build_child<ISO>(a, T, l, cn);
+                build_child<ISO>(a, l, cn);
             }
             __syncthreads();
             if (tid < S) { s_nc[tid] = tid < ns ? s_nnew[tid] : 0; s_off[tid] = s_offn[tid]; }
             if (tid == 0) s_off[S] = s_offn[S];
             __syncthreads();
-            KF_TICK(4);
         }
 
         // ---------------- B6: back-trace + store ----------------
         if (tid < ns) a.n_cand_o[s0 + tid] = s_nc[tid];
-        for (int c = tid; c < s_off[ns]; c += NT) build_output(a, T, s0, c);       // live candidates, densely
+        for (int c = tid; c < s_off[ns]; c += NT) build_output(a, s0, c);       // live candidates, densely
         for (int idx = tid; idx < ns * K; idx += NT) {                            // every slot: charge; unused slots: empty
             const int s = idx / K, j = idx - s * K;
             const int64_t slot = (s0 + s) * K + j;
@@ -596,13 +568,10 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
             }
         }
         __syncthreads();     // the workspace and the shared arrays are reused by the next tile
-        KF_TICK(5);
     }
 }
 
 // ---- host side: tile size, grid and workspace layout (one function, used by the size query and by the launch) ----
-static int g_build_tile = 0;   // 0 = default
-
 static int sm_count() {
     static int n = 0;
     if (n == 0) {
@@ -615,22 +584,32 @@ static int sm_count() {
     return n;
 }
 
-struct BuildPlan { int S, NT, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o_lh, total; };
+struct BuildPlan { int S, NT, ncap, grid; int64_t n_tiles; size_t smem, o_rec, o_lh, total; bool ok; };
 
-static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K) {
+static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K, const kf_options* opt) {
     BuildPlan p;
-    int S = g_build_tile;
-    if (S == 0)      // one wave of 128-seed tiles when the job is that small (latency-sized), otherwise small tiles: more
+    int S = KF_OPT(opt, build_seeds_per_block);
+    const int max_blocks = KF_OPT(opt, build_max_blocks);
+    p.ok = (S == 0 || (S >= 16 && S <= BUILD_MAX_NT && S % 16 == 0)) && max_blocks >= 0;
+    if (!p.ok) S = 0;
+    const bool automatic = S == 0;
+    if (automatic)   // one wave of 128-seed tiles when the job is that small (latency-sized), otherwise small tiles: more
                      // independent blocks per SM, so that the block-level barriers of one tile overlap work of another
         S = n_seeds <= (int64_t)128 * 2 * sm_count() ? 128 : 32;
-    p.S = S;
-    p.NT = S * KF_BUILD_TPS <= 64 ? 64 : (S * KF_BUILD_TPS <= 128 ? 128 : 256);
-    const int SK = S * K;
-    p.ncap = std::min(SK, std::max(std::max(K, 32), (LIST_BYTES_PER_THREAD * p.NT / (8 * K)) & ~31));
-    p.n_tiles = (n_seeds + S - 1) / S;
-    p.smem = (size_t)build_smem(S, K, p.ncap, n_layers).total;
+    for (;;) {
+        p.S = S;
+        p.NT = S * KF_BUILD_TPS <= 64 ? 64 : (S * KF_BUILD_TPS <= 128 ? 128 : 256);
+        const int SK = S * K;
+        p.ncap = std::min(SK, std::max(std::max(K, 32), (LIST_BYTES_PER_THREAD * p.NT / (8 * K)) & ~31));
+        p.smem = (size_t)build_smem(S, K, p.ncap, n_layers).total;
+        if (!automatic || p.smem <= 200 * 1024 || S <= 16) break;      // large K and many layers: a smaller tile fits
+        S /= 2;
+    }
+    const int SK = p.S * K;
+    p.n_tiles = (n_seeds + p.S - 1) / p.S;
     const int by_smem = (int)std::max<size_t>(1, (size_t)(227 * 1024) / (p.smem + 1024));
-    const int resident = sm_count() * std::min(BUILD_THREADS_PER_SM / p.NT, by_smem);
+    int64_t resident = (int64_t)sm_count() * std::min(BUILD_THREADS_PER_SM / p.NT, by_smem);
+    if (max_blocks > 0) resident = std::min<int64_t>(resident, max_blocks);
     p.grid = (int)std::min<int64_t>(std::max<int64_t>(p.n_tiles, 1), resident);
     auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
     size_t o = 0;
@@ -652,30 +631,15 @@ static int launch_build(const BuildArgs& a, const BuildPlan& p, bool iso, cudaSt
 
 }  // namespace kf
 
-#ifdef KF_BUILD_TIMING
-extern "C" void kf_build_timing(unsigned long long* out, int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out, kf::g_build_timing, sizeof(unsigned long long) * 16);
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(kf::g_build_timing, z, sizeof z); }
-}
-#endif
-
-extern "C" size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K) {
+extern "C" size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K, const kf_options* opt) {
     if (!geom || geom->n_layers < 1 || geom->n_layers > KF_MAX_LAYERS || n_seeds < 0 || K < 1 || K > 32) return 0;
-    return kf::build_plan(geom->n_layers, n_seeds, K).total;
-}
-
-// tuning / test hook: seeds per block (16..256, multiple of 16; 0 = automatic).  The result does not depend on it.
-extern "C" int kf_build_set_tile(int32_t seeds_per_block) {
-    if (seeds_per_block != 0 && (seeds_per_block < 16 || seeds_per_block > kf::BUILD_MAX_NT || seeds_per_block % 16))
-        return kf::fail(KF_ERR_INVALID_ARG, "kf_build_set_tile: %d not 0 or a multiple of 16 in 16..256", seeds_per_block);
-    kf::g_build_tile = seeds_per_block;
-    return KF_OK;
+    const kf::BuildPlan p = kf::build_plan(geom->n_layers, n_seeds, K, opt);
+    return p.ok ? p.total : 0;
 }
 
 extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
                         const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,
-                        float n_sigma, kf_cands* out, void* ws, size_t ws_bytes, void* stream) {
+                        float n_sigma, kf_cands* out, const kf_options* opt, void* ws, size_t ws_bytes, void* stream) {
     using namespace kf;
     if (!geom || !hits || !binned || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_build: NULL struct argument");
     int rc = check_geom(geom, "kf_build");
@@ -686,6 +650,8 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     if (seeds->n < 0 || seeds->ld < seeds->n) return fail(KF_ERR_INVALID_ARG, "kf_build: need 0 <= n <= ld for the seeds");
     if (out->ld < seeds->n * K || out->cand.ld != out->ld) return fail(KF_ERR_INVALID_ARG, "kf_build: out->ld must be >= n_seeds*K and equal cand.ld");
     if (binned->n_phi < 8 || (binned->n_phi % 8) || binned->n_z < 1) return fail(KF_ERR_BAD_GEOM, "kf_build: bad bin counts");
+    const BuildPlan p = build_plan(geom->n_layers, seeds->n, K, opt);
+    if (!p.ok) return fail(KF_ERR_INVALID_ARG, "kf_build: options out of range (build_seeds_per_block: 0 or a multiple of 16 in 16..256; build_max_blocks >= 0)");
     out->K = K; out->n_layers = geom->n_layers; out->n_seeds = seeds->n; out->cand.n = seeds->n * K;
     if (seeds->n == 0) return KF_OK;
     if (!seeds->par || !seeds->cov || !seeds->q) return fail(KF_ERR_NULL_PTR, "kf_build: NULL seed array");
@@ -694,7 +660,6 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     const kf_tracks& c = out->cand;
     if (!c.par || !c.cov || !c.q || !c.chi2 || !c.nhits || !c.status || !out->hit_idx || !out->n_cand)
         return fail(KF_ERR_NULL_PTR, "kf_build: NULL output array");
-    const BuildPlan p = build_plan(geom->n_layers, seeds->n, K);
     if (!ws || ws_bytes < p.total) return fail(KF_ERR_WORKSPACE_TOO_SMALL, "kf_build: workspace %zu < %zu bytes", ws_bytes, p.total);
     if (p.smem > 227 * 1024) return fail(KF_ERR_INVALID_ARG, "kf_build: tile of %d seeds with K = %d needs %zu bytes of shared memory (> 227 KB)", p.S, K, p.smem);
     BuildArgs a;
@@ -702,7 +667,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     a.S = p.S; a.ncap = p.ncap; a.n_tiles = p.n_tiles;
     a.kb = KCURV * geom->bz_tesla; a.chi2_cut = chi2_cut; a.n_sigma = n_sigma; a.inv_dphi = host_inv_dphi(binned->n_phi);
     a.n_seeds = seeds->n; a.ld_seed = seeds->ld; a.ld_out = out->ld;
-    a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q; a.seed_event = seed_event; a.seed_hit_idx = seed_hit_idx;
+    a.par = seeds->par; a.cov = seeds->cov; a.chi2_in = seeds->chi2; a.q = seeds->q; a.seed_event = seed_event; a.seed_hit_idx = seed_hit_idx;
     a.xyzp = (const float4*)binned->xyzp; a.bin_off = binned->bin_off;
     a.par_o = c.par; a.cov_o = c.cov; a.chi2_o = c.chi2; a.q_o = c.q; a.nhits_o = c.nhits; a.status_o = c.status;
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;

@@ -1,6 +1,7 @@
 // kf_common.cuh -- host-side plumbing shared by the entry points: error reporting, geometry checks.
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 #include "../../include/kf.h"
 #include "kf_math.cuh"
@@ -10,6 +11,13 @@ namespace kf {
 int fail(int code, const char* fmt, ...);              // records the message for kf_last_error(), returns code
 int check_launch(const char* what);                    // cudaGetLastError() -> KF_OK / KF_ERR_CUDA
 int check_geom(const kf_geom* g, const char* who);
+
+// field of the caller's kf_options; 0 (= automatic) when opt is NULL or the caller's struct is older than the field
+inline int32_t opt_get(const kf_options* o, size_t offset) {
+    if (!o || o->size < offset + sizeof(int32_t)) return 0;
+    return *(const int32_t*)((const char*)o + offset);
+}
+#define KF_OPT(o, field) kf::opt_get(o, offsetof(kf_options, field))
 
 inline LayerC make_layer(const kf_layer& l) {
     LayerC c;

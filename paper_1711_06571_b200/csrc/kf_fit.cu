@@ -53,11 +53,13 @@ __device__ __forceinline__ int fit_layers(const FitArgs& a, int64_t t, float cw,
         int64_t idx = t;
         if (IDX) {
             idx = a.hit_idx[l * a.ld_idx + t];
-            if (idx < 0) continue;           // layer skipped entirely (R8)
+            if (idx < -1) continue;          // layer not crossed: skipped entirely (R8)
         }
+        const bool hole = IDX && idx < 0;    // -1: crossed without a hit -> transport + material, no update (R8)
         // F6: issued before the arithmetic
-        float mx, my, mz;
-        if (EVT) {
+        float mx = 0.f, my = 0.f, mz = 0.f;
+        if (hole) {
+        } else if (EVT) {
             const int64_t h = a.seg_off_dev[seg + l] + idx;
             mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
         } else {
@@ -74,6 +76,7 @@ __device__ __forceinline__ int fit_layers(const FitArgs& a, int64_t t, float cw,
             st |= flag;
             break;
         }
+        if (hole) continue;
         Ldl3 Si;
         float r[3], c2;
         HitCov V;
@@ -201,8 +204,6 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_PAIR_MINB) kf_fit_pair_kernel(co
     *reinterpret_cast<uint2*>(a.status_o + t) = make_uint2(0u, 0u);
 }
 
-static int g_fit_pairs = 1;   // 1 = two tracks per thread where the arguments allow it, 0 = never (test hook)
-
 template <bool IDX, bool EVT>
 static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t st) {
     if (iso) kf_fit_kernel<IDX, EVT, true><<<blocks, FIT_BLOCK, 0, st>>>(a);
@@ -211,15 +212,8 @@ static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t
 
 }  // namespace kf
 
-// test / tuning hook: 1 = two tracks per thread where the arguments allow it (default), 0 = always one track per thread
-extern "C" int kf_fit_set_pairs(int32_t enable) {
-    if (enable != 0 && enable != 1) return kf::fail(KF_ERR_INVALID_ARG, "kf_fit_set_pairs: %d not 0 or 1", enable);
-    kf::g_fit_pairs = enable;
-    return KF_OK;
-}
-
 extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, const int32_t* trk_event,
-                      const kf_tracks* seeds, kf_tracks* out, void* stream) {
+                      const kf_tracks* seeds, kf_tracks* out, const kf_options* opt, void* stream) {
     using namespace kf;
     if (!geom || !hits || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_fit: NULL struct argument");
     int rc = check_geom(geom, "kf_fit");
@@ -232,6 +226,9 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     if (!hits->x || !hits->y || !hits->z || !hits->seg_off) return fail(KF_ERR_NULL_PTR, "kf_fit: NULL hit array");
     if (hits->n_events < 1) return fail(KF_ERR_INVALID_ARG, "kf_fit: n_events < 1");
     if (trk_event && !hits->seg_off_dev) return fail(KF_ERR_NULL_PTR, "kf_fit: trk_event given but hits->seg_off_dev is NULL");
+    if (trk_event && !hit_idx) return fail(KF_ERR_INVALID_ARG, "kf_fit: identity indexing (hit_idx == NULL) needs trk_event == NULL");
+    const int tpt = KF_OPT(opt, fit_tracks_per_thread);
+    if (tpt < 0 || tpt > 2) return fail(KF_ERR_INVALID_ARG, "kf_fit: options: fit_tracks_per_thread = %d not 0, 1 or 2", tpt);
     FitArgs a;
     a.n_layers = geom->n_layers; a.n_events = hits->n_events;
     a.kb = KCURV * geom->bz_tesla;
@@ -250,12 +247,12 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     }
     if (!hit_idx) {   // identity indexing: every segment of event 0 must hold n hits
         for (int l = 0; l < geom->n_layers; ++l)
-            if (!trk_event && hits->seg_off[l + 1] - hits->seg_off[l] < seeds->n)
+            if (hits->seg_off[l + 1] - hits->seg_off[l] < seeds->n)
                 return fail(KF_ERR_INVALID_ARG, "kf_fit: hit_idx == NULL needs >= n hits in every segment");
     }
     const unsigned blocks = (unsigned)((a.n + FIT_BLOCK - 1) / FIT_BLOCK);
     cudaStream_t cs = (cudaStream_t)stream;
-    if (g_fit_pairs && !hit_idx && !trk_event && iso) {
+    if (tpt != 1 && !hit_idx && !trk_event && iso) {
         // two tracks per thread: 8-byte loads and stores of track pairs, so every array and stride must be even
         bool even = (a.ld_in % 2 == 0) && (a.ld_out % 2 == 0);
         const void* ptrs[] = {a.par, a.cov, a.par_o, a.cov_o, a.chi2_o, a.nhits_o, a.status_o};
@@ -269,6 +266,6 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
         }
     }
     if (hit_idx) { if (trk_event) launch_fit<true, true>(a, iso, blocks, cs); else launch_fit<true, false>(a, iso, blocks, cs); }
-    else { if (trk_event) launch_fit<false, true>(a, iso, blocks, cs); else launch_fit<false, false>(a, iso, blocks, cs); }
+    else launch_fit<false, false>(a, iso, blocks, cs);
     return check_launch("kf_fit");
 }

@@ -1,8 +1,9 @@
 // kf_select.cu -- hand-over from building to the final fit (sec. 2: "When a complete track has been
 // reconstructed, a final fit using the KF is performed to provide the best estimate of the track's parameters").
 // kf_select_best copies the hit list of the best candidate of every seed (slot s*K of kf_cands, ranked first by
-// kf_build) into the [n_layers][ld] index layout kf_fit reads; layers without a hit, layers not crossed and the layers
-// already on the seed (< first_layer: the seed state sits behind them) become -1 = skipped.
+// kf_build) into the [n_layers][ld] index layout kf_fit reads, with kf_fit's meaning of the negative entries: -1 =
+// layer crossed without a hit (transported, material added), -2 = not crossed; the layers already on the seed
+// (< first_layer: the seed state sits behind them) become -2.
 #include "kf_common.cuh"
 
 namespace kf {
@@ -12,8 +13,8 @@ __global__ void __launch_bounds__(256) kf_select_best_kernel(const int32_t* __re
     const int64_t s = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (s >= n_seeds) return;
     for (int l = 0; l < n_layers; ++l) {
-        const int32_t h = l < first_layer ? -1 : cand_hit[(int64_t)l * ld_cand + s * K];
-        out[(int64_t)l * ld_out + s] = h < 0 ? -1 : h;
+        const int32_t h = l < first_layer ? -2 : cand_hit[(int64_t)l * ld_cand + s * K];
+        out[(int64_t)l * ld_out + s] = h < -2 ? -2 : h;
     }
 }
 

@@ -26,10 +26,23 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a
 __device__ __forceinline__ float2 mul2(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 
+// The azimuth phi is only ever accumulated (turning angles, update corrections) and written out; the arithmetic uses the
+// carried sin/cos.  It is kept as a 32-bit fixed-point angle, phi = PH * pi / 2^31: integer addition wraps modulo 2 pi
+// exactly and does not round, so the output carries one rounding instead of 2 L of them at the size of the largest
+// intermediate angle (a 0.5 GeV track turns by ~2 rad on the way out; its final |phi| may be 1e-3: the 1e-6 absolute floor
+// of the parity tolerance is then below the accumulated fp32 rounding).
+constexpr float PHI_TO_FIX = 683565275.57643158978f;          // 2^31 / pi
+constexpr float FIX_TO_PHI = 1.46291807926715968105e-9f;      // pi / 2^31
+__device__ __forceinline__ int phi_fix_small(float a) { return __float2int_rn(a * PHI_TO_FIX); }                                // |a| <= pi
+__device__ __forceinline__ int phi_fix(float a) { return (int)__double2ll_rn((double)a * 683565275.57643158978); }            // any a, modulo 2 pi
+__device__ __forceinline__ float phi_float(int f) { return f == (int)0x80000000 ? 3.14159265358979323846f : (float)f * FIX_TO_PHI; }   // (-pi, pi]
+
 // Track state: 6 parameters, carried sin/cos of both angles, 21 covariance elements (+3 duplicates).
 struct State {
     float2 XY;           // x, y
-    float2 ZP;           // z, phi
+    float Z;             // z
+    int PH;              // phi, fixed point
+    float dph;           // last update's correction of phi (finiteness checks only)
     float2 IT;           // 1/pT, theta
     float2 CC, SS;       // (cos phi, cos theta), (sin phi, sin theta)
     float2 P0, P1, P2;   // (C00, C10), (C01, C11), (C02, C12): rows 0,1 x columns 0,1,2
@@ -39,10 +52,13 @@ struct State {
     float C44, C55;
 };
 
-// packed lower-triangular storage <-> State (k = i(i+1)/2 + j)
-template <typename LoadP, typename LoadC>
+// packed lower-triangular storage <-> State (k = i(i+1)/2 + j).  RAW: par(4) is the bit pattern of the fixed-point angle
+// (intermediate records), otherwise phi in radians.
+template <bool RAW = false, typename LoadP, typename LoadC>
 __device__ __forceinline__ void state_set(State& s, LoadP par, LoadC cov) {
-    s.XY = f2(par(0), par(1)); s.ZP = f2(par(2), par(4)); s.IT = f2(par(3), par(5));
+    s.XY = f2(par(0), par(1)); s.Z = par(2); s.IT = f2(par(3), par(5));
+    s.PH = RAW ? __float_as_int(par(4)) : phi_fix(par(4));
+    s.dph = 0.0f;
     const float c10 = cov(pk(1, 0)), c20 = cov(pk(2, 0)), c21 = cov(pk(2, 1));
     s.P0 = f2(cov(pk(0, 0)), c10); s.P1 = f2(c10, cov(pk(1, 1))); s.P2 = f2(c20, c21);
     s.Q0 = f2(c20, cov(pk(4, 0))); s.Q1 = f2(c21, cov(pk(4, 1))); s.Q2 = f2(cov(pk(2, 2)), cov(pk(4, 2)));
@@ -52,9 +68,9 @@ __device__ __forceinline__ void state_set(State& s, LoadP par, LoadC cov) {
 }
 
 // sin / cos of both angles from the angles themselves (start of a track; afterwards they are carried)
-__device__ __forceinline__ void state_trig(State& s) {
+__device__ __forceinline__ void state_trig(State& s, float phi) {
     float sp, cp, st, ct;
-    sincosf(s.ZP.y, &sp, &cp);
+    sincosf(phi, &sp, &cp);
     sincosf(s.IT.y, &st, &ct);
     s.CC = f2(cp, ct); s.SS = f2(sp, st);
 }
@@ -62,13 +78,13 @@ __device__ __forceinline__ void state_trig(State& s) {
 template <typename LoadP, typename LoadC>
 __device__ __forceinline__ void state_load(State& s, LoadP par, LoadC cov) {
     state_set(s, par, cov);
-    state_trig(s);
+    state_trig(s, par(4));
 }
 
-// WRAP: phi wrapped to (-pi, pi] (final output) or left as accumulated (intermediate record)
+// WRAP: phi in radians in (-pi, pi] (final output) or the bit pattern of the fixed-point angle (intermediate record)
 template <bool WRAP = true, typename StoreP, typename StoreC>
 __device__ __forceinline__ void state_store(const State& s, StoreP par, StoreC cov) {
-    par(0, s.XY.x); par(1, s.XY.y); par(2, s.ZP.x); par(3, s.IT.x); par(4, WRAP ? wrap_phi(s.ZP.y) : s.ZP.y); par(5, s.IT.y);
+    par(0, s.XY.x); par(1, s.XY.y); par(2, s.Z); par(3, s.IT.x); par(4, WRAP ? phi_float(s.PH) : __int_as_float(s.PH)); par(5, s.IT.y);
     cov(pk(0, 0), s.P0.x);
     cov(pk(1, 0), s.P0.y); cov(pk(1, 1), s.P1.y);
     cov(pk(2, 0), s.P2.x); cov(pk(2, 1), s.P2.y); cov(pk(2, 2), s.Q2.x);
@@ -80,7 +96,7 @@ __device__ __forceinline__ void state_store(const State& s, StoreP par, StoreC c
 // 0 * inf = NaN, 0 * NaN = NaN: one fused chain over everything
 __device__ __forceinline__ bool state_finite(const State& s) {
     float2 a = mul2(s.XY, 0.0f);
-    a = fma2(s.ZP, 0.0f, a); a = fma2(s.IT, 0.0f, a);
+    a = fma2(f2(s.Z, s.dph), 0.0f, a); a = fma2(s.IT, 0.0f, a);
     a = fma2(s.P0, 0.0f, a); a = fma2(s.P1, 0.0f, a); a = fma2(s.P2, 0.0f, a);
     a = fma2(s.Q0, 0.0f, a); a = fma2(s.Q1, 0.0f, a); a = fma2(s.Q2, 0.0f, a);
     a = fma2(s.R0, 0.0f, a); a = fma2(s.R1, 0.0f, a); a = fma2(s.R2, 0.0f, a);
@@ -90,7 +106,7 @@ __device__ __forceinline__ bool state_finite(const State& s) {
 
 // cheap per-layer check: NaN/Inf anywhere in S or the gain reaches chi2 or the parameters
 __device__ __forceinline__ bool step_finite(const State& s, float chi2) {
-    const float2 a = fma2(s.XY, 0.0f, fma2(s.ZP, 0.0f, mul2(s.IT, 0.0f)));
+    const float2 a = fma2(s.XY, 0.0f, fma2(f2(s.Z, s.dph), 0.0f, mul2(s.IT, 0.0f)));
     return fmaf(0.0f, chi2, a.x + a.y) == 0.0f;
 }
 
@@ -100,7 +116,7 @@ __device__ __forceinline__ uint32_t predict(State& s, float cw, const LayerC& ly
     const float cp = s.CC.x, ct = s.CC.y, sp = s.SS.x, st = s.SS.y;
     const float ist = frcp(st);
     const float cot = ct * ist;
-    const float pp[6] = {s.XY.x, s.XY.y, s.ZP.x, s.IT.x, s.ZP.y, s.IT.y};
+    const float pp[6] = {s.XY.x, s.XY.y, s.Z, s.IT.x, 0.0f, s.IT.y};       // transport works from the carried sin / cos, not from phi
     Transport t;
     const uint32_t flag = transport(pp, cw, cp, sp, cot, ly, t);
     if (flag) return flag;
@@ -174,7 +190,8 @@ __device__ __forceinline__ uint32_t predict(State& s, float cw, const LayerC& ly
     s.C44 = n44 + q44;
     s.C55 += q55;
     s.XY = f2(t.xn, t.yn);
-    s.ZP = f2(t.zn, s.ZP.y + t.alpha);
+    s.Z = t.zn;
+    s.PH += phi_fix_small(t.alpha);
     s.CC.x = t.cpn; s.SS.x = t.spn;
     return 0u;
 }
@@ -187,7 +204,7 @@ __device__ __forceinline__ bool innovation(const State& s, float mx, float my, f
     S.m00 = s.P0.x + V.xx; S.m10 = s.P0.y + V.xy; S.m11 = s.P1.y + V.yy;
     S.m20 = s.P2.x; S.m21 = s.P2.y; S.m22 = s.Q2.x + V.zz;
     const bool ok = ldl3(S, F);
-    r[0] = mx - s.XY.x; r[1] = my - s.XY.y; r[2] = mz - s.ZP.x;
+    r[0] = mx - s.XY.x; r[1] = my - s.XY.y; r[2] = mz - s.Z;
     const float y1 = fmaf(-F.l10, r[0], r[1]);
     const float y2 = fmaf(-F.l21, y1, fmaf(-F.l20, r[0], r[2]));
     chi2 = fmaf(r[0] * r[0], F.i0, fmaf(y1 * y1, F.i1, y2 * y2 * F.i2));
@@ -230,14 +247,16 @@ __device__ __forceinline__ void gain_update(State& s, const Ldl3& F, const HitCo
     s.XY = fma2(KP0, r[0], fma2(KP1, r[1], fma2(KP2, r[2], s.XY)));
     const float2 dZP = fma2(KQ0, r[0], fma2(KQ1, r[1], mul2(KQ2, r[2])));
     const float2 dIT = fma2(KR0, r[0], fma2(KR1, r[1], mul2(KR2, r[2])));
-    s.ZP = add2(s.ZP, dZP);
+    s.Z += dZP.x;
+    s.PH += phi_fix_small(dZP.y);
+    s.dph = dZP.y;
     s.IT = add2(s.IT, dIT);
     const float dphi = dZP.y, dth = dIT.y;
     if (fmaxf(fabsf(dphi), fabsf(dth)) < 0.06f) {
         rotate_poly2(s.CC, s.SS, f2(dphi, dth));
     } else {
         float sp, cp, st, ct;
-        sincosf(s.ZP.y, &sp, &cp);
+        sincosf(phi_float(s.PH), &sp, &cp);
         sincosf(s.IT.y, &st, &ct);
         s.CC = f2(cp, ct); s.SS = f2(sp, st);
     }

@@ -11,7 +11,7 @@ import torch
 
 from oracle import kf_oracle as o
 from paper_1711_06571_b200 import synth
-from tests.parity import compare_tracks
+from tests.parity import assert_parity, compare_tracks
 
 pytestmark = pytest.mark.gpu
 
@@ -98,43 +98,75 @@ def test_window_lookup_bit_exact():
     assert rc.max() > cap and (rc == 0).any()
 
 
-def run_build(bi, K=None, tile=0, first_layer=None):
+def run_build(bi, K=None, opt=None):
+    """opt: dict of kf_options fields (build_seeds_per_block, build_max_blocks) or None = automatic"""
     from paper_1711_06571_b200 import binding as b
     geom, hits, binned = gpu_bin(bi)
     seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    b.kf_build_set_tile(tile)
-    try:
-        out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K if K is None else K,
-                         bi.chi2_cut, bi.n_sigma)
-        torch.cuda.synchronize()
-    finally:
-        b.kf_build_set_tile(0)
+    out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K if K is None else K,
+                     bi.chi2_cut, bi.n_sigma, opt=None if opt is None else b.options(**opt))
+    torch.cuda.synchronize()
     return out.to_host()
 
 
 def ref_build(bi, K=None):
     rb = ref_bin(bi)
     return o.kf_build(bi.geom.layer_table(), bi.geom.bz, rb, bi.seg_off, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx,
-                      bi.first_layer, bi.K if K is None else K, bi.chi2_cut, bi.n_sigma)
+                      bi.first_layer, bi.K if K is None else K, bi.chi2_cut, bi.n_sigma, margins=True)
 
 
 GRAZING_BAND = 0.2   # generator guard on cos(incidence) (DESIGN.md R8); the KF guard is 0.1 (R9)
+# DESIGN.md R16: how close (relative) a decision of the ORACLE must sit to its threshold for fp32 to be allowed to take
+# it the other way: [0] strict window edge, [1] chi2 cut, [2] chi2 of two children adjacent in the ranking, [3] grazing
+# guard / z acceptance, [4] tangency (cos^2 of the incidence of a crossing that only just exists, or the relative gap of
+# one that only just does not: fp32 evaluates the discriminant u^2 + E A to ~1e-6 of its terms).
+MARGIN_TOL = np.array([1e-4, 1e-4, 1e-4, 1e-4, 1e-5])
+# R16b: covariance elements that carry the 1/cos(incidence) factor of the surface Jacobian (everything but the
+# (1/pT, theta) block) get 3x the tolerance on candidates inside the grazing band; parameters and chi2 stay at 1x.
+BAND_COV_SCALE = np.full((6, 6), 3.0)
+for _i in (3, 5):
+    for _j in (3, 5):
+        BAND_COV_SCALE[_i, _j] = 1.0
 
 
-def compare_build(g, r, n_seeds, K, max_mismatch_frac, band_frac=0.02):
-    """Seeds whose valid slots carry identical (n_cand, hit lists, nhits, status) are compared element-wise; the others
-    (fp32 decided a window edge / chi2 cut / rank differently, R16) are counted.
-    Conditioning band (R16b): a candidate whose final state crosses its cylinder with cos(incidence) < 0.2 lies
-    beyond the guard the generator applies to truth tracks (R8) and inside the KF guard band 0.1-0.2 (R9); the surface
-    Jacobian carries 1/cos(incidence) factors, so rounding is amplified up to 4x more than anywhere on a truth track.
-    Such candidates (pT < 0.5 GeV near their turning point; only the configs[4] generator makes them) are compared at
-    3x the tolerances and their share is bounded by `band_frac`; every other candidate at 1x with zero violations."""
+def first_parting_layer(gl, rl, first_layer):
+    """gl, rl: [L][k] hit lists of the valid candidates of one seed on either side.  The first layer at which the two
+    sets of list prefixes differ; first_layer when the sets are equal everywhere (only order / status differ)."""
+    L = gl.shape[0]
+    for l in range(first_layer, L):
+        if {tuple(gl[:l + 1, k]) for k in range(gl.shape[1])} != {tuple(rl[:l + 1, k]) for k in range(rl.shape[1])}:
+            return l
+    return first_layer
+
+
+def compare_build(g, r, n_seeds, K, first_layer, band_frac=0.02, margin_tol=MARGIN_TOL):
+    """Seeds whose valid slots carry identical (n_cand, hit lists, nhits, status) are compared element-wise.  Every
+    other seed must be a PROVEN decision-margin case (R16): a decision that changes the result at layer l_d
+    changes the candidate lists from some layer <= l_d on, so the oracle must have recorded, at or after the first
+    layer where the two results part, a decision within `margin_tol` (relative) of its threshold -- a hit on the window
+    edge, a chi2 at the cut, two competing children with near-equal chi2, a crossing at the grazing or acceptance limit.
+    Anything else fails.
+    Conditioning band (R16b): candidates whose final state crosses its cylinder with cos(incidence) < 0.2 (beyond the
+    generator's guard, inside the KF guard band) get 3x on the covariance elements with the 1/cos(incidence) factor;
+    their share is bounded by `band_frac`."""
     same = g["n_cand"] == r["n_cand"]
     hs = (g["hit_idx"] == r["hit_idx"]).all(axis=0) & (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
     slot_valid = (np.arange(K)[None, :] < r["n_cand"][:, None])
     same &= (hs.reshape(n_seeds, K) | ~slot_valid).all(axis=1)
     frac = 1.0 - same.mean()
+    mg = r["margins"]
+    unexplained = []
+    used = np.zeros(5, int)
+    for s_ in np.nonzero(~same)[0]:
+        gl = g["hit_idx"][:, s_ * K: s_ * K + g["n_cand"][s_]]
+        rl = r["hit_idx"][:, s_ * K: s_ * K + r["n_cand"][s_]]
+        l0 = first_parting_layer(gl, rl, first_layer)
+        m = mg[s_, l0:, :].min(axis=0)
+        if (m < margin_tol).any():
+            used[np.argmin(m / margin_tol)] += 1
+        else:
+            unexplained.append((int(s_), int(l0), [float(x) for x in m]))
     # the best candidate alone (what a user takes as the track)
     best = np.arange(n_seeds) * K
     best_same = (g["hit_idx"][:, best] == r["hit_idx"][:, best]).all(axis=0)
@@ -144,36 +176,41 @@ def compare_build(g, r, n_seeds, K, max_mismatch_frac, band_frac=0.02):
     band = sel & (cosinc < GRAZING_BAND)
     gd = dict(par=g["par"], cov=g["cov"], chi2=g["chi2"])
     rep = compare_tracks(gd, r, sel=sel & ~band)
-    rep_band = compare_tracks(gd, r, sel=band)
-    rep.update(seed_mismatch_frac=float(frac), best_mismatch_frac=float(1 - best_same.mean()), seeds=int(n_seeds),
+    rep_band = compare_tracks(gd, r, sel=band, cov_scale=BAND_COV_SCALE)
+    rep.update(seed_mismatch_frac=float(frac), mismatching_seeds=int((~same).sum()), explained_by=dict(window=int(used[0]), chi2_cut=int(used[1]), rank=int(used[2]), guards=int(used[3]), tangency=int(used[4])),
+               unexplained=unexplained[:10], n_unexplained=len(unexplained), best_mismatch_frac=float(1 - best_same.mean()), seeds=int(n_seeds),
                band=dict(n=rep_band["n"], worst_mom=rep_band["worst_mom"], worst_pos_norm=rep_band["worst_pos_norm"],
                          worst_cov=rep_band["worst_cov"], worst_chi2=rep_band["worst_chi2"]))
     print(rep)
-    assert frac <= max_mismatch_frac, rep
-    assert rep["mom_viol"] == 0 and rep["pos_viol"] == 0 and rep["chi2_viol"] == 0 and rep["cov_viol"] == 0, rep
+    assert not unexplained, rep
+    assert frac <= 0.05, rep          # secondary: the margin cases themselves are rare
+    assert_parity(rep)
     assert rep_band["n"] <= band_frac * max(rep["n"], 1), rep
-    assert max(rep_band["worst_mom"], rep_band["worst_pos_norm"], rep_band["worst_cov"], rep_band["worst_chi2"]) < 3.0, rep
+    assert_parity(rep_band)
     # unused slots
     unused = ~(np.arange(K)[None, :] < g["n_cand"][:, None]).reshape(-1)
     assert (g["nhits"][unused] == 0).all() and (g["hit_idx"][:, unused] == -2).all() and (g["status"][unused] == 0).all()
     return rep
 
 
-@pytest.mark.parametrize("tile", [0, 16, 112, 256])
-def test_build_config3_small(tile):
+@pytest.mark.parametrize("opt", [None, dict(build_seeds_per_block=16), dict(build_seeds_per_block=112), dict(build_seeds_per_block=256),
+                                 dict(build_seeds_per_block=32, build_max_blocks=5)])
+def test_build_config3_small(opt):
+    """The last case runs 25 tiles on each of 5 persistent blocks: workspace, links and shared arrays reused tile after tile."""
     bi = synth.build_inputs(3, n_events=2, tracks=2000)
-    compare_build(run_build(bi, tile=tile), ref_build(bi), bi.n_seeds, bi.K, 2e-3)
+    compare_build(run_build(bi, opt=opt), ref_build(bi), bi.n_seeds, bi.K, bi.first_layer)
 
 
-def test_build_tile_does_not_change_the_result():
-    """Seeds per block (and with it the number of rounds a layer takes: 256 seeds x up to 10 candidates exceed the list
-    area on the outer layers) must not change a single bit of the result."""
+def test_build_options_do_not_change_the_result():
+    """Seeds per warp (and with it the number of passes a layer takes) and the size of the persistent grid must not
+    change a single bit of the result."""
     bi = synth.build_inputs(4, n_events=1, tracks=2000, fake_frac=0.2)
-    base = run_build(bi, tile=128)
-    for tile in (16, 48, 256):
-        other = run_build(bi, tile=tile)
+    base = run_build(bi)
+    for opt in (dict(build_seeds_per_block=16), dict(build_seeds_per_block=48), dict(build_seeds_per_block=256), dict(build_seeds_per_block=32, build_max_blocks=3),
+                dict(build_max_blocks=7)):
+        other = run_build(bi, opt=opt)
         for k in ("n_cand", "hit_idx", "nhits", "status", "chi2"):
-            assert np.array_equal(base[k], other[k]), (tile, k)
+            assert np.array_equal(base[k], other[k]), (opt, k)
         v = base["nhits"] > 0
         assert np.array_equal(base["par"][:, v], other["par"][:, v]) and np.array_equal(base["cov"][:, v], other["cov"][:, v])
 
@@ -183,22 +220,101 @@ def test_build_config4_small():
     bi = synth.build_inputs(4, n_events=1, tracks=3000)
     g, r = run_build(bi), ref_build(bi)
     assert (r["status"] != 0).any() and (r["n_cand"] == bi.K).mean() > 0.03
-    compare_build(g, r, bi.n_seeds, bi.K, 2e-2, band_frac=0.05)
+    compare_build(g, r, bi.n_seeds, bi.K, bi.first_layer, band_frac=0.05)
+
+
+def test_build_config4_eight_events():
+    """configs[4] at 8 of its 64 events (96 000 seeds, 13.5 M hits) in the launch configuration bench.py times: tile 32,
+    64 threads, 3 000 tiles on the 1 184 persistent blocks, i.e. several tiles per block, against the oracle."""
+    bi = synth.build_inputs(4, n_events=8)
+    g, r = run_build(bi), ref_build(bi)
+    rep = compare_build(g, r, bi.n_seeds, bi.K, bi.first_layer, band_frac=0.05)
+    assert rep["seeds"] > 90_000
 
 
 @pytest.mark.parametrize("K", [1, 3, 32])
 def test_build_other_K(K):
     bi = synth.build_inputs(3, n_events=1, tracks=1500, noise=8.0)
-    compare_build(run_build(bi, K=K), ref_build(bi, K=K), bi.n_seeds, K, 5e-3)
+    compare_build(run_build(bi, K=K), ref_build(bi, K=K), bi.n_seeds, K, bi.first_layer)
 
 
-def test_build_dense_windows_exceed_the_child_buffer():
-    """30-sigma windows, chi2 cut 3000, 40x noise: ~37 compatible hits per seed-layer, so the child buffer is pruned
-    several times per layer and K = 10 saturates for every seed."""
+def test_build_K32_with_32_layers():
+    """The largest K with the largest layer count: the automatic tile must shrink until its shared memory fits."""
+    from paper_1711_06571_b200 import binding as b
+    g10 = synth.geometry("barrel10")
+    bi = synth.build_inputs(3, n_events=1, tracks=300, noise=3.0)
+    # 32 layers: the ten radii of the event plus 22 more outside, without hits (every candidate runs through them)
+    lt = np.concatenate([g10.layer_table(), np.tile(g10.layer_table()[-1:], (22, 1))])
+    lt[10:, 0] = 40.0 + 1.5 * np.arange(1, 23)
+    seg = np.concatenate([bi.seg_off, np.full(22, bi.seg_off[-1])])
+    geom = b.Geom(lt, g10.bz)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, seg, 1)
+    binned = b.kf_bin_hits(geom, hits, 64, 8)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 32, 30.0, 3.0)
+    torch.cuda.synchronize()
+    g = out.to_host()
+    rb = o.bin_hits(lt, 1, seg, bi.hit_x, bi.hit_y, bi.hit_z, 64, 8)
+    r = o.kf_build(lt, g10.bz, rb, seg, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx, 3, 32, 30.0, 3.0, margins=True)
+    compare_build(g, r, bi.n_seeds, 32, 3)
+
+
+def test_build_dense_windows_overflow_the_child_pools():
+    """30-sigma windows, chi2 cut 3000, 40x noise: ~37 compatible hits per seed-layer and parent, so every candidate's
+    child list (K entries) is pruned many times per layer and K = 10 saturates for every seed."""
     bi = synth.build_inputs(3, n_events=1, tracks=300, noise=40.0, n_sigma=30.0, chi2_cut=3000.0)
     r = ref_build(bi)
     assert r["counters"]["n_children"] / r["counters"]["n_seed_layers"] > 20
-    compare_build(run_build(bi, tile=64), r, bi.n_seeds, bi.K, 5e-2)
+    compare_build(run_build(bi), r, bi.n_seeds, bi.K, bi.first_layer)
+    compare_build(run_build(bi, opt=dict(build_seeds_per_block=64)), r, bi.n_seeds, bi.K, bi.first_layer)
+
+
+def test_build_seed_chi2_is_the_starting_chi2():
+    """DESIGN.md R10 / SURVEY.md sec. 8c-7: a candidate starts with its seed's chi2."""
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs(3, n_events=1, tracks=500)
+    geom, hits, binned = gpu_bin(bi)
+    rng = np.random.default_rng(3)
+    c0 = rng.uniform(0, 20, bi.n_seeds).astype(np.float32)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q, chi2=c0)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K, bi.chi2_cut, bi.n_sigma)
+    torch.cuda.synchronize()
+    g = out.to_host()
+    r = o.kf_build(bi.geom.layer_table(), bi.geom.bz, ref_bin(bi), bi.seg_off, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx,
+                   bi.first_layer, bi.K, bi.chi2_cut, bi.n_sigma, chi2_in=c0, margins=True)
+    compare_build(g, r, bi.n_seeds, bi.K, bi.first_layer)
+    assert (r["chi2"][::bi.K] >= c0 - 1e-6).all()
+
+
+def test_build_numeric_exits():
+    """The hand-made seeds of tests/test_oracle_build_pins.py::numeric_exit_case on the GPU: S not positive definite with
+    and without a hit inside the window, an update that leaves 1/pT <= 0, a window that is not finite.  Decisions
+    identical to the oracle's, the unchanged / predicted states kept as the oracle keeps them."""
+    from paper_1711_06571_b200 import binding as b
+    from tests.test_oracle_build_pins import numeric_exit_case
+    g_, lt, par, cov, q, seg, hx, hy, hz = numeric_exit_case()
+    K = 3
+    rb = o.bin_hits(lt, 1, seg, hx, hy, hz, 8, 1)
+    r = o.kf_build(lt, g_.bz, rb, seg, par, cov, q, np.zeros(4, np.int32), None, 3, K, 30.0, 3.0, n=4)
+    geom = b.Geom(lt, g_.bz)
+    hits = b.Hits(hx, hy, hz, seg, 1)
+    binned = b.kf_bin_hits(geom, hits, 8, 1)
+    for opt in (None, b.options(build_seeds_per_block=16)):
+        out = b.kf_build(geom, hits, binned, b.Tracks.from_host(par, cov, q), None, None, 3, K, 30.0, 3.0, opt=opt)
+        torch.cuda.synchronize()
+        g = out.to_host()
+        assert (r["status"] == o.NUMERIC).sum() == 3
+        for k in ("n_cand", "nhits", "status", "hit_idx"):
+            assert np.array_equal(g[k], r[k]), (k, g[k], r[k])
+        for t in (0, 2):          # the unchanged seed
+            assert np.array_equal(g["par"][:4, t * K], par[:4, t]) and np.array_equal(g["cov"][:, t * K], cov[:, t])
+        v = (r["nhits"] > 0) & (np.arange(4 * K) // K == 1)           # seed 1: a sane covariance, compared as usual
+        rep = compare_tracks(dict(par=g["par"], cov=g["cov"], chi2=g["chi2"]), r, sel=v)
+        assert rep["n"] >= 2
+        assert_parity(rep)
+        assert abs(np.hypot(g["par"][0, 3 * K], g["par"][1, 3 * K]) - 40.0) < 1e-4       # seed 3 went on to the last layer
 
 
 def test_build_edge_cases():
@@ -226,14 +342,17 @@ def test_build_edge_cases():
     with pytest.raises(b.KfError, match="-4"):
         b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 10, 30.0, 3.0, ws=torch.empty(64, dtype=torch.uint8, device="cuda"))
     with pytest.raises(b.KfError, match="-1"):
-        b.kf_build_set_tile(24)
+        b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), 3, 10, 30.0, 3.0, opt=b.options(build_seeds_per_block=24))
+    # the workspace size is a pure function of its arguments
+    assert b.kf_build_workspace_bytes(geom, 1000, 10, b.options(build_seeds_per_block=64)) == b.kf_build_workspace_bytes(geom, 1000, 10, b.options(build_seeds_per_block=64))
+    assert b.kf_build_workspace_bytes(geom, 10 ** 6, 10, b.options(build_max_blocks=7)) < b.kf_build_workspace_bytes(geom, 10 ** 6, 10)
 
 
 def test_build_config3_full():
     """BASELINE.json configs[3] at full size (16 events x 2 000 tracks), in the launch configuration bench.py times."""
     bi = synth.build_inputs(3)
     g, r = run_build(bi), ref_build(bi)
-    rep = compare_build(g, r, bi.n_seeds, bi.K, 2e-3)
+    rep = compare_build(g, r, bi.n_seeds, bi.K, bi.first_layer)
     assert rep["best_mismatch_frac"] < 1e-3
     best = np.arange(bi.n_seeds) * bi.K
     truth = bi.truth_hit_idx[:, bi.seed_truth]
