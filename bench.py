@@ -2,12 +2,14 @@
 """bench.py -- throughput of the KF hot path on B200 (contract: see DESIGN.md sec. 7).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload fit_c1|fit_c2|fit_c0|build_c3|build_c4]
-                  [--impl ours|reference]
+                  [--impl ours|reference] [--scaling weak|strong]
 
 A "step" is one pass of the hot path over one batch of synthetic input: for the fit workloads one kf_fit call over
 all tracks (steps F1-F9), for the build workloads kf_bin_hits + kf_build over all events (steps B0-B6).  The default
 line is fit_c1 = BASELINE.json configs[1] (the configuration the roofline target is quoted on) and carries, under
-"build", the seeds/s of configs[3] measured the same way in the same run.  `value` is whole-job throughput with
+"fit_c2", "build" (= build_c3) and "build_c4", the other BASELINE.json configs measured the same way in the same run,
+each with its own clock sample, roofline and cpu_baseline.  With --gpus N > 1 and no torchrun environment bench.py starts
+the N ranks itself (torch.distributed.run on 127.0.0.1).  `value` is whole-job throughput with
 inputs resident in HBM; `e2e` is the same through the C-ABI call with pinned HOST buffers, H2D and D2H copies inside
 the timed region.  `--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload
 on the host cores.  Under torchrun every rank works on its own shard of the same size (weak scaling, no collective
@@ -266,8 +268,16 @@ def nbytes(ts):
 def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
     import torch
     from paper_1711_06571_b200 import binding as b
-    # every rank: its own shard of the configured size (weak scaling); events differ by rank
-    fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks, event=d.rank)
+    # weak scaling (default): every rank its own shard of the configured size, events differ by rank;
+    # strong scaling: the configured tracks split over the ranks (shard.track_range)
+    from paper_1711_06571_b200 import shard
+    n_cfg = args.tracks if args.tracks is not None else synth.FIT_CONFIGS[FIT_CFG[workload]]["n"]
+    if args.scaling == "strong":
+        lo_, hi_ = shard.track_range(n_cfg, d.rank, d.world)
+        fi = synth.fit_inputs(FIT_CFG[workload], n=hi_ - lo_, event=d.rank)
+    else:
+        fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks, event=d.rank)
+    n_job = n_cfg if args.scaling == "strong" else fi.n * d.world
     units = fit_units(fi)
     geom = b.Geom(fi.geom.layer_table(), fi.geom.bz)
     hits = b.Hits(fi.hit_x, fi.hit_y, fi.hit_z, fi.seg_off, 1)
@@ -284,56 +294,21 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
     sampler = ClockSampler(d.local) if d.rank == 0 else None
     ms_per_step, per, _, t0, t1 = time_steps(step, args.steps, W, stream, d)
     clocks = sampler.stop(t0, t1) if sampler else None
-    value = fi.n * d.world / (ms_per_step * 1e-3)
+    value = n_job / (ms_per_step * 1e-3)
 
     # ---- end to end: pinned host buffers -> H2D -> kf_fit -> D2H, all inside the timed region ----
-    # The tracks are split into `args.e2e_streams` independent sub-batches, each with its own stream, pinned host
+    # pipeline.FitPipeline: the tracks in `args.e2e_streams` independent sub-batches, each with its own stream, pinned host
     # buffers and device buffers, so that the copies of one sub-batch overlap the fit of another ("multiple events in
     # flight ... to overlap expensive copy operations").
-    L = fi.geom.n_layers
-    n_sub = max(1, min(args.e2e_streams, fi.n))
-    bounds = [fi.n * i // n_sub for i in range(n_sub + 1)]
-    subs = []
-    for c in range(n_sub):
-        lo, hi = bounds[c], bounds[c + 1]
-        m = hi - lo
-        ldc = max(32, (m + 31) // 32 * 32)
-        hp = np.zeros((6, ldc), np.float32); hp[:, :m] = fi.par[:, lo:hi]
-        hc = np.zeros((21, ldc), np.float32); hc[:, :m] = fi.cov[:, lo:hi]
-        hxs = [np.ascontiguousarray(a_.reshape(L, fi.ld)[:, lo:hi]).reshape(-1) for a_ in (fi.hit_x, fi.hit_y, fi.hit_z)]
-        hidx = None
-        if fi.hit_idx is not None:
-            hidx = np.full((L, ldc), -2, np.int32)
-            hidx[:, :m] = np.where(fi.hit_idx[:, lo:hi] >= 0, np.arange(m, dtype=np.int32)[None, :], fi.hit_idx[:, lo:hi])
-        sub = dict(m=m, stream=torch.cuda.Stream(), h_in=[pin(hp), pin(hc), pin(fi.q[lo:hi])] + [pin(x) for x in hxs] + ([pin(hidx)] if hidx is not None else []))
-        sub["seeds"] = b.Tracks.empty(m, ldc)
-        sub["hits"] = b.Hits(hxs[0], hxs[1], hxs[2], np.arange(L + 1, dtype=np.int64) * m, 1)
-        sub["hit_idx"] = None if hidx is None else torch.from_numpy(hidx).cuda()
-        sub["out"] = b.Tracks.empty(m, ldc)
-        sub["out"].q = sub["seeds"].q
-        sub["d_in"] = [sub["seeds"].par, sub["seeds"].cov, sub["seeds"].q, sub["hits"].x, sub["hits"].y, sub["hits"].z] + ([sub["hit_idx"]] if hidx is not None else [])
-        sub["d_out"] = [sub["out"].par, sub["out"].cov, sub["out"].chi2, sub["out"].nhits, sub["out"].status]
-        sub["h_out"] = [torch.empty(t_.shape, dtype=t_.dtype).pin_memory() for t_ in sub["d_out"]]
-        subs.append(sub)
-    h2d = sum(nbytes(sb["h_in"]) for sb in subs)
-    d2h = sum(nbytes(sb["h_out"]) for sb in subs)
+    from paper_1711_06571_b200 import pipeline
+    pipe = pipeline.FitPipeline(geom, fi.n, fi.par, fi.cov, fi.q, fi.hit_x, fi.hit_y, fi.hit_z, fi.ld, hit_idx=fi.hit_idx, n_streams=args.e2e_streams)
+    n_sub, h2d, d2h = len(pipe.subs), pipe.h2d_bytes, pipe.d2h_bytes
 
     def e2e_step(rec):
-        start = torch.cuda.Event(); start.record(stream)
-        for sb in subs:
-            st_ = sb["stream"]
-            st_.wait_event(start)
-            with torch.cuda.stream(st_):
-                for dst, src in zip(sb["d_in"], sb["h_in"]):
-                    dst.copy_(src, non_blocking=True)
-                b.kf_fit(geom, sb["hits"], sb["hit_idx"], None, sb["seeds"], out=sb["out"], stream=st_)
-                for dst, src in zip(sb["h_out"], sb["d_out"]):
-                    dst.copy_(src, non_blocking=True)
-            done = torch.cuda.Event(); done.record(st_)
-            stream.wait_event(done)
+        pipe.run(stream)
 
     e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
-    e2e_value = fi.n * d.world / (e2e_ms * 1e-3)
+    e2e_value = n_job / (e2e_ms * 1e-3)
     if d.rank != 0:
         return None
 
@@ -353,7 +328,7 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
                     frac_of_slower_roof=max(t_alu, t_hbm) / (kern_ms * 1e-3))
     roofline["traffic"] = stored_traffic(workload)
     line = dict(metric="tracks_fitted_per_s", value=value, unit="tracks/s", n_gpus=d.world, steps=args.steps, warmup=W,
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                ms_per_step=ms_per_step, higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="f32", data="synthetic",
                 config=dict(workload=workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=units["track_layers"],
                             l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (units["bytes"] / 1e6)),
                 clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms, streams=n_sub),
@@ -366,13 +341,19 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
 
 
 def stored_traffic(workload):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.csv)."""
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.csv).
+    A row counts only if it was captured with this version of the library (column kf_version): a stale number reads null."""
     import csv
     tr = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(tr):
         return None
+    try:
+        from paper_1711_06571_b200 import binding as b
+        ver = str(b.kf_version())
+    except Exception:
+        return None
     for row in csv.DictReader(open(tr)):
-        if row["workload"] == workload and row["dram_bytes_per_launch"]:
+        if row["workload"] == workload and row["dram_bytes_per_launch"] and row.get("kf_version", "") == ver:
             return float(row["dram_bytes_per_launch"])
     return None
 
@@ -384,7 +365,14 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     import torch
     from paper_1711_06571_b200 import binding as b
     cfg = BUILD_CFG[workload]
-    bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000)
+    if args.scaling == "strong":      # the configured events dealt out whole, balanced by seed count (shard.assign_events)
+        from paper_1711_06571_b200 import shard
+        n_ev_cfg = args.events if args.events is not None else synth.BUILD_CONFIGS[cfg]["n_events"]
+        per_event = synth.BUILD_CONFIGS[cfg]["tracks"] * (1.0 + synth.BUILD_CONFIGS[cfg]["fake_frac"])
+        mine = shard.assign_events([per_event] * n_ev_cfg, d.world)[d.rank]
+        bi = synth.build_inputs(cfg, n_events=max(len(mine), 1), event0=mine[0] if mine else 0)
+    else:
+        bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000)
     L, K = bi.geom.n_layers, bi.K
     geom = b.Geom(bi.geom.layer_table(), bi.geom.bz)
     hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
@@ -412,57 +400,20 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     clocks = sampler.stop(t0, t1) if sampler else None
     bin_ms, build_ms = statistics.mean(seg[1]), statistics.mean(seg[2])
     ms_per_step = d.max_ms(bin_ms + build_ms)          # the L2 flush is not part of the step
-    value = bi.n_seeds * d.world / (ms_per_step * 1e-3)
+    from paper_1711_06571_b200 import shard as _shard
+    n_job = _shard.sum_over_ranks(float(bi.n_seeds), device="cuda")
+    value = n_job / (ms_per_step * 1e-3)
 
     # ---- end to end: hits + seeds H2D, bin + build, candidates D2H ----
-    # The events are split into `args.e2e_streams` groups, each with its own stream and buffers: several events in flight,
-    # copies of one group overlapping the building of another.
-    n_sub = max(1, min(args.e2e_streams, bi.n_events))
-    ev_b = [bi.n_events * i // n_sub for i in range(n_sub + 1)]
-    subs = []
-    for c in range(n_sub):
-        e0, e1 = ev_b[c], ev_b[c + 1]
-        h0, h1 = int(bi.seg_off[e0 * L]), int(bi.seg_off[e1 * L])
-        sel = np.nonzero((bi.seed_event >= e0) & (bi.seed_event < e1))[0]
-        s0_, s1_ = (int(sel[0]), int(sel[-1]) + 1) if len(sel) else (0, 0)
-        m = s1_ - s0_
-        ldc = max(32, (m + 31) // 32 * 32)
-        hp = np.zeros((6, ldc), np.float32); hp[:, :m] = bi.par[:, s0_:s1_]
-        hc = np.zeros((21, ldc), np.float32); hc[:, :m] = bi.cov[:, s0_:s1_]
-        hs = np.full((bi.first_layer, ldc), -1, np.int32); hs[:, :m] = bi.seed_hit_idx[:, s0_:s1_]
-        sub = dict(stream=torch.cuda.Stream(), n_ev=e1 - e0, m=m)
-        sub["hits"] = b.Hits(bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], bi.seg_off[e0 * L: e1 * L + 1] - h0, e1 - e0)
-        sub["binned"] = b.Binned(h1 - h0, (e1 - e0) * L * bi.n_phi * bi.n_z, bi.n_phi, bi.n_z, soa=False)
-        sub["ws"] = torch.empty(max(b.kf_bin_workspace_bytes(geom, sub["hits"], bi.n_phi, bi.n_z), 1), dtype=torch.uint8, device="cuda")
-        sub["seeds"] = b.Tracks.empty(m, ldc)
-        sub["sev"] = torch.zeros(max(m, 1), dtype=torch.int32, device="cuda")[:m]
-        sub["shi"] = torch.empty((bi.first_layer, ldc), dtype=torch.int32, device="cuda")
-        sub["out"] = b.Cands(m, K, L)
-        sub["bws"] = torch.empty(max(b.kf_build_workspace_bytes(geom, m, K), 1), dtype=torch.uint8, device="cuda")
-        sub["h_in"] = [pin(a_) for a_ in (bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], hp, hc, bi.q[s0_:s1_], bi.seed_event[s0_:s1_] - e0, hs)]
-        sub["d_in"] = [sub["hits"].x, sub["hits"].y, sub["hits"].z, sub["seeds"].par, sub["seeds"].cov, sub["seeds"].q, sub["sev"], sub["shi"]]
-        o_ = sub["out"]
-        sub["d_out"] = [o_.tracks.par, o_.tracks.cov, o_.tracks.chi2, o_.tracks.nhits, o_.tracks.status, o_.hit_idx, o_.n_cand]
-        sub["h_out"] = [torch.empty(t_.shape, dtype=t_.dtype).pin_memory() for t_ in sub["d_out"]]
-        subs.append(sub)
-    h = [x for sb in subs for x in sb["h_in"]]
-    ho = [x for sb in subs for x in sb["h_out"]]
+    # pipeline.BuildPipeline: the events in `args.e2e_streams` groups, each with its own stream and buffers: several events in
+    # flight, copies of one group overlapping the building of another.
+    from paper_1711_06571_b200 import pipeline
+    pipe = pipeline.BuildPipeline(geom, bi.n_events, bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_phi, bi.n_z, bi.par, bi.cov, bi.q, bi.seed_event,
+                                  bi.seed_hit_idx, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, n_streams=args.e2e_streams)
+    n_sub = len(pipe.subs)
 
     def e2e_step(rec):
-        start = torch.cuda.Event(); start.record(stream)
-        for sb in subs:
-            st_ = sb["stream"]
-            st_.wait_event(start)
-            with torch.cuda.stream(st_):
-                for dst, src in zip(sb["d_in"], sb["h_in"]):
-                    dst.copy_(src, non_blocking=True)
-                b.kf_bin_hits(geom, sb["hits"], bi.n_phi, bi.n_z, out=sb["binned"], ws=sb["ws"], stream=st_)
-                b.kf_build(geom, sb["hits"], sb["binned"], sb["seeds"], sb["sev"], sb["shi"], bi.first_layer, K, bi.chi2_cut, bi.n_sigma,
-                           out=sb["out"], ws=sb["bws"], stream=st_)
-                for dst, src in zip(sb["h_out"], sb["d_out"]):
-                    dst.copy_(src, non_blocking=True)
-            done = torch.cuda.Event(); done.record(st_)
-            stream.wait_event(done)
+        pipe.run(stream)
 
     e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
     if d.rank != 0:
@@ -474,7 +425,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
                            n_phi=bi.n_phi, n_z=bi.n_z, chi2_cut=bi.chi2_cut, n_sigma=bi.n_sigma,
                            l2="192 MB fill between timed iterations (outside the timed segments)" if flush is not None else
                               "hits + sorted copy + candidates per step exceed the 126 MB L2; no explicit flush"),
-               e2e=dict(value=bi.n_seeds * d.world / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=nbytes(h), d2h_bytes_per_step=nbytes(ho),
+               e2e=dict(value=n_job / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=pipe.h2d_bytes, d2h_bytes_per_step=pipe.d2h_bytes,
                         ms_per_step=e2e_ms, streams=n_sub),
                gpu_launches=args.steps * BUILD_LAUNCHES_PER_STEP, clocks=clocks)
     bin_bytes = BIN_BYTES_PER_HIT * hits.n_hits + 4.0 * n_bins
@@ -552,6 +503,17 @@ def bench_mplex(args, d: Dist):
     return line
 
 
+def spawn_ranks(n: int) -> int:
+    """--gpus N without a torchrun environment: start the N ranks here (one process per GPU, rendezvous on 127.0.0.1)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -559,16 +521,19 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="fit_c1", choices=list(FIT_CFG) + list(BUILD_CFG) + ["mplex"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="weak: every rank a full-size shard; strong: the configured work split over the ranks")
     ap.add_argument("--tracks", type=int, default=None, help="override the track count (debug only; invalidates the metric)")
     ap.add_argument("--events", type=int, default=None, help="override the event count of a build workload (debug only)")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: tracks per step")
     ap.add_argument("--ref-events", type=int, default=16, help="--impl reference: events per step (build workloads)")
     ap.add_argument("--cpu-sample", type=int, default=200_000)
-    ap.add_argument("--cpu-events", type=int, default=16, help="events the oracle builds for cpu_baseline and the build counters")
+    ap.add_argument("--cpu-events", type=int, default=None, help="events the oracle builds for cpu_baseline and the build counters (default: 16 for build_c3, 1 for build_c4)")
     ap.add_argument("--e2e-streams", type=int, default=4, help="sub-batches in flight in the end-to-end leg (copies overlap compute)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-build", action="store_true", help="default line without the configs[3] build leg")
+    ap.add_argument("--no-build", action="store_true", help="default line without the extra legs (fit_c2, build_c3, build_c4)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        return spawn_ranks(args.gpus)
     d = Dist()
 
     if args.impl == "reference":
@@ -584,21 +549,34 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", d.local))
 
+    def build_leg(wl):
+        a2 = argparse.Namespace(**vars(args))
+        if a2.cpu_events is None:
+            a2.cpu_events = 16 if wl == "build_c3" else 1
+        return bench_build(a2, d, wl)
+
     if args.workload == "mplex":
         line = bench_mplex(args, d)
     elif args.workload in FIT_CFG:
         line = bench_fit(args, d, args.workload)
-        if not args.no_build and args.tracks is None:
-            bl = bench_build(args, d, "build_c3", sample_clocks=False)
+        if not args.no_build and args.tracks is None and args.workload == "fit_c1":
+            # the other BASELINE.json configs in the same run, each a compact line of its own
+            f2 = bench_fit(args, d, "fit_c2")
+            b3 = build_leg("build_c3")
+            torch.cuda.empty_cache()
+            b4 = build_leg("build_c4")
             if line is not None:
-                line["build"] = bl
-                line["gpu_launches"] += bl["gpu_launches"]
+                keep = ("metric", "value", "unit", "ms_per_step", "config", "clocks", "roofline", "cpu_baseline", "e2e", "gpu_launches")
+                line["fit_c2"] = {k: f2[k] for k in keep if k in f2}
+                line["build"] = b3
+                line["build_c4"] = b4
+                line["gpu_launches"] += f2["gpu_launches"] + b3["gpu_launches"] + b4["gpu_launches"]
     else:
-        r = bench_build(args, d, args.workload)
+        r = build_leg(args.workload)
         line = None
         if r is not None:
             line = dict(metric=r.pop("metric"), value=r.pop("value"), unit=r.pop("unit"), n_gpus=d.world, steps=args.steps,
-                        warmup=max(args.warmup, 3), ms_per_step=r.pop("ms_per_step"), higher_is_better=True, scaling="weak",
+                        warmup=max(args.warmup, 3), ms_per_step=r.pop("ms_per_step"), higher_is_better=True, scaling=args.scaling,
                         vs_baseline=None, dtype="f32", data="synthetic", **r)
     if d.rank == 0:
         print(json.dumps(line), flush=True)

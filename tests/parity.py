@@ -22,9 +22,9 @@ import numpy as np
 PAR_REL, PAR_ABS, COV_REL, CHI2_REL = 1e-4, 1e-6, 1e-3, 1e-3
 
 
-def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None) -> dict:
+def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None, chi2_scale=1.0) -> dict:
     """gpu: par [6][n] f32, cov [21][n] f32 packed, chi2; ref: par [6][n] f64, cov [n][6][6] f64, chi2.
-    cov_scale: optional [6][6] factors on the covariance tolerance (R16b).
+    cov_scale, chi2_scale: optional factors on the covariance ([6][6]) and chi2 tolerances (R16b).
     Returns violation counts and worst normalised errors (1.0 = at tolerance)."""
     n = ref["par"].shape[1]
     sel = np.ones(n, bool) if sel is None else sel
@@ -46,7 +46,7 @@ def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None) -> dict:
     cerr = np.abs(gc - rc) / (COV_REL * s[:, :, None] * s[:, None, :])
     if cov_scale is not None:
         cerr = cerr / np.asarray(cov_scale, dtype=np.float64)[None, :, :]
-    c2 = np.abs(gpu["chi2"].astype(np.float64)[sel] - ref["chi2"][sel]) / (CHI2_REL * np.maximum(ref["chi2"][sel], 1.0))
+    c2 = np.abs(gpu["chi2"].astype(np.float64)[sel] - ref["chi2"][sel]) / (chi2_scale * CHI2_REL * np.maximum(ref["chi2"][sel], 1.0))
     mom = comp[[3, 5]]
     phi_dir = np.abs(d[4]) / PAR_REL
     return dict(n=int(sel.sum()), worst_mom=float(mom.max(initial=0)), worst_pos_norm=float(pos.max(initial=0)),

@@ -9,7 +9,7 @@ import torch
 from oracle import kf_oracle as o
 from paper_1711_06571_b200 import synth
 from tests.parity import assert_parity, compare_tracks
-from tests.test_build_gpu import BAND_COV_SCALE, GRAZING_BAND
+from tests.test_build_gpu import BAND_CHI2_SCALE, BAND_COV_SCALE, GRAZING_BAND
 
 pytestmark = pytest.mark.gpu
 
@@ -44,7 +44,7 @@ def test_build_then_final_fit(config, kw):
     cosinc = (x * np.cos(ph) + y * np.sin(ph)) / np.maximum(np.hypot(x, y), 1e-30)
     band = cosinc < GRAZING_BAND                               # conditioning band: DESIGN.md R16b
     rep = compare_tracks(g, r, sel=same & ~band)
-    rep_band = compare_tracks(g, r, sel=same & band, cov_scale=BAND_COV_SCALE)
+    rep_band = compare_tracks(g, r, sel=same & band, cov_scale=BAND_COV_SCALE, chi2_scale=BAND_CHI2_SCALE)
     print(rep, rep_band)
     assert rep["n"] > 0.9 * n and rep_band["n"] <= 0.05 * n
     for q_ in (rep, rep_band):
