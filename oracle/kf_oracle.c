@@ -47,13 +47,18 @@ enum { KFO_UNREACHABLE = 1, KFO_LEFT_Z = 2, KFO_GRAZING = 4, KFO_NUMERIC = 8 };
 
 #define KFO_CMIN 0.1 /* KF-side grazing guard on cos(incidence) [R9] */
 
-/* layer table row: r, zmax, xx0, sig_rphi, sig_z, sig_r */
-#define LR(t, l) ((t)[6 * (l) + 0])
-#define LZMAX(t, l) ((t)[6 * (l) + 1])
-#define LXX0(t, l) ((t)[6 * (l) + 2])
-#define LSRPHI(t, l) ((t)[6 * (l) + 3])
-#define LSZ(t, l) ((t)[6 * (l) + 4])
-#define LSR(t, l) ((t)[6 * (l) + 5])
+/* layer table row, 8 columns: r, zmax, xx0, sig_rphi, sig_z, sig_r, kind, rmin.
+ * kind 0 = barrel cylinder of radius r and half length zmax; kind 1 = endcap disk ("cylinder with lids", PAPER.md:L70
+ * sec. 4.1) in the plane z = r (column 0, signed), covering rmin <= radius <= zmax (column 1 = outer radius) [R19]. */
+#define KFO_LW 8
+#define LR(t, l) ((t)[KFO_LW * (l) + 0])
+#define LZMAX(t, l) ((t)[KFO_LW * (l) + 1])
+#define LXX0(t, l) ((t)[KFO_LW * (l) + 2])
+#define LSRPHI(t, l) ((t)[KFO_LW * (l) + 3])
+#define LSZ(t, l) ((t)[KFO_LW * (l) + 4])
+#define LSR(t, l) ((t)[KFO_LW * (l) + 5])
+#define LKIND(t, l) ((int)(t)[KFO_LW * (l) + 6])
+#define LRMIN(t, l) ((t)[KFO_LW * (l) + 7])
 
 int kfo_num_threads(void) {
 #ifdef _OPENMP
@@ -102,6 +107,50 @@ static double g_of(const double p[6], double w, double s, double R, double* dg) 
     helix_at(p, w, s, o);
     if (dg) *dg = 2.0 * (o[0] * cos(o[4]) + o[1] * sin(o[4]));
     return o[0] * o[0] + o[1] * o[1] - R * R;
+}
+
+/* Fixed-path-length partial derivatives of the helix (sec. 8c-3 of SURVEY.md): with a = w s,
+ * dX/d iota = c_w s^2 f1(a), dY/d iota = c_w s^2 f2(a), f1 = (cos a - sin a / a)/a, f2 = (sin a - (1 - cos a)/a)/a. */
+static void helix_curv_partials(double c_w, double w, double s, double* dXdi, double* dYdi) {
+    const double a = w * s;
+    double f1, f2;
+    if (fabs(a) < 1e-2) {
+        double a2 = a * a;
+        f1 = a * (-1.0 / 3.0 + a2 * (1.0 / 30.0 + a2 * (-1.0 / 840.0 + a2 / 45360.0)));
+        f2 = 0.5 + a2 * (-1.0 / 8.0 + a2 * (1.0 / 144.0 - a2 / 5760.0));
+    } else {
+        f1 = (cos(a) - sin(a) / a) / a;
+        f2 = (sin(a) - (1.0 - cos(a)) / a) / a;
+    }
+    *dXdi = c_w * s * s * f1;
+    *dYdi = c_w * s * s * f2;
+}
+
+/* State at transverse path s and the Jacobian of the transport TO THE CYLINDER through that point: fixed-s partials
+ * plus the path-length term, ds/dp from the constraint x'^2 + y'^2 = const (sec. 8c-3).  up = x' cos phi' + y' sin phi'. */
+static void helix_to_cylinder(const double p[6], double w, double c_w, double s, double pout[6], double J[36], double* up_out) {
+    helix_at(p, w, s, pout);
+    const double xn = pout[0], yn = pout[1], phn = pout[4];
+    const double cpn = cos(phn), spn = sin(phn), cp = cos(p[4]), sp = sin(p[4]);
+    const double up = xn * cpn + yn * spn; /* R cos(incidence) */
+    double dXdi, dYdi;
+    helix_curv_partials(c_w, w, s, &dXdi, &dYdi);
+    const double Fxi = cp * dXdi - sp * dYdi, Fyi = sp * dXdi + cp * dYdi;
+    const double Fxp = -(yn - p[1]), Fyp = xn - p[0];
+    const double cot = cos(p[5]) / sin(p[5]), sin2 = sin(p[5]) * sin(p[5]);
+    /* ds/dp from g(p, s(p)) = 0 */
+    const double sx = -xn / up, sy = -yn / up;
+    const double si = -(xn * Fxi + yn * Fyi) / up, sph = -(xn * Fxp + yn * Fyp) / up;
+    memset(J, 0, 36 * sizeof(double));
+    /* columns: x y z iota phi theta */
+    J[0 * 6 + 0] = 1.0 + cpn * sx; J[0 * 6 + 1] = cpn * sy; J[0 * 6 + 3] = Fxi + cpn * si; J[0 * 6 + 4] = Fxp + cpn * sph;
+    J[1 * 6 + 0] = spn * sx; J[1 * 6 + 1] = 1.0 + spn * sy; J[1 * 6 + 3] = Fyi + spn * si; J[1 * 6 + 4] = Fyp + spn * sph;
+    J[2 * 6 + 0] = cot * sx; J[2 * 6 + 1] = cot * sy; J[2 * 6 + 2] = 1.0; J[2 * 6 + 3] = cot * si; J[2 * 6 + 4] = cot * sph;
+    J[2 * 6 + 5] = -s / sin2;
+    J[3 * 6 + 3] = 1.0;
+    J[4 * 6 + 0] = w * sx; J[4 * 6 + 1] = w * sy; J[4 * 6 + 3] = c_w * s + w * si; J[4 * 6 + 4] = 1.0 + w * sph;
+    J[5 * 6 + 5] = 1.0;
+    *up_out = up;
 }
 
 /* Propagate the state to the cylinder of radius R: smallest positive root of g(s) = x'^2 + y'^2 - R^2 [R2].
@@ -168,48 +217,80 @@ static int propagate_ex(const double p[6], int q, double bz, double R, double po
         s = sn;
         if (ds <= 1e-15 * fmax(1.0, fabs(s)) || hi - lo <= 1e-15 * fmax(1.0, fabs(s))) break;
     }
-    helix_at(p, w, s, pout);
-    const double xn = pout[0], yn = pout[1], phn = pout[4];
-    const double cpn = cos(phn), spn = sin(phn), cp = cos(p[4]), sp = sin(p[4]);
-    const double up = xn * cpn + yn * spn; /* R cos(incidence) */
+    double up;
+    helix_to_cylinder(p, w, c_w, s, pout, J, &up);
     if (s_out) *s_out = s;
     if (cosinc_out) *cosinc_out = up / R;
     if (tangency_out) *tangency_out = (up / R) * (up / R);
-
-    /* fixed-s partial derivatives (sec. 8c-3) */
-    const double a = w * s;
-    double f1, f2; /* f1 = (cos a - sinc a)/a, f2 = (sin a - (1-cos a)/a)/a */
-    if (fabs(a) < 1e-2) {
-        double a2 = a * a;
-        f1 = a * (-1.0 / 3.0 + a2 * (1.0 / 30.0 + a2 * (-1.0 / 840.0 + a2 / 45360.0)));
-        f2 = 0.5 + a2 * (-1.0 / 8.0 + a2 * (1.0 / 144.0 - a2 / 5760.0));
-    } else {
-        f1 = (cos(a) - sin(a) / a) / a;
-        f2 = (sin(a) - (1.0 - cos(a)) / a) / a;
-    }
-    const double dXdi = c_w * s * s * f1; /* dX/d iota at fixed s = (s cos a - X)/iota */
-    const double dYdi = c_w * s * s * f2; /* dY/d iota at fixed s = (s sin a - Y)/iota */
-    const double Fxi = cp * dXdi - sp * dYdi, Fyi = sp * dXdi + cp * dYdi;
-    const double Fxp = -(yn - p[1]), Fyp = xn - p[0];
-    const double cot = cos(p[5]) / sin(p[5]), sin2 = sin(p[5]) * sin(p[5]);
-    /* ds/dp from g(p, s(p)) = 0 */
-    const double sx = -xn / up, sy = -yn / up;
-    const double si = -(xn * Fxi + yn * Fyi) / up, sph = -(xn * Fxp + yn * Fyp) / up;
-    memset(J, 0, 36 * sizeof(double));
-    /* columns: x y z iota phi theta */
-    J[0 * 6 + 0] = 1.0 + cpn * sx; J[0 * 6 + 1] = cpn * sy; J[0 * 6 + 3] = Fxi + cpn * si; J[0 * 6 + 4] = Fxp + cpn * sph;
-    J[1 * 6 + 0] = spn * sx; J[1 * 6 + 1] = 1.0 + spn * sy; J[1 * 6 + 3] = Fyi + spn * si; J[1 * 6 + 4] = Fyp + spn * sph;
-    J[2 * 6 + 0] = cot * sx; J[2 * 6 + 1] = cot * sy; J[2 * 6 + 2] = 1.0; J[2 * 6 + 3] = cot * si; J[2 * 6 + 4] = cot * sph;
-    J[2 * 6 + 5] = -s / sin2;
-    J[3 * 6 + 3] = 1.0;
-    J[4 * 6 + 0] = w * sx; J[4 * 6 + 1] = w * sy; J[4 * 6 + 3] = c_w * s + w * si; J[4 * 6 + 4] = 1.0 + w * sph;
-    J[5 * 6 + 5] = 1.0;
     if (!(up / R >= KFO_CMIN)) return KFO_GRAZING;
     return 0;
 }
 int kfo_propagate(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out,
                   double* cosinc_out) {
     return propagate_ex(p, q, bz, R, pout, J, s_out, cosinc_out, NULL);
+}
+
+/* Second step of the two-step propagation (sec. 4.1: "an initial propagation to the average radius of the
+ * barrel ... followed by further propagation steps to the position of each candidate hit") [R20]: from a state on (or
+ * near) a cylinder to the NEAREST crossing of the cylinder of radius R, forwards or backwards -- Newton on
+ * g(s) = x'^2 + y'^2 - R^2 from s = 0, g' = 2 (x' cos phi' + y' sin phi').  Same surface Jacobian.  No material.
+ * Returns 0, or KFO_UNREACHABLE when the iteration does not converge (the hit radius is not within reach of a short step). */
+int kfo_propagate_near(const double p[6], int q, double bz, double R, double pout[6], double J[36], double* s_out) {
+    const double w = -(double)q * KFO_KCURV * bz * p[3], c_w = -(double)q * KFO_KCURV * bz;
+    memcpy(pout, p, 6 * sizeof(double));
+    for (int i = 0; i < 36; ++i) J[i] = (i % 7 == 0) ? 1.0 : 0.0;
+    if (s_out) *s_out = 0.0;
+    double s = 0.0;
+    int ok = 0;
+    for (int it = 0; it < 50; ++it) {
+        double dg, g = g_of(p, w, s, R, &dg);
+        if (!(fabs(dg) > 0.0) || !isfinite(g)) break;
+        double ds = -g / dg;
+        s += ds;
+        if (fabs(ds) <= 1e-14 * fmax(1.0, R)) { ok = 1; break; }       /* the rounding of g = r^2 - R^2 is ~1e-16 R^2, of ds ~1e-16 R */
+        if (!(fabs(s) < 4.0 * R)) break;
+    }
+    if (!ok) return KFO_UNREACHABLE;
+    double up;
+    helix_to_cylinder(p, w, c_w, s, pout, J, &up);
+    if (s_out) *s_out = s;
+    return 0;
+}
+
+/* Propagate to the plane z = Z of an endcap disk [R19]: z' = z + s cot(theta) fixes the transverse path
+ * s = (Z - z) tan(theta).  forward_only: s must be positive (first step: the track has to move towards the disk) and
+ * the turning angle at most half a turn [R2]; otherwise (second step to a hit's own z) any sign of s.
+ * J = fixed-s partials + (dp'/ds)(ds/dp)^T with ds/dz = -tan(theta), ds/dtheta = (Z - z)/cos^2(theta): the z' row
+ * vanishes identically (the state is transported to the surface).  cosinc_out = |cos(theta)| (angle to the disk normal). */
+int kfo_propagate_z(const double p[6], int q, double bz, double Z, int forward_only, double pout[6], double J[36], double* s_out,
+                    double* cosinc_out) {
+    const double w = -(double)q * KFO_KCURV * bz * p[3], c_w = -(double)q * KFO_KCURV * bz;
+    const double st = sin(p[5]), ct = cos(p[5]);
+    memcpy(pout, p, 6 * sizeof(double));
+    for (int i = 0; i < 36; ++i) J[i] = (i % 7 == 0) ? 1.0 : 0.0;
+    if (s_out) *s_out = 0.0;
+    if (cosinc_out) *cosinc_out = fabs(ct);
+    const double s = (Z - p[2]) * st / ct;
+    if (!isfinite(s) || !isfinite(w)) return KFO_UNREACHABLE;
+    if (forward_only && (!(s > 0.0) || !(fabs(w) * s <= KFO_PI))) return KFO_UNREACHABLE;
+    helix_at(p, w, s, pout);
+    pout[2] = Z;
+    const double cpn = cos(pout[4]), spn = sin(pout[4]), cp = cos(p[4]), sp = sin(p[4]);
+    double dXdi, dYdi;
+    helix_curv_partials(c_w, w, s, &dXdi, &dYdi);
+    const double Fxi = cp * dXdi - sp * dYdi, Fyi = sp * dXdi + cp * dYdi;
+    const double Fxp = -(pout[1] - p[1]), Fyp = pout[0] - p[0];
+    const double sz = -st / ct, sth = (Z - p[2]) / (ct * ct);
+    memset(J, 0, 36 * sizeof(double));
+    J[0 * 6 + 0] = 1.0; J[0 * 6 + 2] = cpn * sz; J[0 * 6 + 3] = Fxi; J[0 * 6 + 4] = Fxp; J[0 * 6 + 5] = cpn * sth;
+    J[1 * 6 + 1] = 1.0; J[1 * 6 + 2] = spn * sz; J[1 * 6 + 3] = Fyi; J[1 * 6 + 4] = Fyp; J[1 * 6 + 5] = spn * sth;
+    /* row z': 1 + cot(theta) ds/dz = 0 and -s/sin^2 + cot(theta) ds/dtheta = 0 */
+    J[3 * 6 + 3] = 1.0;
+    J[4 * 6 + 2] = w * sz; J[4 * 6 + 3] = c_w * s; J[4 * 6 + 4] = 1.0; J[4 * 6 + 5] = w * sth;
+    J[5 * 6 + 5] = 1.0;
+    if (s_out) *s_out = s;
+    if (forward_only && !(fabs(ct) >= KFO_CMIN)) return KFO_GRAZING;
+    return 0;
 }
 
 /* remove the rounding-level asymmetry of the dense loops: C <- (C + C^T)/2 */
@@ -359,12 +440,115 @@ int kfo_update(const double p[6], const double C[36], const double m[3], double 
     return 0;
 }
 
+/* Measurement directions of a hit on its tangent plane ("KF updates are performed on the plane tangent to
+ * the hit radius") [R21]: u1 = azimuthal unit vector at the hit, u2 = z axis (barrel hit: measures r-phi and z) or the
+ * radial unit vector at the hit (disk hit: measures r-phi and r). */
+static void hit_axes(const double m[3], int kind, double u1[3], double u2[3]) {
+    const double rm = sqrt(m[0] * m[0] + m[1] * m[1]);
+    u1[0] = -m[1] / rm; u1[1] = m[0] / rm; u1[2] = 0.0;
+    if (kind == 0) { u2[0] = 0.0; u2[1] = 0.0; u2[2] = 1.0; }
+    else { u2[0] = m[0] / rm; u2[1] = m[1] / rm; u2[2] = 0.0; }
+}
+
+/* chi2 of the 2-D residual of hit m on its tangent plane, H = [u1^T 0; u2^T 0], V = diag(s1^2, s2^2).  -1 if S is not PD. */
+int kfo_chi2_2d(const double p[6], const double C[36], const double m[3], int kind, double s1, double s2, double* chi2) {
+    double u[2][3], r[2], S[2][2];
+    hit_axes(m, kind, u[0], u[1]);
+    for (int a = 0; a < 2; ++a) {
+        r[a] = 0.0;
+        for (int i = 0; i < 3; ++i) r[a] += u[a][i] * (m[i] - p[i]);
+        for (int b = 0; b < 2; ++b) {
+            double v = 0.0;
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j) v += u[a][i] * C[i * 6 + j] * u[b][j];
+            S[a][b] = v;
+        }
+    }
+    S[0][0] += s1 * s1; S[1][1] += s2 * s2;
+    const double det = S[0][0] * S[1][1] - S[0][1] * S[1][0];
+    if (!(S[0][0] > 0.0) || !(det > 0.0)) return -1;
+    *chi2 = (S[1][1] * r[0] * r[0] - 2.0 * S[0][1] * r[0] * r[1] + S[0][0] * r[1] * r[1]) / det;
+    return 0;
+}
+
+/* Kalman update with the 2-D measurement of hit m on its tangent plane [R21]: r = H (m - x), S = H C H^T + V (2x2),
+ * K = C H^T S^-1 (6x2), p <- p + K r, C <- (I-KH) C (I-KH)^T + K V K^T (Joseph form).  Flags as kfo_update. */
+int kfo_update_2d(const double p[6], const double C[36], const double m[3], int kind, double s1, double s2, double pout[6],
+                  double Cout[36], double* chi2) {
+    double u[2][3], r[2], S[2][2], Si[2][2], CHt[6][2], K[6][2], A[36], T[36];
+    const double V[2] = {s1 * s1, s2 * s2};
+    hit_axes(m, kind, u[0], u[1]);
+    for (int a = 0; a < 2; ++a) {
+        r[a] = 0.0;
+        for (int i = 0; i < 3; ++i) r[a] += u[a][i] * (m[i] - p[i]);
+    }
+    for (int i = 0; i < 6; ++i)
+        for (int a = 0; a < 2; ++a) {
+            double v = 0.0;
+            for (int j = 0; j < 3; ++j) v += C[i * 6 + j] * u[a][j];
+            CHt[i][a] = v;
+        }
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) {
+            double v = 0.0;
+            for (int i = 0; i < 3; ++i) v += u[a][i] * CHt[i][b];
+            S[a][b] = v + (a == b ? V[a] : 0.0);
+        }
+    const double det = S[0][0] * S[1][1] - S[0][1] * S[1][0];
+    if (!(S[0][0] > 0.0) || !(det > 0.0)) return KFO_NUMERIC;
+    Si[0][0] = S[1][1] / det; Si[1][1] = S[0][0] / det; Si[0][1] = Si[1][0] = -S[0][1] / det;
+    const double c2 = r[0] * (Si[0][0] * r[0] + Si[0][1] * r[1]) + r[1] * (Si[1][0] * r[0] + Si[1][1] * r[1]);
+    for (int i = 0; i < 6; ++i)
+        for (int a = 0; a < 2; ++a) K[i][a] = CHt[i][0] * Si[0][a] + CHt[i][1] * Si[1][a];
+    for (int i = 0; i < 6; ++i) pout[i] = p[i] + K[i][0] * r[0] + K[i][1] * r[1];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double kh = 0.0;
+            if (j < 3) kh = K[i][0] * u[0][j] + K[i][1] * u[1][j];
+            A[i * 6 + j] = (i == j ? 1.0 : 0.0) - kh;
+        }
+    similarity6(A, C, T);
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) Cout[i * 6 + j] = T[i * 6 + j] + K[i][0] * V[0] * K[j][0] + K[i][1] * V[1] * K[j][1];
+    symmetrize6(Cout);
+    *chi2 = c2;
+    for (int i = 0; i < 6; ++i)
+        if (!isfinite(pout[i])) return KFO_NUMERIC;
+    for (int i = 0; i < 36; ++i)
+        if (!isfinite(Cout[i])) return KFO_NUMERIC;
+    if (!(pout[3] > 0.0) || !isfinite(c2)) return KFO_NUMERIC;
+    return 0;
+}
+
+/* Second step [R20]: from the predicted state on the layer's nominal surface to the surface through hit m -- the
+ * cylinder of the hit's own radius (barrel) or the plane of the hit's own z (disk); C2 = J2 Cp J2^T, no material. */
+static int to_hit_surface(int kind, double bz, int q, const double pp[6], const double Cp[36], const double m[3], double p2[6], double C2[36]) {
+    double J[36], s;
+    int f;
+    if (kind == 0) f = kfo_propagate_near(pp, q, bz, sqrt(m[0] * m[0] + m[1] * m[1]), p2, J, &s);
+    else f = kfo_propagate_z(pp, q, bz, m[2], 0, p2, J, &s, NULL);
+    if (f) return f;
+    similarity6(J, Cp, C2);
+    return 0;
+}
+int kfo_to_hit_surface(int kind, double bz, int q, const double pp[6], const double Cp[36], const double m[3], double p2[6], double C2[36]) {
+    return to_hit_surface(kind, bz, q, pp, Cp, m, p2, C2);
+}
+
 /* One KF step: propagate to layer l, add Q, (optionally) update with hit m.  Used by fit and build.
  * Returns flags; on flags != 0 the outputs are not to be used. */
 static int predict_ci(const double* layers, int l, double bz, const double p[6], const double C[36], int q,
                       double pp[6], double Cp[36], double* ci_out, double* tangency_out) {
     double J[36], Q[36], s, ci;
-    int f = propagate_ex(p, q, bz, LR(layers, l), pp, J, &s, &ci, tangency_out);
+    int f;
+    if (LKIND(layers, l) == 0) f = propagate_ex(p, q, bz, LR(layers, l), pp, J, &s, &ci, tangency_out);
+    else {
+        /* disk: cos of the angle to the disk normal is |cos theta|; kfo_ms_noise divides by sin(theta) cos_inc, the cosine
+           of the 3-D angle to a CYLINDER's normal, so hand it |cos theta| / sin theta */
+        f = kfo_propagate_z(p, q, bz, LR(layers, l), 1, pp, J, &s, &ci);
+        if (tangency_out) *tangency_out = 1e300;
+        ci = ci / sin(p[5]);
+    }
     if (ci_out) *ci_out = ci;
     if (f) return f;
     similarity6(J, C, Cp);
@@ -387,8 +571,11 @@ int kfo_predict(const double* layers, int l, double bz, const double p[6], const
  * crossed: skipped entirely;  NULL -> identity.  Hit of track t on layer l is
  * (hx,hy,hz)[seg_off[ev*L + l] + idx], ev = trk_event ? trk_event[t] : 0.
  * A propagation failure or a failed update sets the status bit, stops the track and keeps the last good state.
- * par [6][ld], cov [36][ld] dense in, outputs alike; chi2/nhits/status [n].  chi2_in/nhits_in may be NULL (=0). */
-int kfo_fit(int n_layers, const double* layers, double bz, int64_t n, int64_t ld, const double* par,
+ * par [6][ld], cov [36][ld] dense in, outputs alike; chi2/nhits/status [n].
+ * hit_mode 0: hits lie on the nominal surface, 3-D update there [R5].  hit_mode 1 [R20, R21]: two-step propagation -- to the
+ * nominal surface (material added there), then on to the hit's own radius (barrel) / z (disk) -- and a 2-D update on the
+ * plane tangent to the hit radius; the state then sits on the hit's surface. */
+int kfo_fit(int n_layers, const double* layers, double bz, int hit_mode, int64_t n, int64_t ld, const double* par,
             const double* cov, const int8_t* q, const double* hx, const double* hy, const double* hz,
             const int64_t* seg_off, const int32_t* hit_idx, const int32_t* trk_event, double* par_out,
             double* cov_out, double* chi2_out, int32_t* nhits_out, uint32_t* status_out) {
@@ -413,7 +600,13 @@ int kfo_fit(int n_layers, const double* layers, double bz, int64_t n, int64_t ld
             }
             int64_t h = seg_off[(int64_t)ev * n_layers + l] + idx;
             double m[3] = {hx[h], hy[h], hz[h]}, c2;
-            f = kfo_update(pp, Cp, m, LSRPHI(layers, l), LSZ(layers, l), LSR(layers, l), pu, Cu, &c2);
+            if (hit_mode == 0) f = kfo_update(pp, Cp, m, LSRPHI(layers, l), LSZ(layers, l), LSR(layers, l), pu, Cu, &c2);
+            else {
+                double p2[6], C2[36];
+                const int kind = LKIND(layers, l);
+                f = to_hit_surface(kind, bz, q[t], pp, Cp, m, p2, C2);
+                if (!f) f = kfo_update_2d(p2, C2, m, kind, LSRPHI(layers, l), kind == 0 ? LSZ(layers, l) : LSR(layers, l), pu, Cu, &c2);
+            }
             if (f) { st |= (uint32_t)f; break; }
             memcpy(p, pu, sizeof p);
             memcpy(C, Cu, sizeof C);

@@ -41,6 +41,16 @@ def _d(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
+def _lt(layers):
+    """Layer table for the C side: [L][8] = r (or the z of a disk), zmax (or the outer radius of a disk), xx0, sig_rphi,
+    sig_z, sig_r, kind (0 barrel, 1 disk), rmin.  A [L][6] table (barrel only) is padded with kind = 0, rmin = 0."""
+    t = np.asarray(layers, dtype=np.float64)
+    if t.shape[1] == 6:
+        t = np.concatenate([t, np.zeros((t.shape[0], 2))], axis=1)
+    assert t.shape[1] == 8
+    return np.ascontiguousarray(t)
+
+
 def _p(a, t=C.c_double):
     return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
 
@@ -85,9 +95,44 @@ def chi2(p, Cm, m, sig_rphi, sig_z, sig_r):
 
 def predict(layers, l, bz, p, Cm, q):
     """propagate to layer l + J C J^T + Q  -> (flags, p_pred, C_pred)"""
-    layers = _d(layers); p = _d(p); Cm = _d(Cm).reshape(36); po = np.zeros(6); Co = np.zeros(36)
+    layers = _lt(layers); p = _d(p); Cm = _d(Cm).reshape(36); po = np.zeros(6); Co = np.zeros(36)
     f = lib().kfo_predict(_p(layers), C.c_int(l), C.c_double(bz), _p(p), _p(Cm), C.c_int(int(q)), _p(po), _p(Co))
     return f, po, Co.reshape(6, 6)
+
+
+def propagate_near(p, q, bz, R):
+    """second step to the nearest crossing of the cylinder R (either direction) -> (flags, p_out, J, s)"""
+    p = _d(p); po = np.zeros(6); J = np.zeros(36); s = C.c_double()
+    f = lib().kfo_propagate_near(_p(p), C.c_int(int(q)), C.c_double(bz), C.c_double(R), _p(po), _p(J), C.byref(s))
+    return f, po, J.reshape(6, 6), s.value
+
+
+def propagate_z(p, q, bz, Z, forward_only=True):
+    """to the plane z = Z -> (flags, p_out, J, s, |cos theta|)"""
+    p = _d(p); po = np.zeros(6); J = np.zeros(36); s = C.c_double(); ci = C.c_double()
+    f = lib().kfo_propagate_z(_p(p), C.c_int(int(q)), C.c_double(bz), C.c_double(Z), C.c_int(1 if forward_only else 0), _p(po), _p(J),
+                              C.byref(s), C.byref(ci))
+    return f, po, J.reshape(6, 6), s.value, ci.value
+
+
+def update_2d(p, Cm, m, kind, s1, s2):
+    """2-D update on the plane tangent to the hit radius -> (flags, p_out, C_out, chi2)"""
+    p = _d(p); Cm = _d(Cm).reshape(36); m = _d(m); po = np.zeros(6); Co = np.zeros(36); c2 = C.c_double()
+    f = lib().kfo_update_2d(_p(p), _p(Cm), _p(m), C.c_int(kind), C.c_double(s1), C.c_double(s2), _p(po), _p(Co), C.byref(c2))
+    return f, po, Co.reshape(6, 6), c2.value
+
+
+def chi2_2d(p, Cm, m, kind, s1, s2):
+    p = _d(p); Cm = _d(Cm).reshape(36); m = _d(m); c2 = C.c_double()
+    rc = lib().kfo_chi2_2d(_p(p), _p(Cm), _p(m), C.c_int(kind), C.c_double(s1), C.c_double(s2), C.byref(c2))
+    return rc, c2.value
+
+
+def to_hit_surface(kind, bz, q, pp, Cp, m):
+    """second step of the two-step propagation -> (flags, p2, C2)"""
+    pp = _d(pp); Cp = _d(Cp).reshape(36); m = _d(m); p2 = np.zeros(6); C2 = np.zeros(36)
+    f = lib().kfo_to_hit_surface(C.c_int(kind), C.c_double(bz), C.c_int(int(q)), _p(pp), _p(Cp), _p(m), _p(p2), _p(C2))
+    return f, p2, C2.reshape(6, 6)
 
 
 def _unpack21(cov21):
@@ -101,10 +146,11 @@ def _unpack21(cov21):
     return out
 
 
-def fit(layers, bz, par, cov21, q, hx, hy, hz, seg_off, hit_idx=None, trk_event=None, n=None):
-    """kf_fit_ref.  par [6][ld], cov21 [21][ld] (any float dtype), q [n] int8.
+def fit(layers, bz, par, cov21, q, hx, hy, hz, seg_off, hit_idx=None, trk_event=None, n=None, hit_mode=0):
+    """kf_fit_ref.  par [6][ld], cov21 [21][ld] (any float dtype), q [n] int8.  hit_mode 1: two-step propagation to each
+    hit's own radius / z and 2-D update on the tangent plane.
     -> dict(par [6][n] f64, cov [n][6][6] f64, chi2 [n], nhits [n], status [n])"""
-    layers = _d(layers)
+    layers = _lt(layers)
     L = layers.shape[0]
     par = _d(par); ld = par.shape[1]
     n = len(q) if n is None else n
@@ -117,7 +163,7 @@ def fit(layers, bz, par, cov21, q, hx, hy, hz, seg_off, hit_idx=None, trk_event=
     if hi is not None:
         assert hi.shape == (L, ld)
     po = np.zeros((6, ld)); co = np.zeros((36, ld)); c2 = np.zeros(n); nh = np.zeros(n, dtype=np.int32); st = np.zeros(n, dtype=np.uint32)
-    lib().kfo_fit(C.c_int(L), _p(layers), C.c_double(bz), C.c_int64(n), C.c_int64(ld), _p(par), _p(cov), _p(q, C.c_int8),
+    lib().kfo_fit(C.c_int(L), _p(layers), C.c_double(bz), C.c_int(hit_mode), C.c_int64(n), C.c_int64(ld), _p(par), _p(cov), _p(q, C.c_int8),
                   _p(hx), _p(hy), _p(hz), _p(seg_off, C.c_int64), _p(hi, C.c_int32), _p(te, C.c_int32),
                   _p(po), _p(co), _p(c2), _p(nh, C.c_int32), _p(st, C.c_uint32))
     return dict(par=po[:, :n], cov=co[:, :n].T.reshape(n, 6, 6), chi2=c2, nhits=nh, status=st)
@@ -162,7 +208,7 @@ def window_bins(phi_c, dphi, z_c, dz, zmax, n_phi, n_z):
 
 def bin_hits(layers, n_events, seg_off, hx, hy, hz, n_phi, n_z):
     """kf_bin_hits_ref -> dict(x, y, z sorted f32, perm i32, bin_off i32)"""
-    layers = _d(layers); L = layers.shape[0]
+    layers = _lt(layers); L = layers.shape[0]
     seg_off = np.ascontiguousarray(seg_off, dtype=np.int64)
     assert len(seg_off) == n_events * L + 1
     hx, hy, hz = _f(hx), _f(hy), _f(hz)
@@ -175,7 +221,7 @@ def bin_hits(layers, n_events, seg_off, hx, hy, hz, n_phi, n_z):
 
 
 def window_lookup(layers, binned, event, layer, phi_c, dphi, z_c, dz, cap):
-    layers = _d(layers)
+    layers = _lt(layers)
     event, layer = _i(event), _i(layer)
     phi_c, dphi, z_c, dz = _f(phi_c), _f(dphi), _f(z_c), _f(dz)
     nq = len(event)
@@ -194,7 +240,7 @@ def kf_build(layers, bz, binned, seg_off, par, cov21, q, seed_event, seed_hit_id
     """kf_build_ref.  -> dict(par [6][n*K], cov [n*K][6][6], chi2, nhits, status [n*K], hit_idx [L][n*K], n_cand [n], counters
     [, margins [n][L][5]: smallest relative distance of the seed's decisions on that layer to the window edge, the chi2
     cut, a rank swap, the propagation / acceptance guards, a tangential crossing; 1e300 = none])"""
-    layers = _d(layers); L = layers.shape[0]
+    layers = _lt(layers); L = layers.shape[0]
     par = _d(par); ld = par.shape[1]
     n = len(q) if n is None else n
     cov = _unpack21(_d(cov21))

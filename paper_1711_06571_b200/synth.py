@@ -34,7 +34,10 @@ def rng_for(config: int, event: int = 0, stream: int = 0) -> np.random.Generator
 
 @dataclass
 class Geometry:
-    """Ideal concentric barrel.  One row per layer, increasing radius."""
+    """Ideal concentric barrel, optionally closed by endcap disks ("cylinder with lids", sec. 4.1).
+    One row per layer in the order a track from the vertex crosses them: barrel layers by increasing radius, then the
+    disks of either side by increasing |z|.  kind 0: cylinder of radius r, |z| <= zmax.  kind 1: disk in the plane
+    z = r (signed), rmin <= radius <= zmax."""
     r: np.ndarray
     zmax: np.ndarray
     xx0: np.ndarray
@@ -42,14 +45,29 @@ class Geometry:
     sig_z: np.ndarray
     sig_r: np.ndarray
     bz: float
+    kind: np.ndarray | None = None
+    rmin: np.ndarray | None = None
+
+    def __post_init__(self):
+        if self.kind is None:
+            self.kind = np.zeros(len(self.r), dtype=np.int32)
+        if self.rmin is None:
+            self.rmin = np.zeros(len(self.r))
 
     @property
     def n_layers(self) -> int:
         return len(self.r)
 
+    @property
+    def has_disks(self) -> bool:
+        return bool(np.any(self.kind != 0))
+
     def layer_table(self) -> np.ndarray:
-        """[L][6] float64: r, zmax, xx0, sig_rphi, sig_z, sig_r."""
-        return np.stack([self.r, self.zmax, self.xx0, self.sig_rphi, self.sig_z, self.sig_r], axis=1).astype(np.float64)
+        """[L][6] float64: r, zmax, xx0, sig_rphi, sig_z, sig_r; with disks [L][8]: ..., kind, rmin."""
+        t = np.stack([self.r, self.zmax, self.xx0, self.sig_rphi, self.sig_z, self.sig_r], axis=1).astype(np.float64)
+        if self.has_disks:
+            t = np.concatenate([t, self.kind[:, None].astype(np.float64), self.rmin[:, None].astype(np.float64)], axis=1)
+        return t
 
 
 def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0) -> Geometry:
@@ -61,6 +79,16 @@ def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0) -> Geometry:
     elif kind == "barrel17":
         r = 4.0 + 4.75 * np.arange(17, dtype=np.float64)
         xx0 = np.where(np.arange(17) % 2 == 0, 0.01, 0.03)
+    elif kind == "lids10":
+        # "cylinder with lids": the 10-layer barrel shortened to |z| <= 50 cm, closed on either side by four
+        # disks at |z| = 60, 75, 90, 105 cm covering 4 <= radius <= 44 cm; same resolutions, x/X0 = 0.02 everywhere
+        rb = 4.0 * np.arange(1, 11, dtype=np.float64)
+        zd = np.array([60.0, 75.0, 90.0, 105.0])
+        r = np.concatenate([rb, zd, -zd])
+        n = len(r)
+        knd = np.concatenate([np.zeros(10, np.int32), np.ones(8, np.int32)])
+        return Geometry(r=r, zmax=np.where(knd == 0, 50.0, 44.0), xx0=np.full(n, 0.02) * xx0_scale, sig_rphi=np.full(n, 0.01),
+                        sig_z=np.full(n, 0.1), sig_r=np.full(n, 0.01), bz=bz, kind=knd, rmin=np.where(knd == 0, 0.0, 4.0))
     else:
         raise ValueError(kind)
     n = len(r)
@@ -105,6 +133,9 @@ def particle_gun(rng: np.random.Generator, n: int, kind: str) -> dict:
     elif kind == "wide":
         pt = np.exp(rng.uniform(np.log(0.3), np.log(100.0), n))
         eta = rng.uniform(-1.5, 1.5, n)
+    elif kind == "forward":      # the flat gun opened up to |eta| < 2.2: barrel, both lids and the transition between them
+        pt = rng.uniform(0.5, 10.0, n)
+        eta = rng.uniform(-2.2, 2.2, n)
     else:
         raise ValueError(kind)
     theta = 2.0 * np.arctan(np.exp(-eta))
@@ -170,6 +201,27 @@ def cross_cylinder(x, y, z, ipt, phi, theta, q, bz, R):
     return ok, xs, ys, zn, phn, s, cosinc
 
 
+def cross_plane(x, y, z, ipt, phi, theta, q, bz, Z):
+    """First crossing of the plane z = Z by the truth helix (simulator only): z advances by cot(theta) per unit of
+    transverse path, so s_T = (Z - z) tan(theta) must be positive; the transverse position turns about the centre of
+    curvature by w s_T.  Returns (ok, x', y', z', phi', s_T, cos_inc = |cos theta|); ok needs s_T > 0 and at most half a turn."""
+    x, y, z, ipt, phi, theta = (np.asarray(a, dtype=np.float64) for a in (x, y, z, ipt, phi, theta))
+    w = -np.asarray(q, dtype=np.float64) * K_CURV * bz * ipt
+    s = (Z - z) * np.tan(theta)
+    straight = np.abs(w) * np.abs(s) < 1e-12
+    ws = np.where(straight, 1.0, w)
+    cx, cy = x - np.sin(phi) / ws, y + np.cos(phi) / ws
+    a = ws * s
+    xr, yr = x - cx, y - cy
+    xc = cx + xr * np.cos(a) - yr * np.sin(a)
+    yc = cy + xr * np.sin(a) + yr * np.cos(a)
+    xs = np.where(straight, x + s * np.cos(phi), xc)
+    ys = np.where(straight, y + s * np.sin(phi), yc)
+    phn = np.where(straight, phi, phi + a)
+    ok = (s > 0) & np.isfinite(s) & (np.abs(w) * s <= np.pi)
+    return ok, xs, ys, np.full(xs.shape, float(Z)) if np.ndim(Z) == 0 else Z, phn, s, np.abs(np.cos(theta))
+
+
 def highland_theta0(ipt, theta, cosinc, xx0):
     """Highland/PDG width of the projected scattering angle, beta = 1, unit charge, p = 1/(ipt sin theta),
     path through the layer = xx0 / (sin(theta) * cos_inc)."""
@@ -180,14 +232,18 @@ def highland_theta0(ipt, theta, cosinc, xx0):
 GEN_MIN_COSINC = 0.2  # a truth crossing shallower than this ends the track (reading A9)
 
 
-def simulate(geom: Geometry, gun: dict, rng: np.random.Generator, ms: bool = True, smear: bool = True) -> dict:
+def simulate(geom: Geometry, gun: dict, rng: np.random.Generator, ms: bool = True, smear: bool = True, jitter: float = 0.0) -> dict:
     """Transport every truth particle outward layer by layer; record the crossing, smear the hit on the
-    cylinder surface (phi by N(0, sig_rphi/R), z by N(0, sig_z)), then apply the thin-scatterer kick.
+    surface (barrel: phi by N(0, sig_rphi/R), z by N(0, sig_z); disk: r-phi by N(0, sig_rphi), radius by N(0, sig_r)),
+    then apply the thin-scatterer kick.
 
-    A track ends (that layer and all outer ones get no hit) when the layer is unreachable, the crossing has
-    |z| > zmax, or cos(incidence) < GEN_MIN_COSINC.
-    Returns hits [L][n][3] (NaN where absent), valid [L][n], truth [L][n][6] = state just outside the layer.
-    """
+    Barrel-only geometry: a track ends (that layer and all outer ones get no hit) when the layer is unreachable, the
+    crossing has |z| > zmax, or cos(incidence) < GEN_MIN_COSINC.  With disks a crossing outside the layer's acceptance
+    only skips that layer (the particle flies on to the lids); unreachable / grazing still ends the track.
+    jitter > 0 ("hits at slightly different radii within a layer"): the sensor that is hit sits at
+    R + U(-jitter, jitter) (barrel) or Z + U(-jitter, jitter) (disk); crossing, hit and scattering happen THERE.
+    Returns hits [L][n][3] (NaN where absent), valid [L][n], truth [L][n][6] = state just outside the layer (at the
+    hit's own surface)."""
     n = len(gun["phi"])
     L = geom.n_layers
     x, y, z = gun["x"].copy(), gun["y"].copy(), gun["z"].copy()
@@ -196,27 +252,55 @@ def simulate(geom: Geometry, gun: dict, rng: np.random.Generator, ms: bool = Tru
     hits = np.full((L, n, 3), np.nan)
     valid = np.zeros((L, n), dtype=bool)
     truth = np.full((L, n, 6), np.nan)
+    lids = geom.has_disks
     for l in range(L):
         R = geom.r[l]
+        disk = geom.kind[l] != 0
+        off = rng.uniform(-jitter, jitter, n) if jitter > 0 else 0.0
         with np.errstate(invalid="ignore", divide="ignore"):
-            ok, xn, yn, zn, phn, s, ci = cross_cylinder(x, y, z, ipt, phi, theta, q, geom.bz, R)
-        ok = ok & alive & (np.abs(zn) <= geom.zmax[l]) & (ci >= GEN_MIN_COSINC)
-        alive = ok
+            if disk:
+                ok, xn, yn, zn, phn, s, ci = cross_plane(x, y, z, ipt, phi, theta, q, geom.bz, R + off)
+                ci3 = ci                                     # cosine of the angle to the disk normal
+                rn = np.hypot(xn, yn)
+                inside = (rn >= geom.rmin[l]) & (rn <= geom.zmax[l])
+            else:
+                ok, xn, yn, zn, phn, s, ci = cross_cylinder(x, y, z, ipt, phi, theta, q, geom.bz, R + off)
+                inside = np.abs(zn) <= geom.zmax[l]
+        if lids:
+            crossed = ok & alive & (ci >= GEN_MIN_COSINC)
+            if not disk:
+                alive = alive & crossed                      # a looper that cannot reach / grazes a cylinder is lost
+            ok = crossed & inside
+        else:
+            ok = ok & alive & inside & (ci >= GEN_MIN_COSINC)
+            alive = ok
         x = np.where(ok, xn, x); y = np.where(ok, yn, y); z = np.where(ok, zn, z); phi = np.where(ok, phn, phi)
         # hit, smeared on the surface
-        e_phi = rng.standard_normal(n) * (geom.sig_rphi[l] / R if smear else 0.0)
-        e_z = rng.standard_normal(n) * (geom.sig_z[l] if smear else 0.0)
-        az = np.arctan2(y, x) + e_phi
-        hits[l, :, 0] = np.where(ok, R * np.cos(az), np.nan)
-        hits[l, :, 1] = np.where(ok, R * np.sin(az), np.nan)
-        hits[l, :, 2] = np.where(ok, z + e_z, np.nan)
+        e1 = rng.standard_normal(n)
+        e2 = rng.standard_normal(n)
+        if disk:
+            rr = np.hypot(x, y)
+            az = np.arctan2(y, x) + e1 * (geom.sig_rphi[l] if smear else 0.0) / np.where(rr > 0, rr, 1.0)
+            rh = rr + e2 * (geom.sig_r[l] if smear else 0.0)
+            hits[l, :, 0] = np.where(ok, rh * np.cos(az), np.nan)
+            hits[l, :, 1] = np.where(ok, rh * np.sin(az), np.nan)
+            hits[l, :, 2] = np.where(ok, z, np.nan)
+        else:
+            Rh = R + off
+            az = np.arctan2(y, x) + e1 * (geom.sig_rphi[l] / Rh if smear else 0.0)
+            hits[l, :, 0] = np.where(ok, Rh * np.cos(az), np.nan)
+            hits[l, :, 1] = np.where(ok, Rh * np.sin(az), np.nan)
+            hits[l, :, 2] = np.where(ok, z + e2 * (geom.sig_z[l] if smear else 0.0), np.nan)
         valid[l] = ok
         # multiple scattering: two orthogonal kicks of width theta0, |p| conserved
         k1 = rng.standard_normal(n)
         k2 = rng.standard_normal(n)
         if ms:
             with np.errstate(invalid="ignore", divide="ignore"):
-                th0 = np.where(ok, highland_theta0(ipt, theta, np.where(ok, ci, 1.0), geom.xx0[l]), 0.0)
+                # highland_theta0 takes the in-plane incidence on a cylinder; for a disk hand it |cos theta| / sin theta so
+                # that sin(theta) * cos_inc is the cosine of the angle to the surface normal in both cases
+                cie = np.where(ok, ci / np.sin(theta) if disk else ci, 1.0)
+                th0 = np.where(ok, highland_theta0(ipt, theta, cie, geom.xx0[l]), 0.0)
             th_new = theta + k1 * th0
             phi = phi + k2 * th0 / np.sin(theta)
             ipt = ipt * np.sin(theta) / np.sin(th_new)
@@ -281,21 +365,24 @@ class FitInputs:
 
 
 FIT_CONFIGS = {
+    # "lids": cylinder with lids + sensors staggered by +-0.3 cm about the nominal surfaces;
+    # fitted with kf_geom.hit_mode = 1 (two-step propagation, 2-D update on the tangent plane)
+    "lids": dict(n=100_000, geom="lids10", gun="forward", jitter=0.3),
     0: dict(n=10_000, geom="barrel10", gun="flat"),
     1: dict(n=1_000_000, geom="barrel10", gun="flat"),
     2: dict(n=1_000_000, geom="barrel17", gun="wide"),
 }
 
 
-def fit_inputs(config: int, n: int | None = None, ms: bool = True, smear: bool = True, event: int = 0,
-               force_index: bool = False, bz: float = 3.8) -> FitInputs:
+def fit_inputs(config, n: int | None = None, ms: bool = True, smear: bool = True, event: int = 0,
+               force_index: bool = False, bz: float = 3.8, jitter: float | None = None) -> FitInputs:
     """Inputs of kf_fit for BASELINE.json configs 0-2 (n overrides the track count, e.g. for tests)."""
     cfg = FIT_CONFIGS[config]
     n = cfg["n"] if n is None else n
     geom = geometry(cfg["geom"], bz=bz, xx0_scale=1.0 if ms else 0.0)
-    rng = rng_for(config, event)
+    rng = rng_for(config if isinstance(config, int) else 100, event)
     gun = particle_gun(rng, n, cfg["gun"])
-    sim = simulate(geom, gun, rng, ms=ms, smear=smear)
+    sim = simulate(geom, gun, rng, ms=ms, smear=smear, jitter=cfg.get("jitter", 0.0) if jitter is None else jitter)
     vtx = np.stack([gun["x"], gun["y"], gun["z"], gun["ipt"], gun["phi"], gun["theta"]], axis=1)
     seed, sig = smear_seed(rng, vtx)
     t = _soa_tracks(seed, sig, gun["q"])
