@@ -42,24 +42,31 @@ typedef enum {
     KF_OK = 0,
     KF_ERR_INVALID_ARG = -1,
     KF_ERR_NULL_PTR = -2,
-    KF_ERR_BAD_GEOM = -3,            /* n_layers outside 1..KF_MAX_LAYERS, radii not increasing, n_phi % 8 != 0 ... */
+    KF_ERR_BAD_GEOM = -3,            /* n_layers outside 1..KF_MAX_LAYERS, radii / disk |z| not increasing, n_phi % 8 != 0 ... */
     KF_ERR_WORKSPACE_TOO_SMALL = -4,
     KF_ERR_CUDA = -5,                /* launch / runtime error; text in kf_last_error() */
     KF_ERR_UNIMPLEMENTED = -6
 } kf_status;
 
 /* per-track status bits */
-#define KF_ST_UNREACHABLE 1u /* layer radius not reached within half a turn, or start radius >= layer radius       */
+#define KF_ST_UNREACHABLE 1u /* layer surface not reached within half a turn, start radius >= layer radius, disk behind */
 #define KF_ST_LEFT_Z 2u      /* kf_build only: predicted |z| beyond zmax + window                                   */
-#define KF_ST_GRAZING 4u     /* cos(incidence) < 0.1 at the crossing                                                */
+#define KF_ST_GRAZING 4u     /* cos(incidence) < 0.1 at the crossing (cylinder: in the transverse plane; disk: |cos theta|) */
 #define KF_ST_NUMERIC 8u     /* innovation matrix not positive definite, non-finite result, or 1/pT <= 0            */
 
-/* One barrel layer: cylinder of radius r [cm], half length zmax [cm], thickness xx0 in radiation lengths at
- * normal incidence, hit resolutions [cm] along r-phi, z and r (sig_r regularises the 3-D update; R5). */
-typedef struct { float r, zmax, xx0, sig_rphi, sig_z, sig_r; } kf_layer;
+/* One layer.  kind 0, barrel: cylinder of radius r [cm], half length zmax [cm].  kind 1, endcap disk ("cylinder with
+ * lids", sec. 4.1; R19): the plane z = r (signed), covering rmin <= radius <= zmax.  Thickness xx0
+ * in radiation lengths at normal incidence, hit resolutions [cm] along r-phi, z and r (in a 3-D update the resolution
+ * along the surface normal -- sig_r for a cylinder, sig_z for a disk -- only regularises; R5). */
+typedef struct { float r, zmax, xx0, sig_rphi, sig_z, sig_r; int32_t kind; float rmin; } kf_layer;
 
-/* Geometry: n_layers cylinders sorted by increasing r; uniform field bz_tesla along z.  `layers` is a HOST array. */
-typedef struct { int32_t n_layers; float bz_tesla; const kf_layer* layers; } kf_geom;
+/* Geometry: n_layers layers in the order a track from the vertex crosses them (cylinders by increasing r, then the
+ * disks of either side by increasing |z|); uniform field bz_tesla along z.  `layers` is a HOST array.
+ * hit_mode 0: hits lie on the nominal surfaces, 3-D update there (R5).  hit_mode 1 (R20, R21;
+ * kf_fit only): two-step propagation -- to the nominal surface, where the material is added, then on to the hit's own
+ * radius (barrel) or z (disk) -- and a 2-D update on the plane tangent to the hit radius (r-phi and z for a barrel
+ * hit, r-phi and r for a disk hit); the state then sits on the hit's surface. */
+typedef struct { int32_t n_layers; float bz_tesla; const kf_layer* layers; int32_t hit_mode; } kf_geom;
 
 /* Per-call tuning options (never change a result beyond rounding; kf_build results do not depend on them at all).
  * Pass NULL for the defaults.  `size` = sizeof(kf_options) of the caller's header (versioning: fields beyond it are
@@ -97,8 +104,8 @@ typedef struct {
 
 /* ---------------------------------------------------------------------------------------------------------
  * kf_fit -- forward (inside-out) Kalman filter over a fixed hit list (DESIGN.md sec. 2 F1-F9).
- * For every track t and every layer l in order of increasing radius with hit_idx[l*ld + t] >= -1:
- *   propagate the state and covariance along the exact helix to the first crossing of the cylinder r_l (Jacobian
+ * For every track t and every layer l in list order with hit_idx[l*ld + t] >= -1:
+ *   propagate the state and covariance along the exact helix to the first crossing of the layer's surface (Jacobian
  *   including the path-length term), add the multiple-scattering noise of the layer (Highland) and, if there is a hit,
  *   update with the 3-D hit (residual, 3x3 innovation inverse, chi2, gain, state and covariance update).
  * hit_idx: [n_layers][seeds->ld] index of the hit within its segment; -1 = layer crossed without a hit (transport and

@@ -28,11 +28,11 @@ class KfError(RuntimeError):
 
 
 class kf_layer(C.Structure):
-    _fields_ = [(n, C.c_float) for n in ("r", "zmax", "xx0", "sig_rphi", "sig_z", "sig_r")]
+    _fields_ = [(n, C.c_float) for n in ("r", "zmax", "xx0", "sig_rphi", "sig_z", "sig_r")] + [("kind", C.c_int32), ("rmin", C.c_float)]
 
 
 class kf_geom(C.Structure):
-    _fields_ = [("n_layers", C.c_int32), ("bz_tesla", C.c_float), ("layers", C.POINTER(kf_layer))]
+    _fields_ = [("n_layers", C.c_int32), ("bz_tesla", C.c_float), ("layers", C.POINTER(kf_layer)), ("hit_mode", C.c_int32)]
 
 
 class kf_options(C.Structure):
@@ -109,15 +109,20 @@ def _stream(stream):
 
 
 class Geom:
-    """Host-side kf_geom built from a [L][6] table (r, zmax, xx0, sig_rphi, sig_z, sig_r) and Bz."""
+    """Host-side kf_geom built from a [L][6] table (r, zmax, xx0, sig_rphi, sig_z, sig_r; cylinders) or a [L][8] table
+    (... kind, rmin; cylinders and endcap disks), Bz and the hit mode (0: hits on the nominal surfaces, 3-D update;
+    1: two-step propagation and 2-D update on the tangent plane)."""
 
-    def __init__(self, layer_table, bz: float):
+    def __init__(self, layer_table, bz: float, hit_mode: int = 0):
         tab = np.asarray(layer_table, dtype=np.float32)
         self.n_layers = tab.shape[0]
         self._arr = (kf_layer * max(1, self.n_layers))()
         for i in range(self.n_layers):
-            self._arr[i] = kf_layer(*[float(v) for v in tab[i]])
-        self.c = kf_geom(self.n_layers, float(bz), C.cast(self._arr, C.POINTER(kf_layer)))
+            row = [float(v) for v in tab[i, :6]]
+            kind, rmin = (int(tab[i, 6]), float(tab[i, 7])) if tab.shape[1] >= 8 else (0, 0.0)
+            self._arr[i] = kf_layer(*row, kind, rmin)
+        self.hit_mode = int(hit_mode)
+        self.c = kf_geom(self.n_layers, float(bz), C.cast(self._arr, C.POINTER(kf_layer)), self.hit_mode)
         self.table = tab
         self.bz = float(bz)
 

@@ -1,4 +1,5 @@
 // kf_api.cu -- error plumbing and small entry points of the C ABI (include/kf.h).
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include "kf_common.cuh"
@@ -25,13 +26,23 @@ int check_geom(const kf_geom* g, const char* who) {
     if (!g->layers) return fail(KF_ERR_NULL_PTR, "%s: geom->layers is NULL", who);
     if (g->n_layers < 1 || g->n_layers > KF_MAX_LAYERS)
         return fail(KF_ERR_BAD_GEOM, "%s: n_layers = %d outside 1..%d", who, g->n_layers, KF_MAX_LAYERS);
+    float last_r = 0.f, last_zp = 0.f, last_zn = 0.f;
     for (int l = 0; l < g->n_layers; ++l) {
         const kf_layer& y = g->layers[l];
-        if (!(y.r > 0.f) || (l && !(y.r > g->layers[l - 1].r)))
-            return fail(KF_ERR_BAD_GEOM, "%s: layer radii must be positive and strictly increasing (layer %d)", who, l);
+        if (y.kind == 0) {
+            if (!(y.r > last_r)) return fail(KF_ERR_BAD_GEOM, "%s: cylinder radii must be positive and strictly increasing (layer %d)", who, l);
+            last_r = y.r;
+        } else if (y.kind == 1) {
+            float& last = y.r > 0.f ? last_zp : last_zn;
+            if (!(fabsf(y.r) > last)) return fail(KF_ERR_BAD_GEOM, "%s: disks of one side must come with strictly increasing |z| (layer %d)", who, l);
+            last = fabsf(y.r);
+            if (!(y.rmin >= 0.f) || !(y.zmax > y.rmin)) return fail(KF_ERR_BAD_GEOM, "%s: disk %d needs 0 <= rmin < outer radius", who, l);
+        } else
+            return fail(KF_ERR_BAD_GEOM, "%s: layer %d has kind %d (0 = cylinder, 1 = disk)", who, l, y.kind);
         if (!(y.zmax > 0.f) || !(y.xx0 >= 0.f) || !(y.sig_rphi > 0.f) || !(y.sig_z > 0.f) || !(y.sig_r > 0.f))
             return fail(KF_ERR_BAD_GEOM, "%s: layer %d needs zmax > 0, xx0 >= 0 and positive resolutions", who, l);
     }
+    if (g->hit_mode != 0 && g->hit_mode != 1) return fail(KF_ERR_BAD_GEOM, "%s: hit_mode = %d not 0 or 1", who, g->hit_mode);
     if (!(g->bz_tesla == g->bz_tesla)) return fail(KF_ERR_BAD_GEOM, "%s: bz_tesla is NaN", who);
     return KF_OK;
 }

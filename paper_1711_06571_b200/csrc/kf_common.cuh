@@ -24,6 +24,7 @@ inline LayerC make_layer(const kf_layer& l) {
     c.r = l.r; c.r2 = l.r * l.r; c.zmax = l.zmax; c.xx0r = l.xx0 * l.r;
     c.var_rphi = l.sig_rphi * l.sig_rphi; c.var_z = l.sig_z * l.sig_z; c.var_r = l.sig_r * l.sig_r;
     c.rcmin = l.r * CMIN;
+    c.xx0 = l.xx0; c.rmin = l.rmin; c.kind = l.kind; c.pad_ = 0;
     return c;
 }
 

@@ -11,7 +11,7 @@
 namespace kf {
 
 struct FitArgs {
-    int32_t n_layers, n_events;
+    int32_t n_layers, n_events, hit_mode;
     float kb;                      // k * Bz
     int64_t n, ld_in, ld_out, ld_idx;
     const float* par; const float* cov; const int8_t* q;
@@ -204,6 +204,66 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_PAIR_MINB) kf_fit_pair_kernel(co
     *reinterpret_cast<uint2*>(a.status_o + t) = make_uint2(0u, 0u);
 }
 
+// ---- "cylinder with lids" (R19-R21): disks in the layer list and / or hit_mode 1 (two-step propagation,
+// 2-D update on the tangent plane).  One track per thread, explicit or identity indices, any event, any hit covariance. ----
+__global__ void __launch_bounds__(FIT_BLOCK) kf_fit_lids_kernel(const __grid_constant__ FitArgs a) {
+    const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
+    if (t >= a.n) return;
+    const float cw = -(float)a.q[t] * a.kb;
+    const int64_t seg = a.trk_event ? (int64_t)a.trk_event[t] * a.n_layers : 0;
+    State s;
+    state_load(s, [&](int i) { return a.par[i * a.ld_in + t]; }, [&](int k) { return a.cov[k * a.ld_in + t]; });
+    float chi2 = 0.0f;
+    int nh = 0;
+    uint32_t st = 0u;
+#pragma unroll 1
+    for (int l = 0; l < a.n_layers; ++l) {
+        int64_t idx = t;
+        if (a.hit_idx) {
+            idx = a.hit_idx[l * a.ld_idx + t];
+            if (idx < -1) continue;
+        }
+        const LayerC ly = a.layer[l];
+        const State before = s;                     // a layer that fails leaves the state of the last good layer
+        uint32_t flag = ly.kind ? predict_disk<false>(s, cw, ly, ly.r) : predict(s, cw, ly);
+        if (flag) { st |= flag; break; }
+        if (idx < 0) continue;                      // hole: transported, material added, no update
+        float mx, my, mz;
+        if (a.trk_event) {
+            const int64_t h = a.seg_off_dev[seg + l] + idx;
+            mx = a.hx[h]; my = a.hy[h]; mz = a.hz[h];
+        } else {
+            mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+        }
+        bool ok;
+        float c2;
+        if (a.hit_mode) {
+            if (ly.kind) flag = predict_disk<true>(s, cw, ly, mz);
+            else {
+                LayerC hl = ly;
+                hl.r2 = fmaf(mx, mx, my * my); hl.rcmin = 0.0f; hl.xx0r = 0.0f;
+                flag = predict<true>(s, cw, hl);
+            }
+            if (flag) { s = before; st |= flag; break; }
+            ok = update_2d(s, mx, my, mz, ly.kind, ly.var_rphi, ly.kind ? ly.var_r : ly.var_z, c2);
+        } else {
+            Ldl3 Si;
+            float r[3];
+            const HitCov V = hit_cov(mx, my, ly);
+            ok = innovation(s, mx, my, mz, V, Si, r, c2);
+            gain_update<false>(s, Si, V, r);
+        }
+        ok = ok && step_finite(s, c2) && s.IT.x > 0.0f && state_finite(s);
+        if (!ok) { s = before; st |= ST_NUMERIC; break; }
+        chi2 += c2;
+        nh += 1;
+    }
+    state_store(s, [&](int i, float v) { a.par_o[i * a.ld_out + t] = v; }, [&](int k, float v) { a.cov_o[k * a.ld_out + t] = v; });
+    a.chi2_o[t] = chi2;
+    a.nhits_o[t] = nh;
+    a.status_o[t] = st;
+}
+
 template <bool IDX, bool EVT>
 static void launch_fit(const FitArgs& a, bool iso, unsigned blocks, cudaStream_t st) {
     if (iso) kf_fit_kernel<IDX, EVT, true><<<blocks, FIT_BLOCK, 0, st>>>(a);
@@ -230,18 +290,19 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     const int tpt = KF_OPT(opt, fit_tracks_per_thread);
     if (tpt < 0 || tpt > 2) return fail(KF_ERR_INVALID_ARG, "kf_fit: options: fit_tracks_per_thread = %d not 0, 1 or 2", tpt);
     FitArgs a;
-    a.n_layers = geom->n_layers; a.n_events = hits->n_events;
+    a.n_layers = geom->n_layers; a.n_events = hits->n_events; a.hit_mode = geom->hit_mode;
     a.kb = KCURV * geom->bz_tesla;
     a.n = seeds->n; a.ld_in = seeds->ld; a.ld_out = out->ld; a.ld_idx = seeds->ld;
     a.par = seeds->par; a.cov = seeds->cov; a.q = seeds->q;
     a.hx = hits->x; a.hy = hits->y; a.hz = hits->z;
     a.seg_off_dev = hits->seg_off_dev; a.hit_idx = hit_idx; a.trk_event = trk_event;
     a.par_o = out->par; a.cov_o = out->cov; a.chi2_o = out->chi2; a.nhits_o = out->nhits; a.status_o = out->status;
-    bool iso = true;
+    bool iso = true, lids = geom->hit_mode != 0;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const int ll = l < geom->n_layers ? l : geom->n_layers - 1;
         a.layer[l] = make_layer(geom->layers[ll]);
         iso = iso && geom->layers[ll].sig_r == geom->layers[ll].sig_rphi;
+        lids = lids || geom->layers[ll].kind != 0;
         const int64_t o = hits->seg_off[ll];
         a.hxl[l] = hits->x + o; a.hyl[l] = hits->y + o; a.hzl[l] = hits->z + o;
     }
@@ -252,6 +313,10 @@ extern "C" int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* h
     }
     const unsigned blocks = (unsigned)((a.n + FIT_BLOCK - 1) / FIT_BLOCK);
     cudaStream_t cs = (cudaStream_t)stream;
+    if (lids) {
+        kf_fit_lids_kernel<<<blocks, FIT_BLOCK, 0, cs>>>(a);
+        return check_launch("kf_fit");
+    }
     if (tpt != 1 && !hit_idx && !trk_event && iso) {
         // two tracks per thread: 8-byte loads and stores of track pairs, so every array and stride must be even
         bool even = (a.ld_in % 2 == 0) && (a.ld_out % 2 == 0);

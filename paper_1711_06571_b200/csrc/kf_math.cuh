@@ -15,7 +15,8 @@ enum : uint32_t { ST_UNREACHABLE = 1u, ST_LEFT_Z = 2u, ST_GRAZING = 4u, ST_NUMER
 // per-layer constants, prepared on the host; two 16-byte vectors so that a layer is two constant-bank loads
 struct alignas(16) LayerC {
     float r2, rcmin, xx0r, var_z;     // radius^2, r * CMIN, xx0 * r, hit variance along z
-    float var_r, var_rphi, zmax, r;   // hit variances along r and r-phi, half length, radius
+    float var_r, var_rphi, zmax, r;   // hit variances along r and r-phi, half length (disk: outer radius), radius (disk: z)
+    float xx0, rmin; int32_t kind, pad_;   // thickness, inner radius of a disk, 0 = cylinder / 1 = disk
 };
 
 // 1-ulp hardware approximations (MUFU.RCP / MUFU.RSQ / MUFU.LG2): no IEEE slow paths, no branches.
@@ -66,6 +67,9 @@ struct Transport {
 
 // Closed-form first crossing of the cylinder r (R2): with u, v the position along / across the direction,
 // E = (r^2 - x^2 - y^2)/2, A = 2(1 + v w) - w^2 E, D = u^2 + E A:  tau = tan(alpha/2)/w solves A tau^2 + 2 u tau - E = 0.
+// NEAR (second step of the two-step propagation, R20): the nearest crossing of a radius close to the state's own,
+// forwards or backwards (E of either sign); the state must move outwards (u > 0).
+template <bool NEAR = false>
 __device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, float cp, float sp, float cot,
                                               const LayerC& ly, Transport& t) {
     const float x = p[0], y = p[1];
@@ -78,8 +82,8 @@ __device__ __forceinline__ uint32_t transport(const float (&p)[6], float cw, flo
     // u >= 0 (moving outwards): tau = E / (u + sqrt D), the smaller positive root whatever the sign of A;
     // u < 0: tau = (sqrt D - u) / A, positive only for A > 0 (else the crossing lies beyond half a turn).
     // Branch-free on purpose: the sign of u is random for seeds smeared about the vertex.
-    const bool fwd = u >= 0.0f;
-    if (!(E > 0.0f) || !(D >= 0.0f) || !(fwd || A > 0.0f)) return ST_UNREACHABLE;
+    const bool fwd = NEAR || u >= 0.0f;
+    if (NEAR ? (!(u > 0.0f) || !(D >= 0.0f)) : (!(E > 0.0f) || !(D >= 0.0f) || !(fwd || A > 0.0f))) return ST_UNREACHABLE;
     const float sq = fsqrt(D);
     const float tau = (fwd ? E : sq - u) * frcp(fwd ? u + sq : A);
     const float th = w * tau;                     // tan(alpha/2)

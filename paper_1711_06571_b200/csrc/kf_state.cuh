@@ -112,13 +112,15 @@ __device__ __forceinline__ bool step_finite(const State& s, float chi2) {
 
 // Predict: transport the state to layer ly, C <- J C J^T + Q (R2-R4).  On a non-zero return s is untouched.
 // cw = -q k Bz.
+// NEAR: second step of the two-step propagation (R20): to the nearest crossing of ly.r2, either direction, no material.
+template <bool NEAR = false>
 __device__ __forceinline__ uint32_t predict(State& s, float cw, const LayerC& ly) {
     const float cp = s.CC.x, ct = s.CC.y, sp = s.SS.x, st = s.SS.y;
     const float ist = frcp(st);
     const float cot = ct * ist;
     const float pp[6] = {s.XY.x, s.XY.y, s.Z, s.IT.x, 0.0f, s.IT.y};       // transport works from the carried sin / cos, not from phi
     Transport t;
-    const uint32_t flag = transport(pp, cw, cp, sp, cot, ly, t);
+    const uint32_t flag = transport<NEAR>(pp, cw, cp, sp, cot, ly, t);
     if (flag) return flag;
 
     // ---- Jacobian (R3): rows x', y' as pairs ab_k = (a_k, b_k), rows z', phi' as pairs cd_k = (c_k, d_k) ----
@@ -169,7 +171,7 @@ __device__ __forceinline__ uint32_t predict(State& s, float cw, const LayerC& ly
 #undef KF_ROWS
     // ---- multiple scattering (R4), evaluated at the arriving state ----
     float q33 = 0.0f, q53 = 0.0f, q44 = 0.0f, q55 = 0.0f;
-    if (ly.xx0r > 0.0f) {
+    if (!NEAR && ly.xx0r > 0.0f) {
         const float iota = s.IT.x;
         const float tms = ly.xx0r * ist * iup;                 // xx0 / (sin(theta) cos(inc))
         const float lg = fmaf(0.038f, flog(tms), 1.0f);
@@ -279,5 +281,221 @@ __device__ __forceinline__ void gain_update(State& s, const Ldl3& F, const HitCo
     s.P1.x = s.P0.y;                      // the three duplicates follow the lower triangle
     s.P2 = f2(s.Q0.x, s.Q1.x);
 }
+
+// =====================================================================================================================
+// "Cylinder with lids" (sec. 4.1; R19-R21): endcap disks, the second propagation step to a hit's own
+// surface, the 2-D update on the plane tangent to the hit radius.  Written on a plain packed covariance (21 elements,
+// every index a compile-time constant): this path is about coverage of the geometry, not the FP32 roof.
+// =====================================================================================================================
+struct Dense { float p[6]; float C[21]; };
+#define KF_CD(d, i, j) (d).C[pk(i, j)]
+
+__device__ __forceinline__ void to_dense(const State& s, Dense& d) {
+    state_store<false>(s, [&](int i, float v) { d.p[i] = v; }, [&](int k, float v) { d.C[k] = v; });
+}
+__device__ __forceinline__ void cov_from_dense(State& s, const Dense& d) {
+    const int ph = s.PH;
+    const float2 cc = s.CC, ss = s.SS;
+    const float dph = s.dph;
+    state_set<true>(s, [&](int i) { return i == 4 ? __int_as_float(ph) : d.p[i]; }, [&](int k) { return d.C[k]; });
+    s.CC = cc; s.SS = ss; s.dph = dph;
+}
+
+// curvature partials f1(a) = (cos a - sin a / a)/a, f2(a) = (sin a - (1 - cos a)/a)/a from the turning angle itself
+__device__ __forceinline__ void curv_partials(float alpha, float sa, float ca, float& f1, float& f2) {
+    const float a2 = alpha * alpha;
+    if (a2 < 0.25f) {
+        f1 = alpha * fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 45360.0f, -1.0f / 840.0f), 1.0f / 30.0f), -1.0f / 3.0f);
+        f2 = fmaf(a2, fmaf(a2, fmaf(a2, fmaf(a2, 1.0f / 403200.0f, -1.0f / 5760.0f), 1.0f / 144.0f), -0.125f), 0.5f);
+    } else {
+        const float ia = 1.0f / alpha;
+        f1 = (ca - sa * ia) * ia;
+        f2 = (sa - (1.0f - ca) * ia) * ia;
+    }
+}
+
+// Transport to the plane z = Z (R19): s = (Z - z) tan(theta); J = fixed-s partials + (dp'/ds)(ds/dp)^T with ds/dz = -tan(theta),
+// ds/dtheta = (Z - z)/cos^2(theta); the z' row vanishes.  NEAR: second step to a hit's own z (either direction, no material,
+// no guards).  On a non-zero return s is untouched.
+template <bool NEAR>
+__device__ __noinline__ uint32_t predict_disk(State& s, float cw, const LayerC& ly, float Z) {
+    const float cp = s.CC.x, ct = s.CC.y, sp = s.SS.x, st = s.SS.y;
+    Dense d;
+    to_dense(s, d);
+    const float x = d.p[0], y = d.p[1], iota = d.p[3];
+    const float w = cw * iota;
+    const float dz = Z - d.p[2];
+    const float tanth = st / ct;
+    const float sT = dz * tanth;
+    if (!(fabsf(sT) <= 3.0e38f)) return ST_UNREACHABLE;
+    if (!NEAR) {
+        if (!(sT > 0.0f) || !(fabsf(w) * sT <= 3.14159265358979f)) return ST_UNREACHABLE;
+        if (!(fabsf(ct) >= CMIN)) return ST_GRAZING;
+    }
+    const float alpha = w * sT;
+    float sa, ca;
+    sincosf(alpha, &sa, &ca);
+    float X, Y;
+    if (fabsf(alpha) < 0.02f) {
+        const float a2 = alpha * alpha;
+        X = sT * fmaf(a2, -1.0f / 6.0f, 1.0f);
+        Y = sT * 0.5f * alpha * fmaf(a2, -1.0f / 12.0f, 1.0f);
+    } else {
+        const float iw = 1.0f / w;
+        X = sa * iw;
+        Y = (1.0f - ca) * iw;
+    }
+    const float dx = fmaf(cp, X, -sp * Y), dy = fmaf(sp, X, cp * Y);
+    const float cpn = fmaf(cp, ca, -sp * sa), spn = fmaf(sp, ca, cp * sa);
+    float f1, f2;
+    curv_partials(alpha, sa, ca, f1, f2);
+    const float cs2 = cw * sT * sT;
+    const float Fxi = cs2 * fmaf(cp, f1, -sp * f2), Fyi = cs2 * fmaf(sp, f1, cp * f2);
+    const float sz = -tanth, sth = dz / (ct * ct);
+    // rows of J: x' = (1, 0, a2, a3, a4, a5), y' = (0, 1, b2, b3, b4, b5), z' = 0, phi' = (0, 0, d2, d3, 1, d5); 1/pT and theta unit rows
+    const float a2_ = cpn * sz, a3 = Fxi, a4 = -dy, a5 = cpn * sth;
+    const float b2_ = spn * sz, b3 = Fyi, b4 = dx, b5 = spn * sth;
+    const float d2 = w * sz, d3 = cw * sT, d5 = w * sth;
+    float T0[6], T1[6], T4[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        T0[k] = fmaf(a2_, KF_CD(d, 2, k), fmaf(a3, KF_CD(d, 3, k), fmaf(a4, KF_CD(d, 4, k), fmaf(a5, KF_CD(d, 5, k), KF_CD(d, 0, k)))));
+        T1[k] = fmaf(b2_, KF_CD(d, 2, k), fmaf(b3, KF_CD(d, 3, k), fmaf(b4, KF_CD(d, 4, k), fmaf(b5, KF_CD(d, 5, k), KF_CD(d, 1, k)))));
+        T4[k] = fmaf(d2, KF_CD(d, 2, k), fmaf(d3, KF_CD(d, 3, k), fmaf(d5, KF_CD(d, 5, k), KF_CD(d, 4, k))));
+    }
+    auto colx = [&](const float (&T)[6]) { return fmaf(a2_, T[2], fmaf(a3, T[3], fmaf(a4, T[4], fmaf(a5, T[5], T[0])))); };
+    auto coly = [&](const float (&T)[6]) { return fmaf(b2_, T[2], fmaf(b3, T[3], fmaf(b4, T[4], fmaf(b5, T[5], T[1])))); };
+    auto colp = [&](const float (&T)[6]) { return fmaf(d2, T[2], fmaf(d3, T[3], fmaf(d5, T[5], T[4]))); };
+    Dense n;
+    KF_CD(n, 0, 0) = colx(T0);
+    KF_CD(n, 1, 0) = colx(T1); KF_CD(n, 1, 1) = coly(T1);
+    KF_CD(n, 2, 0) = 0.0f; KF_CD(n, 2, 1) = 0.0f; KF_CD(n, 2, 2) = 0.0f;
+    KF_CD(n, 3, 0) = T0[3]; KF_CD(n, 3, 1) = T1[3]; KF_CD(n, 3, 2) = 0.0f; KF_CD(n, 3, 3) = KF_CD(d, 3, 3);
+    KF_CD(n, 4, 0) = colx(T4); KF_CD(n, 4, 1) = coly(T4); KF_CD(n, 4, 2) = 0.0f; KF_CD(n, 4, 3) = T4[3]; KF_CD(n, 4, 4) = colp(T4);
+    KF_CD(n, 5, 0) = T0[5]; KF_CD(n, 5, 1) = T1[5]; KF_CD(n, 5, 2) = 0.0f; KF_CD(n, 5, 3) = KF_CD(d, 5, 3); KF_CD(n, 5, 4) = T4[5]; KF_CD(n, 5, 5) = KF_CD(d, 5, 5);
+    if (!NEAR && ly.xx0 > 0.0f) {      // scattering (R4) with the path through the disk xx0 / |cos theta|
+        const float ist = 1.0f / st;
+        const float tms = ly.xx0 / fabsf(ct);
+        const float lg = fmaf(0.038f, flog(tms), 1.0f);
+        const float h = 0.0136f * iota * st * lg;
+        const float v = h * h * tms;
+        const float icot = iota * ct * ist;
+        KF_CD(n, 5, 5) += v;
+        KF_CD(n, 4, 4) += v * ist * ist;
+        KF_CD(n, 3, 3) += icot * icot * v;
+        KF_CD(n, 5, 3) += -icot * v;
+    }
+    n.p[0] = x + dx; n.p[1] = y + dy; n.p[2] = Z; n.p[3] = iota; n.p[5] = d.p[5];
+    s.PH += phi_fix_small(alpha);
+    s.CC.x = cpn; s.SS.x = spn;
+    cov_from_dense(s, n);
+    return 0u;
+}
+
+// 2-D update on the plane tangent to the hit radius (R21).  The position block is turned into the hit's own (radial,
+// azimuthal, z) frame; a barrel hit measures (azimuthal, z), a disk hit (azimuthal, radial) -- for the disk the radial and
+// z coordinates swap places, so that the measured pair is always coordinates (1, 2).  Columns of the measured pair are
+// rebuilt as K V (exact, no cancellation; kf_state.cuh gain_update), the rest as C - K (C H^T)^T.
+// v1, v2: variances along the azimuth and along z (barrel) / the radius (disk).  false: S not positive definite.
+static __device__ __noinline__ bool update_2d(State& s, float mx, float my, float mz, int kind, float v1, float v2, float& chi2) {
+    Dense d;
+    to_dense(s, d);
+    const float irm = rsqrtf(fmaf(mx, mx, my * my));
+    const float cn = mx * irm, sn = my * irm;
+    // full symmetric matrix in the rotated frame q = (n, t, z): rows / columns 0, 1 turned by the hit's azimuth
+    float c[6][6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+#pragma unroll
+        for (int j = 0; j < 6; ++j) c[i][j] = KF_CD(d, i, j);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {       // rows
+        const float a = c[0][k], b = c[1][k];
+        c[0][k] = fmaf(cn, a, sn * b); c[1][k] = fmaf(-sn, a, cn * b);
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {       // columns
+        const float a = c[k][0], b = c[k][1];
+        c[k][0] = fmaf(cn, a, sn * b); c[k][1] = fmaf(-sn, a, cn * b);
+    }
+    const float dx = mx - d.p[0], dy = my - d.p[1];
+    float rq[3] = {fmaf(cn, dx, sn * dy), fmaf(-sn, dx, cn * dy), mz - d.p[2]};
+    if (kind) {                         // disk: swap the radial and the z coordinate
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { const float t = c[0][k]; c[0][k] = c[2][k]; c[2][k] = t; }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { const float t = c[k][0]; c[k][0] = c[k][2]; c[k][2] = t; }
+        const float t = rq[0]; rq[0] = rq[2]; rq[2] = t;
+    }
+    const float S11 = c[1][1] + v1, S12 = c[2][1], S22 = c[2][2] + v2;
+    const float det = fmaf(S11, S22, -S12 * S12);
+    const bool ok = (S11 > 0.0f) && (det > 0.0f);
+    const float idet = 1.0f / det;
+    const float r1 = rq[1], r2 = rq[2];
+    chi2 = (fmaf(S22 * r1, r1, fmaf(-2.0f * S12 * r1, r2, S11 * r2 * r2))) * idet;
+    float K1[6], K2[6], dq[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        K1[i] = fmaf(c[i][1], S22, -c[i][2] * S12) * idet;
+        K2[i] = fmaf(-c[i][1], S12, c[i][2] * S11) * idet;
+        dq[i] = fmaf(K1[i], r1, K2[i] * r2);
+    }
+    // covariance: unmeasured block with the old measured columns, measured columns as K V
+    constexpr int U[4] = {0, 3, 4, 5};
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b <= a; ++b) {
+            const int i = U[a], j = U[b];
+            const float v = fmaf(-K1[i], c[j][1], fmaf(-K2[i], c[j][2], c[i][j]));
+            c[i][j] = v; c[j][i] = v;
+        }
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { c[i][1] = K1[i] * v1; c[i][2] = K2[i] * v2; }
+    c[1][2] = c[2][1];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { c[1][i] = c[i][1]; c[2][i] = c[i][2]; }
+    if (kind) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { const float t = c[0][k]; c[0][k] = c[2][k]; c[2][k] = t; }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { const float t = c[k][0]; c[k][0] = c[k][2]; c[k][2] = t; }
+        const float t = dq[0]; dq[0] = dq[2]; dq[2] = t;
+    }
+    // back to (x, y): q = R x  =>  x = R^T q
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float a = c[0][k], b = c[1][k];
+        c[0][k] = fmaf(cn, a, -sn * b); c[1][k] = fmaf(sn, a, cn * b);
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float a = c[k][0], b = c[k][1];
+        c[k][0] = fmaf(cn, a, -sn * b); c[k][1] = fmaf(sn, a, cn * b);
+    }
+    Dense n;
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+#pragma unroll
+        for (int j = 0; j <= i; ++j) KF_CD(n, i, j) = c[i][j];
+    n.p[0] = d.p[0] + fmaf(cn, dq[0], -sn * dq[1]);
+    n.p[1] = d.p[1] + fmaf(sn, dq[0], cn * dq[1]);
+    n.p[2] = d.p[2] + dq[2];
+    n.p[3] = d.p[3] + dq[3];
+    n.p[5] = d.p[5] + dq[5];
+    s.PH += phi_fix_small(dq[4]);
+    s.dph = dq[4];
+    if (fmaxf(fabsf(dq[4]), fabsf(dq[5])) < 0.06f) {
+        rotate_poly2(s.CC, s.SS, f2(dq[4], dq[5]));
+    } else {
+        float sp_, cp_, st_, ct_;
+        sincosf(phi_float(s.PH), &sp_, &cp_);
+        sincosf(n.p[5], &st_, &ct_);
+        s.CC = f2(cp_, ct_); s.SS = f2(sp_, st_);
+    }
+    cov_from_dense(s, n);
+    return ok;
+}
+#undef KF_CD
 
 }  // namespace kf

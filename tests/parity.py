@@ -43,7 +43,8 @@ def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None, chi2_scale=1.
             k += 1
     s = np.sqrt(np.einsum("nii->ni", rc))
     s[:, 0] = s[:, 1] = np.sqrt(rc[:, 0, 0] + rc[:, 1, 1])
-    cerr = np.abs(gc - rc) / (COV_REL * s[:, :, None] * s[:, None, :])
+    with np.errstate(invalid="ignore", divide="ignore"):      # a state on a disk has C_zz = 0 exactly on both sides: 0/0 counts as 0
+        cerr = np.nan_to_num(np.abs(gc - rc) / (COV_REL * s[:, :, None] * s[:, None, :]), nan=0.0, posinf=np.inf)
     if cov_scale is not None:
         cerr = cerr / np.asarray(cov_scale, dtype=np.float64)[None, :, :]
     c2 = np.abs(gpu["chi2"].astype(np.float64)[sel] - ref["chi2"][sel]) / (chi2_scale * CHI2_REL * np.maximum(ref["chi2"][sel], 1.0))
