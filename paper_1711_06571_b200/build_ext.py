@@ -32,7 +32,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", SO]
+    extra = os.environ.get("KF_NVCC_EXTRA", "").split()      # e.g. -DKF_SCAN_B=8 when sweeping a kernel constant
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", SO]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode:
         sys.stderr.write(res.stdout + res.stderr)

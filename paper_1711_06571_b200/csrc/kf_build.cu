@@ -34,14 +34,26 @@ namespace kf {
 #define KF_BUILD_TPS 2     // threads per seed of the tile
 #endif
 constexpr int BUILD_MAX_NT = 256;         // threads per block: 64, 128 or 256 (KF_BUILD_TPS x the seeds of the tile)
-constexpr int BUILD_THREADS_PER_SM = 512; // 128 registers per thread
+#ifndef KF_BUILD_TPSM
+#define KF_BUILD_TPSM 512
+#endif
+constexpr int BUILD_THREADS_PER_SM = KF_BUILD_TPSM; // 512: 128 registers per thread
 constexpr int NREC = 33;                  // words per candidate record
+#ifndef KF_TILE_WAVE
+#define KF_TILE_WAVE 128   // seeds per block when the whole job is one wave of such blocks
+#endif
+#ifndef KF_TILE_SMALL
+#define KF_TILE_SMALL 32   // seeds per block otherwise
+#endif
 #ifndef KF_SCAN_BATCH
 #define KF_SCAN_BATCH 4
 #endif
 constexpr int SCAN_BATCH = KF_SCAN_BATCH;  // hits requested together in the window scan
 constexpr int HITPOS_NONE = 0x7fffffff;
-constexpr int LIST_BYTES_PER_THREAD = 192; // shared memory for the per-candidate child lists, per thread of the block
+#ifndef KF_LIST_BYTES
+#define KF_LIST_BYTES 192
+#endif
+constexpr int LIST_BYTES_PER_THREAD = KF_LIST_BYTES; // shared memory for the per-candidate child lists, per thread of the block
 enum { W_TRIG = 27, W_CHI2 = 31, W_META = 32 };
 // meta word of a record: bits 0-7 nhits, bit 8 finished, bits 16-19 status
 // info word of a parent in a round: bits 0-7 nhits, bit 8 finished (child inherits the unchanged state), bits 16-19 status to add
@@ -446,8 +458,14 @@ __device__ __noinline__ void build_output(const BuildArgs& a, int64_t s0, int c)
 }
 
 template <int NT, bool ISO>
-__global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel(const __grid_constant__ BuildArgs a) {
+__global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel(const __grid_constant__ BuildArgs ga) {
     extern __shared__ __align__(16) unsigned char smem[];
+    // The phase bodies are separate functions that take the arguments by reference: a copy in shared memory keeps their
+    // reads of it short (a reference to the kernel parameters makes every one a generic load of the parameter space).
+    __shared__ BuildArgs sa;
+    for (int w = threadIdx.x; w < (int)(sizeof(BuildArgs) / 4); w += NT) ((int*)&sa)[w] = ((const int*)&ga)[w];
+    __syncthreads();
+    const BuildArgs& a = sa;
     const int S = a.S, K = a.K, L = a.n_layers, ncap = a.ncap, SK = S * K;
     const BuildSmem m = build_smem(S, K, ncap, L);
     int* s_nc = (int*)(smem + m.nc); int* s_off = (int*)(smem + m.off);
@@ -595,19 +613,19 @@ static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K, const kf_optio
     const bool automatic = S == 0;
     if (automatic)   // one wave of 128-seed tiles when the job is that small (latency-sized), otherwise small tiles: more
                      // independent blocks per SM, so that the block-level barriers of one tile overlap work of another
-        S = n_seeds <= (int64_t)128 * 2 * sm_count() ? 128 : 32;
+        S = n_seeds <= (int64_t)KF_TILE_WAVE * 2 * sm_count() ? KF_TILE_WAVE : KF_TILE_SMALL;
     for (;;) {
         p.S = S;
         p.NT = S * KF_BUILD_TPS <= 64 ? 64 : (S * KF_BUILD_TPS <= 128 ? 128 : 256);
         const int SK = S * K;
         p.ncap = std::min(SK, std::max(std::max(K, 32), (LIST_BYTES_PER_THREAD * p.NT / (8 * K)) & ~31));
         p.smem = (size_t)build_smem(S, K, p.ncap, n_layers).total;
-        if (!automatic || p.smem <= 200 * 1024 || S <= 16) break;      // large K and many layers: a smaller tile fits
+        if (!automatic || p.smem + sizeof(BuildArgs) <= 200 * 1024 || S <= 16) break;      // large K and many layers: a smaller tile fits
         S /= 2;
     }
     const int SK = p.S * K;
     p.n_tiles = (n_seeds + p.S - 1) / p.S;
-    const int by_smem = (int)std::max<size_t>(1, (size_t)(227 * 1024) / (p.smem + 1024));
+    const int by_smem = (int)std::max<size_t>(1, (size_t)(227 * 1024) / (p.smem + sizeof(BuildArgs) + 1024));
     int64_t resident = (int64_t)sm_count() * std::min(BUILD_THREADS_PER_SM / p.NT, by_smem);
     if (max_blocks > 0) resident = std::min<int64_t>(resident, max_blocks);
     p.grid = (int)std::min<int64_t>(std::max<int64_t>(p.n_tiles, 1), resident);
@@ -661,7 +679,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     if (!c.par || !c.cov || !c.q || !c.chi2 || !c.nhits || !c.status || !out->hit_idx || !out->n_cand)
         return fail(KF_ERR_NULL_PTR, "kf_build: NULL output array");
     if (!ws || ws_bytes < p.total) return fail(KF_ERR_WORKSPACE_TOO_SMALL, "kf_build: workspace %zu < %zu bytes", ws_bytes, p.total);
-    if (p.smem > 227 * 1024) return fail(KF_ERR_INVALID_ARG, "kf_build: tile of %d seeds with K = %d needs %zu bytes of shared memory (> 227 KB)", p.S, K, p.smem);
+    if (p.smem + sizeof(BuildArgs) > 227 * 1024) return fail(KF_ERR_INVALID_ARG, "kf_build: tile of %d seeds with K = %d needs %zu bytes of shared memory (> 227 KB)", p.S, K, p.smem);
     BuildArgs a;
     a.n_layers = geom->n_layers; a.first_layer = first_layer; a.K = K; a.n_phi = binned->n_phi; a.n_z = binned->n_z;
     a.S = p.S; a.ncap = p.ncap; a.n_tiles = p.n_tiles;

@@ -72,6 +72,36 @@ def test_bin_hits_empty_segments_and_edges():
         b.kf_bin_hits(b.Geom(lt, 3.8), hits, 256, 16, ws=torch.empty(16, dtype=torch.uint8, device="cuda"))
 
 
+def test_bin_hits_both_paths_and_crowded_bins():
+    """Few large and many small segments, few and very many bins, and bins with many hits (more than a warp's worth, which
+    the warp orders together): the index stays bit-exact and crowded bins keep the order of the original indices."""
+    from paper_1711_06571_b200 import binding as b
+    rng = np.random.default_rng(7)
+    lt = synth.geometry("barrel10").layer_table()[:2]
+    n0, n1 = 30000, 5000                                   # event 0: one large segment (layer 0) and a small one
+    r = np.r_[np.full(n0, lt[0][0]), np.full(n1, lt[1][0])]
+    phi = rng.uniform(-np.pi, np.pi, n0 + n1)
+    phi[:200] = 0.3                                        # 200 hits in one bin
+    z = rng.uniform(-100, 100, n0 + n1)
+    z[:200] = 12.0
+    x = (r * np.cos(phi)).astype(np.float32); y = (r * np.sin(phi)).astype(np.float32); z = z.astype(np.float32)
+    seg_off = np.array([0, n0, n0 + n1], np.int64)
+    for n_phi, n_z in ((256, 16), (4096, 16), (64, 4)):     # 4 096, 65 536 and 256 bins per segment
+        hits = b.Hits(x, y, z, seg_off, 1)
+        g = b.kf_bin_hits(b.Geom(lt, 3.8), hits, n_phi, n_z)
+        torch.cuda.synchronize()
+        assert_binned_equal(g.to_host(), o.bin_hits(lt, 1, seg_off, x, y, z, n_phi, n_z))
+    # many small segments with a crowded bin each
+    ne = 100
+    xs = np.tile(x[:4000], ne); ys = np.tile(y[:4000], ne); zs = np.tile(z[:4000], ne)
+    lt1 = lt[:1]
+    seg = np.arange(ne + 1, dtype=np.int64) * 4000
+    hits = b.Hits(xs, ys, zs, seg, ne)
+    g = b.kf_bin_hits(b.Geom(lt1, 3.8), hits, 256, 16)
+    torch.cuda.synchronize()
+    assert_binned_equal(g.to_host(), o.bin_hits(lt1, ne, seg, xs, ys, zs, 256, 16))
+
+
 def test_window_lookup_bit_exact():
     from paper_1711_06571_b200 import binding as b
     bi = synth.build_inputs(3, n_events=2, tracks=1000)
