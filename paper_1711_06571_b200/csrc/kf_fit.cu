@@ -168,6 +168,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_PAIR_MINB) kf_fit_pair_kernel(co
         float s0, c0, s1, c1;
         sincosf(S.p[4].v.x, &s0, &c0); sincosf(S.p[4].v.y, &s1, &c1);
         S.g.sp = mk(s0, s1); S.g.cp = mk(c0, c1);
+        S.pha = phi_fix(S.p[4].v.x); S.phb = phi_fix(S.p[4].v.y);
         sincosf(S.p[5].v.x, &s0, &c0); sincosf(S.p[5].v.y, &s1, &c1);
         S.g.st = mk(s0, s1); S.g.ct = mk(c0, c1);
     }
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, KF_PAIR_MINB) kf_fit_pair_kernel(co
     }
     // F9
     auto st2 = [](float* p_, V v) { *reinterpret_cast<float2*>(p_) = v.v; };
-    S.p[4] = mk(wrap_phi(S.p[4].v.x), wrap_phi(S.p[4].v.y));
+    S.p[4] = mk(phi_float(S.pha), phi_float(S.phb));
 #pragma unroll
     for (int i = 0; i < 6; ++i) st2(a.par_o + i * a.ld_out + t, S.p[i]);
 #pragma unroll

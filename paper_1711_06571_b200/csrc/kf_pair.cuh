@@ -7,6 +7,7 @@
 // Same formulas and operation order as kf_state.cuh (R2-R5); shares nothing with oracle/.
 #pragma once
 #include "kf_math.cuh"
+#include "kf_state.cuh"
 
 namespace kf {
 namespace pair {
@@ -35,7 +36,7 @@ __device__ __forceinline__ bool both_lt(V a, float b) { return a.v.x < b && a.v.
 __device__ __forceinline__ V abs_(V a) { return mk(fabsf(a.v.x), fabsf(a.v.y)); }
 
 struct Trig2 { V cp, sp, st, ct; };
-struct State2 { V p[6]; V C[21]; Trig2 g; };
+struct State2 { V p[6]; V C[21]; Trig2 g; int pha, phb; };   // p[4] is unused: phi is the fixed-point pair (pha, phb), see kf_state.cuh
 
 // rotate (c, s) by d, |d| < 0.06 (polynomial, then one Newton step back to unit norm)
 __device__ __forceinline__ void rotate_poly(V& c, V& s, V d) {
@@ -153,7 +154,8 @@ __device__ __forceinline__ bool predict(State2& S, V cw, const LayerC& ly) {
     C[pk(4, 0)] = n40; C[pk(4, 1)] = n41; C[pk(4, 2)] = n42; C[pk(4, 3)] = T43; C[pk(4, 4)] = n44 + q44;
     C[pk(5, 0)] = T05; C[pk(5, 1)] = T15; C[pk(5, 2)] = T25; C[pk(5, 3)] = C[pk(5, 3)] + q53; C[pk(5, 4)] = T45; C[pk(5, 5)] = C[pk(5, 5)] + q55;
 #undef CC
-    p[0] = xn; p[1] = yn; p[2] = zn; p[4] = p[4] + alpha;
+    p[0] = xn; p[1] = yn; p[2] = zn;
+    S.pha += phi_fix_small(alpha.v.x); S.phb += phi_fix_small(alpha.v.y);
     S.g.cp = cpn; S.g.sp = spn;
     return true;
 }
@@ -195,7 +197,7 @@ __device__ __forceinline__ bool update(State2& S, V mx, V my, V mz, float vr, fl
     for (int i = 0; i < 4; ++i) p[i] = fma(K[i][0], r0, fma(K[i][1], r1, fma(K[i][2], r2, p[i])));
     const V dphi = fma(K[4][0], r0, fma(K[4][1], r1, K[4][2] * r2));
     const V dth = fma(K[5][0], r0, fma(K[5][1], r1, K[5][2] * r2));
-    p[4] = p[4] + dphi;
+    S.pha += phi_fix_small(dphi.v.x); S.phb += phi_fix_small(dphi.v.y);
     p[5] = p[5] + dth;
     ok = ok && both_lt(abs_(dphi), 0.06f) && both_lt(abs_(dth), 0.06f);
     rotate_poly(S.g.cp, S.g.sp, dphi);
@@ -214,14 +216,15 @@ __device__ __forceinline__ bool update(State2& S, V mx, V my, V mz, float vr, fl
         if (i >= 2) C[pk(i, 2)] = K[i][2] * vz;
     }
     // finite and physical: 0 * x is NaN for x = Inf or NaN
-    const V z = fma(chi2, 0.0f, fma(p[0] + p[1], 0.0f, fma(p[2] + p[3], 0.0f, (p[4] + p[5]) * 0.0f)));
+    const V z = fma(chi2, 0.0f, fma(p[0] + p[1], 0.0f, fma(p[2] + p[3], 0.0f, (dphi + p[5]) * 0.0f)));
     return ok && z.v.x == 0.0f && z.v.y == 0.0f && both_gt(p[3], 0.0f);
 }
 
 __device__ __forceinline__ bool all_finite(const State2& S) {
     V acc = S.p[0] * 0.0f;
 #pragma unroll
-    for (int i = 1; i < 6; ++i) acc = fma(S.p[i], 0.0f, acc);
+    for (int i = 1; i < 6; ++i)
+        if (i != 4) acc = fma(S.p[i], 0.0f, acc);
 #pragma unroll
     for (int i = 0; i < 21; ++i) acc = fma(S.C[i], 0.0f, acc);
     return acc.v.x == 0.0f && acc.v.y == 0.0f;
