@@ -659,6 +659,23 @@ int kfo_z_bin(float z, float zmax, int n_z) {
     return iz;
 }
 
+/* X2 for any layer [R22]: row of coordinate v in [lo, hi) cut into n rows.  A barrel layer bins z in [-zmax, zmax) (then this
+ * is kfo_z_bin bit for bit: z - (-zmax) = z + zmax and zmax - (-zmax) = 2 zmax are the same fp32 operations); a disk bins
+ * the radius of the hit, rho = fl32(sqrt(fl32(fl32(x x) + fl32(y y)))), in [rmin, rmax). */
+int kfo_row_bin(float v, float lo, float hi, int n) {
+    float inv = (float)n / (hi - lo);
+    float f = floorf((v - lo) * inv);
+    return (f >= (float)n) ? n - 1 : (f < 0.0f ? 0 : (int)f);
+}
+float kfo_hit_rho(float x, float y) {
+    float xx = x * x, yy = y * y;
+    return sqrtf(xx + yy);
+}
+static void row_range(const double* layers, int l, float* lo, float* hi) {
+    if (LKIND(layers, l) == 0) { *lo = -(float)LZMAX(layers, l); *hi = (float)LZMAX(layers, l); }
+    else { *lo = (float)LRMIN(layers, l); *hi = (float)LZMAX(layers, l); }
+}
+
 /* B0: sorted order = ascending (global bin, original index).  seg_off [n_events*L + 1]; outputs sx, sy, sz,
  * perm [n_hits] (sorted position -> original index within the segment), bin_off [n_events*L*n_z*n_phi + 1]. */
 int kfo_bin_hits(int n_layers, const double* layers, int n_events, const int64_t* seg_off, const float* hx,
@@ -673,10 +690,12 @@ int kfo_bin_hits(int n_layers, const double* layers, int n_events, const int64_t
     int32_t* key = (int32_t*)malloc((size_t)(n_hits > 0 ? n_hits : 1) * sizeof(int32_t));
     for (int64_t sg = 0; sg < nseg; ++sg) {
         int l = (int)(sg % n_layers);
-        float zmax = (float)LZMAX(layers, l);
+        float lo, hi;
+        row_range(layers, l, &lo, &hi);
+        const int disk = LKIND(layers, l) != 0;
         int32_t* cnt = (int32_t*)calloc((size_t)bins_per_seg + 1, sizeof(int32_t));
         for (int64_t h = seg_off[sg]; h < seg_off[sg + 1]; ++h) {
-            int b = kfo_z_bin(hz[h], zmax, n_z) * n_phi + kfo_phi_bin(hx[h], hy[h], n_phi, tab);
+            int b = kfo_row_bin(disk ? kfo_hit_rho(hx[h], hy[h]) : hz[h], lo, hi, n_z) * n_phi + kfo_phi_bin(hx[h], hy[h], n_phi, tab);
             key[h] = b;
             cnt[b + 1] += 1;
         }
@@ -694,9 +713,10 @@ int kfo_bin_hits(int n_layers, const double* layers, int n_events, const int64_t
     return 0;
 }
 
-/* X3: window (phi_c +- dphi, z_c +- dz) -> first phi bin, number of phi bins (wrapping), z rows [iz_lo, iz_hi] */
-void kfo_window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, int n_phi, int n_z, int* first, int* n_b,
-                     int* iz_lo, int* iz_hi) {
+/* X3: window (phi_c +- dphi, c +- d) -> first phi bin, number of phi bins (wrapping), rows [iz_lo, iz_hi] of the row
+ * coordinate (z on a barrel layer, radius on a disk [R22]) binned in [lo, hi) */
+void kfo_window_bins_row(float phi_c, float dphi, float z_c, float dz, float lo, float hi, int n_phi, int n_z, int* first, int* n_b,
+                         int* iz_lo, int* iz_hi) {
     float inv_dphi = (float)((double)n_phi / (2.0 * KFO_PI));
     if (!(dphi * inv_dphi < (float)n_phi)) { /* half width of a full turn or more: every bin, starting at bin 0 [X3] */
         *first = 0;
@@ -710,8 +730,12 @@ void kfo_window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, i
         *n_b = nb;
         *first = ((b_lo % n_phi) + n_phi) % n_phi;
     }
-    *iz_lo = kfo_z_bin(z_c - dz, zmax, n_z);
-    *iz_hi = kfo_z_bin(z_c + dz, zmax, n_z);
+    *iz_lo = kfo_row_bin(z_c - dz, lo, hi, n_z);
+    *iz_hi = kfo_row_bin(z_c + dz, lo, hi, n_z);
+}
+void kfo_window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, int n_phi, int n_z, int* first, int* n_b,
+                     int* iz_lo, int* iz_hi) {
+    kfo_window_bins_row(phi_c, dphi, z_c, dz, -zmax, zmax, n_phi, n_z, first, n_b, iz_lo, iz_hi);
 }
 
 /* kf_window_lookup_ref: bin-granular hit list of each query (rows ascending, bins ascending with wrap, hits in
@@ -721,7 +745,9 @@ int kfo_window_lookup(int n_layers, const double* layers, int n_phi, int n_z, co
                       const float* z_c, const float* dz, int cap, int32_t* count, int32_t* sorted_idx) {
     for (int64_t i = 0; i < n_query; ++i) {
         int first, nb, z0, z1;
-        kfo_window_bins(phi_c[i], dphi[i], z_c[i], dz[i], (float)LZMAX(layers, layer[i]), n_phi, n_z, &first, &nb, &z0, &z1);
+        float lo, hi;
+        row_range(layers, layer[i], &lo, &hi);
+        kfo_window_bins_row(phi_c[i], dphi[i], z_c[i], dz[i], lo, hi, n_phi, n_z, &first, &nb, &z0, &z1);
         int64_t seg = (int64_t)event[i] * n_layers + layer[i];
         int32_t c = 0;
         for (int iz = z0; iz <= z1; ++iz)
@@ -746,7 +772,7 @@ typedef struct {
 } kfo_cand;
 
 typedef struct {
-    int parent, kind; /* kind 0 = hit child, 1 = no compatible hit (-1), 2 = finished (-2) */
+    int parent, kind; /* kind 0 = hit child, 1 = no compatible hit (-1), 2 = finished (-2), 3 = layer skipped (-2, alive) [R22] */
     int64_t hitpos;   /* global sorted position; INT64_MAX for kinds 1, 2 */
     double chi2;
     int nhits;
@@ -766,6 +792,14 @@ static int child_cmp(const void* a_, const void* b_) {
  * the layer's segment (brute force without the spatial index, pin P12).
  * Outputs, slot = s*K + k: par_o [6][ld_out], cov_o [36][ld_out], chi2_o, nhits_o, status_o [n_seeds*K],
  * hit_idx_o [n_layers][ld_out], n_cand [n_seeds]; unused slots: nhits 0, chi2 0, status 0, hit_idx -2, par/cov 0.
+ * Geometry with disks ("cylinder with lids") [R22]: the layers are alternatives, not a sequence every track
+ * goes through -- a candidate that cannot be propagated to a layer (not reached, grazing) or whose window lies off the
+ * layer SKIPS it: one child with the unchanged state, hit = -2, alive, no status bit; only a numeric failure finishes a
+ * candidate.  On a disk the window is in (phi, radius): rho_c = |(x', y')|, d_rho = n_sigma sqrt(var_rho + sig_r^2) with
+ * var_rho = (x'^2 Cxx + 2 x'y' Cxy + y'^2 Cyy)/rho_c^2, dphi = n_sigma sqrt(var_phi + (sig_rphi/rho_c)^2); off the layer when
+ * rho_c > rmax + d_rho or rho_c < rmin - d_rho; strict test |x'm_y - y'm_x| <= dphi rho_c rho_m, x'm_x + y'm_y > 0,
+ * |rho_m - rho_c| <= d_rho; rows of the bins by radius.  chi2 and update: the 3-D ones [R5] (sig_z regularises along the
+ * disk normal).  Barrel-only geometries keep the behaviour of R10 exactly.
  * counters[8]: 0 propagations, 1 hits scanned, 2 pass strict window, 3 pass chi2 cut (hit children), 4 updates,
  *              5 bin rows touched, 6 seed-layers, 7 children ranked.
  * margins (NULL or [n_seeds][n_layers][5], test diagnostics for DESIGN.md R16): the smallest RELATIVE distance of any
@@ -787,6 +821,8 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
               double* margins) {
     if (K < 1 || K > 32 || n_layers > 32 || first_layer < 0 || first_layer > n_layers) return -1;
     int64_t cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int lids = 0;
+    for (int l = 0; l < n_layers; ++l) lids = lids || LKIND(layers, l) != 0;
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : cnt[:8])
     for (int64_t sd = 0; sd < n_seeds; ++sd) {
         kfo_cand* cur = (kfo_cand*)calloc((size_t)K, sizeof(kfo_cand));
@@ -806,7 +842,8 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
         for (int l = 0; l < first_layer; ++l) cur[0].hits[l] = seed_hit_idx ? seed_hit_idx[(int64_t)l * ld_seed + sd] : -1;
 
         for (int l = first_layer; l < n_layers; ++l) {
-            const double R = LR(layers, l), zmax = LZMAX(layers, l);
+            const double R = LR(layers, l), zmax = LZMAX(layers, l), rmin = LRMIN(layers, l);
+            const int disk = LKIND(layers, l) != 0;
             const double srphi = LSRPHI(layers, l), szz = LSZ(layers, l), sr = LSR(layers, l);
             const int64_t seg = (int64_t)ev * n_layers + l;
             n_ch = 0;
@@ -822,28 +859,51 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                 if (!cur[c].finished && (f == 0 || f == KFO_GRAZING)) KFO_MARGIN(3, fabs(ci / KFO_CMIN - 1.0));
                 if (!cur[c].finished) KFO_MARGIN(4, tang);
                 double dphi = 0, dzw = 0;
-                if (f == 0) { /* window (R11) */
+                if (f == 0) { /* window (R11; on a disk R22) */
                     const double x = pp[c][0], y = pp[c][1], r2 = x * x + y * y;
                     double varphi = (x * x * Cp[c][1 * 6 + 1] - 2.0 * x * y * Cp[c][0 * 6 + 1] + y * y * Cp[c][0]) / (r2 * r2);
                     if (varphi < 0.0) varphi = 0.0;
-                    dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R));
-                    dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz);
+                    if (!disk) {
+                        dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R));
+                        dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz);
+                    } else {
+                        double varrho = (x * x * Cp[c][0] + 2.0 * x * y * Cp[c][0 * 6 + 1] + y * y * Cp[c][1 * 6 + 1]) / r2;
+                        if (varrho < 0.0) varrho = 0.0;
+                        dphi = n_sigma * sqrt(varphi + srphi * srphi / r2);
+                        dzw = n_sigma * sqrt(varrho + sr * sr);
+                    }
                     if (!isfinite(dphi) || !isfinite(dzw)) f = KFO_NUMERIC;
-                    else {
+                    else if (!disk) {
                         KFO_MARGIN(3, fabs(fabs(pp[c][2]) / (zmax + dzw) - 1.0));
                         if (fabs(pp[c][2]) > zmax + dzw) f = KFO_LEFT_Z;
+                    } else {
+                        const double rho = sqrt(r2);
+                        KFO_MARGIN(3, fabs(rho / (zmax + dzw) - 1.0));
+                        if (rmin - dzw > 0.0) KFO_MARGIN(3, fabs(rho / (rmin - dzw) - 1.0));
+                        if (rho > zmax + dzw || rho < rmin - dzw) f = KFO_LEFT_Z;
                     }
                 }
-                if (f != 0) { /* finished (or just found unpropagatable): state unchanged */
+                if (f != 0) {
+                    if (lids && !cur[c].finished && f != KFO_NUMERIC) { /* layer not crossed: skipped, the candidate lives on [R22] */
+                        kfo_child skip = {c, 3, INT64_MAX, cur[c].chi2, cur[c].nhits};
+                        if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
+                        ch[n_ch++] = skip;
+                        continue;
+                    }
+                    /* finished (or just found unpropagatable): state unchanged */
                     if (f > 0) pflag[c] = (uint32_t)f;
                     if (n_ch == cap_ch) ch = (kfo_child*)realloc(ch, (cap_ch *= 2) * sizeof(kfo_child));
                     ch[n_ch++] = pass;
                     continue;
                 }
-                const double x = pp[c][0], y = pp[c][1], zc = pp[c][2], rp = sqrt(x * x + y * y);
+                const double x = pp[c][0], y = pp[c][1], rp = sqrt(x * x + y * y);
+                const double zc = disk ? rp : pp[c][2];            /* centre of the window along the row coordinate */
                 int first = 0, nb = 1, z0 = 0, z1 = 0;
-                if (use_bins)
-                    kfo_window_bins((float)atan2(y, x), (float)dphi, (float)zc, (float)dzw, (float)zmax, n_phi, n_z, &first, &nb, &z0, &z1);
+                if (use_bins) {
+                    float lo_, hi_;
+                    row_range(layers, l, &lo_, &hi_);
+                    kfo_window_bins_row((float)atan2(y, x), (float)dphi, (float)zc, (float)dzw, lo_, hi_, n_phi, n_z, &first, &nb, &z0, &z1);
+                }
                 int n_hit_children = 0, s_bad = 0;
                 for (int iz = z0; iz <= z1 && !s_bad; ++iz) {
                     cnt[5] += use_bins ? 1 : 0;
@@ -859,10 +919,11 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                             const double rm = sqrt(m[0] * m[0] + m[1] * m[1]);
                             const int in_phi = fabs(x * m[1] - y * m[0]) <= dphi * rp * rm;
                             const int in_dot = x * m[0] + y * m[1] > 0.0;
-                            const int in_z = fabs(m[2] - zc) <= dzw;
+                            const double mrow = disk ? rm : m[2];
+                            const int in_z = fabs(mrow - zc) <= dzw;
                             if (margins && in_dot && (in_phi || in_z)) { /* distance to the window edges (diagnostics only) */
                                 const double mphi = fabs(fabs(x * m[1] - y * m[0]) / (dphi * rp * rm) - 1.0);
-                                const double mz = fabs(fabs(m[2] - zc) / dzw - 1.0);
+                                const double mz = fabs(fabs(mrow - zc) / dzw - 1.0);
                                 const double near = fmin(in_z ? mphi : 1e300, in_phi ? mz : 1e300);
                                 if (near < mg[0]) {
                                     double c2m;
@@ -915,6 +976,8 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                 if (k->kind == 2) {
                     o->finished = 1;
                     o->status |= pflag[k->parent];
+                    o->hits[l] = -2;
+                } else if (k->kind == 3) {
                     o->hits[l] = -2;
                 } else if (k->kind == 1) {
                     memcpy(o->p, pp[k->parent], sizeof o->p);

@@ -198,6 +198,26 @@ def z_bin(z, zmax, n_z):
     return np.array([l.kfo_z_bin(C.c_float(float(a)), C.c_float(float(zmax)), C.c_int(n_z)) for a in _f(np.atleast_1d(z))], dtype=np.int32)
 
 
+def row_bin(v, lo, hi, n):
+    """X2 for any layer (R22): row of v in [lo, hi) cut into n rows (barrel: z in [-zmax, zmax); disk: radius)."""
+    l = lib(); l.kfo_row_bin.restype = C.c_int
+    return np.array([l.kfo_row_bin(C.c_float(float(a)), C.c_float(float(lo)), C.c_float(float(hi)), C.c_int(n)) for a in _f(np.atleast_1d(v))], dtype=np.int32)
+
+
+def hit_rho(x, y):
+    """fp32 radius of a hit as the disk binning takes it: sqrt(fl(fl(x x) + fl(y y)))."""
+    l = lib(); l.kfo_hit_rho.restype = C.c_float
+    return np.array([l.kfo_hit_rho(C.c_float(float(a)), C.c_float(float(b))) for a, b in zip(_f(np.atleast_1d(x)), _f(np.atleast_1d(y)))], dtype=np.float32)
+
+
+def window_bins_row(phi_c, dphi, c, d, lo, hi, n_phi, n_z):
+    """X3 with the row coordinate binned in [lo, hi) -> (first phi bin, n phi bins, row_lo, row_hi)"""
+    a, b, e, f = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+    lib().kfo_window_bins_row(C.c_float(phi_c), C.c_float(dphi), C.c_float(c), C.c_float(d), C.c_float(lo), C.c_float(hi), C.c_int(n_phi), C.c_int(n_z),
+                              C.byref(a), C.byref(b), C.byref(e), C.byref(f))
+    return a.value, b.value, e.value, f.value
+
+
 def window_bins(phi_c, dphi, z_c, dz, zmax, n_phi, n_z):
     """X3 -> (first phi bin, n phi bins, iz_lo, iz_hi)"""
     a, b, c, d = C.c_int(), C.c_int(), C.c_int(), C.c_int()

@@ -434,6 +434,9 @@ class BuildInputs:
 BUILD_CONFIGS = {
     3: dict(n_events=16, tracks=2_000, geom="barrel10", gun="flat", noise=5, n_phi=256, n_z=16, fake_frac=0.0),
     4: dict(n_events=64, tracks=10_000, geom="barrel17", gun="wide", noise=10, n_phi=1024, n_z=32, fake_frac=0.2),
+    # building on the "cylinder with lids" (R22): the config-3 recipe on the lids10 geometry with the
+    # forward gun; noise on a disk is uniform in phi and in radius over [rmin, rmax]
+    "lids": dict(n_events=8, tracks=2_000, geom="lids10", gun="forward", noise=5, n_phi=256, n_z=16, fake_frac=0.0),
 }
 
 
@@ -469,7 +472,7 @@ def _three_point_seed(p1, p2, p3, bz):
     return np.array([x3, y3, z3, ipt, phi, theta]), q
 
 
-def build_inputs(config: int, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
+def build_inputs(config, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
                  K: int = 10, chi2_cut: float = 30.0, n_sigma: float = 3.0, noise: float | None = None,
                  fake_frac: float | None = None, n_phi: int | None = None, n_z: int | None = None,
                  smear: bool = True, ms: bool = True, event0: int = 0) -> BuildInputs:
@@ -494,7 +497,7 @@ def build_inputs(config: int, n_events: int | None = None, tracks: int | None = 
     seeds, sigs, qs, sev, struth, shit = [], [], [], [], [], []
     truth_hit_idx = np.full((L, n_events * tracks), -1, dtype=np.int32)
     for ev in range(n_events):
-        rng = rng_for(config, ev + event0)     # event0: a rank's own events (weak scaling)
+        rng = rng_for(config if isinstance(config, int) else 101, ev + event0)     # event0: a rank's own events (weak scaling)
         gun = particle_gun(rng, tracks, cfg["gun"])
         sim = simulate(geom, gun, rng, ms=ms, smear=smear)
         ev_hits = []
@@ -504,9 +507,14 @@ def build_inputs(config: int, n_events: int | None = None, tracks: int | None = 
             n_sig = len(ids)
             n_noise = int(round(noise * n_sig))
             az = rng.uniform(-np.pi, np.pi, n_noise)
-            nz = rng.uniform(-geom.zmax[l], geom.zmax[l], n_noise)
-            hx = np.concatenate([sim["hits"][l, ids, 0], geom.r[l] * np.cos(az)])
-            hy = np.concatenate([sim["hits"][l, ids, 1], geom.r[l] * np.sin(az)])
+            if geom.kind[l] == 0:
+                nz = rng.uniform(-geom.zmax[l], geom.zmax[l], n_noise)
+                nr = np.full(n_noise, geom.r[l])
+            else:                                  # disk: in the plane z = Z, radius uniform over the annulus' width
+                nz = np.full(n_noise, geom.r[l])
+                nr = rng.uniform(geom.rmin[l], geom.zmax[l], n_noise)
+            hx = np.concatenate([sim["hits"][l, ids, 0], nr * np.cos(az)])
+            hy = np.concatenate([sim["hits"][l, ids, 1], nr * np.sin(az)])
             hz = np.concatenate([sim["hits"][l, ids, 2], nz])
             ht = np.concatenate([ids + ev * tracks, np.full(n_noise, -1)]).astype(np.int32)
             perm = rng.permutation(len(hx))
