@@ -127,7 +127,9 @@ int kf_fit(const kf_geom* geom, const kf_hits* hits, const int32_t* hit_idx, con
 /* ---------------------------------------------------------------------------------------------------------
  * Binned hit index (DESIGN.md sec. 2 B0, readings X1-X2).  Filled by kf_bin_hits into
  * caller-allocated arrays.  Global bin of a hit = ((event*n_layers + layer)*n_z + iz)*n_phi + iphi; iphi from the
- * azimuth by exact fp32 comparisons against a tangent table (no atan2), iz = clamp(floor((z + zmax)*n_z/(2 zmax))).
+ * azimuth by exact fp32 comparisons against a tangent table (no atan2), iz = clamp(floor((z + zmax)*n_z/(2 zmax))) on a
+ * barrel layer; on a disk (kind 1; R22) the rows are cut along the radius of the hit,
+ * iz = clamp(floor((sqrt(x^2 + y^2) - rmin)*n_z/(rmax - rmin))), every operation one IEEE fp32 rounding.
  * Sorted order = ascending (global bin, original index): unique, hence bit-exact testable. */
 typedef struct {
     int32_t n_phi, n_z;   /* n_phi multiple of 8, 8..4096; n_z 1..1024                                     */
@@ -143,7 +145,8 @@ int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t
                 size_t ws_bytes, void* stream);
 
 /* kf_window_lookup -- test / diagnostic entry: the window hit list of B2-B3 for explicit windows (reading X3).
- * Query i: event[i], layer[i], azimuth window phi_c +- dphi (phi_c in (-pi, pi], dphi >= 0), z window z_c +- dz.
+ * Query i: event[i], layer[i], azimuth window phi_c +- dphi (phi_c in (-pi, pi], dphi >= 0), z window z_c +- dz (on a
+ * disk layer z_c, dz are read as the radius window rho_c +- d_rho).
  * The list is every hit of the bins touched, rows in ascending iz, bins in ascending (wrapping) iphi, hits in
  * sorted order.  count[i] = true length even if > cap; sorted_idx[i*cap + j] = global sorted position, j < min(count, cap). */
 int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, int64_t n_query,
@@ -156,6 +159,10 @@ int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* 
  * n_sigma standard deviations in phi and z, chi2 against every hit of the window, one child per hit with
  * chi2 < chi2_cut (else one child without hit), keep the best K children by (nhits desc, chi2 asc, parent slot asc,
  * sorted hit position asc), update the survivors.
+ * Geometry with endcap disks ("cylinder with lids"; R22; geom->hit_mode must be 0): on a disk the
+ * window is in phi and radius, and on any layer a candidate that cannot be propagated there (not reached, grazing) or
+ * whose window lies off the layer skips it (hit_idx -2, state unchanged, no status bit) and lives on; only a numeric
+ * failure finishes a candidate.  A barrel-only geometry keeps the behaviour below (a failed layer finishes the candidate).
  * Output: slot s*K + k of `cand` (best first), hit_idx[l*ld + slot] = original index within the segment,
  * -1 = no hit on this layer, -2 = layer not crossed (candidate finished); n_cand[s] = number of valid slots.
  */
@@ -179,7 +186,7 @@ typedef struct {
  * next call on the same stream.  opt (NULL = automatic): seeds per thread block and the cap on the persistent grid;
  * the result does not depend on them, the workspace size does (pass the same opt to both calls).
  * Errors: NULL pointers, K / first_layer / cuts / options out of range, bad bin counts, workspace too small (-4),
- * CUDA failure. */
+ * geom->hit_mode != 0 (KF_ERR_UNIMPLEMENTED: the two-step propagation is built for kf_fit), CUDA failure. */
 size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K, const kf_options* opt);
 int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,

@@ -38,7 +38,8 @@ struct BinArgs {
     int32_t* perm;
     float4* xyzp;
     float phi_scale;             // n_phi / (2 pi): first guess of the table search
-    float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
+    float row_lo[KF_MAX_LAYERS], row_inv[KF_MAX_LAYERS];   // X2 rows: z in [-zmax, zmax) on a barrel layer, radius in [rmin, rmax) on a disk
+    int32_t kind[KF_MAX_LAYERS];
     float tan_tab[MAX_TAN_TAB];  // X1: fl32(tan(2 pi k / n_phi)), k = 0 .. n_phi/8 (evaluated in double on the host), last = 1
 };
 
@@ -51,7 +52,8 @@ __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_co
         const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
         const int32_t base = seg * a.n_z * a.n_phi;
         for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
-            const int b = base + z_bin(a.hz[h], a.zmax[l], a.inv_dz[l], a.n_z) * a.n_phi + phi_bin(a.hx[h], a.hy[h], a.n_phi, s_tab, a.phi_scale);
+            const float x = a.hx[h], y = a.hy[h];
+            const int b = base + row_bin(a.kind[l] ? hit_rho(x, y) : a.hz[h], a.row_lo[l], a.row_inv[l], a.n_z) * a.n_phi + phi_bin(x, y, a.n_phi, s_tab, a.phi_scale);
             a.kr[h] = make_int2(b, atomicAdd(&a.bin_off[b + 1], 1));
         }
     }
@@ -142,14 +144,14 @@ struct LookupArgs {
     const int32_t* bin_off;
     int32_t *count, *sorted_idx;
     float inv_dphi;
-    float zmax[KF_MAX_LAYERS], inv_dz[KF_MAX_LAYERS];
+    float row_lo[KF_MAX_LAYERS], row_inv[KF_MAX_LAYERS];
 };
 
 __global__ void __launch_bounds__(BIN_BLOCK) kf_window_lookup_kernel(const __grid_constant__ LookupArgs a) {
     const int64_t i = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
     if (i >= a.n_query) return;
     const int l = a.layer[i];
-    const WindowBins w = window_bins(a.phi_c[i], a.dphi[i], a.z_c[i], a.dz[i], a.zmax[l], a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+    const WindowBins w = window_bins<true>(a.phi_c[i], a.dphi[i], a.z_c[i], a.dz[i], a.row_lo[l], a.row_inv[l], a.inv_dphi, a.n_phi, a.n_z);
     const int64_t seg = (int64_t)a.event[i] * a.n_layers + l;
     int c = 0;
     for (int iz = w.iz_lo; iz <= w.iz_hi; ++iz) {
@@ -237,8 +239,8 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
     a.phi_scale = host_inv_dphi(n_phi);
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
-        a.zmax[l] = y.zmax;
-        a.inv_dz[l] = (float)n_z / (2.0f * y.zmax);      // one IEEE fp32 division of exact operands (X2)
+        host_row_range(y, n_z, &a.row_lo[l], &a.row_inv[l]);      // one IEEE fp32 subtraction and division (X2)
+        a.kind[l] = y.kind;
     }
     // X1 table: T[k] = fl32(tan(2 pi k / N)) evaluated in double on the host, T[N/8] = 1; travels as a kernel argument
     const double two_pi = 6.283185307179586476925286766559;
@@ -281,8 +283,7 @@ extern "C" int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const 
     a.inv_dphi = host_inv_dphi(binned->n_phi);
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
-        a.zmax[l] = y.zmax;
-        a.inv_dz[l] = (float)binned->n_z / (2.0f * y.zmax);
+        host_row_range(y, binned->n_z, &a.row_lo[l], &a.row_inv[l]);
     }
     kf_window_lookup_kernel<<<(unsigned)((n_query + BIN_BLOCK - 1) / BIN_BLOCK), BIN_BLOCK, 0, (cudaStream_t)stream>>>(a);
     return check_launch("kf_window_lookup");

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include "../../include/kf.h"
 
 namespace kf {
 
@@ -23,16 +24,33 @@ __device__ __forceinline__ int phi_bin(float x, float y, int n_phi, const float*
     return (y >= 0.0f) ? (n_phi >> 1) - 1 - a : (n_phi >> 1) + a;
 }
 
-// X2: z row; inv_dz = fl32(n_z / (2 zmax))
+// X2: z row of a barrel layer; inv_dz = fl32(n_z / (2 zmax))
 __device__ __forceinline__ int z_bin(float z, float zmax, float inv_dz, int n_z) {
     const float f = floorf(__fmul_rn(__fadd_rn(z, zmax), inv_dz));
     return (f >= (float)n_z) ? n_z - 1 : (f < 0.0f ? 0 : (int)f);
+}
+// X2 for any layer: row of the coordinate v binned in [lo, hi), inv = fl32(n / fl32(hi - lo)).  Barrel layer: v = z, lo = -zmax (then
+// v - lo = z + zmax and hi - lo = 2 zmax: the original X2); disk (R22): v = hit_rho(x, y), lo = rmin, hi = rmax.
+__device__ __forceinline__ int row_bin(float v, float lo, float inv, int n) {
+    const float f = floorf(__fmul_rn(__fsub_rn(v, lo), inv));
+    return (f >= (float)n) ? n - 1 : (f < 0.0f ? 0 : (int)f);
+}
+// radius of a hit as the disk rows take it: one IEEE rounding per operation
+__device__ __forceinline__ float hit_rho(float x, float y) { return __fsqrt_rn(__fadd_rn(__fmul_rn(x, x), __fmul_rn(y, y))); }
+// per-layer row constants on the host (the same fp32 operations as the oracle)
+inline void host_row_range(const kf_layer& y, int n_z, float* lo, float* inv) {
+    const float l = y.kind ? y.rmin : -y.zmax, h = y.zmax;
+    *lo = l;
+    *inv = (float)n_z / (h - l);
 }
 
 // X3: window -> first phi bin, number of phi bins (wrapping), z rows
 struct WindowBins { int first, n_b, iz_lo, iz_hi; };
 
-__device__ __forceinline__ WindowBins window_bins(float phi_c, float dphi, float z_c, float dz, float zmax, float inv_dz,
+// ROW = false: barrel layer, rows of z (a = zmax, b = inv_dz); ROW = true: any layer, rows of the coordinate binned in
+// [lo, hi) (a = lo, b = inv): the same bins for a barrel layer, written with the operations of X2 / of row_bin
+template <bool ROW = false>
+__device__ __forceinline__ WindowBins window_bins(float phi_c, float dphi, float z_c, float dz, float a, float b,
                                                   float inv_dphi, int n_phi, int n_z) {
     WindowBins w;
     if (!(__fmul_rn(dphi, inv_dphi) < (float)n_phi)) {      // half width of a full turn or more (or not a number): every bin, from bin 0
@@ -46,8 +64,8 @@ __device__ __forceinline__ WindowBins window_bins(float phi_c, float dphi, float
         int f = b_lo % n_phi;
         w.first = f < 0 ? f + n_phi : f;
     }
-    w.iz_lo = z_bin(__fsub_rn(z_c, dz), zmax, inv_dz, n_z);
-    w.iz_hi = z_bin(__fadd_rn(z_c, dz), zmax, inv_dz, n_z);
+    w.iz_lo = ROW ? row_bin(__fsub_rn(z_c, dz), a, b, n_z) : z_bin(__fsub_rn(z_c, dz), a, b, n_z);
+    w.iz_hi = ROW ? row_bin(__fadd_rn(z_c, dz), a, b, n_z) : z_bin(__fadd_rn(z_c, dz), a, b, n_z);
     return w;
 }
 

@@ -56,7 +56,8 @@ constexpr int HITPOS_NONE = 0x7fffffff;
 constexpr int LIST_BYTES_PER_THREAD = KF_LIST_BYTES; // shared memory for the per-candidate child lists, per thread of the block
 enum { W_TRIG = 27, W_CHI2 = 31, W_META = 32 };
 // meta word of a record: bits 0-7 nhits, bit 8 finished, bits 16-19 status
-// info word of a parent in a round: bits 0-7 nhits, bit 8 finished (child inherits the unchanged state), bits 16-19 status to add
+// info word of a parent in a round: bits 0-7 nhits, bit 8 finished (child inherits the unchanged state), bit 9 layer skipped
+// (the same, but the candidate lives on: R22), bits 16-19 status to add
 
 struct BuildArgs {
     int32_t n_layers, first_layer, K, n_phi, n_z, S, ncap;
@@ -69,7 +70,9 @@ struct BuildArgs {
     float* ws_rec;            // [grid][2][NREC4][S*K] float4
     int32_t* ws_link_hit;     // [grid][n_layers][S*K]
     LayerC layer[KF_MAX_LAYERS];
-    float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax); (sig_rphi/r)^2
+    float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax) (disk: n_z/(rmax - rmin)); (sig_rphi/r)^2
+    float row_lo[KF_MAX_LAYERS];   // X2 rows of any layer start at -zmax (disk: rmin)
+    int32_t lids;             // the geometry has disks (R22)
 };
 
 // Records are stored as NREC4 = 9 groups of four words, group g of record c at float4 index g * SK + c: a record moves
@@ -212,7 +215,8 @@ __device__ __forceinline__ Tile tile_of(const BuildArgs& a) {
 // inlined into one kernel they need 228 registers and spill ~480 bytes at the 128 the launch bounds allow.
 
 // phase 1, one live candidate: dense index base + i, round-local index i
-template <bool ISO>
+// LIDS: the geometry has disks (R22); a barrel-only geometry compiles without any of it
+template <bool ISO, bool LIDS>
 __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base, int i, int64_t s0) {
     const Tile T = tile_of(a);
     // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
@@ -240,30 +244,76 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
     Ldl3 F = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     bool fok = false;
     WindowBins wb = {0, 0, 0, -1};
-    if (!fin) {
-        flag = predict(st, cw, ly);
-        if (!flag) {
-            px = st.XY.x; py = st.XY.y; pz = st.Z;
-            c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
-            const float r2 = fmaf(px, px, py * py);
-            const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
-            const float varphi = fmaxf(num / (r2 * r2), 0.0f);
-            const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
-            dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
-            if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
-            else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
-            else {
-                thr2 = dphi * dphi * r2;
-                wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
-                if (ISO) {
-                    Sym3 Sm;
-                    Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
-                    Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
-                    fok = ldl3(Sm, F);
+    [[maybe_unused]] float wrow = 0.f;          // LIDS: centre of the window along the row coordinate (z or radius)
+    [[maybe_unused]] bool skip = false, disk = false;
+    if constexpr (!LIDS) {
+        if (!fin) {
+            flag = predict(st, cw, ly);
+            if (!flag) {
+                px = st.XY.x; py = st.XY.y; pz = st.Z;
+                c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
+                const float r2 = fmaf(px, px, py * py);
+                const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
+                const float varphi = fmaxf(num / (r2 * r2), 0.0f);
+                const float dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
+                dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+                if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
+                else if (fabsf(pz) > ly.zmax + dzw) flag = ST_LEFT_Z;
+                else {
+                    thr2 = dphi * dphi * r2;
+                    wb = window_bins(atan2f(py, px), dphi, pz, dzw, ly.zmax, a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+                    if (ISO) {
+                        Sym3 Sm;
+                        Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
+                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
+                        fok = ldl3(Sm, F);
+                    }
                 }
             }
+            fin = flag != 0u;
         }
-        fin = flag != 0u;
+    } else {
+        // Geometry with disks (R22): on a disk the window is in (phi, radius); a layer that is not reached or whose window
+        // lies off it is skipped and the candidate lives on; only a numeric failure finishes it.
+        disk = ly.kind != 0;
+        if (!fin) {
+            flag = disk ? predict_disk<false>(st, cw, ly, ly.r) : predict(st, cw, ly);
+            if (!flag) {
+                px = st.XY.x; py = st.XY.y; pz = st.Z;
+                c00 = st.P0.x; c10 = st.P0.y; c11 = st.P1.y; c20 = st.P2.x; c21 = st.P2.y; c22 = st.Q2.x;
+                const float r2 = fmaf(px, px, py * py);
+                const float num = fmaf(px * px, c11, fmaf(-2.0f * px * py, c10, py * py * c00));
+                const float varphi = fmaxf(num / (r2 * r2), 0.0f);
+                float dphi;
+                bool off;
+                if (!disk) {
+                    dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
+                    dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+                    wrow = pz;
+                    off = fabsf(pz) > ly.zmax + dzw;
+                } else {
+                    const float varrho = fmaxf(fmaf(px * px, c00, fmaf(2.0f * px * py, c10, py * py * c11)) / r2, 0.0f);
+                    dphi = a.n_sigma * sqrtf(varphi + ly.var_rphi / r2);
+                    dzw = a.n_sigma * sqrtf(varrho + ly.var_r);
+                    wrow = sqrtf(r2);
+                    off = wrow > ly.zmax + dzw || wrow < ly.rmin - dzw;
+                }
+                if (!(dphi <= 3.0e38f) || !(dzw <= 3.0e38f)) flag = ST_NUMERIC;      // NaN or Inf
+                else if (off) flag = ST_LEFT_Z;
+                else {
+                    thr2 = dphi * dphi * r2;
+                    wb = window_bins<true>(atan2f(py, px), dphi, wrow, dzw, a.row_lo[l], a.inv_dz[l], a.inv_dphi, a.n_phi, a.n_z);
+                    if (ISO) {
+                        Sym3 Sm;
+                        Sm.m00 = c00 + ly.var_r; Sm.m10 = c10; Sm.m11 = c11 + ly.var_r;
+                        Sm.m20 = c20; Sm.m21 = c21; Sm.m22 = c22 + ly.var_z;
+                        fok = ldl3(Sm, F);
+                    }
+                }
+            }
+            if (flag != 0u && flag != ST_NUMERIC) { skip = true; flag = 0u; }
+            fin = flag != 0u || skip;
+        }
     }
     int cnt = 0;
     if (!fin) {
@@ -302,8 +352,15 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
                     for (int u = 0; u < SCAN_BATCH; ++u) {
                         const float mx = hv[u].x, my = hv[u].y, mz = hv[u].z;
                         const float cr = fmaf(px, my, -py * mx);
-                        const bool in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
-                                            (fabsf(mz - pz) <= dzw);
+                        bool in_win;
+                        if constexpr (!LIDS) {
+                            in_win = (t0 + u < nab) && (cr * cr <= thr2 * fmaf(mx, mx, my * my)) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                     (fabsf(mz - pz) <= dzw);
+                        } else {
+                            const float rm2 = fmaf(mx, mx, my * my);
+                            in_win = (t0 + u < nab) && (cr * cr <= thr2 * rm2) && (fmaf(px, mx, py * my) > 0.0f) &&
+                                     (fabsf((disk ? sqrtf(rm2) : mz) - wrow) <= dzw);
+                        }
                         inside |= in_win ? (1u << u) : 0u;
                     }
                     while (inside) {
@@ -350,7 +407,7 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
     if (fin) rec_copy(recA, c, recB, c, SK);
     s_lcnt[i] = (unsigned char)cnt;
     s_pchi2[i] = chi2;
-    s_pinfo[i] = (meta & 255) | (fin ? 256 : 0) | (int)(flag << 16);
+    s_pinfo[i] = (meta & 255) | (fin ? (LIDS && skip ? 512 : 256) : 0) | (int)(flag << 16);
 }
 
 // phase 3, one surviving child: dense index cn among the children of the tile
@@ -379,6 +436,8 @@ __device__ __noinline__ void build_child(const BuildArgs& a, int l, int cn) {
         if (pkd & (1 << 16)) {
             const int meta = __float_as_int(rec_word(recB, SK, cp, W_META)) | 256 | (((pkd >> 24) & 15) << 16);
             rec_set_word(recA, SK, cn, W_META, __int_as_float(meta));
+            link = -2;
+        } else if (pkd & (1 << 17)) {      // layer skipped: the record is the unchanged state, the candidate lives on
             link = -2;
         } else {
             link = -1;
@@ -457,7 +516,7 @@ __device__ __noinline__ void build_output(const BuildArgs& a, int64_t s0, int c)
     }
 }
 
-template <int NT, bool ISO>
+template <int NT, bool ISO, bool LIDS>
 __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel(const __grid_constant__ BuildArgs ga) {
     extern __shared__ __align__(16) unsigned char smem[];
     // The phase bodies are separate functions that take the arguments by reference: a copy in shared memory keeps their
@@ -518,7 +577,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                 const int nround = s_off[r1] - base;
                 // ---------------- phase 1: predict + window + scan, thread per candidate ----------------
                 for (int i = tid; i < nround; i += NT) {
-                    build_candidate<ISO>(a, l, base, i, s0);
+                    build_candidate<ISO, LIDS>(a, l, base, i, s0);
                 }
                 __syncthreads();
                 // ---------------- phase 2: best K children of a seed (B4), thread per seed ----------------
@@ -544,7 +603,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
                         const int cnt = s_lcnt[i];
                         sel_chi2[s * K + n_out] = __uint_as_float((unsigned)(best >> 10));
                         sel_hit[s * K + n_out] = cnt ? s_lhit[j * ncap + i] : HITPOS_NONE;
-                        sel_pk[s * K + n_out] = k | (nh << 8) | (s_pinfo[i] & 0x000f0100) << 8;   // bit 16 finished, bits 24-27 status
+                        sel_pk[s * K + n_out] = k | (nh << 8) | (s_pinfo[i] & 0x000f0300) << 8;   // bit 16 finished, bit 17 skipped, bits 24-27 status
                         s_hkey[i] = (j + 1 < cnt) ? child_key(nh, s_lchi2[(j + 1) * ncap + i], k, j + 1) : ~0ull;
                     }
                     s_nnew[s] = n_out;
@@ -637,14 +696,18 @@ static BuildPlan build_plan(int n_layers, int64_t n_seeds, int K, const kf_optio
     return p;
 }
 
+template <int NT, bool ISO, bool LIDS>
+static int launch_build3(const BuildArgs& a, const BuildPlan& p, cudaStream_t st) {
+    cudaError_t e = cudaFuncSetAttribute(kf_build_kernel<NT, ISO, LIDS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
+    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+    kf_build_kernel<NT, ISO, LIDS><<<p.grid, NT, p.smem, st>>>(a);
+    return check_launch("kf_build");
+}
+
 template <int NT>
 static int launch_build(const BuildArgs& a, const BuildPlan& p, bool iso, cudaStream_t st) {
-    cudaError_t e = iso ? cudaFuncSetAttribute(kf_build_kernel<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem)
-                        : cudaFuncSetAttribute(kf_build_kernel<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
-    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_build: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
-    if (iso) kf_build_kernel<NT, true><<<p.grid, NT, p.smem, st>>>(a);
-    else kf_build_kernel<NT, false><<<p.grid, NT, p.smem, st>>>(a);
-    return check_launch("kf_build");
+    if (a.lids) return iso ? launch_build3<NT, true, true>(a, p, st) : launch_build3<NT, false, true>(a, p, st);
+    return iso ? launch_build3<NT, true, false>(a, p, st) : launch_build3<NT, false, false>(a, p, st);
 }
 
 }  // namespace kf
@@ -662,6 +725,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     if (!geom || !hits || !binned || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_build: NULL struct argument");
     int rc = check_geom(geom, "kf_build");
     if (rc) return rc;
+    if (geom->hit_mode != 0) return fail(KF_ERR_UNIMPLEMENTED, "kf_build: hit_mode 1 (two-step propagation, 2-D update) is built for kf_fit only");
     if (K < 1 || K > 32) return fail(KF_ERR_INVALID_ARG, "kf_build: K = %d outside 1..32", K);
     if (first_layer < 0 || first_layer > geom->n_layers) return fail(KF_ERR_INVALID_ARG, "kf_build: first_layer outside 0..n_layers");
     if (!(chi2_cut > 0.f) || !(n_sigma > 0.f)) return fail(KF_ERR_INVALID_ARG, "kf_build: chi2_cut and n_sigma must be positive");
@@ -691,10 +755,12 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;
     a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh);
     bool iso = true;
+    a.lids = 0;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
         a.layer[l] = make_layer(y);
-        a.inv_dz[l] = (float)binned->n_z / (2.0f * y.zmax);
+        host_row_range(y, binned->n_z, &a.row_lo[l], &a.inv_dz[l]);
+        a.lids = a.lids || y.kind != 0;
         a.sphi_over_r2[l] = (y.sig_rphi / y.r) * (y.sig_rphi / y.r);
         iso = iso && y.sig_r == y.sig_rphi;
     }

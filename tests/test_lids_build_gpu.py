@@ -1,0 +1,106 @@
+"""Parity of the CUDA binning / window lookup / combinatorial building on the "cylinder with lids" (sec. 4.1;
+DESIGN.md R22: rows of a disk's bins by radius, window in (phi, radius), layers that are not crossed are skipped) with the
+fp64 oracle, through the C ABI.  Bins and window lists bit-exact; built candidates as in tests/test_build_gpu.py (every
+seed whose lists differ proven to be a decision-margin case); then the build -> select -> final fit chain on the lids."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kf_oracle as o
+from paper_1711_06571_b200 import synth
+from tests.parity import assert_parity, compare_tracks
+from tests.test_build_gpu import assert_binned_equal, compare_build, gpu_bin, ref_bin, ref_build, run_build
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("kw", [dict(n_events=1, tracks=50), dict(n_events=3, tracks=1500), dict(n_events=2, tracks=800, n_phi=1024, n_z=32)])
+def test_lids_bin_hits_bit_exact(kw):
+    bi = synth.build_inputs("lids", **kw)
+    _, _, binned = gpu_bin(bi)
+    assert_binned_equal(binned.to_host(), ref_bin(bi))
+
+
+def test_lids_window_lookup_bit_exact():
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs("lids", n_events=2, tracks=1000)
+    lt = bi.geom.layer_table()
+    geom, hits, binned = gpu_bin(bi)
+    rb = ref_bin(bi)
+    rng = np.random.default_rng(5)
+    nq = 4000
+    ev = rng.integers(0, bi.n_events, nq).astype(np.int32)
+    ly = rng.integers(0, lt.shape[0], nq).astype(np.int32)           # barrel layers and disks
+    phc = rng.uniform(-np.pi, np.pi, nq).astype(np.float32); dph = np.abs(rng.normal(0, 0.05, nq)).astype(np.float32)
+    disk = lt[ly, 6] != 0
+    c = np.where(disk, rng.uniform(0, 50, nq), rng.uniform(-60, 60, nq)).astype(np.float32)
+    d = np.abs(rng.normal(0, 3, nq)).astype(np.float32)
+    cap = 512
+    t = lambda a: torch.from_numpy(a).cuda()
+    cnt, idx = b.kf_window_lookup(geom, hits, binned, t(ev), t(ly), t(phc), t(dph), t(c), t(d), cap)
+    torch.cuda.synchronize()
+    rc, ri = o.window_lookup(lt, rb, ev, ly, phc, dph, c, d, cap)
+    cnt, idx = cnt.cpu().numpy(), idx.cpu().numpy()
+    assert np.array_equal(cnt, rc)
+    for i in range(nq):
+        n = min(rc[i], cap)
+        assert np.array_equal(idx[i, :n], ri[i, :n])
+    assert disk.sum() > 1000 and rc[disk].sum() > 1000
+
+
+@pytest.mark.parametrize("kw,K", [(dict(n_events=4, tracks=2000), None), (dict(n_events=2, tracks=1500), 3), (dict(n_events=2, tracks=1500, noise=0.0), None)])
+def test_lids_build_parity(kw, K):
+    bi = synth.build_inputs("lids", **kw)
+    K_ = bi.K if K is None else K
+    g, r = run_build(bi, K=K), ref_build(bi, K=K)
+    rep = compare_build(g, r, bi.n_seeds, K_, bi.first_layer)
+    # the lids are used: candidates with hits on disks, layers skipped by candidates that live on, no status bits
+    best = np.arange(bi.n_seeds) * K_
+    on_disk = (r["hit_idx"][10:, best] >= 0).any(axis=0)
+    assert on_disk.mean() > 0.3 and (g["hit_idx"][10:, best] >= 0).any(axis=0).mean() > 0.3
+    skipped_then_hit = ((r["hit_idx"][3:10, best] == -2).any(axis=0)) & on_disk
+    assert skipped_then_hit.sum() > 50
+    assert (g["status"][best] == 0).all()
+    assert rep["seed_mismatch_frac"] < 0.02
+
+
+def test_lids_build_then_final_fit():
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs("lids", n_events=3, tracks=1500)
+    K, n = bi.K, bi.n_seeds
+    lt = bi.geom.layer_table()
+    geom = b.Geom(lt, bi.geom.bz)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    binned = b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    sev = t(bi.seed_event)
+    cands = b.kf_build(geom, hits, binned, seeds, sev, t(bi.seed_hit_idx), bi.first_layer, K, bi.chi2_cut, bi.n_sigma)
+    idx = b.kf_select_best(cands, bi.first_layer, seeds.ld)
+    fitted = b.kf_fit(geom, hits, idx, sev, seeds)
+    torch.cuda.synchronize()
+    g, c, hi = fitted.to_host(), cands.to_host(), idx.cpu().numpy()
+    best = np.arange(n) * K
+    r = o.fit(lt, bi.geom.bz, bi.par, bi.cov, bi.q, bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, hit_idx=hi, trk_event=bi.seed_event)
+    # a layer the build skipped is skipped by the fit (-2); a hole the build crossed may, within rounding of a guard, stop the fit
+    same = (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
+    assert (~same).sum() <= 2e-3 * n, int((~same).sum())
+    ok = same & (r["status"] == 0)
+    assert ok.mean() > 0.97
+    assert_parity(compare_tracks(g, r, sel=ok))
+    # the refit reproduces the built candidate
+    m = ok & (c["status"][best] == 0)
+    assert np.array_equal(g["nhits"][m] + bi.first_layer, c["nhits"][best][m])
+    assert np.allclose(g["chi2"][m], c["chi2"][best][m], rtol=2e-4, atol=1e-4)
+
+
+def test_build_with_hit_mode_1_is_unimplemented():
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs("lids", n_events=1, tracks=50)
+    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz, hit_mode=1)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    binned = b.kf_bin_hits(b.Geom(bi.geom.layer_table(), bi.geom.bz), hits, bi.n_phi, bi.n_z)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    with pytest.raises(b.KfError, match="-6"):
+        b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K, bi.chi2_cut, bi.n_sigma)
