@@ -778,6 +778,17 @@ typedef struct {
     int nhits;
 } kfo_child;
 
+/* chi2 of hit m against the predicted state (pp, Cp) on the layer's nominal surface: hit_mode 0 the 3-D one [R5];
+ * hit_mode 1 second step to the hit's own surface, then the 2-D one on its tangent plane [R20, R21, R23].
+ * 0 = ok, -1 = S not positive definite, 1 = the second step does not reach the hit. */
+static int build_hit_chi2(int hit_mode, int disk, double bz, int q, const double pp[6], const double Cp[36], const double m[3],
+                          double srphi, double szz, double sr, double* c2) {
+    if (hit_mode == 0) return kfo_chi2(pp, Cp, m, srphi, szz, sr, c2) ? -1 : 0;
+    double p2[6], C2[36];
+    if (to_hit_surface(disk, bz, q, pp, Cp, m, p2, C2)) return 1;
+    return kfo_chi2_2d(p2, C2, m, disk, srphi, disk ? sr : szz, c2) ? -1 : 0;
+}
+
 static int child_cmp(const void* a_, const void* b_) {
     const kfo_child *a = (const kfo_child*)a_, *b = (const kfo_child*)b_;
     if (a->nhits != b->nhits) return a->nhits > b->nhits ? -1 : 1;
@@ -800,6 +811,13 @@ static int child_cmp(const void* a_, const void* b_) {
  * rho_c > rmax + d_rho or rho_c < rmin - d_rho; strict test |x'm_y - y'm_x| <= dphi rho_c rho_m, x'm_x + y'm_y > 0,
  * |rho_m - rho_c| <= d_rho; rows of the bins by radius.  chi2 and update: the 3-D ones [R5] (sig_z regularises along the
  * disk normal).  Barrel-only geometries keep the behaviour of R10 exactly.
+ * hit_mode 1 ("followed by further propagation steps to the position of each candidate hit.  KF updates are
+ * performed on the plane tangent to the hit radius") [R23]: the window is opened on the layer's nominal surface as above,
+ * widened by the displacement of the sensors about it (r.m.s. sig_r along the normal of a cylinder, sig_z along that of a disk);
+ * every hit inside it is reached by the second propagation step [R20] from the predicted state and judged by the chi2 of
+ * the 2-D residual on its tangent plane [R21]; a hit the second step cannot reach is not compatible; the kept hit
+ * children are updated there (2-D update; the state then sits on the hit's own surface).  hit_mode 0: 3-D chi2 and
+ * update on the nominal surface [R5].
  * counters[8]: 0 propagations, 1 hits scanned, 2 pass strict window, 3 pass chi2 cut (hit children), 4 updates,
  *              5 bin rows touched, 6 seed-layers, 7 children ranked.
  * margins (NULL or [n_seeds][n_layers][5], test diagnostics for DESIGN.md R16): the smallest RELATIVE distance of any
@@ -816,7 +834,7 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
               const float* sz, const int32_t* perm, const int32_t* bin_off, const int64_t* seg_off, int64_t n_seeds,
               int64_t ld_seed, const double* par, const double* cov, const int8_t* q, const double* chi2_in,
               const int32_t* seed_event, const int32_t* seed_hit_idx, int first_layer, int K, double chi2_cut,
-              double n_sigma, int use_bins, int64_t ld_out, double* par_o, double* cov_o, double* chi2_o,
+              double n_sigma, int use_bins, int hit_mode, int64_t ld_out, double* par_o, double* cov_o, double* chi2_o,
               int32_t* nhits_o, uint32_t* status_o, int32_t* hit_idx_o, int32_t* n_cand, int64_t* counters,
               double* margins) {
     if (K < 1 || K > 32 || n_layers > 32 || first_layer < 0 || first_layer > n_layers) return -1;
@@ -863,14 +881,29 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                     const double x = pp[c][0], y = pp[c][1], r2 = x * x + y * y;
                     double varphi = (x * x * Cp[c][1 * 6 + 1] - 2.0 * x * y * Cp[c][0 * 6 + 1] + y * y * Cp[c][0]) / (r2 * r2);
                     if (varphi < 0.0) varphi = 0.0;
+                    /* hit_mode 1 [R23]: the sensors sit off the nominal surface by an r.m.s. sig_n along its normal (sig_r on a
+                       cylinder, sig_z on a disk: the resolutions the 2-D update does not use); a sensor displaced by d along
+                       the normal is crossed d cot(theta)/cos(inc) further in z and d tan(inc)/r further in azimuth (cylinder),
+                       at most d tan(theta) further in radius and d tan(theta)/rho in azimuth (disk) */
+                    double wphi2 = 0.0, wrow2 = 0.0;
+                    if (hit_mode && !disk) {
+                        const double cinc = (x * cos(pp[c][4]) + y * sin(pp[c][4])) / sqrt(r2);
+                        const double cot = cos(pp[c][5]) / sin(pp[c][5]);
+                        wrow2 = (sr * cot / cinc) * (sr * cot / cinc);
+                        wphi2 = sr * sr * (1.0 - cinc * cinc) / (cinc * cinc) / r2;
+                    } else if (hit_mode) {
+                        const double tth = sin(pp[c][5]) / cos(pp[c][5]);
+                        wrow2 = szz * tth * szz * tth;
+                        wphi2 = wrow2 / r2;
+                    }
                     if (!disk) {
-                        dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R));
-                        dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz);
+                        dphi = n_sigma * sqrt(varphi + (srphi / R) * (srphi / R) + wphi2);
+                        dzw = n_sigma * sqrt(Cp[c][2 * 6 + 2] + szz * szz + wrow2);
                     } else {
                         double varrho = (x * x * Cp[c][0] + 2.0 * x * y * Cp[c][0 * 6 + 1] + y * y * Cp[c][1 * 6 + 1]) / r2;
                         if (varrho < 0.0) varrho = 0.0;
-                        dphi = n_sigma * sqrt(varphi + srphi * srphi / r2);
-                        dzw = n_sigma * sqrt(varrho + sr * sr);
+                        dphi = n_sigma * sqrt(varphi + srphi * srphi / r2 + wphi2);
+                        dzw = n_sigma * sqrt(varrho + sr * sr + wrow2);
                     }
                     if (!isfinite(dphi) || !isfinite(dzw)) f = KFO_NUMERIC;
                     else if (!disk) {
@@ -927,7 +960,8 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                                 const double near = fmin(in_z ? mphi : 1e300, in_phi ? mz : 1e300);
                                 if (near < mg[0]) {
                                     double c2m;
-                                    if (kfo_chi2(pp[c], Cp[c], m, srphi, szz, sr, &c2m) || c2m < chi2_cut) mg[0] = near;
+                                    int fm = build_hit_chi2(hit_mode, disk, bz, q[sd], pp[c], Cp[c], m, srphi, szz, sr, &c2m);
+                                    if (fm < 0 || (fm == 0 && c2m < chi2_cut)) mg[0] = near;
                                 }
                             }
                             if (!in_phi) continue;
@@ -935,7 +969,9 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                             if (!in_z) continue;
                             cnt[2] += 1;
                             double c2;
-                            if (kfo_chi2(pp[c], Cp[c], m, srphi, szz, sr, &c2)) { s_bad = 1; break; }
+                            const int fh = build_hit_chi2(hit_mode, disk, bz, q[sd], pp[c], Cp[c], m, srphi, szz, sr, &c2);
+                            if (fh < 0) { s_bad = 1; break; }
+                            if (fh > 0) continue;          /* hit_mode 1: the second step does not reach the hit's surface */
                             KFO_MARGIN(1, fabs(c2 / chi2_cut - 1.0));
                             if (!(c2 < chi2_cut)) continue;
                             cnt[3] += 1;
@@ -987,7 +1023,13 @@ int kfo_build(int n_layers, const double* layers, double bz, int n_phi, int n_z,
                     const double m[3] = {sx[k->hitpos], sy[k->hitpos], sz[k->hitpos]};
                     double c2;
                     cnt[4] += 1;
-                    int f = kfo_update(pp[k->parent], Cp[k->parent], m, srphi, szz, sr, o->p, o->C, &c2);
+                    int f;
+                    if (hit_mode == 0) f = kfo_update(pp[k->parent], Cp[k->parent], m, srphi, szz, sr, o->p, o->C, &c2);
+                    else {
+                        double p2[6], C2[36];
+                        f = to_hit_surface(disk, bz, q[sd], pp[k->parent], Cp[k->parent], m, p2, C2);
+                        if (f == 0) f = kfo_update_2d(p2, C2, m, disk, srphi, disk ? sr : szz, o->p, o->C, &c2);
+                    }
                     o->chi2 = k->chi2;
                     o->nhits = k->nhits;
                     o->hits[l] = perm[k->hitpos];

@@ -256,7 +256,7 @@ COUNTERS = ("n_prop", "n_scan", "n_window", "n_children", "n_upd", "n_rows", "n_
 
 
 def kf_build(layers, bz, binned, seg_off, par, cov21, q, seed_event, seed_hit_idx, first_layer, K, chi2_cut, n_sigma,
-          chi2_in=None, use_bins=True, n=None, margins=False):
+          chi2_in=None, use_bins=True, n=None, margins=False, hit_mode=0):
     """kf_build_ref.  -> dict(par [6][n*K], cov [n*K][6][6], chi2, nhits, status [n*K], hit_idx [L][n*K], n_cand [n], counters
     [, margins [n][L][5]: smallest relative distance of the seed's decisions on that layer to the window edge, the chi2
     cut, a rank swap, the propagation / acceptance guards, a tangential crossing; 1e300 = none])"""
@@ -280,7 +280,7 @@ def kf_build(layers, bz, binned, seg_off, par, cov21, q, seed_event, seed_hit_id
                      _p(binned["x"], C.c_float), _p(binned["y"], C.c_float), _p(binned["z"], C.c_float), _p(binned["perm"], C.c_int32),
                      _p(binned["bin_off"], C.c_int32), _p(seg_off, C.c_int64), C.c_int64(n), C.c_int64(ld), _p(par), _p(cov), _p(q, C.c_int8),
                      _p(ci), _p(se, C.c_int32), _p(sh, C.c_int32), C.c_int(first_layer), C.c_int(K), C.c_double(chi2_cut), C.c_double(n_sigma),
-                     C.c_int(1 if use_bins else 0), C.c_int64(ldo), _p(po), _p(co), _p(c2), _p(nh, C.c_int32), _p(st, C.c_uint32),
+                     C.c_int(1 if use_bins else 0), C.c_int(hit_mode), C.c_int64(ldo), _p(po), _p(co), _p(c2), _p(nh, C.c_int32), _p(st, C.c_uint32),
                      _p(hi, C.c_int32), _p(nc, C.c_int32), _p(cnt, C.c_int64), _p(mg))
     assert rc == 0, rc
     m = n * K

@@ -70,7 +70,7 @@ class Geometry:
         return t
 
 
-def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0) -> Geometry:
+def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0, depth: float = 0.0) -> Geometry:
     """kind 'barrel10' (configs 0,1,3): r = 4,8..40 cm, x/X0 = 0.02.
     kind 'barrel17' (configs 2,4): 17 layers r = 4..80 uniformly, x/X0 alternating 0.01/0.03."""
     if kind == "barrel10":
@@ -87,8 +87,11 @@ def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0) -> Geometry:
         r = np.concatenate([rb, zd, -zd])
         n = len(r)
         knd = np.concatenate([np.zeros(10, np.int32), np.ones(8, np.int32)])
+        # depth > 0 (building with kf_geom.hit_mode = 1, R23): the resolution along a surface's normal -- which the
+        # 2-D update does not use -- carries the r.m.s. displacement of the sensors about the nominal surface
         return Geometry(r=r, zmax=np.where(knd == 0, 50.0, 44.0), xx0=np.full(n, 0.02) * xx0_scale, sig_rphi=np.full(n, 0.01),
-                        sig_z=np.full(n, 0.1), sig_r=np.full(n, 0.01), bz=bz, kind=knd, rmin=np.where(knd == 0, 0.0, 4.0))
+                        sig_z=np.where((knd == 1) & (depth > 0), depth, 0.1), sig_r=np.where((knd == 0) & (depth > 0), depth, 0.01),
+                        bz=bz, kind=knd, rmin=np.where(knd == 0, 0.0, 4.0))
     else:
         raise ValueError(kind)
     n = len(r)
@@ -475,9 +478,11 @@ def _three_point_seed(p1, p2, p3, bz):
 def build_inputs(config, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
                  K: int = 10, chi2_cut: float = 30.0, n_sigma: float = 3.0, noise: float | None = None,
                  fake_frac: float | None = None, n_phi: int | None = None, n_z: int | None = None,
-                 smear: bool = True, ms: bool = True, event0: int = 0) -> BuildInputs:
+                 smear: bool = True, ms: bool = True, event0: int = 0, jitter: float = 0.0) -> BuildInputs:
     """Inputs of kf_bin_hits / kf_build for BASELINE.json configs 3-4 (sizes can be overridden for tests).
 
+    jitter > 0: sensors sit at R + U(-jitter, jitter) / Z + U(-jitter, jitter) ("hits at slightly different radii within a
+    layer"), truth and noise hits alike: inputs for kf_geom.hit_mode = 1.
     Per event: truth tracks from the particle gun; hits per layer = truth hits + `noise` x (number of truth
     hits on that layer) uniform in (phi, z) on the cylinder; each segment is shuffled.  One seed per truth
     track that reaches layer `first_layer-1`: truth state just outside that layer, smeared (smear_seed),
@@ -490,7 +495,7 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
     fake_frac = cfg["fake_frac"] if fake_frac is None else fake_frac
     n_phi = cfg["n_phi"] if n_phi is None else n_phi
     n_z = cfg["n_z"] if n_z is None else n_z
-    geom = geometry(cfg["geom"], xx0_scale=1.0 if ms else 0.0)
+    geom = geometry(cfg["geom"], xx0_scale=1.0 if ms else 0.0, **({"depth": jitter / np.sqrt(3.0)} if jitter > 0 else {}))
     L = geom.n_layers
     xs, ys, zs, tr = [], [], [], []
     seg_off = [0]
@@ -499,7 +504,7 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
     for ev in range(n_events):
         rng = rng_for(config if isinstance(config, int) else 101, ev + event0)     # event0: a rank's own events (weak scaling)
         gun = particle_gun(rng, tracks, cfg["gun"])
-        sim = simulate(geom, gun, rng, ms=ms, smear=smear)
+        sim = simulate(geom, gun, rng, ms=ms, smear=smear, jitter=jitter)
         ev_hits = []
         for l in range(L):
             v = sim["valid"][l]
@@ -513,6 +518,12 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
             else:                                  # disk: in the plane z = Z, radius uniform over the annulus' width
                 nz = np.full(n_noise, geom.r[l])
                 nr = rng.uniform(geom.rmin[l], geom.zmax[l], n_noise)
+            if jitter > 0:                         # the sensor a noise hit sits on is displaced like any other
+                off = rng.uniform(-jitter, jitter, n_noise)
+                if geom.kind[l] == 0:
+                    nr = nr + off
+                else:
+                    nz = nz + off
             hx = np.concatenate([sim["hits"][l, ids, 0], nr * np.cos(az)])
             hy = np.concatenate([sim["hits"][l, ids, 1], nr * np.sin(az)])
             hz = np.concatenate([sim["hits"][l, ids, 2], nz])

@@ -5,7 +5,9 @@ The paper gives no formula for any of it; what fixes the oracle here is (B1) the
 to X2 and the disk rows to a plain fp64 floor, (B2) the sorted index against a brute-force key, (B3) bins = no bins,
 (B4) the window list against brute force, (B5) the acceptance edges recomputed in numpy from the one-step primitives,
 (B6) an exhaustive Python enumeration of the rules from those primitives, (B7) best candidate = the fit of its hit list,
-(B8) truth purity on noise-free events with tracks that end on a disk."""
+(B8) truth purity on noise-free events with tracks that end on a disk; and for hit_mode 1 (second propagation step to every
+candidate hit, 2-D chi2 and update on its tangent plane; R23) the same four on events with staggered sensors
+(B9-B12)."""
 import numpy as np
 import pytest
 
@@ -20,9 +22,9 @@ def _event(n_events=2, tracks=300, **kw):
     return bi, lt, b
 
 
-def _build(bi, lt, b, K=None, use_bins=True, margins=False, n=None):
+def _build(bi, lt, b, K=None, use_bins=True, margins=False, n=None, hit_mode=0):
     return o.kf_build(lt, bi.geom.bz, b, bi.seg_off, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx, bi.first_layer,
-                      bi.K if K is None else K, bi.chi2_cut, bi.n_sigma, use_bins=use_bins, margins=margins, n=n)
+                      bi.K if K is None else K, bi.chi2_cut, bi.n_sigma, use_bins=use_bins, margins=margins, n=n, hit_mode=hit_mode)
 
 
 def test_B1_row_bin_barrel_is_X2_and_disk_is_a_floor():
@@ -108,12 +110,12 @@ def test_B4_window_list_on_a_disk_vs_brute_force():
         assert set(s0 + np.nonzero(inside)[0]) <= set(exp)
 
 
-def _disk_window(pp, Cp, n_sigma, srphi, sr):
+def _disk_window(pp, Cp, n_sigma, srphi, sr, wphi2=0.0, wrow2=0.0):
     x, y = pp[0], pp[1]
     r2 = x * x + y * y
     varphi = max((x * x * Cp[1, 1] - 2 * x * y * Cp[0, 1] + y * y * Cp[0, 0]) / r2 ** 2, 0.0)
     varrho = max((x * x * Cp[0, 0] + 2 * x * y * Cp[0, 1] + y * y * Cp[1, 1]) / r2, 0.0)
-    return np.sqrt(r2), n_sigma * np.sqrt(varphi + srphi ** 2 / r2), n_sigma * np.sqrt(varrho + sr ** 2)
+    return np.sqrt(r2), n_sigma * np.sqrt(varphi + srphi ** 2 / r2 + wphi2), n_sigma * np.sqrt(varrho + sr ** 2 + wrow2)
 
 
 def test_B5_disk_acceptance_edges():
@@ -152,8 +154,8 @@ def test_B5_disk_acceptance_edges():
     assert skipped >= 8 and crossed >= 8
 
 
-def _enumerate(bi, lt, b, s, K):
-    """Exhaustive Python version of R10 / R11 / R22 for one seed, built from the oracle's one-step primitives."""
+def _enumerate(bi, lt, b, s, K, hit_mode=0):
+    """Exhaustive Python version of R10 / R11 / R22 (hit_mode 1: R23) for one seed, built from the oracle's one-step primitives."""
     L = lt.shape[0]
     ev = bi.seed_event[s]
     cands = [dict(p=bi.par[:, s].astype(np.float64), C=synth.unpack_sym(bi.cov[:, s].astype(np.float64)), chi2=0.0, nh=bi.first_layer,
@@ -172,13 +174,22 @@ def _enumerate(bi, lt, b, s, K):
                 children.append((-c["nh"], c["chi2"], ci, np.inf, "skip", 0)); continue
             x, y = pp[0], pp[1]
             r2 = x * x + y * y
+            # hit_mode 1 (R23): sensors displaced along the surface normal by an r.m.s. sig_r (cylinder) / sig_z (disk) widen the window
+            wphi2 = wrow2 = 0.0
+            if hit_mode and kind == 0:
+                cinc = (x * np.cos(pp[4]) + y * np.sin(pp[4])) / np.sqrt(r2)
+                wrow2 = (sr / np.tan(pp[5]) / cinc) ** 2
+                wphi2 = sr ** 2 * (1 - cinc ** 2) / cinc ** 2 / r2
+            elif hit_mode:
+                wrow2 = (sz * np.tan(pp[5])) ** 2
+                wphi2 = wrow2 / r2
             if kind == 0:
-                dphi = bi.n_sigma * np.sqrt(max((x * x * Cp[1, 1] - 2 * x * y * Cp[0, 1] + y * y * Cp[0, 0]) / r2 ** 2, 0) + (srphi / R) ** 2)
-                dw = bi.n_sigma * np.sqrt(Cp[2, 2] + sz * sz)
+                dphi = bi.n_sigma * np.sqrt(max((x * x * Cp[1, 1] - 2 * x * y * Cp[0, 1] + y * y * Cp[0, 0]) / r2 ** 2, 0) + (srphi / R) ** 2 + wphi2)
+                dw = bi.n_sigma * np.sqrt(Cp[2, 2] + sz * sz + wrow2)
                 off = abs(pp[2]) > zmax + dw
                 row, rowc = hz, pp[2]
             else:
-                rho, dphi, dw = _disk_window(pp, Cp, bi.n_sigma, srphi, sr)
+                rho, dphi, dw = _disk_window(pp, Cp, bi.n_sigma, srphi, sr, wphi2, wrow2)
                 off = rho > zmax + dw or rho < rmin - dw
                 row, rowc = np.hypot(hx, hy), rho
             if off:
@@ -187,9 +198,18 @@ def _enumerate(bi, lt, b, s, K):
             got = False
             for h in s0 + np.nonzero(inside)[0]:
                 m = np.array([b["x"][h], b["y"][h], b["z"][h]], dtype=np.float64)
-                rc, c2 = o.chi2(pp, Cp, m, srphi, sz, sr)
-                if rc == 0 and c2 < bi.chi2_cut:
-                    children.append((-(c["nh"] + 1), c["chi2"] + c2, ci, h, "hit", (pp, Cp, m)))
+                if hit_mode == 0:
+                    rc, c2 = o.chi2(pp, Cp, m, srphi, sz, sr)
+                    at = (pp, Cp, m)
+                else:           # second step to the hit's own surface, 2-D chi2 on its tangent plane
+                    f2, p2, C2 = o.to_hit_surface(int(kind), bi.geom.bz, bi.q[s], pp, Cp, m)
+                    if f2:
+                        continue
+                    rc, c2 = o.chi2_2d(p2, C2, m, int(kind), srphi, sr if kind else sz)
+                    at = (p2, C2, m)
+                assert rc == 0
+                if c2 < bi.chi2_cut:
+                    children.append((-(c["nh"] + 1), c["chi2"] + c2, ci, h, "hit", at))
                     got = True
             if not got:
                 children.append((-c["nh"], c["chi2"], ci, np.inf, "miss", (pp, Cp, None)))
@@ -205,7 +225,10 @@ def _enumerate(bi, lt, b, s, K):
                 hits[l] = -1
                 new.append(dict(p=aux[0], C=aux[1], chi2=c["chi2"], nh=c["nh"], hits=hits, fin=False, st=c["st"]))
             else:
-                f, pu, Cu, _ = o.update(aux[0], aux[1], aux[2], srphi, sz, sr)
+                if hit_mode == 0:
+                    f, pu, Cu, _ = o.update(aux[0], aux[1], aux[2], srphi, sz, sr)
+                else:
+                    f, pu, Cu, _ = o.update_2d(aux[0], aux[1], aux[2], int(kind), srphi, sr if kind else sz)
                 assert f == 0
                 hits[l] = int(b["perm"][h])
                 new.append(dict(p=pu, C=Cu, chi2=chi2, nh=-mnh, hits=hits, fin=False, st=c["st"]))
@@ -259,3 +282,67 @@ def test_B8_truth_purity_on_noise_free_lids_events():
     ends_on_disk = (truth[10:] >= 0).any(axis=0)
     assert ends_on_disk.sum() > 100 and same[ends_on_disk].mean() > 0.90, (ends_on_disk.sum(), same[ends_on_disk].mean())
     assert (r["status"][::K][:bi.n_seeds] == 0).all()
+
+
+# ------------------------------------------------------------------------------------------------ hit_mode 1 (R23)
+def _event_j(n_events=1, tracks=120, **kw):
+    return _event(n_events=n_events, tracks=tracks, jitter=0.3, **kw)
+
+
+@pytest.mark.parametrize("K", [1, 4])
+def test_B9_two_step_build_equals_exhaustive_python_enumeration(K):
+    bi, lt, b = _event_j(n_events=1, tracks=120)
+    r = _build(bi, lt, b, K=K, hit_mode=1)
+    checked = ends_on_disk = 0
+    for s in range(0, bi.n_seeds, 3):
+        ref = _enumerate(bi, lt, b, s, K, hit_mode=1)
+        assert r["n_cand"][s] == len(ref)
+        for k, c in enumerate(ref):
+            slot = s * K + k
+            assert list(r["hit_idx"][:, slot]) == c["hits"], (s, k)
+            assert r["nhits"][slot] == c["nh"] and abs(r["chi2"][slot] - c["chi2"]) <= 1e-9 * max(1, c["chi2"])
+            pe = c["p"].copy(); pe[4] = np.angle(np.exp(1j * pe[4]))
+            assert np.max(np.abs(r["par"][:, slot] - pe)) < 1e-9 and np.max(np.abs(r["cov"][slot] - c["C"])) < 1e-9 * np.abs(c["C"]).max()
+            checked += 1
+            ends_on_disk += max(i for i, h in enumerate(c["hits"]) if h >= 0) >= 10
+    assert checked >= 30 and ends_on_disk >= 5
+
+
+def test_B10_two_step_best_candidate_is_the_two_step_fit_of_its_hit_list():
+    bi, lt, b = _event_j(n_events=2, tracks=300)
+    r = _build(bi, lt, b, hit_mode=1)
+    K, n = bi.K, bi.n_seeds
+    hi = np.full((lt.shape[0], bi.ld), -2, np.int32)
+    hi[:, :n] = r["hit_idx"][:, ::K]
+    hi[:bi.first_layer] = -2
+    f = o.fit(lt, bi.geom.bz, bi.par, bi.cov, bi.q, bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, hit_idx=hi, trk_event=bi.seed_event, n=n, hit_mode=1)
+    assert np.array_equal(f["nhits"] + bi.first_layer, r["nhits"][::K]) and (f["status"] == 0).all()
+    assert np.allclose(f["chi2"], r["chi2"][::K], rtol=1e-9, atol=1e-9)
+    assert np.allclose(f["par"][[0, 1, 2, 3, 5]], r["par"][[0, 1, 2, 3, 5]][:, ::K], rtol=1e-9, atol=1e-9)
+    assert np.allclose(f["cov"], r["cov"][::K], rtol=1e-8, atol=1e-14)
+    # and the states do sit on the hits' own surfaces, off the nominal ones
+    last = np.array([max(i for i in range(lt.shape[0]) if hi[i, t] >= 0) if (hi[:, t] >= 0).any() else -1 for t in range(n)])
+    crossed = np.array([max(i for i in range(lt.shape[0]) if hi[i, t] >= -1) if (hi[:, t] >= -1).any() else -1 for t in range(n)])
+    barrel = (last >= 3) & (last < 10) & (crossed == last)          # the last layer crossed carries a hit
+    off = np.abs(np.hypot(r["par"][0, ::K][barrel], r["par"][1, ::K][barrel]) - lt[last[barrel], 0])
+    assert barrel.sum() > 50 and off.max() <= 0.3 + 1e-6 and np.median(off) > 0.05
+
+
+def test_B11_two_step_bins_equal_brute_force_and_truth_purity():
+    bi, lt, b = _event_j(n_events=2, tracks=300)
+    a = _build(bi, lt, b, hit_mode=1)
+    c = _build(bi, lt, b, hit_mode=1, use_bins=False)
+    for k in ("n_cand", "hit_idx", "nhits", "status", "chi2", "par"):
+        assert np.array_equal(a[k], c[k]), k
+    bi, lt, b = _event_j(n_events=2, tracks=300, noise=0.0)
+    r = _build(bi, lt, b, hit_mode=1)
+    K = bi.K
+    best = r["hit_idx"][:, ::K][:, :bi.n_seeds]
+    truth = bi.truth_hit_idx[:, bi.seed_truth]
+    truth = np.where(truth >= 0, truth, -9)
+    same = ((best == truth) | ((truth == -9) & (best < 0)))[bi.first_layer:].all(axis=0)
+    assert same.mean() > 0.93, same.mean()
+    # chi2 of the 2-D residuals: 2 per hit added (R21)
+    full = same & (r["nhits"][::K][:bi.n_seeds] >= 8)
+    per_hit = r["chi2"][::K][:bi.n_seeds][full] / (r["nhits"][::K][:bi.n_seeds][full] - bi.first_layer)
+    assert full.sum() > 200 and 1.7 < per_hit.mean() < 2.3, (full.sum(), per_hit.mean())
