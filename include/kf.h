@@ -62,8 +62,8 @@ typedef struct { float r, zmax, xx0, sig_rphi, sig_z, sig_r; int32_t kind; float
 
 /* Geometry: n_layers layers in the order a track from the vertex crosses them (cylinders by increasing r, then the
  * disks of either side by increasing |z|); uniform field bz_tesla along z.  `layers` is a HOST array.
- * hit_mode 0: hits lie on the nominal surfaces, 3-D update there (R5).  hit_mode 1 (R20, R21;
- * kf_fit only): two-step propagation -- to the nominal surface, where the material is added, then on to the hit's own
+ * hit_mode 0: hits lie on the nominal surfaces, 3-D update there (R5).  hit_mode 1 (R20, R21; kf_fit
+ * and kf_build): two-step propagation -- to the nominal surface, where the material is added, then on to the hit's own
  * radius (barrel) or z (disk) -- and a 2-D update on the plane tangent to the hit radius (r-phi and z for a barrel
  * hit, r-phi and r for a disk hit); the state then sits on the hit's surface. */
 typedef struct { int32_t n_layers; float bz_tesla; const kf_layer* layers; int32_t hit_mode; } kf_geom;
@@ -159,10 +159,15 @@ int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const kf_binned* 
  * n_sigma standard deviations in phi and z, chi2 against every hit of the window, one child per hit with
  * chi2 < chi2_cut (else one child without hit), keep the best K children by (nhits desc, chi2 asc, parent slot asc,
  * sorted hit position asc), update the survivors.
- * Geometry with endcap disks ("cylinder with lids"; R22; geom->hit_mode must be 0): on a disk the
- * window is in phi and radius, and on any layer a candidate that cannot be propagated there (not reached, grazing) or
- * whose window lies off the layer skips it (hit_idx -2, state unchanged, no status bit) and lives on; only a numeric
- * failure finishes a candidate.  A barrel-only geometry keeps the behaviour below (a failed layer finishes the candidate).
+ * Geometry with endcap disks ("cylinder with lids"; R22): on a disk the window is in phi and
+ * radius, and on any layer a candidate that cannot be propagated there (not reached, grazing) or whose window lies off the
+ * layer skips it (hit_idx -2, state unchanged, no status bit) and lives on; only a numeric failure finishes a candidate.
+ * A barrel-only geometry keeps the behaviour below (a failed layer finishes the candidate).
+ * geom->hit_mode 1 ("further propagation steps to the position of each candidate hit"; R23): every hit
+ * of the window is reached by a second propagation step from the predicted state and judged by the chi2 of its 2-D residual
+ * on the plane tangent to the hit radius; survivors are updated there (state on the hit's own surface).  The window is
+ * widened by the displacement of the sensors about the nominal surface, whose r.m.s. is read from the resolution along the
+ * surface normal (sig_r of a cylinder, sig_z of a disk), which the 2-D update does not use.
  * Output: slot s*K + k of `cand` (best first), hit_idx[l*ld + slot] = original index within the segment,
  * -1 = no hit on this layer, -2 = layer not crossed (candidate finished); n_cand[s] = number of valid slots.
  */
@@ -186,7 +191,7 @@ typedef struct {
  * next call on the same stream.  opt (NULL = automatic): seeds per thread block and the cap on the persistent grid;
  * the result does not depend on them, the workspace size does (pass the same opt to both calls).
  * Errors: NULL pointers, K / first_layer / cuts / options out of range, bad bin counts, workspace too small (-4),
- * geom->hit_mode != 0 (KF_ERR_UNIMPLEMENTED: the two-step propagation is built for kf_fit), CUDA failure. */
+ * CUDA failure. */
 size_t kf_build_workspace_bytes(const kf_geom* geom, int64_t n_seeds, int32_t K, const kf_options* opt);
 int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binned* binned, const kf_tracks* seeds,
              const int32_t* seed_event, const int32_t* seed_hit_idx, int32_t first_layer, int32_t K, float chi2_cut,

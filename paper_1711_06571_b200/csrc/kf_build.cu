@@ -72,7 +72,7 @@ struct BuildArgs {
     LayerC layer[KF_MAX_LAYERS];
     float inv_dz[KF_MAX_LAYERS], sphi_over_r2[KF_MAX_LAYERS];   // n_z/(2 zmax) (disk: n_z/(rmax - rmin)); (sig_rphi/r)^2
     float row_lo[KF_MAX_LAYERS];   // X2 rows of any layer start at -zmax (disk: rmin)
-    int32_t lids;             // the geometry has disks (R22)
+    int32_t lids, hit_mode;   // the geometry has disks (R22); two-step propagation and 2-D update per candidate hit (R23)
 };
 
 // Records are stored as NREC4 = 9 groups of four words, group g of record c at float4 index g * SK + c: a record moves
@@ -214,6 +214,21 @@ __device__ __forceinline__ Tile tile_of(const BuildArgs& a) {
 // The three per-thread bodies are separate functions (not inlined) so that each gets its own register allocation:
 // inlined into one kernel they need 228 registers and spill ~480 bytes at the 128 the launch bounds allow.
 
+// hit_mode 1 (R20, R21, R23): second propagation step from the predicted state s on the layer's nominal surface to the surface
+// through the hit (its own radius / its own z), then the 2-D update on the plane tangent to the hit radius; chi2 = that of
+// the 2-D residual.  0 = done, 1 = the second step does not reach the hit (s untouched), -1 = S not positive definite.
+static __device__ __noinline__ int two_step_update(State& s, float cw, const LayerC& ly, float mx, float my, float mz, float& chi2) {
+    uint32_t flag;
+    if (ly.kind) flag = predict_disk<true>(s, cw, ly, mz);
+    else {
+        LayerC hl = ly;
+        hl.r2 = fmaf(mx, mx, my * my); hl.rcmin = 0.0f; hl.xx0r = 0.0f;
+        flag = predict<true>(s, cw, hl);
+    }
+    if (flag) return 1;
+    return update_2d(s, mx, my, mz, ly.kind, ly.var_rphi, ly.kind ? ly.var_r : ly.var_z, chi2) ? 0 : -1;
+}
+
 // phase 1, one live candidate: dense index base + i, round-local index i
 // LIDS: the geometry has disks (R22); a barrel-only geometry compiles without any of it
 template <bool ISO, bool LIDS>
@@ -286,15 +301,29 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
                 const float varphi = fmaxf(num / (r2 * r2), 0.0f);
                 float dphi;
                 bool off;
+                // hit_mode 1 (R23): sensors displaced along the surface normal (r.m.s. sig_r on a cylinder, sig_z on a disk) are
+                // crossed elsewhere than on the nominal surface: the window grows by that
+                float wphi2 = 0.0f, wrow2 = 0.0f;
+                if (a.hit_mode && !disk) {
+                    const float cinc = fmaf(px, st.CC.x, py * st.SS.x) * rsqrtf(r2);
+                    const float cot = st.CC.y / st.SS.y;
+                    const float t = cot / cinc;
+                    wrow2 = ly.var_r * t * t;
+                    wphi2 = ly.var_r * (1.0f - cinc * cinc) / (cinc * cinc) / r2;
+                } else if (a.hit_mode) {
+                    const float tth = st.SS.y / st.CC.y;
+                    wrow2 = ly.var_z * tth * tth;
+                    wphi2 = wrow2 / r2;
+                }
                 if (!disk) {
-                    dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l]);
-                    dzw = a.n_sigma * sqrtf(c22 + ly.var_z);
+                    dphi = a.n_sigma * sqrtf(varphi + a.sphi_over_r2[l] + wphi2);
+                    dzw = a.n_sigma * sqrtf(c22 + ly.var_z + wrow2);
                     wrow = pz;
                     off = fabsf(pz) > ly.zmax + dzw;
                 } else {
                     const float varrho = fmaxf(fmaf(px * px, c00, fmaf(2.0f * px * py, c10, py * py * c11)) / r2, 0.0f);
-                    dphi = a.n_sigma * sqrtf(varphi + ly.var_rphi / r2);
-                    dzw = a.n_sigma * sqrtf(varrho + ly.var_r);
+                    dphi = a.n_sigma * sqrtf(varphi + ly.var_rphi / r2 + wphi2);
+                    dzw = a.n_sigma * sqrtf(varrho + ly.var_r + wrow2);
                     wrow = sqrtf(r2);
                     off = wrow > ly.zmax + dzw || wrow < ly.rmin - dzw;
                 }
@@ -311,7 +340,7 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
                     }
                 }
             }
-            if (flag != 0u && flag != ST_NUMERIC) { skip = true; flag = 0u; }
+            if (a.lids && flag != 0u && flag != ST_NUMERIC) { skip = true; flag = 0u; }
             fin = flag != 0u || skip;
         }
     }
@@ -372,6 +401,20 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
                         for (int v = 1; v < SCAN_BATCH; ++v)
                             if (u == v) { m4 = hv[v]; h = hpos[v]; }
                         const float mx = m4.x, my = m4.y, mz = m4.z;
+                        if constexpr (LIDS) {
+                            if (a.hit_mode) {      // second step to the hit, 2-D chi2 there (the updated copy is dropped)
+                                State t2 = st;
+                                float c2h;
+                                const int r2s = two_step_update(t2, cw, ly, mx, my, mz, c2h);
+                                if (r2s < 0) { sbad = true; continue; }
+                                if (r2s > 0) continue;
+                                if (c2h < a.chi2_cut) {
+                                    if (cnt < K) { lc[cnt * ncap] = chi2 + c2h; lh[cnt * ncap] = h; ++cnt; }
+                                    else list_replace_worst(lc, lh, ncap, K, chi2 + c2h, h);
+                                }
+                                continue;
+                            }
+                        }
                         bool ok = fok;
                         if (!ISO) {
                             const HitCov V = hit_cov(mx, my, ly);
@@ -411,7 +454,7 @@ __device__ __noinline__ void build_candidate(const BuildArgs& a, int l, int base
 }
 
 // phase 3, one surviving child: dense index cn among the children of the tile
-template <bool ISO>
+template <bool ISO, bool LIDS>
 __device__ __noinline__ void build_child(const BuildArgs& a, int l, int cn) {
     const Tile T = tile_of(a);
     // shared arrays are re-derived from the block's shared window (so that they stay LDS / STS, not generic accesses)
@@ -454,8 +497,16 @@ __device__ __noinline__ void build_child(const BuildArgs& a, int l, int cn) {
         else V = hit_cov(mx, my, ly);
         Ldl3 F;
         float r[3], c2;
-        bool ok = innovation(st, mx, my, mz, V, F, r, c2);
-        gain_update<ISO>(st, F, V, r);
+        bool ok;
+        bool two_step = false;
+        if constexpr (LIDS) two_step = a.hit_mode != 0;
+        if (two_step) {
+            const int64_t s0 = *reinterpret_cast<const long long*>(smem + m.misc + 4 * 36);      // first seed of the tile
+            ok = two_step_update(st, -(float)a.q[s0 + s] * a.kb, ly, mx, my, mz, c2) == 0;
+        } else {
+            ok = innovation(st, mx, my, mz, V, F, r, c2);
+            gain_update<ISO>(st, F, V, r);
+        }
         ok = ok && state_finite(st) && st.IT.x > 0.0f;
         if (ok) {
             rec_store(st, chi2c, (meta & ~255) | nh, recA, SK, cn);
@@ -543,6 +594,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
     for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t s0 = tile * S;
         const int ns = (int)min((int64_t)S, a.n_seeds - s0);
+        if constexpr (LIDS) { if (tid == 0) *reinterpret_cast<long long*>(s_misc + 36) = s0; }
         // ---- seeds -> one candidate each, dense index = seed ----
         if (tid < S) {
             if (tid < ns) {
@@ -624,7 +676,7 @@ __global__ void __launch_bounds__(NT, BUILD_THREADS_PER_SM / NT) kf_build_kernel
             // ---------------- phase 3: update the survivors, thread per child (B5) ----------------
             const int nchild = s_offn[S];
             for (int cn = tid; cn < nchild; cn += NT) {
-                build_child<ISO>(a, l, cn);
+                build_child<ISO, LIDS>(a, l, cn);
             }
             __syncthreads();
             if (tid < S) { s_nc[tid] = tid < ns ? s_nnew[tid] : 0; s_off[tid] = s_offn[tid]; }
@@ -706,7 +758,7 @@ static int launch_build3(const BuildArgs& a, const BuildPlan& p, cudaStream_t st
 
 template <int NT>
 static int launch_build(const BuildArgs& a, const BuildPlan& p, bool iso, cudaStream_t st) {
-    if (a.lids) return iso ? launch_build3<NT, true, true>(a, p, st) : launch_build3<NT, false, true>(a, p, st);
+    if (a.lids || a.hit_mode) return iso ? launch_build3<NT, true, true>(a, p, st) : launch_build3<NT, false, true>(a, p, st);
     return iso ? launch_build3<NT, true, false>(a, p, st) : launch_build3<NT, false, false>(a, p, st);
 }
 
@@ -725,7 +777,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     if (!geom || !hits || !binned || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_build: NULL struct argument");
     int rc = check_geom(geom, "kf_build");
     if (rc) return rc;
-    if (geom->hit_mode != 0) return fail(KF_ERR_UNIMPLEMENTED, "kf_build: hit_mode 1 (two-step propagation, 2-D update) is built for kf_fit only");
+    if (geom->hit_mode != 0 && geom->hit_mode != 1) return fail(KF_ERR_INVALID_ARG, "kf_build: hit_mode must be 0 or 1");
     if (K < 1 || K > 32) return fail(KF_ERR_INVALID_ARG, "kf_build: K = %d outside 1..32", K);
     if (first_layer < 0 || first_layer > geom->n_layers) return fail(KF_ERR_INVALID_ARG, "kf_build: first_layer outside 0..n_layers");
     if (!(chi2_cut > 0.f) || !(n_sigma > 0.f)) return fail(KF_ERR_INVALID_ARG, "kf_build: chi2_cut and n_sigma must be positive");
@@ -755,7 +807,7 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     a.hit_idx_o = out->hit_idx; a.n_cand_o = out->n_cand;
     a.ws_rec = (float*)((char*)ws + p.o_rec); a.ws_link_hit = (int32_t*)((char*)ws + p.o_lh);
     bool iso = true;
-    a.lids = 0;
+    a.lids = 0; a.hit_mode = geom->hit_mode;
     for (int l = 0; l < KF_MAX_LAYERS; ++l) {
         const kf_layer& y = geom->layers[l < geom->n_layers ? l : geom->n_layers - 1];
         a.layer[l] = make_layer(y);

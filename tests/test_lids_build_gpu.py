@@ -94,13 +94,61 @@ def test_lids_build_then_final_fit():
     assert np.allclose(g["chi2"][m], c["chi2"][best][m], rtol=2e-4, atol=1e-4)
 
 
-def test_build_with_hit_mode_1_is_unimplemented():
+def _run_two_step(bi, K=None):
+    from paper_1711_06571_b200 import binding as b
+    lt = bi.geom.layer_table()
+    geom = b.Geom(lt, bi.geom.bz, hit_mode=1)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    binned = b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    sev = t(bi.seed_event)
+    K = bi.K if K is None else K
+    cands = b.kf_build(geom, hits, binned, seeds, sev, t(bi.seed_hit_idx), bi.first_layer, K, bi.chi2_cut, bi.n_sigma)
+    idx = b.kf_select_best(cands, bi.first_layer, seeds.ld)
+    fitted = b.kf_fit(geom, hits, idx, sev, seeds)
+    torch.cuda.synchronize()
+    rb = ref_bin(bi)
+    r = o.kf_build(lt, bi.geom.bz, rb, bi.seg_off, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx, bi.first_layer, K, bi.chi2_cut, bi.n_sigma,
+                   margins=True, hit_mode=1)
+    return cands.to_host(), r, fitted.to_host(), idx.cpu().numpy()
+
+
+@pytest.mark.parametrize("kw,K", [(dict(n_events=3, tracks=2000), None), (dict(n_events=2, tracks=1500), 3), (dict(n_events=2, tracks=1500, noise=0.0), None)])
+def test_lids_two_step_build_parity(kw, K):
+    """kf_build with hit_mode = 1 (R23) on sensors staggered by +-0.3 cm: second step to every candidate hit, 2-D chi2
+    and update on its tangent plane; then the final fit of the best candidates with the same hit mode."""
+    bi = synth.build_inputs("lids", jitter=0.3, **kw)
+    K_ = bi.K if K is None else K
+    g, r, gf, hi = _run_two_step(bi, K)
+    rep = compare_build(g, r, bi.n_seeds, K_, bi.first_layer, band_frac=0.05)
+    best = np.arange(bi.n_seeds) * K_
+    assert (r["hit_idx"][10:, best] >= 0).any(axis=0).mean() > 0.3 and rep["seed_mismatch_frac"] < 0.03
+    # states sit on the hits' own surfaces: off the nominal radius of the last barrel layer with a hit
+    hl = r["hit_idx"][:, best]
+    last_hit = np.array([max([i for i in range(hl.shape[0]) if hl[i, t] >= 0], default=-1) for t in range(bi.n_seeds)])
+    last_x = np.array([max([i for i in range(hl.shape[0]) if hl[i, t] >= -1], default=-1) for t in range(bi.n_seeds)])
+    sel = (last_hit >= 3) & (last_hit < 10) & (last_x == last_hit)
+    off = np.abs(np.hypot(g["par"][0, best][sel], g["par"][1, best][sel]) - bi.geom.layer_table()[last_hit[sel], 0])
+    assert sel.sum() > 100 and off.max() <= 0.3 + 1e-4 and np.median(off) > 0.05
+    # final fit with the same hit mode against the oracle's fit of the same lists
+    rf = o.fit(bi.geom.layer_table(), bi.geom.bz, bi.par, bi.cov, bi.q, bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, hit_idx=hi, trk_event=bi.seed_event, hit_mode=1)
+    same = (gf["nhits"] == rf["nhits"]) & (gf["status"] == rf["status"])
+    assert (~same).sum() <= 3e-3 * bi.n_seeds, int((~same).sum())
+    x, y, ph = rf["par"][0], rf["par"][1], rf["par"][4]
+    cosinc = (x * np.cos(ph) + y * np.sin(ph)) / np.maximum(np.hypot(x, y), 1e-30)
+    ok = same & (rf["status"] == 0) & (cosinc >= 0.25)
+    assert ok.mean() > 0.9
+    assert_parity(compare_tracks(gf, rf, sel=ok))
+
+
+def test_build_rejects_an_unknown_hit_mode():
     from paper_1711_06571_b200 import binding as b
     bi = synth.build_inputs("lids", n_events=1, tracks=50)
-    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz, hit_mode=1)
+    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz, hit_mode=2)
     hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
     binned = b.kf_bin_hits(b.Geom(bi.geom.layer_table(), bi.geom.bz), hits, bi.n_phi, bi.n_z)
     seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    with pytest.raises(b.KfError, match="-6"):
+    with pytest.raises(b.KfError, match="-3"):
         b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K, bi.chi2_cut, bi.n_sigma)
