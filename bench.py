@@ -44,7 +44,11 @@ BUILD_FLOP = dict(n_prop=458.0, n_scan=15.0, n_window=40.0, n_upd=250.0)
 BIN_BYTES_PER_HIT = 28.0   # algorithmic: read x, y, z (12), write the sorted 16-byte record (16); + 4 per bin for bin_off
 SM_COUNT, FP32_LANES = 148, 128
 FIT_CFG = {"fit_c0": 0, "fit_c1": 1, "fit_c2": 2}
-BUILD_CFG = {"build_c3": 3, "build_c4": 4}
+BUILD_CFG = {"build_c3": 3, "build_c4": 4, "build_lids": "lids", "build_lids_two_step": "lids"}
+# building on the "cylinder with lids" (R22, R23): hits on the nominal surfaces / sensors
+# staggered by +-0.3 cm with the second propagation step to every candidate hit (kf_geom.hit_mode = 1); not in the default line
+BUILD_KW = {"build_lids_two_step": dict(jitter=0.3)}
+BUILD_HIT_MODE = {"build_lids_two_step": 1}
 
 
 def peaks():
@@ -152,7 +156,7 @@ def oracle_fit(fi, n_s, steps, warmup):
                 sample=f"first {n_s} tracks of the {fi.n}-track workload per step", ms_per_step=dt * 1e3)
 
 
-def oracle_build(bi, n_ev, steps, warmup):
+def oracle_build(bi, n_ev, steps, warmup, hit_mode=0):
     """kfo_bin_hits + kfo_build on the first n_ev events (whole events: seeds only see hits of their own event)."""
     from oracle import kf_oracle as o
     L = bi.geom.n_layers
@@ -168,7 +172,7 @@ def oracle_build(bi, n_ev, steps, warmup):
     def call():
         rb = o.bin_hits(lt, n_ev, seg, bi.hit_x[:n_h], bi.hit_y[:n_h], bi.hit_z[:n_h], bi.n_phi, bi.n_z)
         res["r"] = o.kf_build(lt, bi.geom.bz, rb, seg, bi.par, bi.cov, bi.q[:n_s], bi.seed_event[:n_s], bi.seed_hit_idx, bi.first_layer,
-                              bi.K, bi.chi2_cut, bi.n_sigma, n=n_s)
+                              bi.K, bi.chi2_cut, bi.n_sigma, n=n_s, hit_mode=hit_mode)
     for _ in range(warmup):
         call()
     t0 = time.perf_counter()
@@ -199,8 +203,8 @@ def run_reference(args, workload):
         cb = dict(value=m / dt, unit="multiplies/s", cores=1, kind="oracle", sample=f"{m} matrices per step, numpy fp64 matmul", ms_per_step=dt * 1e3)
         metric, cfg = "mat66_multiplies_per_s", dict(workload=workload, matrices=args.tracks or 4_000_000)
     else:
-        bi = synth.build_inputs(BUILD_CFG[workload], n_events=args.events)
-        cb, _, _ = oracle_build(bi, args.ref_events, args.steps, args.warmup)
+        bi = synth.build_inputs(BUILD_CFG[workload], n_events=args.events, **BUILD_KW.get(workload, {}))
+        cb, _, _ = oracle_build(bi, args.ref_events, args.steps, args.warmup, hit_mode=BUILD_HIT_MODE.get(workload, 0))
         metric, cfg = "seeds_built_per_s", dict(workload=workload, events=bi.n_events, seeds=bi.n_seeds, layers=bi.geom.n_layers, K=bi.K)
     ms = cb.pop("ms_per_step")
     return dict(impl="reference", metric=metric, value=cb["value"], unit=cb["unit"], n_gpus=args.gpus, steps=args.steps,
@@ -370,11 +374,11 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
         n_ev_cfg = args.events if args.events is not None else synth.BUILD_CONFIGS[cfg]["n_events"]
         per_event = synth.BUILD_CONFIGS[cfg]["tracks"] * (1.0 + synth.BUILD_CONFIGS[cfg]["fake_frac"])
         mine = shard.assign_events([per_event] * n_ev_cfg, d.world)[d.rank]
-        bi = synth.build_inputs(cfg, n_events=max(len(mine), 1), event0=mine[0] if mine else 0)
+        bi = synth.build_inputs(cfg, n_events=max(len(mine), 1), event0=mine[0] if mine else 0, **BUILD_KW.get(workload, {}))
     else:
-        bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000)
+        bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000, **BUILD_KW.get(workload, {}))
     L, K = bi.geom.n_layers, bi.K
-    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz)
+    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz, hit_mode=BUILD_HIT_MODE.get(workload, 0))
     hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
     n_bins = bi.n_events * L * bi.n_phi * bi.n_z
     binned = b.Binned(hits.n_hits, n_bins, bi.n_phi, bi.n_z, soa=False)     # the records and bin_off: all the build reads
@@ -432,7 +436,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     res["bin_roofline"] = dict(bound="hbm", achieved=bin_bytes / (bin_ms * 1e-3) / 1e9, peak=pk["hbm_gbs"], unit="GB/s",
                                frac=bin_bytes / (bin_ms * 1e-3) / 1e9 / pk["hbm_gbs"], alg_bytes_per_step=bin_bytes, kernels="kf_bin_* (memset + 4 launches)")
     if not args.no_cpu_baseline:
-        cb, counters, n_s = oracle_build(bi, args.cpu_events, 1, 0)
+        cb, counters, n_s = oracle_build(bi, args.cpu_events, 1, 0, hit_mode=BUILD_HIT_MODE.get(workload, 0))
         cb.pop("ms_per_step")
         u = build_units(counters, bi.n_seeds, K, L, scale=bi.n_seeds / max(n_s, 1))
         peak = fp32_peak_tflops(pk)
@@ -552,7 +556,7 @@ def main():
     def build_leg(wl):
         a2 = argparse.Namespace(**vars(args))
         if a2.cpu_events is None:
-            a2.cpu_events = 16 if wl == "build_c3" else 1
+            a2.cpu_events = 1 if wl == "build_c4" else 16
         return bench_build(a2, d, wl)
 
     if args.workload == "mplex":
