@@ -13,7 +13,7 @@
 //                   segments are independent, so there is no carry between blocks and one launch does it
 //   3. bin_scatter: thread per hit: record (x, y, z, original index) to bin_off[key] + rank (the hits travel with their
 //                   index: no gather through the index later)
-//   4. bin_place:   thread per bin (a bin holds a handful of hits): order the records of the bin by original index ->
+//   4. bin_place:   lane per record, warp per 32 consecutive bins: order the records of a bin by original index ->
 //                   deterministic, stable; writes the 16-byte records the build scan reads and, if asked for, the
 //                   sorted x, y, z, perm arrays
 #include <cmath>
@@ -104,34 +104,37 @@ __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_scatter_kernel(const __grid_
     }
 }
 
-// record i of the bin [o0, o1) to its place: rank of its original index among the bin's records
-template <bool SOA>
-__device__ __forceinline__ void place_one(const BinArgs& a, int o0, int o1, int i) {
-    const float4 me = a.tmp[i];
-    const int idx = __float_as_int(me.w);
-    int rank = 0;
-    for (int j = o0; j < o1; ++j) rank += __float_as_int(a.tmp[j].w) < idx ? 1 : 0;
-    const int dst = o0 + rank;
-    a.xyzp[dst] = me;
-    if (SOA) { a.sx[dst] = me.x; a.sy[dst] = me.y; a.sz[dst] = me.z; a.perm[dst] = idx; }
-}
-
+// A warp takes 32 consecutive bins and with them one contiguous run of records; a LANE takes a record (not a bin: bins hold
+// 0 to a dozen records, so a thread per bin leaves two thirds of the lanes waiting for the fullest one).  The record's bin
+// is found among the warp's 33 offsets (held one per lane) by a shuffle binary search; its place is the rank of its
+// original index among the records of that bin (L1-resident re-reads of the index word).
 template <bool SOA>
 __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_place_kernel(const __grid_constant__ BinArgs a, int64_t n_bins) {
-    const int64_t b = (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x;
-    int o0 = 0, o1 = 0;
-    if (b < n_bins) { o0 = a.bin_off[b]; o1 = a.bin_off[b + 1]; }
-    const bool big = o1 - o0 > 32;
-    if (!big)
-        for (int i = o0; i < o1; ++i) place_one<SOA>(a, o0, o1, i);
-    // crowded bins (degenerate input): the whole warp shares the work of each of them
-    unsigned todo = __ballot_sync(0xffffffffu, big);
     const int lane = threadIdx.x & 31;
-    while (todo) {
-        const int src = __ffs(todo) - 1;
-        todo &= todo - 1;
-        const int q0 = __shfl_sync(0xffffffffu, o0, src), q1 = __shfl_sync(0xffffffffu, o1, src);
-        for (int i = q0 + lane; i < q1; i += 32) place_one<SOA>(a, q0, q1, i);
+    const int64_t b0 = ((int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x) - lane;      // first bin of the warp
+    if (b0 >= n_bins) return;
+    const int64_t bl = min(b0 + lane, n_bins);
+    const int off = a.bin_off[bl], off1 = a.bin_off[min(bl + 1, n_bins)];           // [off, off1): this lane's bin
+    const int start = __shfl_sync(0xffffffffu, off, 0), end = __shfl_sync(0xffffffffu, off1, 31);
+    for (int base = start; base < end; base += 32) {
+        const int i = base + lane;
+        const bool valid = i < end;
+        int lo = 0;                                        // largest lane whose bin starts at or before record i
+#pragma unroll
+        for (int step = 16; step >= 1; step >>= 1) {
+            const int v = __shfl_sync(0xffffffffu, off, lo + step);
+            if (v <= i) lo += step;
+        }
+        const int o0 = __shfl_sync(0xffffffffu, off, lo), o1 = __shfl_sync(0xffffffffu, off1, lo);
+        if (valid) {
+            const float4 me = a.tmp[i];
+            const int idx = __float_as_int(me.w);
+            int rank = 0;
+            for (int j = o0; j < o1; ++j) rank += __float_as_int(a.tmp[j].w) < idx ? 1 : 0;
+            const int dst = o0 + rank;
+            a.xyzp[dst] = me;
+            if (SOA) { a.sx[dst] = me.x; a.sy[dst] = me.y; a.sz[dst] = me.z; a.perm[dst] = idx; }
+        }
     }
 }
 
