@@ -43,6 +43,10 @@ struct BinArgs {
     float tan_tab[MAX_TAN_TAB];  // X1: fl32(tan(2 pi k / n_phi)), k = 0 .. n_phi/8 (evaluated in double on the host), last = 1
 };
 
+// BIN_ILP hits per thread, all their loads requested before the first is used and all their atomics before the first rank
+// is stored: the chain load -> atomic -> store is two memory round trips per hit otherwise
+constexpr int BIN_ILP = 2;
+
 __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_constant__ BinArgs a) {
     extern __shared__ float s_tab[];
     for (int i = threadIdx.x; i <= a.n_phi / 8; i += BIN_BLOCK) s_tab[i] = a.tan_tab[i];
@@ -51,10 +55,25 @@ __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_count_kernel(const __grid_co
         const int l = seg % a.n_layers;
         const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
         const int32_t base = seg * a.n_z * a.n_phi;
-        for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
-            const float x = a.hx[h], y = a.hy[h];
-            const int b = base + row_bin(a.kind[l] ? hit_rho(x, y) : a.hz[h], a.row_lo[l], a.row_inv[l], a.n_z) * a.n_phi + phi_bin(x, y, a.n_phi, s_tab, a.phi_scale);
-            a.kr[h] = make_int2(b, atomicAdd(&a.bin_off[b + 1], 1));
+        const bool disk = a.kind[l] != 0;
+        const float lo = a.row_lo[l], inv = a.row_inv[l];
+        for (int64_t hb = h0 + (int64_t)blockIdx.x * (BIN_BLOCK * BIN_ILP) + threadIdx.x; hb < h1; hb += (int64_t)gridDim.x * (BIN_BLOCK * BIN_ILP)) {
+            float x[BIN_ILP], y[BIN_ILP], z[BIN_ILP];
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u) {
+                const int64_t h = min(hb + u * BIN_BLOCK, h1 - 1);
+                x[u] = a.hx[h]; y[u] = a.hy[h]; z[u] = a.hz[h];
+            }
+            int b[BIN_ILP], r[BIN_ILP];
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u)
+                b[u] = base + row_bin(disk ? hit_rho(x[u], y[u]) : z[u], lo, inv, a.n_z) * a.n_phi + phi_bin(x[u], y[u], a.n_phi, s_tab, a.phi_scale);
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u)
+                if (hb + u * BIN_BLOCK < h1) r[u] = atomicAdd(&a.bin_off[b[u] + 1], 1);
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u)
+                if (hb + u * BIN_BLOCK < h1) a.kr[hb + u * BIN_BLOCK] = make_int2(b[u], r[u]);
         }
     }
 }
@@ -95,11 +114,21 @@ __global__ void __launch_bounds__(SCAN_BLOCK) kf_bin_scan_kernel(int32_t* __rest
 __global__ void __launch_bounds__(BIN_BLOCK) kf_bin_scatter_kernel(const __grid_constant__ BinArgs a) {
     for (int seg = blockIdx.y; seg < a.n_seg; seg += gridDim.y) {
         const int64_t h0 = a.seg_off[seg], h1 = a.seg_off[seg + 1];
-        for (int64_t h = h0 + (int64_t)blockIdx.x * BIN_BLOCK + threadIdx.x; h < h1; h += (int64_t)gridDim.x * BIN_BLOCK) {
-            const int2 kr = a.kr[h];
-            const float x = a.hx[h], y = a.hy[h], z = a.hz[h];
-            const int pos = __ldg(a.bin_off + kr.x) + kr.y;
-            a.tmp[pos] = make_float4(x, y, z, __int_as_float((int)(h - h0)));
+        for (int64_t hb = h0 + (int64_t)blockIdx.x * (BIN_BLOCK * BIN_ILP) + threadIdx.x; hb < h1; hb += (int64_t)gridDim.x * (BIN_BLOCK * BIN_ILP)) {
+            int2 kr[BIN_ILP];
+            float x[BIN_ILP], y[BIN_ILP], z[BIN_ILP];
+            int pos[BIN_ILP];
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u) {
+                const int64_t h = min(hb + u * BIN_BLOCK, h1 - 1);
+                kr[u] = a.kr[h];
+                x[u] = a.hx[h]; y[u] = a.hy[h]; z[u] = a.hz[h];
+            }
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u) pos[u] = __ldg(a.bin_off + kr[u].x) + kr[u].y;
+#pragma unroll
+            for (int u = 0; u < BIN_ILP; ++u)
+                if (hb + u * BIN_BLOCK < h1) a.tmp[pos[u]] = make_float4(x[u], y[u], z[u], __int_as_float((int)(hb + u * BIN_BLOCK - h0)));
         }
     }
 }
@@ -253,7 +282,7 @@ extern "C" int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_p
 
     cudaMemsetAsync(out->bin_off, 0, (size_t)(n_bins + 1) * sizeof(int32_t), st);
     if (n_hits > 0) {
-        const unsigned gx = (unsigned)std::min<int64_t>((max_seg + BIN_BLOCK - 1) / BIN_BLOCK, 4096);
+        const unsigned gx = (unsigned)std::min<int64_t>((max_seg + BIN_BLOCK * BIN_ILP - 1) / (BIN_BLOCK * BIN_ILP), 4096);
         const dim3 grid(gx ? gx : 1, (unsigned)std::min(n_seg, 65535));
         kf_bin_count_kernel<<<grid, BIN_BLOCK, (size_t)(n_phi / 8 + 1) * sizeof(float), st>>>(a);
         kf_bin_scan_kernel<<<n_seg, SCAN_BLOCK, 0, st>>>(out->bin_off, hits->seg_off_dev, n_phi * n_z);
