@@ -31,3 +31,8 @@ def test_reference_arm_build():
     d = run("--workload", "build_c3", "--events", "2", "--ref-events", "1")
     assert KEYS <= set(d) and d["metric"] == "seeds_built_per_s" and d["unit"] == "seeds/s" and d["value"] > 0
     assert d["config"]["workload"] == "build_c3"
+
+
+def test_reference_arm_build_on_the_cylinder_with_lids():
+    d = run("--workload", "build_lids_two_step", "--events", "1", "--ref-events", "1")
+    assert KEYS <= set(d) and d["metric"] == "seeds_built_per_s" and d["value"] > 0 and d["config"]["layers"] == 18
