@@ -144,6 +144,29 @@ size_t kf_bin_workspace_bytes(const kf_geom* geom, const kf_hits* hits, int32_t 
 int kf_bin_hits(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* ws,
                 size_t ws_bytes, void* stream);
 
+/* kf_bin_hits_static -- kf_bin_hits for callers that have no device memory to lend as workspace and may not allocate any.
+ * Who that is: a reconstruction module running inside an event-processing framework whose device memory is handed out by the
+ * framework's own pool (a direct cudaMalloc is forbidden there, or simply fails because the pool already holds the card),
+ * and a trigger-style loop that must not hit cudaMalloc's device-wide synchronisation and unbounded latency between events.
+ * Same arguments, same result (bit for bit) as kf_bin_hits, minus ws / ws_bytes: the 24 bytes per hit of scratch (bin key +
+ * arrival rank, then the record in arrival order) live in ONE fixed array compiled into the library, sized for
+ * KF_BIN_STATIC_MAX_HITS hits.  Cost of that: every GPU on which the library's device code gets loaded carries the array
+ * (24 MiB) until the process exits, whether or not this entry is ever called.
+ *   - hits->n_hits > KF_BIN_STATIC_MAX_HITS is refused with KF_ERR_INVALID_ARG and a message naming both numbers (bin larger
+ *     batches in pieces of whole events, or use kf_bin_hits with your own workspace).
+ *   - The call itself performs no cudaMalloc / cudaFree and uses no library routine that allocates; inputs and outputs are the
+ *     caller's as before.
+ *   - The device that is CURRENT on the calling thread must be the one that owns `stream` and every array passed in.  The first
+ *     call on each device looks up the array's device address (cudaGetSymbolAddress; this may make the runtime load the
+ *     library's device code on that GPU) and remembers it per device; make that first call during set-up, before any stream
+ *     capture is begun.  Later calls only launch.
+ *   - All calls on a device share the one array and it keeps whatever the previous call left.  Nothing in it needs to start
+ *     from zero -- each call writes the entries of its own n_hits hits before it reads them -- but two calls whose kernels can
+ *     overlap on the GPU (different streams without an ordering between them, or host threads racing) overwrite each other's
+ *     scratch and give wrong bins: order them on one stream or with events. */
+#define KF_BIN_STATIC_MAX_HITS (1 << 20)
+int kf_bin_hits_static(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* stream);
+
 /* kf_window_lookup -- test / diagnostic entry: the window hit list of B2-B3 for explicit windows (reading X3).
  * Query i: event[i], layer[i], azimuth window phi_c +- dphi (phi_c in (-pi, pi], dphi >= 0), z window z_c +- dz (on a
  * disk layer z_c, dz are read as the radius window rho_c +- d_rho).

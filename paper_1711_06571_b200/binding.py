@@ -19,7 +19,7 @@ _lib = None
 KF_MAX_LAYERS = 32
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
-EXPORTS = ["kf_options_init", "kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_window_lookup", "kf_build_workspace_bytes",
+EXPORTS = ["kf_options_init", "kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_bin_hits_static", "kf_window_lookup", "kf_build_workspace_bytes",
            "kf_build", "kf_select_best", "kf_mat66_multiply", "kf_last_error", "kf_version"]
 
 
@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
         l.kf_options_init.restype = None
         l.kf_fit.argtypes = [C.c_void_p] * 8
         l.kf_bin_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        l.kf_bin_hits_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         l.kf_window_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 6 + [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_mat66_multiply.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_select_best.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p]
@@ -259,6 +260,20 @@ def kf_bin_hits(geom: Geom, hits: Hits, n_phi: int, n_z: int, out: Binned | None
     rc = lib().kf_bin_hits(C.byref(geom.c), C.byref(hits.c), n_phi, n_z, C.byref(out.c), C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
     _check(rc, "kf_bin_hits")
     out._ws = ws    # keep the workspace alive until the stream has consumed it
+    return out
+
+
+BIN_STATIC_MAX_HITS = 1 << 20      # KF_BIN_STATIC_MAX_HITS of include/kf.h
+
+
+def kf_bin_hits_static(geom: Geom, hits: Hits, n_phi: int, n_z: int, out: Binned, stream=None) -> Binned:
+    """include/kf.h kf_bin_hits_static: kf_bin_hits without a workspace argument, for callers that may not allocate device
+    memory (a module fed from a framework-owned memory pool, a loop that cannot take cudaMalloc's synchronisation).  The scratch
+    is a fixed array inside the library, good for BIN_STATIC_MAX_HITS hits; larger batches raise KfError (-1).  `out` must be
+    given -- this wrapper allocates nothing either.  Calls share the array: keep them ordered on the GPU (one stream)."""
+    _require_cuda()
+    rc = lib().kf_bin_hits_static(C.byref(geom.c), C.byref(hits.c), n_phi, n_z, C.byref(out.c), _stream(stream))
+    _check(rc, "kf_bin_hits_static")
     return out
 
 

@@ -320,3 +320,49 @@ extern "C" int kf_window_lookup(const kf_geom* geom, const kf_hits* hits, const 
     kf_window_lookup_kernel<<<(unsigned)((n_query + BIN_BLOCK - 1) / BIN_BLOCK), BIN_BLOCK, 0, (cudaStream_t)stream>>>(a);
     return check_launch("kf_window_lookup");
 }
+
+// ---- kf_bin_hits_static: the same binning with its scratch in a fixed array of this library (include/kf.h) ----
+// For callers that cannot get device memory themselves: a module inside a framework that owns all device memory through its
+// pool, or a loop that cannot afford cudaMalloc's device-wide synchronisation.  Nothing here allocates.
+#include <mutex>
+
+namespace kf {
+
+constexpr size_t align256_c(size_t x) { return (x + 255) & ~(size_t)255; }
+// the layout of bin_ws_layout() for the largest batch accepted: (key, rank) pairs, then the records in arrival order
+constexpr size_t STATIC_WS_BYTES = align256_c((size_t)KF_BIN_STATIC_MAX_HITS * sizeof(int2)) + align256_c((size_t)KF_BIN_STATIC_MAX_HITS * sizeof(float4));
+
+// Lives in the global memory of every GPU that loads this module, until the process ends.  In HOST code the name below is only
+// a handle for cudaGetSymbolAddress -- it is not a device pointer and must never be handed to a kernel as one.
+static __device__ __align__(256) unsigned char g_bin_scratch[STATIC_WS_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static void* g_bin_scratch_addr[STATIC_MAX_DEVICES];     // device address of g_bin_scratch on device d; NULL = not looked up yet
+static std::mutex g_bin_scratch_mutex;
+
+}  // namespace kf
+
+extern "C" int kf_bin_hits_static(const kf_geom* geom, const kf_hits* hits, int32_t n_phi, int32_t n_z, kf_binned* out, void* stream) {
+    using namespace kf;
+    if (!geom || !hits || !out) return fail(KF_ERR_NULL_PTR, "kf_bin_hits_static: NULL struct argument");
+    if (hits->n_hits > (int64_t)KF_BIN_STATIC_MAX_HITS)
+        return fail(KF_ERR_INVALID_ARG, "kf_bin_hits_static: n_hits = %lld exceeds KF_BIN_STATIC_MAX_HITS = %d, the size of the library's fixed scratch array "
+                    "(bin fewer events per call, or use kf_bin_hits with a workspace of your own)", (long long)hits->n_hits, (int)KF_BIN_STATIC_MAX_HITS);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(KF_ERR_CUDA, "kf_bin_hits_static: cudaGetDevice failed: %d (%s)", (int)e, cudaGetErrorString(e));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(KF_ERR_INVALID_ARG, "kf_bin_hits_static: device ordinal %d outside 0..%d", dev, STATIC_MAX_DEVICES - 1);
+    void* scratch = nullptr;
+    {   // once per device, with that device current: the array's address THERE (each GPU has its own copy)
+        std::lock_guard<std::mutex> lock(g_bin_scratch_mutex);
+        scratch = g_bin_scratch_addr[dev];
+        if (!scratch) {
+            e = cudaGetSymbolAddress(&scratch, g_bin_scratch);
+            if (e != cudaSuccess || !scratch)
+                return fail(KF_ERR_CUDA, "kf_bin_hits_static: cudaGetSymbolAddress on device %d failed: %d (%s)", dev, (int)e, cudaGetErrorString(e));
+            g_bin_scratch_addr[dev] = scratch;
+        }
+    }
+    // every scratch entry of a hit is written (count, scatter) before it is read (scatter, place): nothing to clear between calls
+    return kf_bin_hits(geom, hits, n_phi, n_z, out, scratch, STATIC_WS_BYTES, stream);
+}
