@@ -17,6 +17,7 @@ _SO = os.path.join(_HERE, "libkf_b200.so")
 _lib = None
 
 KF_MAX_LAYERS = 32
+MIN_KF_VERSION = 220      # struct layouts and signatures of include/kf.h as they stand (kf_layer.kind, kf_geom.hit_mode, opt)
 ST_UNREACHABLE, ST_LEFT_Z, ST_GRAZING, ST_NUMERIC = 1, 2, 4, 8
 
 EXPORTS = ["kf_options_init", "kf_fit", "kf_bin_workspace_bytes", "kf_bin_hits", "kf_bin_hits_static", "kf_window_lookup", "kf_build_workspace_bytes",
@@ -81,6 +82,10 @@ def lib() -> C.CDLL:
         l.kf_mat66_multiply.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         l.kf_select_best.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p]
         l.kf_build.argtypes = [C.c_void_p] * 6 + [C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        # kf_layer (32 bytes with kind / rmin), kf_geom.hit_mode and the opt arguments date from version 220: only kf_options
+        # carries a size field, so an older library would misread the structs below instead of rejecting them
+        if l.kf_version() < MIN_KF_VERSION:
+            raise KfError(f"{_SO} is version {l.kf_version()}, this binding needs >= {MIN_KF_VERSION}: rebuild with `python -m paper_1711_06571_b200.build_ext --force`")
         _lib = l
     return _lib
 
@@ -192,7 +197,8 @@ def kf_version() -> int:
 
 
 def options(**fields) -> kf_options:
-    """kf_options with the library's defaults (kf_options_init) and the given fields set, e.g. options(build_seeds_per_block=4)."""
+    """kf_options with the library's defaults (kf_options_init) and the given fields set, e.g. options(build_seeds_per_block=64)
+    (build_seeds_per_block: 0 or a multiple of 16 in 16..256)."""
     o = kf_options()
     lib().kf_options_init(C.byref(o))
     for k, v in fields.items():

@@ -781,7 +781,6 @@ extern "C" int kf_build(const kf_geom* geom, const kf_hits* hits, const kf_binne
     if (!geom || !hits || !binned || !seeds || !out) return fail(KF_ERR_NULL_PTR, "kf_build: NULL struct argument");
     int rc = check_geom(geom, "kf_build");
     if (rc) return rc;
-    if (geom->hit_mode != 0 && geom->hit_mode != 1) return fail(KF_ERR_INVALID_ARG, "kf_build: hit_mode must be 0 or 1");
     if (K < 1 || K > 32) return fail(KF_ERR_INVALID_ARG, "kf_build: K = %d outside 1..32", K);
     if (first_layer < 0 || first_layer > geom->n_layers) return fail(KF_ERR_INVALID_ARG, "kf_build: first_layer outside 0..n_layers");
     if (!(chi2_cut > 0.f) || !(n_sigma > 0.f)) return fail(KF_ERR_INVALID_ARG, "kf_build: chi2_cut and n_sigma must be positive");

@@ -8,8 +8,10 @@ north_star: parameters within 1e-4 relative (1e-6 absolute floor), covariance wi
   * covariance: |dC_ij| <= 1e-3 s_i s_j, s_i = sqrt(C_ii), with s_x = s_y = sqrt(C_xx + C_yy) (the x-y block is
     singular by construction and rotates with the azimuth);
   * phi is an azimuth: its zero is a choice of frame, so "relative to |phi|" is as frame-dependent as it is for x and y.
-    Read like the position (A12): the transverse direction (cos phi, sin phi) within 1e-4 of its norm, i.e.
-    |d phi| <= 1e-4 rad (`phi_viol`), AND the strict per-component rule |d phi| <= max(1e-4 |phi|, 1e-6) counted and
+    Read like the position (A12) -- the transverse direction (cos phi, sin phi), not the number phi -- but NOT with the
+    1e-4 of its norm that reading would allow (1e-4 rad is a hundred times what the kernels do and would let a real
+    regression through): the flat bound is |d phi| <= PHI_DIR_ABS = 1e-5 rad (`phi_viol`; worst measured over the GPU suite
+    below 1e-6 rad on the fits), AND the strict per-component rule |d phi| <= max(1e-4 |phi|, 1e-6) counted and
     bounded (`strict_phi_viol`, `worst_phi_strict`): a track that turns by 2 rad carries d phi = 2 rad x d(1/pT)/(1/pT),
     so a 1/pT that is right to 1e-6 -- a hundred times inside ITS tolerance -- already moves phi by 2e-6 rad, which only
     shows where |phi| happens to be below 0.01 (assert_parity: at most 1e-4 of the tracks, none beyond 4x);
@@ -20,6 +22,7 @@ north_star: parameters within 1e-4 relative (1e-6 absolute floor), covariance wi
 import numpy as np
 
 PAR_REL, PAR_ABS, COV_REL, CHI2_REL = 1e-4, 1e-6, 1e-3, 1e-3
+PHI_DIR_ABS = 1e-5      # rad: the frame-independent bound on d phi (module docstring)
 
 
 def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None, chi2_scale=1.0) -> dict:
@@ -49,7 +52,7 @@ def compare_tracks(gpu: dict, ref: dict, sel=None, cov_scale=None, chi2_scale=1.
         cerr = cerr / np.asarray(cov_scale, dtype=np.float64)[None, :, :]
     c2 = np.abs(gpu["chi2"].astype(np.float64)[sel] - ref["chi2"][sel]) / (chi2_scale * CHI2_REL * np.maximum(ref["chi2"][sel], 1.0))
     mom = comp[[3, 5]]
-    phi_dir = np.abs(d[4]) / PAR_REL
+    phi_dir = np.abs(d[4]) / PHI_DIR_ABS
     return dict(n=int(sel.sum()), worst_mom=float(mom.max(initial=0)), worst_pos_norm=float(pos.max(initial=0)),
                 strict_pos_viol=int((comp[:3] > 1).any(axis=0).sum()), mom_viol=int((mom > 1).any(axis=0).sum()),
                 phi_viol=int((phi_dir > 1).sum()), worst_phi_dir=float(phi_dir.max(initial=0)),
