@@ -124,6 +124,26 @@ def fit_units(fi) -> dict:
     return dict(track_layers=n_upd, flops=n_upd * FIT_FLOP_PER_TRACK_LAYER, flops_survey=n_upd * FIT_FLOP_PER_TRACK_LAYER_SURVEY, bytes=by)
 
 
+def fit_config(workload: str, fi) -> dict:
+    """`config` of a fit line: the same keys and values from the GPU arm and the reference arm (the driver compares them)."""
+    u = fit_units(fi)
+    return dict(workload=workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=u["track_layers"],
+                l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (u["bytes"] / 1e6))
+
+
+def build_needs_flush(n_hits: int) -> bool:
+    return n_hits * 28 < (160 << 20)      # working set of a step below the 126 MB L2
+
+
+def build_config(workload: str, bi) -> dict:
+    """`config` of a build line: the same keys and values from both arms."""
+    n_hits = int(bi.seg_off[-1])
+    return dict(workload=workload, events_per_gpu=bi.n_events, seeds_per_gpu=bi.n_seeds, hits_per_gpu=n_hits, layers=bi.geom.n_layers, K=bi.K,
+                n_phi=bi.n_phi, n_z=bi.n_z, chi2_cut=bi.chi2_cut, n_sigma=bi.n_sigma,
+                l2="192 MB fill between timed iterations (outside the timed segments)" if build_needs_flush(n_hits) else
+                   "hits + sorted copy + candidates per step exceed the 126 MB L2; no explicit flush")
+
+
 def build_units(counters: dict, n_seeds: int, K: int, L: int, scale: float = 1.0) -> dict:
     """Algorithmic flops / bytes of one kf_build call from the oracle's own counters."""
     c = {k: v * scale for k, v in counters.items()}
@@ -135,6 +155,33 @@ def build_units(counters: dict, n_seeds: int, K: int, L: int, scale: float = 1.0
 # ----------------------------------------------------------------------------------------------------------------
 # the oracle on the host cores (cpu_baseline leg and --impl reference)
 # ----------------------------------------------------------------------------------------------------------------
+class oracle_threads:
+    """`with oracle_threads(1):` -- the oracle's OpenMP loops on n host threads, set through the libgomp the oracle is linked
+    against (omp_set_num_threads), so that the oracle itself stays as it stands.  SURVEY.md sec. 8d asks for the single-thread
+    rate beside the all-cores one."""
+
+    def __init__(self, n: int):
+        import ctypes
+        from oracle import kf_oracle as o
+        o.lib()                                   # libgomp is in the process once the oracle is loaded
+        self.gomp = ctypes.CDLL("libgomp.so.1")
+        self.n = n
+
+    def __enter__(self):
+        self.prev = int(self.gomp.omp_get_max_threads())
+        self.gomp.omp_set_num_threads(self.n)
+        return self
+
+    def __exit__(self, *exc):
+        self.gomp.omp_set_num_threads(self.prev)
+
+
+def one_core(cb: dict, cb1: dict) -> dict:
+    """adds the single-thread leg to a cpu_baseline object"""
+    cb.update(value_1_core=cb1["value"], sample_1_core=cb1["sample"])
+    return cb
+
+
 def oracle_fit(fi, n_s, steps, warmup):
     from oracle import kf_oracle as o
     n_s = min(fi.n, n_s)
@@ -188,7 +235,7 @@ def run_reference(args, workload):
     if workload in FIT_CFG:
         fi = synth.fit_inputs(FIT_CFG[workload], n=args.tracks)
         cb = oracle_fit(fi, args.ref_sample, args.steps, args.warmup)
-        metric, cfg = "tracks_fitted_per_s", dict(workload=workload, tracks=fi.n, layers=fi.geom.n_layers)
+        metric, cfg = "tracks_fitted_per_s", fit_config(workload, fi)
     elif workload == "mplex":
         from oracle import kf_oracle as o
         m = 2_000_000
@@ -205,7 +252,7 @@ def run_reference(args, workload):
     else:
         bi = synth.build_inputs(BUILD_CFG[workload], n_events=args.events, **BUILD_KW.get(workload, {}))
         cb, _, _ = oracle_build(bi, args.ref_events, args.steps, args.warmup, hit_mode=BUILD_HIT_MODE.get(workload, 0))
-        metric, cfg = "seeds_built_per_s", dict(workload=workload, events=bi.n_events, seeds=bi.n_seeds, layers=bi.geom.n_layers, K=bi.K)
+        metric, cfg = "seeds_built_per_s", build_config(workload, bi)
     ms = cb.pop("ms_per_step")
     return dict(impl="reference", metric=metric, value=cb["value"], unit=cb["unit"], n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
@@ -331,16 +378,19 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
                     hbm_achieved_gbs=units["bytes"] / (kern_ms * 1e-3) / 1e9, hbm_peak_gbs=pk["hbm_gbs"],
                     frac_of_slower_roof=max(t_alu, t_hbm) / (kern_ms * 1e-3))
     roofline["traffic"] = stored_traffic(workload)
+    roofline["traffic_note"] = traffic_note(workload)
     line = dict(metric="tracks_fitted_per_s", value=value, unit="tracks/s", n_gpus=d.world, steps=args.steps, warmup=W,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="f32", data="synthetic",
-                config=dict(workload=workload, tracks_per_gpu=fi.n, layers=fi.geom.n_layers, track_layers=units["track_layers"],
-                            l2="inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no explicit flush" % (units["bytes"] / 1e6)),
+                config=fit_config(workload, fi),
                 clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms, streams=n_sub),
                 gpu_launches=args.steps, roofline=roofline)
     if not args.no_cpu_baseline:
         cb = oracle_fit(fi, args.cpu_sample, 1, 0)
         cb.pop("ms_per_step")
-        line["cpu_baseline"] = cb
+        with oracle_threads(1):
+            cb1 = oracle_fit(fi, max(args.cpu_sample // 10, 1), 1, 0)
+            assert cb1["cores"] == 1
+        line["cpu_baseline"] = one_core(cb, cb1)
     return line
 
 
@@ -362,6 +412,22 @@ def stored_traffic(workload):
     return None
 
 
+def traffic_note(workload):
+    """why `traffic` is what it is: the capture it comes from, or why there is none for this library version"""
+    import csv
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        from paper_1711_06571_b200 import binding as b
+        ver = str(b.kf_version())
+        rows = [r for r in csv.DictReader(open(tr)) if r["workload"] == workload and r["dram_bytes_per_launch"]]
+    except Exception as e:
+        return f"profiles/traffic.csv unreadable: {e}"
+    if any(r.get("kf_version", "") == ver for r in rows):
+        return f"ncu --set full capture at library version {ver} (profiles/traffic.csv)"
+    have = sorted({r.get("kf_version", "?") for r in rows})
+    return f"no capture at library version {ver} in profiles/traffic.csv (captures at: {', '.join(have) or 'none'}); a stale number is not reported"
+
+
 BUILD_LAUNCHES_PER_STEP = 5   # bin: count, scan, scatter, place; build (the memset of bin_off is not a kernel)
 
 
@@ -369,12 +435,14 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     import torch
     from paper_1711_06571_b200 import binding as b
     cfg = BUILD_CFG[workload]
+    idle = False
     if args.scaling == "strong":      # the configured events dealt out whole, balanced by seed count (shard.assign_events)
         from paper_1711_06571_b200 import shard
         n_ev_cfg = args.events if args.events is not None else synth.BUILD_CONFIGS[cfg]["n_events"]
         per_event = synth.BUILD_CONFIGS[cfg]["tracks"] * (1.0 + synth.BUILD_CONFIGS[cfg]["fake_frac"])
         mine = shard.assign_events([per_event] * n_ev_cfg, d.world)[d.rank]
-        bi = synth.build_inputs(cfg, n_events=max(len(mine), 1), event0=mine[0] if mine else 0, **BUILD_KW.get(workload, {}))
+        idle = not mine           # more ranks than events: this rank holds placeholder inputs, launches nothing and counts no seeds
+        bi = synth.build_inputs(cfg, events=mine if mine else [0], **BUILD_KW.get(workload, {}))      # exactly the events dealt to this rank
     else:
         bi = synth.build_inputs(cfg, n_events=args.events, event0=d.rank * 1000, **BUILD_KW.get(workload, {}))
     L, K = bi.geom.n_layers, bi.K
@@ -388,12 +456,15 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     out = b.Cands(bi.n_seeds, K, L)
     bws = torch.empty(max(b.kf_build_workspace_bytes(geom, bi.n_seeds, K), 1), dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
-    flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda") if hits.n_hits * 28 < (160 << 20) else None
+    flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda") if build_needs_flush(hits.n_hits) else None
 
     def step(rec):
         if flush is not None:
             flush.fill_(1)        # working set below the 126 MB L2: flush between timed iterations
         rec(0)
+        if idle:
+            rec(1)
+            return
         b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned, ws=ws, stream=stream)
         rec(1)
         b.kf_build(geom, hits, binned, seeds, sev, shi, bi.first_layer, K, bi.chi2_cut, bi.n_sigma, out=out, ws=bws, stream=stream)
@@ -405,7 +476,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     bin_ms, build_ms = statistics.mean(seg[1]), statistics.mean(seg[2])
     ms_per_step = d.max_ms(bin_ms + build_ms)          # the L2 flush is not part of the step
     from paper_1711_06571_b200 import shard as _shard
-    n_job = _shard.sum_over_ranks(float(bi.n_seeds), device="cuda")
+    n_job = _shard.sum_over_ranks(0.0 if idle else float(bi.n_seeds), device="cuda")
     value = n_job / (ms_per_step * 1e-3)
 
     # ---- end to end: hits + seeds H2D, bin + build, candidates D2H ----
@@ -417,7 +488,8 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     n_sub = len(pipe.subs)
 
     def e2e_step(rec):
-        pipe.run(stream)
+        if not idle:
+            pipe.run(stream)
 
     e2e_ms, _, _, _, _ = time_steps(e2e_step, max(3, min(args.steps, 10)), 2, stream, d)
     if d.rank != 0:
@@ -425,10 +497,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     pk = peaks()
     res = dict(metric="seeds_built_per_s", value=value, unit="seeds/s", ms_per_step=ms_per_step, bin_ms=bin_ms, build_ms=build_ms,
                hits_binned_per_s=hits.n_hits / (bin_ms * 1e-3),
-               config=dict(workload=workload, events_per_gpu=bi.n_events, seeds_per_gpu=bi.n_seeds, hits_per_gpu=hits.n_hits, layers=L, K=K,
-                           n_phi=bi.n_phi, n_z=bi.n_z, chi2_cut=bi.chi2_cut, n_sigma=bi.n_sigma,
-                           l2="192 MB fill between timed iterations (outside the timed segments)" if flush is not None else
-                              "hits + sorted copy + candidates per step exceed the 126 MB L2; no explicit flush"),
+               config=build_config(workload, bi),
                e2e=dict(value=n_job / (e2e_ms * 1e-3), unit="seeds/s", h2d_bytes_per_step=pipe.h2d_bytes, d2h_bytes_per_step=pipe.d2h_bytes,
                         ms_per_step=e2e_ms, streams=n_sub),
                gpu_launches=args.steps * BUILD_LAUNCHES_PER_STEP, clocks=clocks)
@@ -438,6 +507,9 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
     if not args.no_cpu_baseline:
         cb, counters, n_s = oracle_build(bi, args.cpu_events, 1, 0, hit_mode=BUILD_HIT_MODE.get(workload, 0))
         cb.pop("ms_per_step")
+        with oracle_threads(1):
+            cb1, _, _ = oracle_build(bi, 1, 1, 0, hit_mode=BUILD_HIT_MODE.get(workload, 0))
+        one_core(cb, cb1)
         u = build_units(counters, bi.n_seeds, K, L, scale=bi.n_seeds / max(n_s, 1))
         peak = fp32_peak_tflops(pk)
         t_alu, t_hbm = u["flops"] / (peak * 1e12), u["bytes"] / (pk["hbm_gbs"] * 1e9)
@@ -447,7 +519,7 @@ def bench_build(args, d: Dist, workload: str, sample_clocks=True):
         else:
             ach = u["bytes"] / (build_ms * 1e-3) / 1e9
             rf = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"])
-        rf.update(traffic=stored_traffic(workload), kernel="kf_build_kernel", kernel_ms=build_ms, kernel_share_of_step=build_ms / (bin_ms + build_ms),
+        rf.update(traffic=stored_traffic(workload), traffic_note=traffic_note(workload), kernel="kf_build_kernel", kernel_ms=build_ms, kernel_share_of_step=build_ms / (bin_ms + build_ms),
                   alg_flops_per_launch=u["flops"], alg_bytes_per_launch=u["bytes"], counters=u["counters"],
                   counters_source="oracle run of the cpu_baseline sample, scaled by seeds")
         res["roofline"] = rf
@@ -531,7 +603,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: tracks per step")
     ap.add_argument("--ref-events", type=int, default=16, help="--impl reference: events per step (build workloads)")
     ap.add_argument("--cpu-sample", type=int, default=200_000)
-    ap.add_argument("--cpu-events", type=int, default=None, help="events the oracle builds for cpu_baseline and the build counters (default: 16 for build_c3, 1 for build_c4)")
+    ap.add_argument("--cpu-events", type=int, default=None, help="events the oracle builds for cpu_baseline and the build counters (default: 16 for build_c3, 4 for build_c4)")
     ap.add_argument("--e2e-streams", type=int, default=None, help="sub-batches in flight in the end-to-end leg (copies overlap compute); default 4, build_c4: 8 (measured: 40.9 / 37.4 / 36.6 ms with 4 / 8 / 16 groups of events; build_c3 1.44 / 1.64 ms with 4 / 8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-build", action="store_true", help="default line without the extra legs (fit_c2, build_c3, build_c4)")
@@ -556,7 +628,7 @@ def main():
     def build_leg(wl):
         a2 = argparse.Namespace(**vars(args))
         if a2.cpu_events is None:
-            a2.cpu_events = 1 if wl == "build_c4" else 16
+            a2.cpu_events = 4 if wl == "build_c4" else 16
         return bench_build(a2, d, wl)
 
     if args.workload == "mplex":

@@ -432,6 +432,7 @@ class BuildInputs:
     seed_hit_idx: np.ndarray  # [first_layer][ld] i32 index within segment
     seed_truth: np.ndarray    # [n_seeds] i32 global truth-track id, -1 = fake seed
     truth_hit_idx: np.ndarray  # [L][n_tracks_total] i32 index within segment of each truth track's hit, -1 none
+    event_ids: np.ndarray = None   # [n_events] i64 global id (generator stream) of each event of the call
 
 
 BUILD_CONFIGS = {
@@ -478,7 +479,7 @@ def _three_point_seed(p1, p2, p3, bz):
 def build_inputs(config, n_events: int | None = None, tracks: int | None = None, first_layer: int = 3,
                  K: int = 10, chi2_cut: float = 30.0, n_sigma: float = 3.0, noise: float | None = None,
                  fake_frac: float | None = None, n_phi: int | None = None, n_z: int | None = None,
-                 smear: bool = True, ms: bool = True, event0: int = 0, jitter: float = 0.0) -> BuildInputs:
+                 smear: bool = True, ms: bool = True, event0: int = 0, jitter: float = 0.0, events=None) -> BuildInputs:
     """Inputs of kf_bin_hits / kf_build for BASELINE.json configs 3-4 (sizes can be overridden for tests).
 
     jitter > 0: sensors sit at R + U(-jitter, jitter) / Z + U(-jitter, jitter) ("hits at slightly different radii within a
@@ -487,9 +488,17 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
     hits on that layer) uniform in (phi, z) on the cylinder; each segment is shuffled.  One seed per truth
     track that reaches layer `first_layer-1`: truth state just outside that layer, smeared (smear_seed),
     diagonal covariance (reading A6b).  Config 4 adds `fake_frac` x tracks fake seeds from random
-    hit triplets on layers 0-2 (reading A18)."""
+    hit triplets on layers 0-2 (reading A18).
+    Which events: event e of the call is drawn from the generator of global event id event_ids[e]; by default the ids are
+    event0, event0 + 1, ...; `events` = an explicit list of global ids (a rank's share under strong scaling, shard.assign_events)
+    overrides n_events and event0.  The ids are returned in BuildInputs.event_ids."""
     cfg = dict(BUILD_CONFIGS[config])
+    if events is not None:
+        n_events = len(events)
+        if n_events < 1:
+            raise ValueError("build_inputs: `events` must name at least one event")
     n_events = cfg["n_events"] if n_events is None else n_events
+    event_ids = np.asarray(events if events is not None else np.arange(n_events) + event0, dtype=np.int64)
     tracks = cfg["tracks"] if tracks is None else tracks
     noise = cfg["noise"] if noise is None else noise
     fake_frac = cfg["fake_frac"] if fake_frac is None else fake_frac
@@ -502,7 +511,7 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
     seeds, sigs, qs, sev, struth, shit = [], [], [], [], [], []
     truth_hit_idx = np.full((L, n_events * tracks), -1, dtype=np.int32)
     for ev in range(n_events):
-        rng = rng_for(config if isinstance(config, int) else 101, ev + event0)     # event0: a rank's own events (weak scaling)
+        rng = rng_for(config if isinstance(config, int) else 101, int(event_ids[ev]))     # a rank's own events
         gun = particle_gun(rng, tracks, cfg["gun"])
         sim = simulate(geom, gun, rng, ms=ms, smear=smear, jitter=jitter)
         ev_hits = []
@@ -607,4 +616,4 @@ def build_inputs(config, n_events: int | None = None, tracks: int | None = None,
                        first_layer=first_layer, hit_x=np.concatenate(xs), hit_y=np.concatenate(ys), hit_z=np.concatenate(zs),
                        seg_off=np.array(seg_off, dtype=np.int64), hit_truth=np.concatenate(tr), n_seeds=n_seeds, ld=ld,
                        par=t["par"], cov=t["cov"], q=t["q"], seed_event=np.concatenate(sev), seed_hit_idx=seed_hit_idx,
-                       seed_truth=np.concatenate(struth), truth_hit_idx=truth_hit_idx)
+                       seed_truth=np.concatenate(struth), truth_hit_idx=truth_hit_idx, event_ids=event_ids)

@@ -50,9 +50,14 @@ def _worker(rank, world, port, q):
         total = shard.sum_over_ranks(float(fi.n))
         # every rank computes the same event table
         table = shard.assign_events([bi.n_seeds + 3 * k for k in range(6)], world)
+        # strong scaling of a build as bench.py does it: the rank generates exactly the events the table deals to it
+        mine = shard.assign_events([50.0] * 5, world)[rank]
+        sb = synth.build_inputs(3, events=mine, tracks=50)
         gathered = [None] * world
         dist.all_gather_object(gathered, dict(rank=rank, ms=ms, total=total, range=(b, e), table=table,
-                                              par0=float(fi.par[3, 0]), hit0=float(bi.hit_x[0])))
+                                              par0=float(fi.par[3, 0]), hit0=float(bi.hit_x[0]),
+                                              strong_events=[int(v) for v in sb.event_ids], strong_n_events=sb.n_events,
+                                              strong_first_hits=[float(sb.hit_x[sb.seg_off[k * sb.geom.n_layers]]) for k in range(sb.n_events)]))
         if rank == 0:
             q.put(gathered)
     finally:
@@ -76,6 +81,15 @@ def test_world_size_2_gloo():
     assert g[0]["range"] == (0, 501) and g[1]["range"] == (501, 1001)
     assert g[0]["table"] == g[1]["table"]
     assert g[0]["par0"] != g[1]["par0"] and g[0]["hit0"] != g[1]["hit0"]   # ranks work on different events
+    # strong-scaled build: the ranks' events partition 0..4 -- no event is built twice, none is left out
+    ev = [x["strong_events"] for x in g]
+    assert sorted(ev[0] + ev[1]) == [0, 1, 2, 3, 4] and not set(ev[0]) & set(ev[1])
+    assert [x["strong_n_events"] for x in g] == [len(ev[0]), len(ev[1])]
+    # and an event's content depends on its global id only, not on the rank or its place in the call
+    ref = synth.build_inputs(3, n_events=5, tracks=50)
+    first = [float(ref.hit_x[ref.seg_off[k * ref.geom.n_layers]]) for k in range(5)]
+    for x in g:
+        assert x["strong_first_hits"] == [first[e] for e in x["strong_events"]]
 
 
 PORT = _free_port()
