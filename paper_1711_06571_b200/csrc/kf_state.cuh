@@ -1,10 +1,8 @@
 // kf_state.cuh -- the per-layer Kalman-filter step on a register-resident state laid out for Blackwell's packed
 // fp32 arithmetic (FFMA2 / FMUL2 / FADD2: two fp32 lanes per instruction; sm_100a).
 //
-// Why: on B200 a scalar three-register FFMA issues at best every ~1.7 cycles per SM sub-partition (measured), a
-// packed FFMA2 every ~2.2 cycles for two FMAs, and FFMA2 takes any scalar register as a free broadcast operand.
-// The 148 x 128 x 2 FP32 peak is therefore only reachable with packed instructions, and a candidate's step takes
-// 452 instead of 560 warp instructions.  The 6x6 algebra of the
+// Why: a packed FFMA2 does two fp32 FMAs in one issue slot and takes any scalar register as a free broadcast operand, so
+// a candidate's step takes 452 instead of 560 warp instructions.  The 6x6 algebra of the
 // step is arranged so that its long, regular chains run two rows (or two columns) of a matrix at a time:
 //   rows (x, y) and rows (z, phi) of T = J C and of J C J^T,        columns (1/pT, theta) of T,
 //   rows (0,1), (2,4), (3,5) of the gain K = C H^T S^-1 and of the covariance update.
