@@ -58,4 +58,4 @@ extern "C" void kf_options_init(kf_options* opt) {
 }
 
 extern "C" const char* kf_last_error(void) { return kf::g_err; }
-extern "C" int kf_version(void) { return 220; }
+extern "C" int kf_version(void) { return 230; }

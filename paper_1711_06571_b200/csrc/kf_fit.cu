@@ -29,6 +29,10 @@ struct FitArgs {
 #ifndef KF_FIT_MINB
 #define KF_FIT_MINB 5
 #endif
+#ifndef KF_FIT_IDX_MINB
+#define KF_FIT_IDX_MINB KF_FIT_MINB   // explicit indices, gather requested a layer ahead: 96 registers without spills beat 80 with
+                                      // (config 2 on B200: 0.334 ms at 5 blocks per SM, 0.365 at 6, 0.342 at 4; before the pipelined gather 0.354 at 6)
+#endif
 constexpr int FIT_BLOCK = KF_FIT_BLOCK;
 
 // IDX: explicit hit_idx (else identity), EVT: per-track event (else event 0), ISO: sig_r == sig_rphi on every layer.
@@ -48,12 +52,29 @@ __device__ __forceinline__ int fit_layers(const FitArgs& a, int64_t t, float cw,
     // F6 with identity indexing: the hit of the next layer is requested one layer ahead
     float nx = 0.f, ny = 0.f, nz = 0.f;
     if (!IDX && !EVT && limit > 0) { nx = a.hxl[0][t]; ny = a.hyl[0][t]; nz = a.hzl[0][t]; }
+    // F6 with explicit indices (event 0): the same one layer ahead, which takes the index two layers ahead -- the index of
+    // layer l+2 and the hit of layer l+1 (whose index arrived during layer l-1) are requested before the arithmetic of layer l,
+    // instead of index -> dependent gather -> arithmetic in every layer
+    constexpr bool PIPE = IDX && !EVT;
+    int i1 = -2, i2 = -2;                    // indices of this layer and the next
+    if (PIPE) {
+        if (limit > 0) i1 = a.hit_idx[t];
+        if (limit > 1) i2 = a.hit_idx[a.ld_idx + t];
+        if (i1 >= 0) { nx = a.hxl[0][i1]; ny = a.hyl[0][i1]; nz = a.hzl[0][i1]; }
+    }
 #pragma unroll 1
     for (int l = 0; l < limit; ++l) {
         int64_t idx = t;
-        if (IDX) {
-            idx = a.hit_idx[l * a.ld_idx + t];
+        float px = nx, py = ny, pz = nz;     // PIPE: the hit of this layer, requested a layer ago
+        if (PIPE) {
+            idx = i1;
+            i1 = i2;
+            i2 = l + 2 < limit ? a.hit_idx[(int64_t)(l + 2) * a.ld_idx + t] : -2;
+            if (i1 >= 0) { nx = a.hxl[l + 1][i1]; ny = a.hyl[l + 1][i1]; nz = a.hzl[l + 1][i1]; }
             if (idx < -1) continue;          // layer not crossed: skipped entirely (R8)
+        } else if (IDX) {
+            idx = a.hit_idx[l * a.ld_idx + t];
+            if (idx < -1) continue;
         }
         const bool hole = IDX && idx < 0;    // -1: crossed without a hit -> transport + material, no update (R8)
         // F6: issued before the arithmetic
@@ -67,7 +88,7 @@ __device__ __forceinline__ int fit_layers(const FitArgs& a, int64_t t, float cw,
                 mx = nx; my = ny; mz = nz;
                 if (l + 1 < limit) { nx = a.hxl[l + 1][t]; ny = a.hyl[l + 1][t]; nz = a.hzl[l + 1][t]; }
             } else {
-                mx = a.hxl[l][idx]; my = a.hyl[l][idx]; mz = a.hzl[l][idx];
+                mx = px; my = py; mz = pz;
             }
         }
         const LayerC ly = a.layer[l];
@@ -115,7 +136,7 @@ __device__ __noinline__ void fit_redo(const FitArgs& a, int64_t t, float cw, int
 }
 
 template <bool IDX, bool EVT, bool ISO>
-__global__ void __launch_bounds__(FIT_BLOCK, IDX ? KF_FIT_MINB + 1 : KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {   // gathered hits: one more block
+__global__ void __launch_bounds__(FIT_BLOCK, IDX ? KF_FIT_IDX_MINB : KF_FIT_MINB) kf_fit_kernel(const __grid_constant__ FitArgs a) {
     const int64_t t = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x;
     if (t >= a.n) return;
     const float cw = -(float)a.q[t] * a.kb;

@@ -95,8 +95,9 @@ def geometry(kind: str, bz: float = 3.8, xx0_scale: float = 1.0, depth: float = 
     else:
         raise ValueError(kind)
     n = len(r)
+    # depth > 0 (hit_mode 1 on staggered sensors, R23): sig_r carries the r.m.s. radial displacement of the sensors
     return Geometry(r=r, zmax=np.full(n, 100.0), xx0=xx0 * xx0_scale, sig_rphi=np.full(n, 0.01),
-                    sig_z=np.full(n, 0.1), sig_r=np.full(n, 0.01), bz=bz)
+                    sig_z=np.full(n, 0.1), sig_r=np.full(n, depth if depth > 0 else 0.01), bz=bz)
 
 
 def pack_index(i: int, j: int) -> int:

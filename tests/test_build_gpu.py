@@ -154,9 +154,9 @@ GRAZING_BAND = 0.2   # generator guard on cos(incidence) (R8); the KF 
 MARGIN_TOL = np.array([1e-4, 1e-4, 1e-4, 1e-4, 1e-5])
 # R16b: on candidates inside the grazing band (final cos(incidence) < 0.2) the covariance elements that carry the
 # 1/cos(incidence) factor of the surface Jacobian (everything but the (1/pT, theta) block) and chi2 (whose last
-# increments are taken against that covariance) get 3x the tolerance; parameters stay at 1x.  Measured worst cases
-# (configs[4], 96 000 seeds): covariance 1.58x, chi2 1.72x at cos(incidence) = 0.11.
-BAND_CHI2_SCALE = 3.0
+# increments are taken against that covariance) get a wider tolerance; parameters stay at 1x.  Measured worst cases over all
+# build / chain / lids / pipeline tests (round 3, B200): chi2 1.72x at cos(incidence) = 0.11 -> 2x; covariance 2.9x -> 3x.
+BAND_CHI2_SCALE = 2.0
 BAND_COV_SCALE = np.full((6, 6), 3.0)
 for _i in (3, 5):
     for _j in (3, 5):
@@ -181,7 +181,7 @@ def compare_build(g, r, n_seeds, K, first_layer, band_frac=0.02, margin_tol=MARG
     edge, a chi2 at the cut, two competing children with near-equal chi2, a crossing at the grazing or acceptance limit.
     Anything else fails.
     Conditioning band (R16b): candidates whose final state crosses its cylinder with cos(incidence) < 0.2 (beyond the
-    generator's guard, inside the KF guard band) get 3x on the covariance elements with the 1/cos(incidence) factor and
+    generator's guard, inside the KF guard band) get 3x on the covariance elements with the 1/cos(incidence) factor and 2x
     on chi2; their share is bounded by `band_frac`."""
     same = g["n_cand"] == r["n_cand"]
     hs = (g["hit_idx"] == r["hit_idx"]).all(axis=0) & (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
@@ -263,6 +263,81 @@ def test_build_config4_eight_events():
     g, r = run_build(bi), ref_build(bi)
     rep = compare_build(g, r, bi.n_seeds, bi.K, bi.first_layer, band_frac=0.05)
     assert rep["seeds"] > 90_000
+
+
+def test_build_config4_full_sampled():
+    """BASELINE.json configs[4] at FULL size -- all 64 events, 768 000 seeds, 1.08e8 hits, 24 000 tiles on the persistent grid: the
+    very call every build_c4 number of bench.py is timed on.  The oracle redoes events 0, 21, 42 and 63 on their own (an event's
+    seeds only see its hits): bins bit-exact, candidates through compare_build (every mismatching seed proven from the oracle's
+    margins); all other events: properties that hold at any size."""
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs(4)
+    assert bi.n_events == 64
+    L, K, nb = bi.geom.n_layers, bi.K, bi.n_phi * bi.n_z
+    geom = b.Geom(bi.geom.layer_table(), bi.geom.bz)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    binned = b.Binned(hits.n_hits, bi.n_events * L * nb, bi.n_phi, bi.n_z, soa=False)        # as bench.py: records and offsets only
+    b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z, out=binned)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, K, bi.chi2_cut, bi.n_sigma)
+    torch.cuda.synchronize()
+    n_cand = out.n_cand.cpu().numpy()
+    nhits = out.tracks.nhits.cpu().numpy(); status = out.tracks.status.cpu().numpy(); chi2 = out.tracks.chi2.cpu().numpy()
+    # any size: every seed keeps at least one candidate, valid slots are finite and carry at least the seed's hits, unused slots are blank
+    valid = (np.arange(K)[None, :] < n_cand[:, None]).reshape(-1)
+    assert (n_cand >= 1).all() and (n_cand <= K).all()
+    assert (nhits[:bi.n_seeds * K][valid] >= bi.first_layer).all() and np.isfinite(chi2[:bi.n_seeds * K][valid]).all() and (chi2[:bi.n_seeds * K] >= 0).all()
+    assert (nhits[:bi.n_seeds * K][~valid] == 0).all() and (status[:bi.n_seeds * K][~valid] == 0).all()
+    assert bool(torch.isfinite(out.tracks.par[:, :bi.n_seeds * K][:, torch.from_numpy(valid).cuda()]).all())
+    lt = bi.geom.layer_table()
+    total = 0
+    for e in (0, 21, 42, 63):
+        h0, h1 = int(bi.seg_off[e * L]), int(bi.seg_off[(e + 1) * L])
+        seg = bi.seg_off[e * L:(e + 1) * L + 1] - h0
+        rb = o.bin_hits(lt, 1, seg, bi.hit_x[h0:h1], bi.hit_y[h0:h1], bi.hit_z[h0:h1], bi.n_phi, bi.n_z)
+        # bins of the event: offsets relative to its first hit, records in the same order
+        assert np.array_equal(binned.bin_off[e * L * nb:(e + 1) * L * nb + 1].cpu().numpy() - h0, rb["bin_off"])
+        p4 = binned.xyzp[h0:h1].cpu().numpy()
+        assert np.array_equal(p4[:, 0], rb["x"]) and np.array_equal(p4[:, 1], rb["y"]) and np.array_equal(p4[:, 2], rb["z"])
+        assert np.array_equal(np.ascontiguousarray(p4[:, 3]).view(np.int32), rb["perm"])
+        sd = np.nonzero(bi.seed_event == e)[0]
+        s0, s1 = int(sd[0]), int(sd[-1]) + 1
+        assert s1 - s0 == len(sd)
+        n = s1 - s0
+        r = o.kf_build(lt, bi.geom.bz, rb, seg, np.ascontiguousarray(bi.par[:, s0:s1]), np.ascontiguousarray(bi.cov[:, s0:s1]), bi.q[s0:s1],
+                       np.zeros(n, np.int32), np.ascontiguousarray(bi.seed_hit_idx[:, s0:s1]), bi.first_layer, K, bi.chi2_cut, bi.n_sigma, margins=True)
+        sl = slice(s0 * K, s1 * K)
+        g = dict(par=out.tracks.par[:, sl].cpu().numpy(), cov=out.tracks.cov[:, sl].cpu().numpy(), chi2=chi2[sl], nhits=nhits[sl],
+                 status=status[sl].view(np.uint32), hit_idx=out.hit_idx[:, sl].cpu().numpy(), n_cand=n_cand[s0:s1])
+        rep = compare_build(g, r, n, K, bi.first_layer, band_frac=0.05)
+        total += rep["seeds"]
+    assert total > 45_000
+
+
+def test_two_step_build_on_a_barrel_only_geometry():
+    """hit_mode 1 WITHOUT disks (config-3 recipe, sensors staggered by +-0.3 cm radially): the kernel instantiation that handles
+    the second propagation step but, having no lids, finishes a candidate on a layer it cannot reach instead of skipping the
+    layer (kf_build.cu, a.lids == 0)."""
+    from paper_1711_06571_b200 import binding as b
+    bi = synth.build_inputs(3, n_events=3, tracks=1500, jitter=0.3)
+    lt = bi.geom.layer_table()
+    geom = b.Geom(lt, bi.geom.bz, hit_mode=1)
+    hits = b.Hits(bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, bi.n_events)
+    binned = b.kf_bin_hits(geom, hits, bi.n_phi, bi.n_z)
+    seeds = b.Tracks.from_host(bi.par, bi.cov, bi.q)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g = b.kf_build(geom, hits, binned, seeds, t(bi.seed_event), t(bi.seed_hit_idx), bi.first_layer, bi.K, bi.chi2_cut, bi.n_sigma)
+    torch.cuda.synchronize()
+    r = o.kf_build(lt, bi.geom.bz, ref_bin(bi), bi.seg_off, bi.par, bi.cov, bi.q, bi.seed_event, bi.seed_hit_idx, bi.first_layer, bi.K,
+                   bi.chi2_cut, bi.n_sigma, margins=True, hit_mode=1)
+    rep = compare_build(g.to_host(), r, bi.n_seeds, bi.K, bi.first_layer, band_frac=0.05)
+    best = np.arange(bi.n_seeds) * bi.K
+    assert rep["seed_mismatch_frac"] < 0.03 and (r["nhits"][best] >= 8).mean() > 0.8        # the staggered hits are found
+    # the states sit on the hits' own radii
+    off = np.abs(np.hypot(g.tracks.par[0].cpu().numpy()[best], g.tracks.par[1].cpu().numpy()[best]) - lt[-1][0])
+    full = r["hit_idx"][-1, best] >= 0
+    assert full.sum() > 1000 and off[full].max() <= 0.3 + 1e-4 and np.median(off[full]) > 0.05
 
 
 @pytest.mark.parametrize("K", [1, 3, 32])

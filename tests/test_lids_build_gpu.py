@@ -135,11 +135,22 @@ def test_lids_two_step_build_parity(kw, K):
     rf = o.fit(bi.geom.layer_table(), bi.geom.bz, bi.par, bi.cov, bi.q, bi.hit_x, bi.hit_y, bi.hit_z, bi.seg_off, hit_idx=hi, trk_event=bi.seed_event, hit_mode=1)
     same = (gf["nhits"] == rf["nhits"]) & (gf["status"] == rf["status"])
     assert (~same).sum() <= 3e-3 * bi.n_seeds, int((~same).sum())
+    # cos(incidence) on the surface the fitted state sits on: in the transverse plane on a cylinder, |cos theta| on a disk
     x, y, ph = rf["par"][0], rf["par"][1], rf["par"][4]
-    cosinc = (x * np.cos(ph) + y * np.sin(ph)) / np.maximum(np.hypot(x, y), 1e-30)
-    ok = same & (rf["status"] == 0) & (cosinc >= 0.25)
-    assert ok.mean() > 0.9
-    assert_parity(compare_tracks(gf, rf, sel=ok))
+    kind = bi.geom.layer_table()[:, 6]
+    crossed = hi[:, :bi.n_seeds] >= -1
+    last = np.where(crossed.any(axis=0), crossed.shape[0] - 1 - np.argmax(crossed[::-1], axis=0), 0)
+    cosinc = np.where(kind[last] == 0, (x * np.cos(ph) + y * np.sin(ph)) / np.maximum(np.hypot(x, y), 1e-30), np.abs(np.cos(rf["par"][5])))
+    from tests.test_build_gpu import BAND_CHI2_SCALE, BAND_COV_SCALE
+    from tests.test_lids_gpu import TWO_STEP_BAND
+    ok = same & (rf["status"] == 0) & (rf["nhits"] > 0)
+    inband = cosinc < TWO_STEP_BAND
+    assert (ok & ~inband).mean() > 0.9
+    assert_parity(compare_tracks(gf, rf, sel=ok & ~inband))
+    # the conditioning band (R16b) is compared too, with its scales, and its share is bounded
+    rb = compare_tracks(gf, rf, sel=ok & inband, cov_scale=BAND_COV_SCALE, chi2_scale=BAND_CHI2_SCALE)
+    assert rb["n"] <= 0.05 * bi.n_seeds, rb
+    assert_parity(rb)
 
 
 def test_build_rejects_an_unknown_hit_mode():

@@ -32,7 +32,7 @@ TWO_STEP_BAND = 0.25   # DESIGN.md R16b for hit_mode 1: two covariance transport
 
 def check(g, r, max_decision_mismatch=1e-4, band=0.0):
     """band > 0: tracks whose final state crosses its cylinder with cos(incidence) < band are compared with the R16b scales
-    (3x on the covariance elements carrying the 1/cos(incidence) factor and on chi2), their share bounded at 2 %."""
+    (3x on the covariance elements carrying the 1/cos(incidence) factor, 2x on chi2), their share bounded at 2 %."""
     from tests.test_build_gpu import BAND_CHI2_SCALE, BAND_COV_SCALE
     same = (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
     assert (~same).sum() <= max_decision_mismatch * len(same), int((~same).sum())
