@@ -182,7 +182,25 @@ def one_core(cb: dict, cb1: dict) -> dict:
     return cb
 
 
-def oracle_fit(fi, n_s, steps, warmup):
+def parity_summary(out, r, sample: str) -> dict:
+    """The timed kernel's output against the oracle run of the cpu_baseline leg (same tracks), with the rules of tests/parity.py:
+    a report, not a gate -- the gate is `pytest -m gpu`.  Worst errors are in units of their tolerance (1.0 = at tolerance)."""
+    try:
+        from tests.parity import compare_tracks, PHI_DIR_ABS
+        n = len(r["chi2"])
+        g = dict(par=out.par[:, :n].cpu().numpy(), cov=out.cov[:, :n].cpu().numpy(), chi2=out.chi2[:n].cpu().numpy(),
+                 nhits=out.nhits[:n].cpu().numpy(), status=out.status[:n].cpu().numpy().view(np.uint32))
+        same = (g["nhits"] == r["nhits"]) & (g["status"] == r["status"])
+        rep = compare_tracks(g, r, sel=same & (r["nhits"] > 0))
+        keys = ("n", "mom_viol", "pos_viol", "cov_viol", "chi2_viol", "phi_viol", "strict_phi_viol", "worst_mom", "worst_pos_norm", "worst_cov",
+                "worst_chi2", "worst_phi_strict")
+        return dict(sample=sample, decisions_differ=int((~same).sum()), worst_dphi_rad=rep["worst_phi_dir"] * PHI_DIR_ABS, **{k: rep[k] for k in keys})
+    except Exception as e:                      # never let the report break the bench line
+        return dict(error=f"{type(e).__name__}: {e}")
+
+
+def oracle_fit(fi, n_s, steps, warmup, keep=None):
+    """keep: a dict that receives the oracle's result of the last call under "r" (for the parity summary of the line)"""
     from oracle import kf_oracle as o
     n_s = min(fi.n, n_s)
     L, ld = fi.geom.n_layers, fi.ld
@@ -192,13 +210,18 @@ def oracle_fit(fi, n_s, steps, warmup):
     hi = None if fi.hit_idx is None else np.ascontiguousarray(fi.hit_idx[:, :n_s])
     par = np.ascontiguousarray(fi.par[:, :n_s]); cov = np.ascontiguousarray(fi.cov[:, :n_s]); q = fi.q[:n_s]
     seg = np.arange(L + 1) * n_s
-    call = lambda: o.fit(fi.geom.layer_table(), fi.geom.bz, par, cov, q, hx, hy, hz, seg, hi)
+    last = {}
+
+    def call():
+        last["r"] = o.fit(fi.geom.layer_table(), fi.geom.bz, par, cov, q, hx, hy, hz, seg, hi)
     for _ in range(warmup):
         call()
     t0 = time.perf_counter()
     for _ in range(steps):
         call()
     dt = (time.perf_counter() - t0) / steps
+    if keep is not None:
+        keep.update(last)
     return dict(value=n_s / dt, unit="tracks/s", cores=o.num_threads(), kind="oracle",
                 sample=f"first {n_s} tracks of the {fi.n}-track workload per step", ms_per_step=dt * 1e3)
 
@@ -385,8 +408,10 @@ def bench_fit(args, d: Dist, workload: str, sampler_cb=None):
                 clocks=clocks, e2e=dict(value=e2e_value, unit="tracks/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_ms, streams=n_sub),
                 gpu_launches=args.steps, roofline=roofline)
     if not args.no_cpu_baseline:
-        cb = oracle_fit(fi, args.cpu_sample, 1, 0)
+        keep = {}
+        cb = oracle_fit(fi, args.cpu_sample, 1, 0, keep=keep)
         cb.pop("ms_per_step")
+        line["parity_sample"] = parity_summary(out, keep.get("r"), cb["sample"])
         with oracle_threads(1):
             cb1 = oracle_fit(fi, max(args.cpu_sample // 10, 1), 1, 0)
             assert cb1["cores"] == 1
@@ -642,7 +667,7 @@ def main():
             torch.cuda.empty_cache()
             b4 = build_leg("build_c4")
             if line is not None:
-                keep = ("metric", "value", "unit", "ms_per_step", "config", "clocks", "roofline", "cpu_baseline", "e2e", "gpu_launches")
+                keep = ("metric", "value", "unit", "ms_per_step", "config", "clocks", "roofline", "cpu_baseline", "parity_sample", "e2e", "gpu_launches")
                 line["fit_c2"] = {k: f2[k] for k in keep if k in f2}
                 line["build"] = b3
                 line["build_c4"] = b4
